@@ -1,0 +1,212 @@
+"""Seeded synthetic inputs and weights for the Evoformer trunk (shared by tests, bench and smoke).
+
+This module holds NONE of the method's arithmetic: it only draws seeded random numbers, names the
+parameters of one Evoformer block in the blob order of SURVEY.md Appendix B, and packs / unpacks
+that blob.  Both the fp64 oracle (``oracle/``) and the CUDA path (``paper_2111_06340_b200``) are fed
+from here so that they see bit-identical inputs; neither of them imports the other.
+
+Readings used: R2 (mask shapes), R8 (init recipe), R10 (cfg5 length law),
+R11 (cfg2 msa_mask law), R15 (weights are bf16-representable on the bf16 path).
+Workload shapes stand in for the paper's data sets, which are not available:
+PAPER.md:130-132 (small / medium / large sets), PAPER.md:113 (batches of similar-length proteins).
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass
+
+import numpy as np
+
+# ----------------------------------------------------------------------------------------------
+# dimensions (BASELINE.json north_star / configs[0]; SURVEY.md §8 header)
+# ----------------------------------------------------------------------------------------------
+
+
+@dataclass(frozen=True)
+class Dims:
+    c_m: int = 256
+    c_z: int = 128
+    heads_msa: int = 8
+    heads_pair: int = 4
+    head_dim: int = 32
+    c_opm: int = 32
+    c_tri: int = 128
+    transition_n: int = 4
+
+
+AF2 = Dims()
+
+
+def _attn_spec(c, heads, with_pair_bias, c_bias_in):
+    hd = c  # heads * head_dim == c
+    spec = [("ln_g", (c,), "gamma"), ("ln_b", (c,), "beta")]
+    if with_pair_bias == "row":
+        spec += [("ln_z_g", (c_bias_in,), "gamma"), ("ln_z_b", (c_bias_in,), "beta")]
+    if with_pair_bias:
+        spec += [("w_bias", (c_bias_in, heads), "W")]
+    spec += [("wq", (c, hd), "W"), ("wk", (c, hd), "W"), ("wv", (c, hd), "W"),
+             ("wg", (c, hd), "W"), ("bg", (hd,), "bias"),
+             ("wo", (hd, c), "W"), ("bo", (c,), "bias")]
+    return spec
+
+
+def block_spec(d: Dims = AF2):
+    """Ordered list of (module, [(name, shape, kind)]) for one block — SURVEY.md Appendix B.
+
+    kind: "W" (N(0,1)/sqrt(fan_in), bf16-rounded on the bf16 path), "bias" (0.1 N(0,1)),
+    "gamma" (1 + 0.1 N(0,1)), "beta" (0.1 N(0,1))  — reading R8.
+    """
+    cm, cz, n = d.c_m, d.c_z, d.transition_n
+    tri_mul = [("ln_in_g", (cz,), "gamma"), ("ln_in_b", (cz,), "beta"),
+               ("w_ap", (cz, d.c_tri), "W"), ("b_ap", (d.c_tri,), "bias"),
+               ("w_ag", (cz, d.c_tri), "W"), ("b_ag", (d.c_tri,), "bias"),
+               ("w_bp", (cz, d.c_tri), "W"), ("b_bp", (d.c_tri,), "bias"),
+               ("w_bg", (cz, d.c_tri), "W"), ("b_bg", (d.c_tri,), "bias"),
+               ("w_g", (cz, cz), "W"), ("b_g", (cz,), "bias"),
+               ("ln_out_g", (d.c_tri,), "gamma"), ("ln_out_b", (d.c_tri,), "beta"),
+               ("w_z", (d.c_tri, cz), "W"), ("b_z", (cz,), "bias")]
+    return [
+        ("row", _attn_spec(cm, d.heads_msa, "row", cz)),
+        ("col", _attn_spec(cm, d.heads_msa, None, 0)),
+        ("msa_trans", [("ln_g", (cm,), "gamma"), ("ln_b", (cm,), "beta"),
+                       ("w1", (cm, n * cm), "W"), ("b1", (n * cm,), "bias"),
+                       ("w2", (n * cm, cm), "W"), ("b2", (cm,), "bias")]),
+        ("opm", [("ln_g", (cm,), "gamma"), ("ln_b", (cm,), "beta"),
+                 ("wa", (cm, d.c_opm), "W"), ("ba", (d.c_opm,), "bias"),
+                 ("wb", (cm, d.c_opm), "W"), ("bb", (d.c_opm,), "bias"),
+                 ("wout", (d.c_opm * d.c_opm, cz), "W"), ("bout", (cz,), "bias")]),
+        ("tri_mul_out", list(tri_mul)),
+        ("tri_mul_in", list(tri_mul)),
+        ("tri_att_start", _attn_spec(cz, d.heads_pair, "self", cz)),
+        ("tri_att_end", _attn_spec(cz, d.heads_pair, "self", cz)),
+        ("pair_trans", [("ln_g", (cz,), "gamma"), ("ln_b", (cz,), "beta"),
+                        ("w1", (cz, n * cz), "W"), ("b1", (n * cz,), "bias"),
+                        ("w2", (n * cz, cz), "W"), ("b2", (cz,), "bias")]),
+    ]
+
+
+def block_floats(d: Dims = AF2) -> int:
+    return sum(int(np.prod(shape)) for _, items in block_spec(d) for _, shape, _ in items)
+
+
+# ----------------------------------------------------------------------------------------------
+# random numbers: counter-based Philox, one stream per (seed, purpose)
+# ----------------------------------------------------------------------------------------------
+
+def rng(seed: int, stream: int = 0) -> np.random.Generator:
+    return np.random.Generator(np.random.Philox(key=[int(seed) & 0xFFFFFFFFFFFFFFFF, int(stream)]))
+
+
+def round_to_bf16(x: np.ndarray) -> np.ndarray:
+    """Round fp32 to the nearest bf16-representable value (ties to even); returns fp32.
+
+    Storage-format rounding of *parameters* (reading R15), not part of the method.
+    """
+    x = np.ascontiguousarray(x, dtype=np.float32)
+    u = x.view(np.uint32).astype(np.uint64)
+    lsb = (u >> 16) & 1
+    u = (u + 0x7FFF + lsb) & 0xFFFF0000
+    return u.astype(np.uint32).view(np.float32).reshape(x.shape)
+
+
+def make_block_weights(seed: int, block: int, d: Dims = AF2, bf16_weights: bool = False):
+    """dict[module][name] -> fp32 ndarray for one block (R8; R15 when bf16_weights)."""
+    g = rng(seed, 1000 + block)
+    out = {}
+    for module, items in block_spec(d):
+        mod = {}
+        for name, shape, kind in items:
+            r = g.standard_normal(shape, dtype=np.float32)
+            if kind == "W":
+                w = r / np.float32(np.sqrt(shape[0]))
+                mod[name] = round_to_bf16(w) if bf16_weights else w.astype(np.float32)
+            elif kind == "gamma":
+                mod[name] = (1.0 + 0.1 * r).astype(np.float32)
+            else:  # bias, beta
+                mod[name] = (0.1 * r).astype(np.float32)
+        out[module] = mod
+    return out
+
+
+def make_weights(seed: int, n_blocks: int, d: Dims = AF2, bf16_weights: bool = False):
+    return [make_block_weights(seed, b, d, bf16_weights) for b in range(n_blocks)]
+
+
+def pack_blob(blocks, d: Dims = AF2) -> np.ndarray:
+    """Flatten a list of per-block weight dicts into the fp32 blob of Appendix B (row-major [in,out])."""
+    parts = []
+    for w in blocks:
+        for module, items in block_spec(d):
+            for name, shape, _ in items:
+                a = np.asarray(w[module][name], dtype=np.float32)
+                assert a.shape == tuple(shape), (module, name, a.shape, shape)
+                parts.append(a.reshape(-1))
+    return np.ascontiguousarray(np.concatenate(parts))
+
+
+def unpack_blob(blob: np.ndarray, n_blocks: int, d: Dims = AF2):
+    blob = np.asarray(blob, dtype=np.float32).reshape(-1)
+    off, out = 0, []
+    for _ in range(n_blocks):
+        w = {}
+        for module, items in block_spec(d):
+            mod = {}
+            for name, shape, _ in items:
+                n = int(np.prod(shape))
+                mod[name] = blob[off:off + n].reshape(shape).copy()
+                off += n
+            w[module] = mod
+        out.append(w)
+    assert off == blob.size
+    return out
+
+
+# ----------------------------------------------------------------------------------------------
+# inputs
+# ----------------------------------------------------------------------------------------------
+
+def make_inputs(seed: int, B: int, S: int, N: int, d: Dims = AF2, lengths=None,
+                msa_mask_frac_max: float = 0.0):
+    """msa[B,S,N,c_m], pair[B,N,N,c_z] ~ N(0,1) everywhere, padding included (garbage, not zeros);
+    seq_mask[b,i] = 1[i < lengths[b]] (R2); msa_mask per R11: per protein f ~ U[0, frac_max],
+    floor(f*S) rows drawn without replacement from rows 1..S-1 are zeroed (row 0 always kept, R3).
+    """
+    g = rng(seed, 1)
+    msa = g.standard_normal((B, S, N, d.c_m), dtype=np.float32)
+    pair = g.standard_normal((B, N, N, d.c_z), dtype=np.float32)
+    seq_mask = np.ones((B, N), dtype=np.float32)
+    if lengths is not None:
+        for b, L in enumerate(lengths):
+            seq_mask[b, int(L):] = 0.0
+    msa_mask = np.ones((B, S), dtype=np.float32)
+    if msa_mask_frac_max > 0.0 and S > 1:
+        gm = rng(seed, 2)
+        for b in range(B):
+            f = gm.uniform(0.0, msa_mask_frac_max)
+            k = int(np.floor(f * S))
+            if k > 0:
+                rows = gm.choice(np.arange(1, S), size=min(k, S - 1), replace=False)
+                msa_mask[b, rows] = 0.0
+    return msa, pair, seq_mask, msa_mask
+
+
+def cfg2_lengths(seed: int, B: int = 64, lo: int = 50, hi: int = 128) -> np.ndarray:
+    """BASELINE.json configs[1]: lengths uniform in [lo, hi]."""
+    return rng(seed, 3).integers(lo, hi + 1, size=B)
+
+
+def cfg5_lengths(seed: int, n: int = 2000) -> np.ndarray:
+    """BASELINE.json configs[4] with reading R10: log-normal(mu=ln 140, sigma=0.45), rounded, clipped to [50,300]."""
+    x = rng(seed, 4).lognormal(mean=np.log(140.0), sigma=0.45, size=n)
+    return np.clip(np.rint(x), 50, 300).astype(np.int64)
+
+
+CFG5_BUCKETS = (64, 128, 192, 256, 320)
+
+
+def gemm_flops_per_block(S: int, N: int, d: Dims = AF2) -> float:
+    """Algorithmic GEMM FLOPs (2*MAC) of one block for one protein — SURVEY.md §8(d) formula F(S,N)."""
+    cm, cz, co = d.c_m, d.c_z, d.c_opm
+    return (36.0 * S * N * cm * cm + 4.0 * S * N * N * cm + 4.0 * N * S * S * cm
+            + 4.0 * S * N * cm * co + 2.0 * S * N * N * co * co + 2.0 * N * N * co * co * cz
+            + 60.0 * N * N * cz * cz + 12.0 * N ** 3 * cz
+            + 2.0 * N * N * cz * d.heads_msa + 4.0 * N * N * cz * d.heads_pair)
