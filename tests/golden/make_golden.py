@@ -40,5 +40,5 @@ if __name__ == "__main__":
         f.write("# oracle.evoformer_block on cfg1 (seed=1, S=16, N=32, AF2 dims, masks all 1); tensor i0 i1 c value(fp64)\n")
         f.write("# source: tests/golden/make_golden.py (oracle only); reading: SURVEY.md Appendix A, R0-R16\n")
         for t, a, b, c, v in samples():
-            f.write(f"{t} {a} {b} {c} {v!r}\n")
+            f.write(f"{t} {a} {b} {c} {float(v)!r}\n")
     print("wrote", path)
