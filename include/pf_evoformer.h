@@ -1,0 +1,128 @@
+/*
+ * pf_evoformer.h — C ABI of the B200-native Evoformer trunk (the GPU stage ParaFold separates out).
+ *
+ * What is computed: the forward pass of AlphaFold's Evoformer trunk (named at PAPER.md:27 and
+ * PAPER.md:61; AlphaFold v2.0.1 monomer), n_blocks blocks of the nine sub-steps of
+ * SURVEY.md Appendix A.1-A.9, over a batch of proteins padded to one length bucket (PAPER.md:113:
+ * proteins of similar length share one compiled model; here: one binary, runtime shapes).
+ * BASELINE.json:north_star defines the two entry points (create / forward) and the scheduler.
+ *
+ * Conventions
+ *   - Plain C, no torch types.  "dev" = CUDA device pointer on the current device, "host" = host pointer.
+ *   - All tensors row-major, channels last.  B = batch, S = N_seq, N = N_res (padded bucket length).
+ *   - Residual streams msa / pair are fp32 in HBM on both compute paths and are
+ *     updated IN PLACE.
+ *   - Masks are fp32 0/1: seq_mask[B,N], msa_mask[B,S] (R2).  Precondition: msa_mask[b,0]=1 and every
+ *     protein has at least one unmasked residue.  Outputs at masked positions are unspecified but finite (R3).
+ *   - Every call returns a pf_status; nothing throws or aborts across the ABI.  pf_last_error() gives a
+ *     thread-local message for the last non-OK status.
+ *   - A handle is not thread-safe; use one handle per stream.
+ */
+#ifndef PF_EVOFORMER_H_
+#define PF_EVOFORMER_H_
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct pf_evoformer pf_evoformer_t;   /* opaque; owns device weights and a grow-only workspace */
+
+typedef enum {
+  PF_OK = 0,
+  PF_ERR_INVALID_ARG = 1,
+  PF_ERR_SHAPE = 2,
+  PF_ERR_ALLOC = 3,
+  PF_ERR_CUDA = 4,
+  PF_ERR_ARCH = 5,            /* device is not compute capability 10.x */
+  PF_ERR_UNIMPLEMENTED = 6
+} pf_status;
+
+typedef enum {
+  PF_F32 = 0,        /* fp32 SIMT arithmetic everywhere (cfg1; tolerance max-abs 1e-4) */
+  PF_BF16 = 1,       /* bf16 operands, fp32 accumulation on tcgen05 tensor cores, fp32 residual streams */
+  PF_BF16_SIMT = 2   /* debug: same bf16 storage points, contractions on the SIMT kernels */
+} pf_dtype;
+
+typedef struct {
+  int c_m;            /* MSA channels (256) */
+  int c_z;            /* pair channels (128) */
+  int heads_msa;      /* 8  (heads_msa  * head_dim == c_m) */
+  int heads_pair;     /* 4  (heads_pair * head_dim == c_z) */
+  int head_dim;       /* must be 32 */
+  int c_opm;          /* outer-product-mean hidden (32) */
+  int c_tri;          /* triangle-multiplication hidden (128) */
+  int transition_n;   /* transition expansion factor (4) */
+  int n_blocks_max;   /* number of blocks whose weights the blob holds */
+  pf_dtype dtype;
+} pf_config;
+
+/* Number of fp32 values one block occupies in the weights blob (SURVEY.md Appendix B layout,
+ * every matrix row-major [in, out]); 1,829,952 for the AlphaFold dims. */
+size_t pf_evoformer_block_floats(const pf_config* cfg);
+
+/* Create a trunk.  weights_host: host fp32 blob of cfg->n_blocks_max blocks in Appendix-B order,
+ * n_weight_floats its length (checked).  The blob is copied / converted to the device; the caller may
+ * free it afterwards.  Errors: INVALID_ARG (null), SHAPE (bad dims, head_dim != 32, wrong blob length),
+ * ARCH (not CC 10.x), ALLOC, CUDA.  (= north_star pf_evoformer_create(weights, c_m, c_z, heads).) */
+pf_status pf_evoformer_create(pf_evoformer_t** out, const float* weights_host, size_t n_weight_floats,
+                              const pf_config* cfg);
+
+/* Run blocks [0, n_blocks) on dev msa[B,S,N,c_m] and dev pair[B,N,N,c_z] in place, asynchronously on
+ * cuda_stream (a cudaStream_t, NULL = default stream).  Does not synchronise; reports launch-time errors.
+ * Shapes are runtime arguments: a new (B,S,N) costs a workspace growth at most, never a rebuild.
+ * Sub-step order inside a block: 1 row attention with pair bias (A.1), 2 column attention
+ * (A.2), 3 MSA transition (A.3), 4 outer-product-mean (A.4, reads the updated msa), 5/6 triangle
+ * multiplication outgoing/incoming (A.5/A.6), 7/8 triangle attention starting/ending node (A.7/A.8),
+ * 9 pair transition (A.9). */
+pf_status pf_evoformer_forward(pf_evoformer_t* h, float* msa_dev, float* pair_dev,
+                               const float* seq_mask_dev, const float* msa_mask_dev,
+                               int B, int S, int N, int n_blocks, void* cuda_stream);
+
+/* Test hook: run only sub-step `substep` (1..9) of block `block`. */
+pf_status pf_evoformer_forward_substep(pf_evoformer_t* h, float* msa_dev, float* pair_dev,
+                                       const float* seq_mask_dev, const float* msa_mask_dev,
+                                       int B, int S, int N, int block, int substep, void* cuda_stream);
+
+/* End-to-end convenience: the same computation with HOST buffers (pinned or pageable).  Copies msa, pair
+ * and masks host->device on cuda_stream, runs forward, copies msa and pair back, and synchronises the
+ * stream before returning.  Device staging buffers are owned by the handle (grow-only). */
+pf_status pf_evoformer_forward_host(pf_evoformer_t* h, float* msa_host, float* pair_host,
+                                    const float* seq_mask_host, const float* msa_mask_host,
+                                    int B, int S, int N, int n_blocks, void* cuda_stream);
+
+/* Bytes of device workspace forward() needs for (B,S,N) (excluding msa/pair themselves and weights). */
+size_t pf_evoformer_workspace_bytes(const pf_evoformer_t* h, int B, int S, int N);
+
+/* Number of kernel launches the last forward()/forward_substep() call on this handle issued. */
+long long pf_evoformer_last_launch_count(const pf_evoformer_t* h);
+
+void pf_evoformer_destroy(pf_evoformer_t* h);
+
+const char* pf_last_error(void);
+
+/* ------------------------------------------------------------------------------------------------
+ * Length-bucketing batch scheduler ("sort by length ... share the compiled model";
+ * SURVEY.md §3(iv)).  Host only.  Proteins are sorted by descending length (largest first, as the paper
+ * compiles for the largest), assigned to the smallest bucket >= length, and cut into batches of at most
+ * max(1, floor(mem_budget_bytes / bytes_per_protein(bucket, S))) proteins of one bucket.
+ * ---------------------------------------------------------------------------------------------- */
+typedef struct pf_sched pf_sched_t;
+
+/* buckets: ascending padded lengths (host ints).  S: N_seq used for the footprint estimate.
+ * Errors: INVALID_ARG (null / not ascending / n_buckets < 1 / S < 1). */
+pf_status pf_sched_create(pf_sched_t** out, const int* buckets, int n_buckets, size_t mem_budget_bytes, int S);
+/* Errors: SHAPE if length < 1 or length > largest bucket. */
+pf_status pf_sched_add(pf_sched_t* s, int protein_id, int length);
+/* Writes up to cap protein ids and their lengths (lengths_out may be NULL) of the next batch and its bucket;
+ * returns the batch size B (0 when drained, -1 on invalid arguments).  The first call freezes the queue order. */
+int pf_sched_next_batch(pf_sched_t* s, int* ids_out, int* lengths_out, int cap, int* bucket_out);
+/* Footprint model used for batching: residual streams + workspace, bytes per protein. */
+size_t pf_sched_bytes_per_protein(int bucket, int S);
+void pf_sched_destroy(pf_sched_t* s);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PF_EVOFORMER_H_ */

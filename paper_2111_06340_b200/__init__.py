@@ -1,0 +1,205 @@
+"""Thin ctypes binding over the C ABI of include/pf_evoformer.h (argument marshalling only).
+
+Every step of the Evoformer trunk runs in the CUDA kernels of ``csrc/``; this module only loads
+``libpf_evoformer.so`` (built in-tree by ``python -m paper_2111_06340_b200.build``), converts arguments to
+pointers and sizes, and raises on non-OK status.  There is no CPU fallback: if the library is missing or a
+call fails, an exception is raised.  The fp64 oracle under ``oracle/`` is never imported from here.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from ctypes import POINTER, Structure, byref, c_char_p, c_float, c_int, c_longlong, c_size_t, c_void_p
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libpf_evoformer.so")
+
+PF_OK = 0
+PF_F32, PF_BF16, PF_BF16_SIMT = 0, 1, 2
+STATUS_NAMES = {0: "PF_OK", 1: "PF_ERR_INVALID_ARG", 2: "PF_ERR_SHAPE", 3: "PF_ERR_ALLOC", 4: "PF_ERR_CUDA",
+                5: "PF_ERR_ARCH", 6: "PF_ERR_UNIMPLEMENTED"}
+
+EXPORTED_SYMBOLS = (
+    "pf_evoformer_block_floats", "pf_evoformer_create", "pf_evoformer_forward", "pf_evoformer_forward_substep",
+    "pf_evoformer_forward_host", "pf_evoformer_workspace_bytes", "pf_evoformer_last_launch_count",
+    "pf_evoformer_destroy", "pf_last_error", "pf_sched_create", "pf_sched_add", "pf_sched_next_batch",
+    "pf_sched_bytes_per_protein", "pf_sched_destroy",
+)
+
+
+class PfConfig(Structure):
+    _fields_ = [("c_m", c_int), ("c_z", c_int), ("heads_msa", c_int), ("heads_pair", c_int), ("head_dim", c_int),
+                ("c_opm", c_int), ("c_tri", c_int), ("transition_n", c_int), ("n_blocks_max", c_int),
+                ("dtype", c_int)]
+
+
+class PfError(RuntimeError):
+    def __init__(self, status, msg):
+        super().__init__(f"{STATUS_NAMES.get(status, status)}: {msg}")
+        self.status = status
+
+
+_lib = None
+
+
+def lib() -> ctypes.CDLL:
+    """Load the shared library (once).  Raises if it has not been built — never falls back."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} not built; run `python -m paper_2111_06340_b200.build`")
+        L = ctypes.CDLL(LIB_PATH)
+        L.pf_evoformer_block_floats.restype = c_size_t
+        L.pf_evoformer_block_floats.argtypes = [POINTER(PfConfig)]
+        L.pf_evoformer_create.restype = c_int
+        L.pf_evoformer_create.argtypes = [POINTER(c_void_p), c_void_p, c_size_t, POINTER(PfConfig)]
+        fwd = [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_int, c_int, c_int]
+        L.pf_evoformer_forward.restype = c_int
+        L.pf_evoformer_forward.argtypes = fwd + [c_int, c_void_p]
+        L.pf_evoformer_forward_substep.restype = c_int
+        L.pf_evoformer_forward_substep.argtypes = fwd + [c_int, c_int, c_void_p]
+        L.pf_evoformer_forward_host.restype = c_int
+        L.pf_evoformer_forward_host.argtypes = fwd + [c_int, c_void_p]
+        L.pf_evoformer_workspace_bytes.restype = c_size_t
+        L.pf_evoformer_workspace_bytes.argtypes = [c_void_p, c_int, c_int, c_int]
+        L.pf_evoformer_last_launch_count.restype = c_longlong
+        L.pf_evoformer_last_launch_count.argtypes = [c_void_p]
+        L.pf_evoformer_destroy.restype = None
+        L.pf_evoformer_destroy.argtypes = [c_void_p]
+        L.pf_last_error.restype = c_char_p
+        L.pf_sched_create.restype = c_int
+        L.pf_sched_create.argtypes = [POINTER(c_void_p), POINTER(c_int), c_int, c_size_t, c_int]
+        L.pf_sched_add.restype = c_int
+        L.pf_sched_add.argtypes = [c_void_p, c_int, c_int]
+        L.pf_sched_next_batch.restype = c_int
+        L.pf_sched_next_batch.argtypes = [c_void_p, POINTER(c_int), POINTER(c_int), c_int, POINTER(c_int)]
+        L.pf_sched_bytes_per_protein.restype = c_size_t
+        L.pf_sched_bytes_per_protein.argtypes = [c_int, c_int]
+        L.pf_sched_destroy.restype = None
+        L.pf_sched_destroy.argtypes = [c_void_p]
+        _lib = L
+    return _lib
+
+
+def _check(status: int):
+    if status != PF_OK:
+        raise PfError(status, lib().pf_last_error().decode())
+
+
+def _ptr(t):
+    """Device/host pointer of a torch tensor, numpy array or raw int."""
+    if t is None:
+        return None
+    if isinstance(t, int):
+        return t
+    if isinstance(t, np.ndarray):
+        return t.ctypes.data
+    return t.data_ptr()
+
+
+def make_config(n_blocks_max: int, dtype: int = PF_BF16, c_m=256, c_z=128, heads_msa=8, heads_pair=4, head_dim=32,
+                c_opm=32, c_tri=128, transition_n=4) -> PfConfig:
+    return PfConfig(c_m, c_z, heads_msa, heads_pair, head_dim, c_opm, c_tri, transition_n, n_blocks_max, dtype)
+
+
+def pf_evoformer_block_floats(cfg: PfConfig) -> int:
+    return int(lib().pf_evoformer_block_floats(byref(cfg)))
+
+
+class Evoformer:
+    """Handle wrapper: pf_evoformer_create / forward / forward_substep / forward_host / destroy."""
+
+    def __init__(self, weights_blob: np.ndarray, cfg: PfConfig):
+        blob = np.ascontiguousarray(weights_blob, dtype=np.float32)
+        self._h = c_void_p()
+        self.cfg = cfg
+        _check(lib().pf_evoformer_create(byref(self._h), blob.ctypes.data, blob.size, byref(cfg)))
+
+    def _stream(self, stream):
+        if stream is None:
+            import torch
+            return torch.cuda.current_stream().cuda_stream
+        return stream
+
+    def forward(self, msa, pair, seq_mask, msa_mask, n_blocks: int, stream=None):
+        B, S, N = msa.shape[0], msa.shape[1], msa.shape[2]
+        _check(lib().pf_evoformer_forward(self._h, _ptr(msa), _ptr(pair), _ptr(seq_mask), _ptr(msa_mask),
+                                          B, S, N, n_blocks, self._stream(stream)))
+
+    def forward_substep(self, msa, pair, seq_mask, msa_mask, block: int, substep: int, stream=None):
+        B, S, N = msa.shape[0], msa.shape[1], msa.shape[2]
+        _check(lib().pf_evoformer_forward_substep(self._h, _ptr(msa), _ptr(pair), _ptr(seq_mask), _ptr(msa_mask),
+                                                  B, S, N, block, substep, self._stream(stream)))
+
+    def forward_host(self, msa, pair, seq_mask, msa_mask, n_blocks: int, stream=None):
+        B, S, N = msa.shape[0], msa.shape[1], msa.shape[2]
+        _check(lib().pf_evoformer_forward_host(self._h, _ptr(msa), _ptr(pair), _ptr(seq_mask), _ptr(msa_mask),
+                                               B, S, N, n_blocks, self._stream(stream)))
+
+    def workspace_bytes(self, B: int, S: int, N: int) -> int:
+        return int(lib().pf_evoformer_workspace_bytes(self._h, B, S, N))
+
+    def last_launch_count(self) -> int:
+        return int(lib().pf_evoformer_last_launch_count(self._h))
+
+    def close(self):
+        if self._h:
+            lib().pf_evoformer_destroy(self._h)
+            self._h = c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+class Scheduler:
+    """pf_sched_* wrapper: length-bucketing batch scheduler."""
+
+    def __init__(self, buckets, mem_budget_bytes: int, S: int):
+        arr = (c_int * len(buckets))(*buckets)
+        self._s = c_void_p()
+        st = lib().pf_sched_create(byref(self._s), arr, len(buckets), mem_budget_bytes, S)
+        if st != PF_OK:
+            raise PfError(st, "pf_sched_create")
+
+    def add(self, protein_id: int, length: int):
+        st = lib().pf_sched_add(self._s, protein_id, length)
+        if st != PF_OK:
+            raise PfError(st, f"pf_sched_add(id={protein_id}, length={length})")
+
+    def next_batch(self, cap: int = 4096):
+        ids = (c_int * cap)()
+        lens = (c_int * cap)()
+        bucket = c_int()
+        n = lib().pf_sched_next_batch(self._s, ids, lens, cap, byref(bucket))
+        if n < 0:
+            raise PfError(1, "pf_sched_next_batch")
+        if n == 0:
+            return None
+        return list(ids[:n]), list(lens[:n]), bucket.value
+
+    def batches(self, cap: int = 4096):
+        while True:
+            b = self.next_batch(cap)
+            if b is None:
+                return
+            yield b
+
+    def close(self):
+        if self._s:
+            lib().pf_sched_destroy(self._s)
+            self._s = c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def bytes_per_protein(bucket: int, S: int) -> int:
+    return int(lib().pf_sched_bytes_per_protein(bucket, S))

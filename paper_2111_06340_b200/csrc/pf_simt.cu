@@ -1,0 +1,331 @@
+// SIMT (CUDA-core, fp32 arithmetic) kernels of the Evoformer block, templated on the storage type of
+// intermediates (float for the PF_F32 path, bf16 for PF_BF16_SIMT and for the parts of PF_BF16 that are
+// not contractions).  Formulas: SURVEY.md Appendix A; readings R3-R7, R12.
+#include "pf_internal.h"
+#include "pf_device.cuh"
+
+namespace pf {
+
+// ---------------------------------------------------------------------------------------------
+// LayerNorm over channels of fp32 residual rows (R4), optional transposed row gather.
+// One warp per row, 128-bit loads, warp-shuffle reductions, two-pass variance.
+// ---------------------------------------------------------------------------------------------
+template <typename T, int NV>   // C = NV * 128
+__global__ void __launch_bounds__(256) ln_rows_kernel(const float* __restrict__ x, T* __restrict__ y,
+                                                      const float* __restrict__ gamma, const float* __restrict__ beta,
+                                                      long rows, RowGeom g, int transposed) {
+  const int C = NV * 128;
+  long r = (long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  if (r >= rows) return;
+  int lane = threadIdx.x & 31;
+  long src = transposed ? transposed_row(r, g) : r;
+  const float4* xp = reinterpret_cast<const float4*>(x + src * C);
+  float4 v[NV];
+  float s = 0.f;
+#pragma unroll
+  for (int i = 0; i < NV; ++i) {
+    v[i] = ld_nc_f4(xp + lane + 32 * i);
+    s += v[i].x + v[i].y + v[i].z + v[i].w;
+  }
+  float mean = warp_sum(s) * (1.0f / C);
+  float q = 0.f;
+#pragma unroll
+  for (int i = 0; i < NV; ++i) {
+    float a = v[i].x - mean, b = v[i].y - mean, c = v[i].z - mean, d = v[i].w - mean;
+    q += a * a + b * b + c * c + d * d;
+  }
+  float rstd = rsqrtf(warp_sum(q) * (1.0f / C) + 1e-5f);
+#pragma unroll
+  for (int i = 0; i < NV; ++i) {
+    int c4 = lane + 32 * i;
+    float4 gm = __ldg(reinterpret_cast<const float4*>(gamma) + c4);
+    float4 bt = __ldg(reinterpret_cast<const float4*>(beta) + c4);
+    float4 o;
+    o.x = (v[i].x - mean) * rstd * gm.x + bt.x;
+    o.y = (v[i].y - mean) * rstd * gm.y + bt.y;
+    o.z = (v[i].z - mean) * rstd * gm.z + bt.z;
+    o.w = (v[i].w - mean) * rstd * gm.w + bt.w;
+    store4(y + r * C + c4 * 4, o);
+  }
+}
+
+template <typename T>
+void launch_ln_rows(const float* x, T* y, const float* gamma, const float* beta, long rows, int C, RowGeom geom,
+                    int transposed, cudaStream_t st) {
+  int wpb = 8;
+  unsigned grid = (unsigned)((rows + wpb - 1) / wpb);
+  if (C == 128)
+    ln_rows_kernel<T, 1><<<grid, wpb * 32, 0, st>>>(x, y, gamma, beta, rows, geom, transposed);
+  else
+    ln_rows_kernel<T, 2><<<grid, wpb * 32, 0, st>>>(x, y, gamma, beta, rows, geom, transposed);
+}
+template void launch_ln_rows<float>(const float*, float*, const float*, const float*, long, int, RowGeom, int, cudaStream_t);
+template void launch_ln_rows<bf16>(const float*, bf16*, const float*, const float*, long, int, RowGeom, int, cudaStream_t);
+
+// ---------------------------------------------------------------------------------------------
+// Generic SIMT GEMM  acc[r,n] = sum_k A[r,k] W[k,n]  (+ second accumulator with W2 for gated pairs),
+// 64x64 tile, 16-deep k-slices, 4x4 micro-tile per thread, shared epilogue (pf_device.cuh).
+// ---------------------------------------------------------------------------------------------
+template <typename T, bool DUAL>
+__global__ void __launch_bounds__(256) gemm_simt_kernel(const T* __restrict__ A, int lda, const float* __restrict__ W,
+                                                        const float* __restrict__ W2, int ldw, long R, int K, int Nout,
+                                                        Epi epi) {
+  __shared__ float As[16][64 + 4];
+  __shared__ float Bs[16][64];
+  __shared__ float Bs2[DUAL ? 16 : 1][64];
+  int tx = threadIdx.x & 15, ty = threadIdx.x >> 4;
+  long r0 = (long)blockIdx.x * 64;
+  int n0 = blockIdx.y * 64;
+  float acc[4][4] = {}, acc2[4][4] = {};
+  for (int k0 = 0; k0 < K; k0 += 16) {
+    // A tile: 64 rows x 16 k  (thread -> row = tid/4, 4 consecutive k)
+    {
+      int row = threadIdx.x >> 2, kk = (threadIdx.x & 3) * 4;
+      long r = r0 + row;
+#pragma unroll
+      for (int j = 0; j < 4; ++j) As[kk + j][row] = (r < R) ? to_f32(A[r * lda + k0 + kk + j]) : 0.f;
+    }
+    // W tile: 16 k x 64 n  (thread -> k = tid/16, 4 consecutive n)
+    {
+      int kk = threadIdx.x >> 4, nn = (threadIdx.x & 15) * 4;
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        int n = n0 + nn + j;
+        Bs[kk][nn + j] = (n < Nout) ? __ldg(W + (long)(k0 + kk) * ldw + n) : 0.f;
+        if (DUAL) Bs2[kk][nn + j] = (n < Nout) ? __ldg(W2 + (long)(k0 + kk) * ldw + n) : 0.f;
+      }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int kk = 0; kk < 16; ++kk) {
+      float a[4], b[4], b2[4];
+#pragma unroll
+      for (int i = 0; i < 4; ++i) a[i] = As[kk][ty * 4 + i];
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        b[j] = Bs[kk][tx * 4 + j];
+        if (DUAL) b2[j] = Bs2[kk][tx * 4 + j];
+      }
+#pragma unroll
+      for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          acc[i][j] = fmaf(a[i], b[j], acc[i][j]);
+          if (DUAL) acc2[i][j] = fmaf(a[i], b2[j], acc2[i][j]);
+        }
+    }
+    __syncthreads();
+  }
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    long r = r0 + ty * 4 + i;
+    if (r >= R) continue;
+    RowInfo ri = row_info(r, epi);
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      int n = n0 + tx * 4 + j;
+      if (n < Nout) epilogue_elem<T>(epi, ri, r, n, Nout, acc[i][j], acc2[i][j]);
+    }
+  }
+}
+
+template <typename T>
+void launch_gemm_simt(const T* A, int lda, const float* W, const float* W2, int ldw, long R, int K, int Nout,
+                      const Epi& epi, cudaStream_t st) {
+  dim3 grid((unsigned)((R + 63) / 64), (unsigned)((Nout + 63) / 64));
+  if (W2)
+    gemm_simt_kernel<T, true><<<grid, 256, 0, st>>>(A, lda, W, W2, ldw, R, K, Nout, epi);
+  else
+    gemm_simt_kernel<T, false><<<grid, 256, 0, st>>>(A, lda, W, W2, ldw, R, K, Nout, epi);
+}
+template void launch_gemm_simt<float>(const float*, int, const float*, const float*, int, long, int, int, const Epi&, cudaStream_t);
+template void launch_gemm_simt<bf16>(const bf16*, int, const float*, const float*, int, long, int, int, const Epi&, cudaStream_t);
+
+// ---------------------------------------------------------------------------------------------
+// Gated attention core (A.1/A.2/A.7/A.8 after the row permutation): one warp per query row.
+//   qkg [(b,r,l), 3C] = [q/sqrt(d) | k | gate],  vt [((b,r),h,d), Lpad],  bias [(b,h,i), Lpad] or null,
+//   keymask [b, L] in {0,1};  o[(b,r,i), h*32+d] = gate * sum_j softmax_j(q.k/sqrt(d) + bias + NEG) v
+// ---------------------------------------------------------------------------------------------
+template <typename T>
+__global__ void __launch_bounds__(128) attn_simt_kernel(const T* __restrict__ qkg, const T* __restrict__ vt,
+                                                        const T* __restrict__ bias, const float* __restrict__ keymask,
+                                                        T* __restrict__ o, int B, int R, int L, int Lpad, int H) {
+  extern __shared__ float sc[];   // [4 warps][L]
+  int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  int i = blockIdx.x * 4 + warp;
+  int h = blockIdx.y;
+  int br = blockIdx.z;           // b*R + r
+  int b = br / R;
+  if (i >= L) return;
+  int C = H * 32;
+  float* s = sc + warp * L;
+  const T* qrow = qkg + ((long)br * L + i) * (3 * C) + h * 32;
+  float q = to_f32(qrow[lane]);
+  float mx = -INFINITY;
+  for (int j = 0; j < L; ++j) {
+    const T* krow = qkg + ((long)br * L + j) * (3 * C) + C + h * 32;
+    float d = warp_sum(q * to_f32(krow[lane]));   // q already carries 1/sqrt(d) (R12)
+    if (bias) d += to_f32(bias[(((long)b * H + h) * L + i) * Lpad + j]);
+    d += 1e9f * (keymask[(long)b * L + j] - 1.0f);
+    if (lane == 0) s[j] = d;
+    mx = fmaxf(mx, d);
+  }
+  __syncwarp();
+  float sum = 0.f;
+  for (int j = lane; j < L; j += 32) {
+    float e = expf(s[j] - mx);
+    s[j] = e;
+    sum += e;
+  }
+  sum = warp_sum(sum);
+  __syncwarp();
+  // lane = d
+  const T* vrow = vt + (((long)br * H + h) * 32 + lane) * Lpad;
+  float acc = 0.f;
+  for (int j = 0; j < L; ++j) acc = fmaf(s[j], to_f32(vrow[j]), acc);
+  float gate = to_f32(qrow[2 * C + lane]);
+  store1(o + ((long)br * L + i) * C + h * 32 + lane, gate * acc / sum);
+}
+
+template <typename T>
+void launch_attn_simt(const T* qkg, const T* vt, const T* bias, const float* keymask, T* o, int B, int R, int L,
+                      int Lpad, int H, cudaStream_t st) {
+  dim3 grid((L + 3) / 4, H, B * R);
+  attn_simt_kernel<T><<<grid, 128, 4 * L * sizeof(float), st>>>(qkg, vt, bias, keymask, o, B, R, L, Lpad, H);
+}
+template void launch_attn_simt<float>(const float*, const float*, const float*, const float*, float*, int, int, int, int, int, cudaStream_t);
+template void launch_attn_simt<bf16>(const bf16*, const bf16*, const bf16*, const float*, bf16*, int, int, int, int, int, cudaStream_t);
+
+// ---------------------------------------------------------------------------------------------
+// Triangle einsum (A.5 after the permutation): t[bc, i, j] = sum_k a[bc, i, k] b[bc, j, k]   (batched NT GEMM)
+// ---------------------------------------------------------------------------------------------
+template <typename T>
+__global__ void __launch_bounds__(256) tri_einsum_simt_kernel(const T* __restrict__ a, const T* __restrict__ b,
+                                                              float* __restrict__ t, int N, int Npad) {
+  __shared__ float As[16][33], Bs[16][33];
+  long base = (long)blockIdx.z * N * Npad;
+  int i0 = blockIdx.y * 32, j0 = blockIdx.x * 32;
+  int tx = threadIdx.x & 15, ty = threadIdx.x >> 4;   // 16 x 16 threads, 2x2 each
+  float acc[2][2] = {};
+  for (int k0 = 0; k0 < N; k0 += 16) {
+    for (int e = threadIdx.x; e < 512; e += 256) {
+      int row = e >> 4, kk = e & 15;
+      int k = k0 + kk;
+      As[kk][row] = (i0 + row < N && k < N) ? to_f32(a[base + (long)(i0 + row) * Npad + k]) : 0.f;
+      Bs[kk][row] = (j0 + row < N && k < N) ? to_f32(b[base + (long)(j0 + row) * Npad + k]) : 0.f;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int kk = 0; kk < 16; ++kk) {
+      float a0 = As[kk][ty * 2], a1 = As[kk][ty * 2 + 1], b0 = Bs[kk][tx * 2], b1 = Bs[kk][tx * 2 + 1];
+      acc[0][0] = fmaf(a0, b0, acc[0][0]);
+      acc[0][1] = fmaf(a0, b1, acc[0][1]);
+      acc[1][0] = fmaf(a1, b0, acc[1][0]);
+      acc[1][1] = fmaf(a1, b1, acc[1][1]);
+    }
+    __syncthreads();
+  }
+#pragma unroll
+  for (int ii = 0; ii < 2; ++ii)
+#pragma unroll
+    for (int jj = 0; jj < 2; ++jj) {
+      int i = i0 + ty * 2 + ii, j = j0 + tx * 2 + jj;
+      if (i < N && j < N) t[base + (long)i * Npad + j] = acc[ii][jj];
+    }
+}
+
+template <typename T>
+void launch_tri_einsum_simt(const T* a_cm, const T* b_cm, float* t_cm, int batch, int N, int Npad, cudaStream_t st) {
+  dim3 grid((N + 31) / 32, (N + 31) / 32, batch);
+  tri_einsum_simt_kernel<T><<<grid, 256, 0, st>>>(a_cm, b_cm, t_cm, N, Npad);
+}
+template void launch_tri_einsum_simt<float>(const float*, const float*, float*, int, int, int, cudaStream_t);
+template void launch_tri_einsum_simt<bf16>(const bf16*, const bf16*, float*, int, int, int, cudaStream_t);
+
+// ---------------------------------------------------------------------------------------------
+// LayerNorm across channels of the channel-major fp32 einsum output: t[(b,c), i, Npad] -> y[(b,i,j), C]
+// Block = 32 positions (consecutive j) x C channels via shared memory.
+// ---------------------------------------------------------------------------------------------
+template <typename T>
+__global__ void __launch_bounds__(256) lnc_kernel(const float* __restrict__ t, T* __restrict__ y,
+                                                  const float* __restrict__ gamma, const float* __restrict__ beta,
+                                                  int C, int N, int Npad) {
+  extern __shared__ float tile[];   // [C][33]
+  int j0 = blockIdx.x * 32, i = blockIdx.y, b = blockIdx.z;
+  int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  for (int c = warp; c < C; c += 8) {
+    int j = j0 + lane;
+    tile[c * 33 + lane] = (j < N) ? t[(((long)b * C + c) * N + i) * Npad + j] : 0.f;
+  }
+  __syncthreads();
+  // warp w handles positions w, w+8, ... ; lanes over channels
+  for (int p = warp; p < 32; p += 8) {
+    int j = j0 + p;
+    if (j >= N) continue;
+    float s = 0.f;
+    for (int c = lane; c < C; c += 32) s += tile[c * 33 + p];
+    float mean = warp_sum(s) / C;
+    float q = 0.f;
+    for (int c = lane; c < C; c += 32) {
+      float d = tile[c * 33 + p] - mean;
+      q += d * d;
+    }
+    float rstd = rsqrtf(warp_sum(q) / C + 1e-5f);
+    long row = ((long)b * N + i) * N + j;
+    for (int c = lane; c < C; c += 32)
+      store1(y + row * C + c, (tile[c * 33 + p] - mean) * rstd * __ldg(gamma + c) + __ldg(beta + c));
+  }
+}
+
+template <typename T>
+void launch_lnc(const float* t_cm, T* y, const float* gamma, const float* beta, int B, int C, int N, int Npad,
+                cudaStream_t st) {
+  dim3 grid((N + 31) / 32, N, B);
+  lnc_kernel<T><<<grid, 256, C * 33 * sizeof(float), st>>>(t_cm, y, gamma, beta, C, N, Npad);
+}
+template void launch_lnc<float>(const float*, float*, const float*, const float*, int, int, int, int, cudaStream_t);
+template void launch_lnc<bf16>(const float*, bf16*, const float*, const float*, int, int, int, int, cudaStream_t);
+
+// ---------------------------------------------------------------------------------------------
+// Outer-product-mean core (A.4): one block per (b, i, j).  a, b: [(b,s,i), c_opm] already masked by mu.
+//   z[b,i,j,:] += ( vec(sum_s a[s,i] (x) b[s,j]) / (1e-3 + n_ij) ) Wout + bout,   n_ij = sum_s mu_si mu_sj
+// ---------------------------------------------------------------------------------------------
+template <typename T>
+__global__ void __launch_bounds__(256) opm_simt_kernel(const T* __restrict__ a, const T* __restrict__ bb,
+                                                       const float* __restrict__ wout, const float* __restrict__ bout,
+                                                       const float* __restrict__ seq_mask,
+                                                       const float* __restrict__ msa_mask, float* __restrict__ z, int S,
+                                                       int N, int co, int cz) {
+  extern __shared__ float O[];   // [co*co]
+  int j = blockIdx.x, i = blockIdx.y, b = blockIdx.z;
+  for (int e = threadIdx.x; e < co * co; e += blockDim.x) {
+    int c1 = e / co, c2 = e % co;
+    float acc = 0.f;
+    for (int s = 0; s < S; ++s)
+      acc = fmaf(to_f32(a[(((long)b * S + s) * N + i) * co + c1]), to_f32(bb[(((long)b * S + s) * N + j) * co + c2]), acc);
+    O[e] = acc;
+  }
+  float n = 0.f;
+  for (int s = 0; s < S; ++s) n += msa_mask[(long)b * S + s];
+  n *= seq_mask[(long)b * N + i] * seq_mask[(long)b * N + j];
+  float inv = 1.0f / (1e-3f + n);
+  __syncthreads();
+  for (int e = threadIdx.x; e < cz; e += blockDim.x) {
+    float acc = 0.f;
+    for (int k = 0; k < co * co; ++k) acc = fmaf(O[k], __ldg(wout + (long)k * cz + e), acc);
+    long idx = (((long)b * N + i) * N + j) * cz + e;
+    z[idx] += acc * inv + __ldg(bout + e);
+  }
+}
+
+template <typename T>
+void launch_opm_simt(const T* a, const T* b, const float* wout, const float* bout, const float* seq_mask,
+                     const float* msa_mask, float* z, int B, int S, int N, int c_opm, int c_z, cudaStream_t st) {
+  dim3 grid(N, N, B);
+  opm_simt_kernel<T><<<grid, 256, c_opm * c_opm * sizeof(float), st>>>(a, b, wout, bout, seq_mask, msa_mask, z, S, N,
+                                                                       c_opm, c_z);
+}
+template void launch_opm_simt<float>(const float*, const float*, const float*, const float*, const float*, const float*, float*, int, int, int, int, int, cudaStream_t);
+template void launch_opm_simt<bf16>(const bf16*, const bf16*, const float*, const float*, const float*, const float*, float*, int, int, int, int, int, cudaStream_t);
+
+}  // namespace pf
