@@ -98,6 +98,18 @@ size_t pf_evoformer_workspace_bytes(const pf_evoformer_t* h, int B, int S, int N
 /* Number of kernel launches the last forward()/forward_substep() call on this handle issued. */
 long long pf_evoformer_last_launch_count(const pf_evoformer_t* h);
 
+/* Per-launch timing (measurement aid).  While enabled, every kernel launch of forward() is
+ * bracketed by two CUDA events on the launch stream and tagged with its kernel kind and its algorithmic FLOPs
+ * (2*MAC of the contraction) and algorithmic HBM bytes (operands read once + results written once).
+ * set_profiling(h, 1) clears earlier records and starts recording; set_profiling(h, 0) stops and clears.
+ * get_profile synchronises on the recorded events and returns, for one kind in [0, pf_evoformer_profile_kinds()),
+ * the totals since profiling was enabled: launches, device milliseconds, FLOPs, bytes. */
+pf_status pf_evoformer_set_profiling(pf_evoformer_t* h, int enable);
+int pf_evoformer_profile_kinds(void);
+const char* pf_evoformer_profile_name(int kind);
+pf_status pf_evoformer_get_profile(pf_evoformer_t* h, int kind, long long* launches, double* ms, double* flops,
+                                   double* bytes);
+
 void pf_evoformer_destroy(pf_evoformer_t* h);
 
 const char* pf_last_error(void);

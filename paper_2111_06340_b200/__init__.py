@@ -24,7 +24,8 @@ STATUS_NAMES = {0: "PF_OK", 1: "PF_ERR_INVALID_ARG", 2: "PF_ERR_SHAPE", 3: "PF_E
 EXPORTED_SYMBOLS = (
     "pf_evoformer_block_floats", "pf_evoformer_create", "pf_evoformer_forward", "pf_evoformer_forward_substep",
     "pf_evoformer_forward_host", "pf_evoformer_workspace_bytes", "pf_evoformer_last_launch_count",
-    "pf_evoformer_destroy", "pf_last_error", "pf_sched_create", "pf_sched_add", "pf_sched_next_batch",
+    "pf_evoformer_set_profiling", "pf_evoformer_profile_kinds", "pf_evoformer_profile_name",
+    "pf_evoformer_get_profile", "pf_evoformer_destroy", "pf_last_error", "pf_sched_create", "pf_sched_add", "pf_sched_next_batch",
     "pf_sched_bytes_per_protein", "pf_sched_destroy",
 )
 
@@ -66,6 +67,15 @@ def lib() -> ctypes.CDLL:
         L.pf_evoformer_workspace_bytes.argtypes = [c_void_p, c_int, c_int, c_int]
         L.pf_evoformer_last_launch_count.restype = c_longlong
         L.pf_evoformer_last_launch_count.argtypes = [c_void_p]
+        L.pf_evoformer_set_profiling.restype = c_int
+        L.pf_evoformer_set_profiling.argtypes = [c_void_p, c_int]
+        L.pf_evoformer_profile_kinds.restype = c_int
+        L.pf_evoformer_profile_kinds.argtypes = []
+        L.pf_evoformer_profile_name.restype = c_char_p
+        L.pf_evoformer_profile_name.argtypes = [c_int]
+        L.pf_evoformer_get_profile.restype = c_int
+        L.pf_evoformer_get_profile.argtypes = [c_void_p, c_int, POINTER(c_longlong), POINTER(ctypes.c_double),
+                                               POINTER(ctypes.c_double), POINTER(ctypes.c_double)]
         L.pf_evoformer_destroy.restype = None
         L.pf_evoformer_destroy.argtypes = [c_void_p]
         L.pf_last_error.restype = c_char_p
@@ -140,6 +150,19 @@ class Evoformer:
 
     def workspace_bytes(self, B: int, S: int, N: int) -> int:
         return int(lib().pf_evoformer_workspace_bytes(self._h, B, S, N))
+
+    def set_profiling(self, enable: bool):
+        _check(lib().pf_evoformer_set_profiling(self._h, 1 if enable else 0))
+
+    def get_profile(self) -> dict:
+        """{kind name: {"launches", "ms", "flops", "bytes"}} since set_profiling(True)."""
+        out = {}
+        for k in range(lib().pf_evoformer_profile_kinds()):
+            n, ms, fl, by = c_longlong(), ctypes.c_double(), ctypes.c_double(), ctypes.c_double()
+            _check(lib().pf_evoformer_get_profile(self._h, k, byref(n), byref(ms), byref(fl), byref(by)))
+            out[lib().pf_evoformer_profile_name(k).decode()] = {
+                "launches": n.value, "ms": ms.value, "flops": fl.value, "bytes": by.value}
+        return out
 
     def last_launch_count(self) -> int:
         return int(lib().pf_evoformer_last_launch_count(self._h))

@@ -138,7 +138,24 @@ struct pf_evoformer {
   unsigned tc_mask = 0;      // bit0 gemm, bit1 attention, bit2 triangle einsum, bit3 opm
   long long launches = 0;
   TmaCtx* tma = nullptr;
+  // per-launch CUDA-event profiling (pf_evoformer_set_profiling)
+  bool prof_on = false;
+  struct ProfRec { int kind; cudaEvent_t e0, e1; double flops, bytes; };
+  std::vector<ProfRec> prof;
+  std::vector<cudaEvent_t> ev_pool;
+  size_t ev_used = 0;
+  cudaEvent_t next_event() {
+    if (ev_used == ev_pool.size()) {
+      cudaEvent_t e;
+      cudaEventCreate(&e);
+      ev_pool.push_back(e);
+    }
+    return ev_pool[ev_used++];
+  }
 };
+
+enum KernelKind { KK_LN = 0, KK_GEMM, KK_ATTN, KK_TRI, KK_LNC, KK_OPM, KK_COUNT };
+static const char* const kKindNames[KK_COUNT] = {"ln_rows", "gemm", "attn_core", "tri_einsum", "ln_channels", "opm_core"};
 
 static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 static int pad8(int v) { return (v + 7) / 8 * 8; }
@@ -329,7 +346,38 @@ extern "C" void pf_evoformer_destroy(pf_evoformer_t* h) {
   cudaFree(h->ws);
   cudaFree(h->stage);
   if (h->tma) tma_ctx_destroy(h->tma);
+  for (cudaEvent_t e : h->ev_pool) cudaEventDestroy(e);
   delete h;
+}
+
+extern "C" pf_status pf_evoformer_set_profiling(pf_evoformer_t* h, int enable) {
+  if (!h) return fail(PF_ERR_INVALID_ARG, "null handle");
+  h->prof_on = enable != 0;
+  h->prof.clear();
+  h->ev_used = 0;
+  return PF_OK;
+}
+
+extern "C" int pf_evoformer_profile_kinds(void) { return KK_COUNT; }
+
+extern "C" const char* pf_evoformer_profile_name(int kind) {
+  return (kind >= 0 && kind < KK_COUNT) ? kKindNames[kind] : "";
+}
+
+extern "C" pf_status pf_evoformer_get_profile(pf_evoformer_t* h, int kind, long long* launches, double* ms,
+                                              double* flops, double* bytes) {
+  if (!h || !launches || !ms || !flops || !bytes) return fail(PF_ERR_INVALID_ARG, "null argument");
+  if (kind < 0 || kind >= KK_COUNT) return fail(PF_ERR_INVALID_ARG, "kind out of range");
+  *launches = 0; *ms = 0; *flops = 0; *bytes = 0;
+  for (const auto& r : h->prof) {
+    if (r.kind != kind) continue;
+    cudaError_t e = cudaEventSynchronize(r.e1);
+    float t = 0.f;
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&t, r.e0, r.e1);
+    if (e != cudaSuccess) return fail(PF_ERR_CUDA, std::string("profile events: ") + cudaGetErrorString(e));
+    *launches += 1; *ms += t; *flops += r.flops; *bytes += r.bytes;
+  }
+  return PF_OK;
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -355,6 +403,19 @@ struct Driver {
 
   bool tc(unsigned bit) const { return (h->tc_mask >> bit) & 1u; }
 
+  // one kernel launch: counts it and, when profiling, brackets it with events on the launch stream
+  void pb(int kind, double flops, double bytes) {
+    h->launches++;
+    if (!h->prof_on) return;
+    pf_evoformer::ProfRec r{kind, h->next_event(), h->next_event(), flops, bytes};
+    cudaEventRecord(r.e0, st);
+    h->prof.push_back(r);
+  }
+  void pe() {
+    if (h->prof_on) cudaEventRecord(h->prof.back().e1, st);
+  }
+  static constexpr double es() { return (double)sizeof(T); }
+
   static Epi epi_base(int kind, RowGeom g) {
     Epi e;
     memset(&e, 0, sizeof(e));
@@ -368,32 +429,45 @@ struct Driver {
   // acc = A[R,K] W[K,Nout]; W (and W2) fp32 [K, ldw] for SIMT; wt bf16 [Nout(*2), K] for tcgen05
   bool gemm(const T* A, int lda, const float* W, const float* W2, int ldw, const bf16* wt, long R, int K, int Nout,
             const Epi& e) {
-    h->launches++;
+    double nacc = (e.kind == EPI_GATED_CM) ? 2.0 : 1.0;
+    double out_b = (e.kind == EPI_RESID) ? 8.0 + (e.gate ? es() : 0.0) : es();
+    pb(KK_GEMM, 2.0 * R * K * Nout * nacc, (double)R * K * es() + (double)R * Nout * out_b + nacc * K * Nout * 2.0);
     if constexpr (std::is_same<T, bf16>::value) {
       if (tc(0) && wt) {
         if (launch_gemm_tc(h->tma, A, lda, wt, R, K, Nout, e, h->num_sms, st) != 0) {
           err = std::string("gemm_tc: ") + tc_last_error();
           return false;
         }
+        pe();
         return true;
       }
     }
     launch_gemm_simt<T>(A, lda, W, W2, ldw, R, K, Nout, e, st);
+    pe();
     return true;
   }
 
+  void ln_rows(const float* x, T* y, const float* gamma, const float* beta, long rows, int C, RowGeom g, int transposed) {
+    pb(KK_LN, 0.0, (double)rows * C * (4.0 + es()));
+    launch_ln_rows<T>(x, y, gamma, beta, rows, C, g, transposed, st);
+    pe();
+  }
+
   bool attention(const T* qkg, const T* vt, const T* bias, const float* keymask, T* o, int R, int L, int H) {
-    h->launches++;
+    double rows = (double)B * R * L, C = H * 32.0;
+    pb(KK_ATTN, 4.0 * rows * L * C, 5.0 * rows * C * es() + (bias ? (double)B * H * L * L * es() : 0.0));
     if constexpr (std::is_same<T, bf16>::value) {
       if (tc(1)) {
         if (launch_attn_tc(h->tma, qkg, vt, bias, keymask, o, B, R, L, pad8(L), H, h->num_sms, st) != 0) {
           err = std::string("attn_tc: ") + tc_last_error();
           return false;
         }
+        pe();
         return true;
       }
     }
     launch_attn_simt<T>(qkg, vt, bias, keymask, o, B, R, L, pad8(L), H, st);
+    pe();
     return true;
   }
 
@@ -411,16 +485,14 @@ struct Driver {
     if (bias_src_ln_g) {   // A.1: bias from LN'(z), own LayerNorm; z rows (b, i, j)
       long P = (long)B * N * N;
       RowGeom gz{B, N, N};
-      launch_ln_rows<T>(pair, X, bias_src_ln_g, bias_src_ln_b, P, h->cfg.c_z, gz, 0, st);
-      h->launches++;
+      ln_rows(pair, X, bias_src_ln_g, bias_src_ln_b, P, h->cfg.c_z, gz, 0);
       BIAS = buf<T>(ar.bias);
       Epi e = epi_base(EPI_HEADS, gz);
       e.out = BIAS;
       e.Lpad = pad8(N);
       if (!gemm(X, h->cfg.c_z, w + a.w_bias, nullptr, H, nullptr, P, h->cfg.c_z, H, e)) return false;
     }
-    launch_ln_rows<T>(res, X, w + a.ln_g, w + a.ln_b, R, C, g, transposed ? 1 : 0, st);
-    h->launches++;
+    ln_rows(res, X, w + a.ln_g, w + a.ln_b, R, C, g, transposed ? 1 : 0);
     if (self_bias) {       // A.7 / A.8: bias from the same LN(z) rows
       BIAS = buf<T>(ar.bias);
       Epi e = epi_base(EPI_HEADS, g);
@@ -466,8 +538,7 @@ struct Driver {
     RowGeom g{1, 1, (int)R};
     T* X = buf<T>(ar.x);
     T* Hb = buf<T>(ar.qkg);
-    launch_ln_rows<T>(res, X, w + t.ln_g, w + t.ln_b, R, C, g, 0, st);
-    h->launches++;
+    ln_rows(res, X, w + t.ln_g, w + t.ln_b, R, C, g, 0);
     Epi e1 = epi_base(EPI_STORE, g);
     e1.out = Hb; e1.ldo = n * C;
     e1.bias = w + t.b1;
@@ -487,8 +558,7 @@ struct Driver {
     T* X = buf<T>(ar.x);
     T* OA = buf<T>(ar.oa);
     T* OB = buf<T>(ar.ob);
-    launch_ln_rows<T>(msa, X, w + o.ln_g, w + o.ln_b, M, c.c_m, g, 0, st);
-    h->launches++;
+    ln_rows(msa, X, w + o.ln_g, w + o.ln_b, M, c.c_m, g, 0);
     for (int part = 0; part < 2; ++part) {
       Epi e = epi_base(EPI_STORE, g);
       e.out = part ? OB : OA; e.ldo = c.c_opm;
@@ -496,8 +566,12 @@ struct Driver {
       e.rowmask = RM_MSA; e.seq_mask = seq_mask; e.msa_mask = msa_mask;
       if (!gemm(X, c.c_m, w + (part ? o.wb : o.wa), nullptr, c.c_opm, nullptr, M, c.c_m, c.c_opm, e)) return false;
     }
-    launch_opm_simt<T>(OA, OB, w + o.wout, w + o.bout, seq_mask, msa_mask, pair, B, S, N, c.c_opm, c.c_z, st);
-    h->launches++;
+    {
+      double P = (double)B * N * N, cc = (double)c.c_opm * c.c_opm;
+      pb(KK_OPM, 2.0 * P * cc * S + 2.0 * P * cc * c.c_z, 2.0 * M * c.c_opm * es() + 8.0 * P * c.c_z);
+      launch_opm_simt<T>(OA, OB, w + o.wout, w + o.bout, seq_mask, msa_mask, pair, B, S, N, c.c_opm, c.c_z, st);
+      pe();
+    }
     return true;
   }
 
@@ -513,8 +587,7 @@ struct Driver {
     T* G = buf<T>(ar.g);
     float* TCM = buf<float>(ar.tcm);
     T* TN = buf<T>(ar.tn);
-    launch_ln_rows<T>(pair, X, w + t.ln_in_g, w + t.ln_in_b, P, c.c_z, g, incoming ? 1 : 0, st);
-    h->launches++;
+    ln_rows(pair, X, w + t.ln_in_g, w + t.ln_in_b, P, c.c_z, g, incoming ? 1 : 0);
     size_t wa16 = incoming ? h->tc.ti_wa : h->tc.to_wa, wb16 = incoming ? h->tc.ti_wb : h->tc.to_wb;
     size_t wg16 = incoming ? h->tc.ti_wg : h->tc.to_wg, wz16 = incoming ? h->tc.ti_wz : h->tc.to_wz;
     for (int part = 0; part < 2; ++part) {
@@ -538,7 +611,7 @@ struct Driver {
       e.act = ACT_SIGMOID; e.act_lo = 0; e.act_hi = c.c_z;
       if (!gemm(X, c.c_z, w + t.w_g, nullptr, c.c_z, w16 ? w16 + wg16 : nullptr, P, c.c_z, c.c_z, e)) return false;
     }
-    h->launches++;
+    pb(KK_TRI, 2.0 * B * c.c_tri * (double)N * N * N, (double)B * c.c_tri * N * Np * (2.0 * es() + 4.0));
     bool done = false;
     if constexpr (std::is_same<T, bf16>::value) {
       if (tc(2)) {
@@ -550,8 +623,10 @@ struct Driver {
       }
     }
     if (!done) launch_tri_einsum_simt<T>(ACM, BCM, TCM, B * c.c_tri, N, Np, st);
+    pe();
+    pb(KK_LNC, 0.0, (double)P * c.c_tri * (4.0 + es()));
     launch_lnc<T>(TCM, TN, w + t.ln_out_g, w + t.ln_out_b, B, c.c_tri, N, Np, st);
-    h->launches++;
+    pe();
     Epi e = epi_base(EPI_RESID, g);
     e.bias = w + t.b_z;
     e.resid = pair; e.ldr = c.c_z;
