@@ -3,6 +3,7 @@
 #include <cuda_runtime.h>
 #include <cuda_bf16.h>
 #include <stdint.h>
+#include <string>
 
 typedef __nv_bfloat16 bf16;
 
@@ -72,6 +73,7 @@ struct TmaCtx;   // holds the driver entry point for cuTensorMapEncodeTiled
 TmaCtx* tma_ctx_create();
 void tma_ctx_destroy(TmaCtx*);
 const char* tc_last_error();
+void tc_set_error(const std::string& s);
 int launch_gemm_tc(TmaCtx* ctx, const bf16* A, int lda, const bf16* Wt, long R, int K, int Nout, const Epi& epi,
                    int num_sms, cudaStream_t st);
 int launch_attn_tc(TmaCtx* ctx, const bf16* qkg, const bf16* vt, const bf16* bias, const float* keymask, bf16* o,

@@ -1,0 +1,91 @@
+"""bf16 CUDA path (tcgen05 tensor cores, fp32 accumulation, fp32 residual streams) vs the fp64 oracle, through the C ABI.
+
+Tolerances (BASELINE.json north_star): max-abs 3e-2 and mean-rel 1e-2 per block output, mean-rel in the
+ratio-of-means reading R14.  Weights are bf16-representable on both sides (R15).  Every sub-step is also gated on
+its own (R16): the oracle is applied to the same fp32 input the GPU sub-step received (teacher forcing, R1).
+"""
+import numpy as np
+import pytest
+
+import paper_2111_06340_b200 as pf
+import pf_synth as ps
+from gpu_util import errors, run_cuda, run_oracle, valid_masks
+
+pytestmark = pytest.mark.gpu
+
+TOL_ABS, TOL_REL = 3e-2, 1e-2
+
+
+@pytest.fixture(scope="module")
+def ragged():
+    """Several 128-row tiles with a ragged tail, masked residues and masked MSA rows, B > 1."""
+    B, S, N = 2, 20, 72
+    blocks = ps.make_weights(5, 1, bf16_weights=True)
+    msa, pair, sm, mm = ps.make_inputs(6, B, S, N, lengths=[72, 51], msa_mask_frac_max=0.3)
+    return blocks, msa, pair, sm, mm
+
+
+def _check(m, z, mr, zr, sm, mm, what):
+    vm, vz = valid_masks(sm, mm)
+    em, rm = errors(m, mr, vm)
+    ez, rz = errors(z, zr, vz)
+    print(f"{what}: m max-abs {em:.3e} mean-rel {rm:.3e}; z max-abs {ez:.3e} mean-rel {rz:.3e}")
+    assert em <= TOL_ABS and ez <= TOL_ABS, (what, em, ez)
+    assert rm <= TOL_REL and rz <= TOL_REL, (what, rm, rz)
+
+
+@pytest.mark.parametrize("substep", range(1, 10))
+def test_every_substep(ragged, substep):
+    blocks, msa, pair, sm, mm = ragged
+    m, z = run_cuda(pf.PF_BF16, blocks, msa, pair, sm, mm, block=0, substep=substep)
+    mr, zr = run_oracle(blocks, msa, pair, sm, mm, block=0, substep=substep)
+    _check(m, z, mr, zr, sm, mm, f"substep {substep}")
+    if substep <= 3:
+        assert np.array_equal(z, pair)
+    else:
+        assert np.array_equal(m, msa)
+
+
+def test_block(ragged):
+    blocks, msa, pair, sm, mm = ragged
+    m, z = run_cuda(pf.PF_BF16, blocks, msa, pair, sm, mm)
+    mr, zr = run_oracle(blocks, msa, pair, sm, mm)
+    _check(m, z, mr, zr, sm, mm, "block")
+
+
+@pytest.mark.parametrize("B,S,N", [(1, 1, 9), (3, 17, 50), (1, 3, 129), (2, 130, 33)])
+def test_runtime_shapes(B, S, N):
+    """One binary, many shapes (H11): sizes that are not multiples of any tile, S=1, keys spanning two key tiles."""
+    blocks = ps.make_weights(8, 1, bf16_weights=True)
+    lengths = ps.rng(B * 1000 + N, 7).integers(max(1, N // 2), N + 1, size=B)
+    msa, pair, sm, mm = ps.make_inputs(9, B, S, N, lengths=lengths, msa_mask_frac_max=0.4)
+    m, z = run_cuda(pf.PF_BF16, blocks, msa, pair, sm, mm)
+    mr, zr = run_oracle(blocks, msa, pair, sm, mm)
+    _check(m, z, mr, zr, sm, mm, f"B{B} S{S} N{N}")
+
+
+def test_simt_and_tensor_core_paths_agree(ragged):
+    """Same storage points, contractions on CUDA cores (PF_BF16_SIMT) vs tcgen05 (PF_BF16): both within tolerance
+    of the oracle and close to each other (they differ only in accumulation order and fast-math sigmoid)."""
+    blocks, msa, pair, sm, mm = ragged
+    m1, z1 = run_cuda(pf.PF_BF16, blocks, msa, pair, sm, mm)
+    m2, z2 = run_cuda(pf.PF_BF16_SIMT, blocks, msa, pair, sm, mm)
+    vm, vz = valid_masks(sm, mm)
+    assert np.abs(m1[vm] - m2[vm]).max() <= TOL_ABS and np.abs(z1[vz] - z2[vz]).max() <= TOL_ABS
+
+
+def test_cfg2_full_size_sampled_proteins():
+    """BASELINE.json configs[1] at full size in bench.py's launch configuration (B=64, N_seq=128, bucket 128, masks per
+    R11), one teacher-forced block; the oracle recomputes two whole proteins of the batch (the two shortest, to bound
+    CPU time) element by element, and every output of the batch must be finite."""
+    B, S, N = 64, 128, 128
+    blocks = ps.make_weights(7, 1, bf16_weights=True)
+    lengths = ps.cfg2_lengths(100, B)
+    msa, pair, sm, mm = ps.make_inputs(100, B, S, N, lengths=lengths, msa_mask_frac_max=0.3)
+    m, z = run_cuda(pf.PF_BF16, blocks, msa, pair, sm, mm)
+    assert np.isfinite(m).all() and np.isfinite(z).all()
+    pick = np.argsort(lengths)[:2]
+    for b in pick:
+        sl = slice(int(b), int(b) + 1)
+        mr, zr = run_oracle(blocks, msa[sl], pair[sl], sm[sl], mm[sl])
+        _check(m[sl], z[sl], mr, zr, sm[sl], mm[sl], f"cfg2 protein {int(b)} (len {int(lengths[b])})")
