@@ -331,7 +331,7 @@ extern "C" pf_status pf_evoformer_create(pf_evoformer_t** out, const float* weig
       pf_evoformer_destroy(h);
       return fail(PF_ERR_CUDA, std::string("TMA driver entry point: ") + tc_last_error());
     }
-    h->tc_mask = 0x1;   // bit0 projection GEMMs on tcgen05; attention / triangle einsum / OPM bits as kernels land
+    h->tc_mask = 0x3;   // bit0 projection GEMMs on tcgen05; attention / triangle einsum / OPM bits as kernels land
     if (const char* e = getenv("PF_TC_MASK")) h->tc_mask = (unsigned)strtoul(e, nullptr, 0);   // debug bisect only
   }
   *out = h;
