@@ -331,7 +331,7 @@ extern "C" pf_status pf_evoformer_create(pf_evoformer_t** out, const float* weig
       pf_evoformer_destroy(h);
       return fail(PF_ERR_CUDA, std::string("TMA driver entry point: ") + tc_last_error());
     }
-    h->tc_mask = 0x3;   // bit0 projection GEMMs on tcgen05; attention / triangle einsum / OPM bits as kernels land
+    h->tc_mask = 0xF;   // bit0 projection GEMMs on tcgen05; attention / triangle einsum / OPM bits as kernels land
     if (const char* e = getenv("PF_TC_MASK")) h->tc_mask = (unsigned)strtoul(e, nullptr, 0);   // debug bisect only
   }
   *out = h;
@@ -554,8 +554,30 @@ struct Driver {
     const pf_config& c = h->cfg;
     const OpmW& o = h->off.opm;
     long M = (long)B * S * N;
-    RowGeom g{B, S, N};
+    double P = (double)B * N * N, cc = (double)c.c_opm * c.c_opm;
     T* X = buf<T>(ar.x);
+    if constexpr (std::is_same<T, bf16>::value) {
+      if (tc(0) && tc(3) && S <= 512) {
+        // rows (b, i, s): the projection epilogue writes a|b transposed, [(b,i), 64, Spad], s contiguous
+        RowGeom gt{B, N, S};
+        int Sp = pad8(S);
+        T* ABT = buf<T>(ar.vt);
+        ln_rows(msa, X, w + o.ln_g, w + o.ln_b, M, c.c_m, gt, 1);
+        Epi e = epi_base(EPI_STORE, gt);
+        e.bias = wf + h->tc.opm_bias_ab;
+        e.rowmask = RM_MSA; e.seq_mask = seq_mask; e.msa_mask = msa_mask; e.mask_transposed = 1;
+        e.vt_from = 0; e.vt = ABT; e.Lpad = Sp;
+        if (!gemm(X, c.c_m, nullptr, nullptr, 0, w16 + h->tc.opm_wab, M, c.c_m, 2 * c.c_opm, e)) return false;
+        pb(KK_OPM, 2.0 * P * cc * S + 2.0 * P * cc * c.c_z, 2.0 * M * c.c_opm * es() + 8.0 * P * c.c_z);
+        if (launch_opm_tc(h->tma, ABT, w16 + h->tc.opm_wout, w + o.bout, seq_mask, msa_mask, pair, B, S, Sp, N, st) != 0) {
+          err = std::string("opm_tc: ") + tc_last_error();
+          return false;
+        }
+        pe();
+        return true;
+      }
+    }
+    RowGeom g{B, S, N};
     T* OA = buf<T>(ar.oa);
     T* OB = buf<T>(ar.ob);
     ln_rows(msa, X, w + o.ln_g, w + o.ln_b, M, c.c_m, g, 0);
@@ -566,12 +588,9 @@ struct Driver {
       e.rowmask = RM_MSA; e.seq_mask = seq_mask; e.msa_mask = msa_mask;
       if (!gemm(X, c.c_m, w + (part ? o.wb : o.wa), nullptr, c.c_opm, nullptr, M, c.c_m, c.c_opm, e)) return false;
     }
-    {
-      double P = (double)B * N * N, cc = (double)c.c_opm * c.c_opm;
-      pb(KK_OPM, 2.0 * P * cc * S + 2.0 * P * cc * c.c_z, 2.0 * M * c.c_opm * es() + 8.0 * P * c.c_z);
-      launch_opm_simt<T>(OA, OB, w + o.wout, w + o.bout, seq_mask, msa_mask, pair, B, S, N, c.c_opm, c.c_z, st);
-      pe();
-    }
+    pb(KK_OPM, 2.0 * P * cc * S + 2.0 * P * cc * c.c_z, 2.0 * M * c.c_opm * es() + 8.0 * P * c.c_z);
+    launch_opm_simt<T>(OA, OB, w + o.wout, w + o.bout, seq_mask, msa_mask, pair, B, S, N, c.c_opm, c.c_z, st);
+    pe();
     return true;
   }
 

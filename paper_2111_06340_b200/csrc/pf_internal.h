@@ -78,6 +78,9 @@ int launch_gemm_tc(TmaCtx* ctx, const bf16* A, int lda, const bf16* Wt, long R, 
                    int num_sms, cudaStream_t st);
 int launch_attn_tc(TmaCtx* ctx, const bf16* qkg, const bf16* vt, const bf16* bias, const float* keymask, bf16* o,
                    int B, int R, int L, int Lpad, int H, int num_sms, cudaStream_t st);
+// ab_t: [(b,i), 64 channels (a | b), Spad] bf16 masked projections; wout_t: [c_z, c_opm*c_opm] bf16
+int launch_opm_tc(TmaCtx* ctx, const bf16* ab_t, const bf16* wout_t, const float* bout, const float* seq_mask,
+                  const float* msa_mask, float* z, int B, int S, int Spad, int N, cudaStream_t st);
 int launch_tri_einsum_tc(TmaCtx* ctx, const bf16* a_cm, const bf16* b_cm, float* t_cm, int batch, int N, int Npad,
                          int num_sms, cudaStream_t st);
 

@@ -1,0 +1,251 @@
+// Outer-product-mean core on tcgen05 tensor cores (A.4, reading R5/R6):
+//     z[b,i,j,:] += ( vec_{c1,c2}( sum_s a[s,i,c1] b[s,j,c2] ) / (1e-3 + n_ij) ) W_out + b_out,   n_ij = sum_s mu_si mu_sj
+// a, b arrive masked and transposed from the projection epilogue as ab_t[(b,i), ch, Spad] (ch 0..31 = a, 32..63 = b;
+// s contiguous), so both operands of the first contraction are K-major tiles TMA can fetch directly.
+// One CTA = 128 residues i x 2 residues j of one protein.  For c1 = 0..31 (software-pipelined over two TMEM buffers):
+//   GEMM1  D1[i, (j,c2)] = sum_s a[s,i,c1] b[s,j,c2]        M=128, N=64,  K=S     (a streamed per c1, b resident)
+//   epilogue warps: D1 fp32 (TMEM) -> bf16 -> two K-major 128x32 tiles in shared memory (64B swizzle)
+//   GEMM2  acc_j[i, e] += sum_c2 D1[i,(j,c2)] W_out[c1*32+c2, e]   M=128, N=128, K=32  per j, accumulated over c1 in TMEM
+// so the 32x32 outer product per pair never reaches HBM (north_star bullet 3).  Final: acc_j / (1e-3 + n_ij) + b_out
+// added to the fp32 pair stream, 512 contiguous bytes per thread.
+#include "pf_internal.h"
+#include "pf_device.cuh"
+#include "pf_tc.cuh"
+
+namespace pf {
+
+int tma_encode_bf16(TmaCtx* ctx, CUtensorMap* out, const void* base, int rank, const uint64_t* dims,
+                    const uint64_t* strides_elems, const uint32_t* box, int swizzle_bytes);
+
+constexpr int OP_BI = 128, OP_BJ = 2, OP_C = 32, OP_CZ = 128, OP_BK = 64;
+constexpr int OP_MAX_KB = 8;       // S <= 512
+constexpr int OP_A_STAGES = 4;
+constexpr int OP_THREADS = 192;
+
+struct OpmSmem {
+  static constexpr int B_OFF = 0;                                        // OP_MAX_KB x (64 rows x 128 B) = 64 KB
+  static constexpr int B_KB_BYTES = OP_BJ * OP_C * 128;                  // 8 KB
+  static constexpr int A_OFF = B_OFF + OP_MAX_KB * B_KB_BYTES;
+  static constexpr int A_BYTES = OP_BI * 128;                            // 16 KB
+  static constexpr int W_OFF = A_OFF + OP_A_STAGES * A_BYTES;
+  static constexpr int W_BYTES = OP_CZ * 64;                             // 128 e x 32 c2 bf16 = 8 KB
+  static constexpr int OV_OFF = W_OFF + 2 * W_BYTES;
+  static constexpr int OV_TILE = OP_BI * 64;                             // 128 i x 32 c2 bf16 = 8 KB
+  static constexpr int BAR_OFF = OV_OFF + 2 * OP_BJ * OV_TILE;
+  static constexpr int TOTAL = BAR_OFF + 256 + 1024;
+};
+
+__global__ void __launch_bounds__(OP_THREADS, 1)
+opm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
+              const __grid_constant__ CUtensorMap tmW, const float* __restrict__ bout, const float* __restrict__ seq_mask,
+              const float* __restrict__ msa_mask, float* __restrict__ z, int S, int N) {
+  using SM = OpmSmem;
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + SM::BAR_OFF);
+  uint64_t* b_full = bars;
+  uint64_t* a_full = bars + 1;                    // [OP_A_STAGES]
+  uint64_t* a_empty = a_full + OP_A_STAGES;       // [OP_A_STAGES]
+  uint64_t* w_full = a_empty + OP_A_STAGES;       // [2]
+  uint64_t* w_empty = w_full + 2;                 // [2]
+  uint64_t* d1_full = w_empty + 2;                // [2]
+  uint64_t* d1_empty = d1_full + 2;               // [2]
+  uint64_t* ov_full = d1_empty + 2;               // [2]
+  uint64_t* ov_empty = ov_full + 2;               // [2]
+  uint64_t* acc_full = ov_empty + 2;
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(acc_full + 1);
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int j0 = blockIdx.x * OP_BJ, i0 = blockIdx.y * OP_BI, b = blockIdx.z;
+  const int n_kb = (S + OP_BK - 1) / OP_BK;
+
+  if (warp == 0 && lane == 0) {
+    tc::prefetch_tmap(&tmA);
+    tc::prefetch_tmap(&tmB);
+    tc::prefetch_tmap(&tmW);
+    tc::mbar_init(b_full, 1);
+    for (int s = 0; s < OP_A_STAGES; ++s) {
+      tc::mbar_init(&a_full[s], 1);
+      tc::mbar_init(&a_empty[s], 1);
+    }
+    for (int s = 0; s < 2; ++s) {
+      tc::mbar_init(&w_full[s], 1);
+      tc::mbar_init(&w_empty[s], 1);
+      tc::mbar_init(&d1_full[s], 1);
+      tc::mbar_init(&d1_empty[s], 128);
+      tc::mbar_init(&ov_full[s], 128);
+      tc::mbar_init(&ov_empty[s], 1);
+    }
+    tc::mbar_init(acc_full, 1);
+    tc::fence_barrier_init();
+  }
+  if (warp == 1) tc::tmem_alloc<512>(tmem_slot);
+  tc::tc_fence_before();
+  __syncthreads();
+  tc::tc_fence_after();
+  const uint32_t tmem_base = *tmem_slot;
+  const uint32_t tmem_acc = tmem_base;            // 2 x 128 columns
+  const uint32_t tmem_d1 = tmem_base + 256;       // 2 x 64 columns
+
+  if (warp == 0) {
+    if (tc::elect_one()) {
+      tc::mbar_arrive_expect_tx(b_full, (uint32_t)n_kb * SM::B_KB_BYTES);
+      for (int kb = 0; kb < n_kb; ++kb)
+        tc::tma_load_3d(smem + SM::B_OFF + kb * SM::B_KB_BYTES, &tmB, b_full, kb * OP_BK, OP_C, b * N + j0);
+      int it = 0;
+      for (int c1 = 0; c1 < OP_C; ++c1) {
+        for (int kb = 0; kb < n_kb; ++kb, ++it) {
+          int s = it % OP_A_STAGES;
+          tc::mbar_wait(&a_empty[s], ((it / OP_A_STAGES) & 1) ^ 1);
+          tc::mbar_arrive_expect_tx(&a_full[s], SM::A_BYTES);
+          tc::tma_load_3d(smem + SM::A_OFF + s * SM::A_BYTES, &tmA, &a_full[s], kb * OP_BK, c1, b * N + i0);
+        }
+        int ws = c1 & 1;
+        tc::mbar_wait(&w_empty[ws], ((c1 >> 1) & 1) ^ 1);
+        tc::mbar_arrive_expect_tx(&w_full[ws], SM::W_BYTES);
+        tc::tma_load_2d(smem + SM::W_OFF + ws * SM::W_BYTES, &tmW, &w_full[ws], c1 * OP_C, 0);
+      }
+    }
+  } else if (warp == 1) {
+    if (tc::elect_one()) {
+      constexpr uint32_t idesc1 = tc::idesc_bf16_f32(OP_BI, OP_BJ * OP_C);
+      constexpr uint32_t idesc2 = tc::idesc_bf16_f32(OP_BI, OP_CZ);
+      tc::mbar_wait(b_full, 0);
+      int it = 0;
+      for (int c1 = 0; c1 <= OP_C; ++c1) {
+        if (c1 < OP_C) {
+          int buf = c1 & 1;
+          tc::mbar_wait(&d1_empty[buf], ((c1 >> 1) & 1) ^ 1);
+          tc::tc_fence_after();
+          for (int kb = 0; kb < n_kb; ++kb, ++it) {
+            int s = it % OP_A_STAGES;
+            tc::mbar_wait(&a_full[s], (it / OP_A_STAGES) & 1);
+            tc::tc_fence_after();
+            uint64_t a_desc = tc::smem_desc_kmajor<128>(tc::smem_u32(smem + SM::A_OFF + s * SM::A_BYTES));
+            uint64_t b_desc = tc::smem_desc_kmajor<128>(tc::smem_u32(smem + SM::B_OFF + kb * SM::B_KB_BYTES));
+#pragma unroll
+            for (int k = 0; k < OP_BK / 16; ++k)
+              tc::mma_bf16(tmem_d1 + buf * 64, a_desc + 2 * k, b_desc + 2 * k, idesc1, (kb | k) != 0);
+            tc::mma_commit(&a_empty[s]);
+          }
+          tc::mma_commit(&d1_full[buf]);
+        }
+        if (c1 >= 1) {
+          int p = c1 - 1, pb = p & 1;
+          tc::mbar_wait(&ov_full[pb], (p >> 1) & 1);
+          tc::mbar_wait(&w_full[pb], (p >> 1) & 1);
+          tc::tc_fence_after();
+          uint64_t w_desc = tc::smem_desc_kmajor<64>(tc::smem_u32(smem + SM::W_OFF + pb * SM::W_BYTES));
+#pragma unroll
+          for (int j = 0; j < OP_BJ; ++j) {
+            uint64_t o_desc = tc::smem_desc_kmajor<64>(tc::smem_u32(smem + SM::OV_OFF + (pb * OP_BJ + j) * SM::OV_TILE));
+            tc::mma_bf16(tmem_acc + j * OP_CZ, o_desc, w_desc, idesc2, p != 0);
+            tc::mma_bf16(tmem_acc + j * OP_CZ, o_desc + 2, w_desc + 2, idesc2, true);
+          }
+          tc::mma_commit(&ov_empty[pb]);
+          tc::mma_commit(&w_empty[pb]);
+        }
+      }
+      tc::mma_commit(acc_full);
+    }
+  } else {
+    const int quarter = warp & 3;
+    const int row = quarter * 32 + lane;
+    const int i = i0 + row;
+    const uint32_t lane_addr = (uint32_t)(quarter * 32) << 16;
+    for (int c1 = 0; c1 < OP_C; ++c1) {
+      int buf = c1 & 1;
+      tc::mbar_wait(&d1_full[buf], (c1 >> 1) & 1);
+      tc::tc_fence_after();
+      uint32_t v[2][32];
+      tc::tmem_ld32(tmem_d1 + buf * 64 + lane_addr, v[0]);
+      tc::tmem_ld32(tmem_d1 + buf * 64 + lane_addr + 32, v[1]);
+      tc::tmem_ld_wait();
+      tc::tc_fence_before();
+      tc::mbar_arrive(&d1_empty[buf]);
+      tc::mbar_wait(&ov_empty[buf], ((c1 >> 1) & 1) ^ 1);
+#pragma unroll
+      for (int j = 0; j < OP_BJ; ++j) {
+        uint8_t* tile = smem + SM::OV_OFF + (buf * OP_BJ + j) * SM::OV_TILE;
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+          uint32_t pk[4];
+#pragma unroll
+          for (int e = 0; e < 4; ++e) {
+            __nv_bfloat162 pp = __floats2bfloat162_rn(__uint_as_float(v[j][c * 8 + 2 * e]),
+                                                      __uint_as_float(v[j][c * 8 + 2 * e + 1]));
+            pk[e] = *reinterpret_cast<uint32_t*>(&pp);
+          }
+          *reinterpret_cast<uint4*>(tile + tc::swz_offset<64>(row, c)) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
+        }
+      }
+      tc::fence_proxy_async_smem();
+      tc::mbar_arrive(&ov_full[buf]);
+    }
+    // n_ij = (sum_s rho_s) sigma_i sigma_j   (R5)
+    float cnt = 0.f;
+    for (int s = lane; s < S; s += 32) cnt += msa_mask[(long)b * S + s];
+    cnt = warp_sum(cnt);
+    tc::mbar_wait(acc_full, 0);
+    tc::tc_fence_after();
+    const float si = (i < N) ? seq_mask[(long)b * N + i] : 0.f;
+#pragma unroll 1
+    for (int j = 0; j < OP_BJ; ++j) {
+      const int jj = j0 + j;
+      const bool ok = (i < N) && (jj < N);
+      const float inv = ok ? 1.0f / (1e-3f + cnt * si * seq_mask[(long)b * N + jj]) : 0.f;
+      float* dst = z + (((long)b * N + i) * N + jj) * OP_CZ;
+#pragma unroll 1
+      for (int c0 = 0; c0 < OP_CZ; c0 += 32) {
+        uint32_t v[32];
+        tc::tmem_ld32(tmem_acc + j * OP_CZ + lane_addr + c0, v);
+        tc::tmem_ld_wait();
+        if (ok) {
+#pragma unroll
+          for (int e = 0; e < 32; e += 4) {
+            float4 o = *reinterpret_cast<float4*>(dst + c0 + e);
+            float4 bo = __ldg(reinterpret_cast<const float4*>(bout + c0 + e));
+            o.x += __uint_as_float(v[e]) * inv + bo.x;
+            o.y += __uint_as_float(v[e + 1]) * inv + bo.y;
+            o.z += __uint_as_float(v[e + 2]) * inv + bo.z;
+            o.w += __uint_as_float(v[e + 3]) * inv + bo.w;
+            *reinterpret_cast<float4*>(dst + c0 + e) = o;
+          }
+        }
+      }
+    }
+  }
+  tc::tc_fence_before();
+  __syncthreads();
+  if (warp == 1) tc::tmem_dealloc<512>(tmem_base);
+}
+
+int launch_opm_tc(TmaCtx* ctx, const bf16* ab_t, const bf16* wout_t, const float* bout, const float* seq_mask,
+                  const float* msa_mask, float* z, int B, int S, int Spad, int N, cudaStream_t st) {
+  if (S > OP_MAX_KB * OP_BK) {
+    tc_set_error("opm_tc: N_seq above 512 not supported");
+    return -1;
+  }
+  CUtensorMap tmA, tmB, tmW;
+  uint64_t d[3] = {(uint64_t)S, 2 * OP_C, (uint64_t)B * N}, s[2] = {(uint64_t)Spad, (uint64_t)2 * OP_C * Spad};
+  uint32_t bxA[3] = {OP_BK, 1, OP_BI}, bxB[3] = {OP_BK, OP_C, OP_BJ};
+  if (tma_encode_bf16(ctx, &tmA, ab_t, 3, d, s, bxA, 128) != 0) return -1;
+  if (tma_encode_bf16(ctx, &tmB, ab_t, 3, d, s, bxB, 128) != 0) return -1;
+  uint64_t dw[2] = {(uint64_t)OP_C * OP_C, OP_CZ}, sw[1] = {(uint64_t)OP_C * OP_C};
+  uint32_t bxW[2] = {OP_C, OP_CZ};
+  if (tma_encode_bf16(ctx, &tmW, wout_t, 2, dw, sw, bxW, 64) != 0) return -1;
+  static bool configured = false;
+  if (!configured) {
+    cudaError_t e = cudaFuncSetAttribute(opm_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, OpmSmem::TOTAL);
+    if (e != cudaSuccess) {
+      tc_set_error(std::string("cudaFuncSetAttribute(opm_tc): ") + cudaGetErrorString(e));
+      return -1;
+    }
+    configured = true;
+  }
+  dim3 grid((N + OP_BJ - 1) / OP_BJ, (N + OP_BI - 1) / OP_BI, B);
+  opm_tc_kernel<<<grid, OP_THREADS, OpmSmem::TOTAL, st>>>(tmA, tmB, tmW, bout, seq_mask, msa_mask, z, S, N);
+  return 0;
+}
+
+}  // namespace pf
