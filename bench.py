@@ -219,7 +219,7 @@ def cpu_baseline(wl, wl_name, budget_s=25.0):
 # the CUDA path
 # ------------------------------------------------------------------------------------------------
 KIND_BOUND = {"gemm": "tensor", "attn_core": "tensor", "tri_einsum": "tensor", "opm_core": "tensor",
-              "ln_rows": "hbm", "ln_channels": "hbm"}
+              "ln_rows": "hbm", "ln_channels": "hbm", "ln_gemm": "hbm"}
 
 
 def roofline_from_profile(prof, peaks, n_steps):
@@ -273,7 +273,7 @@ def run_ours(args, wl, wl_name):
         dist.init_process_group("nccl", device_id=dev)
     pf.lib()                                                     # fail loudly if the extension is not built
 
-    dtype = pf.PF_F32 if args.dtype == "f32" else (pf.PF_BF16_SIMT if args.dtype == "bf16_simt" else pf.PF_BF16)
+    dtype = pf.PF_F32 if args.dtype == "f32" else pf.PF_BF16
     B, S, N, nb = wl["B"], wl["S"], wl["N"], wl["n_blocks"]
     # the weights of nb distinct blocks (R8/R15); for 48-block workloads the same seeded recipe
     blocks = ps.make_weights(7, nb, bf16_weights=(dtype != pf.PF_F32))
@@ -355,7 +355,7 @@ def run_ours(args, wl, wl_name):
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": {"f32": "f32", "bf16": "bf16", "bf16_simt": "bf16"}[args.dtype], "data": "synthetic",
+        "dtype": args.dtype, "data": "synthetic",
         "config": {"workload": wl_name, "desc": wl["desc"], "B": B, "N_seq": S, "N_res": N, "n_blocks": nb,
                    "parallelism": f"replicas x{world}", "l2": "inputs larger than L2 (msa+pair residual streams "
                    f"{(m0.numel() + z0.numel()) * 4 / 1e6:.0f} MB per step)", "path": args.dtype},
@@ -386,7 +386,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg2", choices=sorted(WORKLOADS))
-    ap.add_argument("--dtype", default="bf16", choices=["bf16", "f32", "bf16_simt"])
+    ap.add_argument("--dtype", default="bf16", choices=["bf16", "f32"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup

@@ -41,8 +41,8 @@ typedef enum {
 
 typedef enum {
   PF_F32 = 0,        /* fp32 SIMT arithmetic everywhere (cfg1; tolerance max-abs 1e-4) */
-  PF_BF16 = 1,       /* bf16 operands, fp32 accumulation on tcgen05 tensor cores, fp32 residual streams */
-  PF_BF16_SIMT = 2   /* debug: same bf16 storage points, contractions on the SIMT kernels */
+  PF_BF16 = 1        /* 16-bit operands (bf16; fp16 for LayerNorm outputs, their weights and gates), fp32 accumulation on
+                        tcgen05 tensor cores, fp32 residual streams */
 } pf_dtype;
 
 typedef struct {

@@ -17,7 +17,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libpf_evoformer.so")
 
 PF_OK = 0
-PF_F32, PF_BF16, PF_BF16_SIMT = 0, 1, 2
+PF_F32, PF_BF16 = 0, 1
 STATUS_NAMES = {0: "PF_OK", 1: "PF_ERR_INVALID_ARG", 2: "PF_ERR_SHAPE", 3: "PF_ERR_ALLOC", 4: "PF_ERR_CUDA",
                 5: "PF_ERR_ARCH", 6: "PF_ERR_UNIMPLEMENTED"}
 

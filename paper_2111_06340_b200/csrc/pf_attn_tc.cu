@@ -233,8 +233,8 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQK, const __grid_constant__
       bf16* op = o + ((long)br * L + i) * C + h * 32;
 #pragma unroll
       for (int d = 0; d < 32; d += 8) {
-        uint4 gu = *reinterpret_cast<const uint4*>(gp + d);
-        const __nv_bfloat162* g2 = reinterpret_cast<const __nv_bfloat162*>(&gu);
+        uint4 gu = *reinterpret_cast<const uint4*>(gp + d);   // the gate is stored as fp16 (bounded in [0,1], not an MMA operand)
+        const __half2* g2 = reinterpret_cast<const __half2*>(&gu);
         uint32_t pk[4];
 #pragma unroll
         for (int e = 0; e < 4; ++e) {

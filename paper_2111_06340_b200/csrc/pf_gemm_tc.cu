@@ -67,6 +67,34 @@ int tma_encode_bf16(TmaCtx* ctx, CUtensorMap* out, const void* base, int rank, c
   return 0;
 }
 
+// General form: elem_kind 0 = bf16, 1 = fp16, 2 = fp32; rank <= 4; strides in BYTES for dims 1.. (multiples of 16).
+int tma_encode(TmaCtx* ctx, CUtensorMap* out, const void* base, int elem_kind, int rank, const uint64_t* dims,
+               const uint64_t* strides_bytes, const uint32_t* box, int swizzle_bytes) {
+  cuuint64_t gd[4];
+  cuuint64_t gs[3];
+  cuuint32_t bx[4], es[4];
+  for (int i = 0; i < rank; ++i) {
+    gd[i] = dims[i];
+    bx[i] = box[i];
+    es[i] = 1;
+  }
+  for (int i = 0; i + 1 < rank; ++i) gs[i] = strides_bytes[i];
+  CUtensorMapDataType dt = elem_kind == 2 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32
+                           : elem_kind == 1 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT16
+                                            : CU_TENSOR_MAP_DATA_TYPE_BFLOAT16;
+  CUtensorMapSwizzle sw = swizzle_bytes == 128 ? CU_TENSOR_MAP_SWIZZLE_128B
+                          : swizzle_bytes == 64 ? CU_TENSOR_MAP_SWIZZLE_64B
+                                                : CU_TENSOR_MAP_SWIZZLE_NONE;
+  CUresult r = ctx->encode(out, dt, (cuuint32_t)rank, const_cast<void*>(base), gd, gs, bx, es,
+                           CU_TENSOR_MAP_INTERLEAVE_NONE, sw, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) {
+    g_tc_err = "cuTensorMapEncodeTiled (rank " + std::to_string(rank) + ") failed with CUresult " + std::to_string((int)r);
+    return -1;
+  }
+  return 0;
+}
+
 // ------------------------------------------------------------------------------------------------
 // epilogue: 32 consecutive output columns [n0, n0+32) of one row, values in registers
 // ------------------------------------------------------------------------------------------------

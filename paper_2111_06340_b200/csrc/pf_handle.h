@@ -1,0 +1,113 @@
+// The handle behind pf_evoformer_t, the weight-blob offsets and the device weight layout of the
+// tensor-core path.  Shared by pf_api.cu (C ABI, fp32 SIMT driver) and pf_trunk_tc.cu (tcgen05 driver).
+#pragma once
+#include "../../include/pf_evoformer.h"
+#include "pf_internal.h"
+
+#include <string>
+#include <vector>
+
+namespace pf {
+
+// ---- offsets (floats, within one block) into the fp32 blob, Appendix B order ----
+struct AttnW {
+  size_t ln_g, ln_b, ln_z_g, ln_z_b, w_bias, wq, wk, wv, wg, bg, wo, bo;
+};
+struct TransW {
+  size_t ln_g, ln_b, w1, b1, w2, b2;
+};
+struct OpmW {
+  size_t ln_g, ln_b, wa, ba, wb, bb, wout, bout;
+};
+struct TriMulW {
+  size_t ln_in_g, ln_in_b, w_ap, b_ap, w_ag, b_ag, w_bp, b_bp, w_bg, b_bg, w_g, b_g, ln_out_g, ln_out_b, w_z, b_z;
+};
+struct BlockW {
+  AttnW row, col, tri_start, tri_end;
+  TransW msa_trans, pair_trans;
+  OpmW opm;
+  TriMulW tri_out, tri_in;
+  size_t total;
+};
+BlockW block_offsets(const pf_config& c);
+
+// ---- tensor-core weight set: 16-bit matrices [Nout, K] (K contiguous), offsets in 16-bit elements within one block.
+// Matrices that multiply a LayerNorm output are stored as fp16 (reading R17: the values are the bf16-rounded
+// weights of R15, which fp16 represents exactly), all others as bf16.  Fused bias vectors are fp32 (offsets in floats).
+struct AttnT {
+  size_t w_in;   // fp16 [4C (+H), C]: q | k | gate | v (| pair-bias heads for triangle attention)
+  size_t b_in;   // fp32 [4C (+H)]: gate bias in its column range, zero elsewhere
+  size_t wo;     // bf16 [C, C]
+};
+struct TcBlock {
+  AttnT row, col, tri_start, tri_end;
+  size_t row_wbias;                      // fp16 [H_m, c_z]  (LN'(z) -> pair bias of row attention)
+  size_t mt_w1, mt_w2, pt_w1, pt_w2;     // transitions: W1 fp16 [4C, C], W2 bf16 [C, 4C]
+  size_t opm_wab, opm_bias_ab, opm_wout; // fp16 [2 c_opm, c_m], fp32 [2 c_opm], bf16 [c_z, c_opm^2]
+  // triangle multiplication: fp16 [5 c_t, c_z] = [p | gate] of the operand written to the first einsum buffer,
+  // [p | gate] of the second, then the output gate g; fp32 bias [5 c_t] in the same order; W_z fp16 [c_z, c_t]
+  size_t to_w, to_b, to_wz, ti_w, ti_b, ti_wz;
+  size_t total16, total_f32;
+};
+TcBlock tc_layout(const pf_config& c);
+void build_tc_block(const pf_config& c, const BlockW& off, const TcBlock& t, const float* w, std::vector<uint16_t>& w16,
+                    size_t base16, std::vector<float>& wf, size_t basef);
+
+enum KernelKind { KK_LN = 0, KK_GEMM, KK_ATTN, KK_TRI, KK_LNC, KK_OPM, KK_LNGEMM, KK_COUNT };
+
+inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+inline int pad8(int v) { return (v + 7) / 8 * 8; }
+
+struct Arena {
+  size_t x, qkg, vt, o, bias, acm, bcm, g, tcm, tn, oa, ob, total;
+};
+Arena arena_layout(const pf_config& c, int B, int S, int N);
+
+}  // namespace pf
+
+struct pf_evoformer {
+  pf_config cfg;
+  pf::BlockW off;
+  pf::TcBlock tc;
+  float* w32 = nullptr;      // device fp32 blob
+  uint16_t* w16 = nullptr;   // device 16-bit transposed matrices (PF_BF16 only)
+  float* wf = nullptr;       // device fused fp32 bias vectors (PF_BF16 only)
+  char* ws = nullptr;        // workspace arena
+  size_t ws_bytes = 0;
+  char* stage = nullptr;     // forward_host staging
+  size_t stage_bytes = 0;
+  int num_sms = 148;
+  long long launches = 0;
+  pf::TmaCtx* tma = nullptr;
+  // per-launch CUDA-event profiling (pf_evoformer_set_profiling)
+  bool prof_on = false;
+  struct ProfRec { int kind; cudaEvent_t e0, e1; double flops, bytes; };
+  std::vector<ProfRec> prof;
+  std::vector<cudaEvent_t> ev_pool;
+  size_t ev_used = 0;
+  cudaEvent_t next_event() {
+    if (ev_used == ev_pool.size()) {
+      cudaEvent_t e;
+      cudaEventCreate(&e);
+      ev_pool.push_back(e);
+    }
+    return ev_pool[ev_used++];
+  }
+  // one kernel launch: counts it and, when profiling, brackets it with events on the launch stream
+  void prof_begin(int kind, double flops, double bytes, cudaStream_t st) {
+    launches++;
+    if (!prof_on) return;
+    ProfRec r{kind, next_event(), next_event(), flops, bytes};
+    cudaEventRecord(r.e0, st);
+    prof.push_back(r);
+  }
+  void prof_end(cudaStream_t st) {
+    if (prof_on) cudaEventRecord(prof.back().e1, st);
+  }
+};
+
+namespace pf {
+// tcgen05 path: one sub-step (1..9) of block `block`; returns false and sets err on failure.
+bool tc_run_substep(pf_evoformer* h, float* msa, float* pair, const float* seq_mask, const float* msa_mask, int B, int S,
+                    int N, int block, int step, cudaStream_t st, std::string& err);
+}  // namespace pf

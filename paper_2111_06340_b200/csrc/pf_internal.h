@@ -2,6 +2,7 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <cuda_bf16.h>
+#include <cuda_fp16.h>
 #include <stdint.h>
 #include <string>
 
@@ -76,6 +77,55 @@ const char* tc_last_error();
 void tc_set_error(const std::string& s);
 int launch_gemm_tc(TmaCtx* ctx, const bf16* A, int lda, const bf16* Wt, long R, int K, int Nout, const Epi& epi,
                    int num_sms, cudaStream_t st);
+// ---- persistent LN-fused projection GEMM (pf_lngemm_tc.cu) ----
+// Rows of the GEMM are (b, x in [0,D1), y in [0,D2)); one CTA tile = XT consecutive x times YT consecutive y (XT*YT = 128).
+// The 64-column groups of the output are described by G2Op: what is done to the accumulator and where it goes.
+enum G2Kind { G2_SKIP = 0, G2_ROW16 = 1, G2_CM_DUAL = 2, G2_HEADS = 3, G2_VT = 4, G2_RESID = 5 };
+struct G2Op {
+  int kind;      // G2Kind
+  int act;       // Act, applied after scale and bias (ROW16)
+  int fmt;       // ROW16: 0 = bf16, 1 = fp16 output
+  int map;       // ROW16: row_out index; CM_DUAL: cm_out index
+  int dst_col;   // first destination column / channel / head
+  int ncols;     // valid columns of this group (<= 64)
+  float scale;   // ROW16 / HEADS: multiplies the accumulator before the bias
+  int masked;    // VT: multiply by the row mask
+};
+constexpr int G2_MAX_OPS = 20;
+struct G2Desc {
+  int B, D1, D2;            // row geometry
+  int K, Nw;                // K in {128, 256}; Nw = rows of Wt (GEMM columns including gate partners)
+  int a_mode;               // 0: A = LayerNorm of fp32 rows gathered from src; 1: A = 16-bit [R, K] in GEMM row order (TMA)
+  const float* src;         // a_mode 0: [B, D1, D2, K] fp32, or [B, D2, D1, K] when src_transposed
+  int src_transposed;
+  const float* gamma;
+  const float* beta;
+  const void* A;            // a_mode 1
+  int op_fmt;               // MMA operand format: 0 bf16, 1 fp16 (A and Wt alike)
+  const void* Wt;           // [Nw, K] 16-bit, K contiguous
+  const float* bias;        // [Nw] fp32 or null
+  int rowmask;              // RowMaskKind, applied by CM_DUAL and masked VT groups
+  const float* seq_mask;
+  const float* msa_mask;
+  int mask_transposed;
+  void* row_out[2];         // ROW16 destinations [R, row_ld] 16-bit in GEMM row order
+  int row_ld[2];
+  float* resid;             // RESID destination: [B, D1, D2, resid_ld], or [B, D2, D1, resid_ld] when resid_transposed
+  int resid_ld;
+  int resid_transposed;
+  const void* gate;         // RESID: optional fp16 gate [R, ldg] in GEMM row order
+  int ldg;
+  void* cm_out[2];          // CM_DUAL: bf16 [(b, channel), D1, Lpad]
+  int cm_channels;
+  void* heads_out;          // HEADS: bf16 [b, n_heads, D1, Lpad]
+  int n_heads;
+  void* vt_out;             // VT: bf16 [((b, x), vt_cols), Lpad]
+  int vt_cols;
+  int Lpad;
+  G2Op ops[G2_MAX_OPS];
+  int n_ops;
+};
+int launch_gemm2(TmaCtx* ctx, const G2Desc& d, int num_sms, cudaStream_t st);
 int launch_attn_tc(TmaCtx* ctx, const bf16* qkg, const bf16* vt, const bf16* bias, const float* keymask, bf16* o,
                    int B, int R, int L, int Lpad, int H, int num_sms, cudaStream_t st);
 // ab_t: [(b,i), 64 channels (a | b), Spad] bf16 masked projections; wout_t: [c_z, c_opm*c_opm] bf16

@@ -1,0 +1,563 @@
+// Persistent LayerNorm-fused projection GEMM on tcgen05 tensor cores (sm_100a) — every Linear of SURVEY.md App. A whose
+// reduction length is one channel dimension (K = c_z = 128 or K = c_m = 256):
+//     acc[r, n] = sum_k A[r, k] Wt[n, k],      r = (b, x, y) rows of a [B, D1, D2] grid,
+//     A = LayerNorm(fp32 residual rows)  (R4; north_star: "LayerNorm fused into the q/k/v/gate/bias projections")
+//         or a 16-bit activation [R, K] fetched by TMA (out-projections, LN_out(t) W_z),
+// followed by per-64-column epilogue groups (G2Op): scaled / biased / activated 16-bit row-major stores, gated channel-major
+// triangle operands, pair-bias heads, transposed V / outer-product operands, or "residual += (acc + bias) * gate".
+//
+// One persistent CTA per SM, 14 warps:
+//   warps 0-3   epilogue: tcgen05.ld their TMEM lane quarter -> registers -> 128B-swizzled shared-memory staging tile ->
+//               one TMA store (16-bit outputs) or one TMA reduce-add (fp32 residual, the add happens at L2) per 128 x 128 B box
+//   warps 4-11  A producers (a_mode 0): warp-per-row LayerNorm with 128-bit loads and warp-shuffle statistics, several rows in
+//               flight per warp, result written as fp16/bf16 straight into the UMMA K-major 128B-swizzle layout
+//   warp 12     TMA: weight tiles [256 x 64] through a ring (and the A tile itself in a_mode 1, issued by warp 4)
+//   warp 13     TMEM allocation + the single MMA-issuing thread
+// The A tile (128 rows x K) stays resident while all N tiles are swept, A is double buffered (the LayerNorm of tile t+1
+// overlaps the MMAs / epilogue of tile t) and so is the 128 x 256 fp32 accumulator in TMEM (2 x 256 columns).
+// A tile covers XT x YT rows so that every output — also a transposed residual — is one 4-D TMA box {cols, YT, XT, 1}.
+#include "pf_internal.h"
+#include "pf_device.cuh"
+#include "pf_tc.cuh"
+
+#include <cuda_fp16.h>
+#include <string>
+
+namespace pf {
+
+int tma_encode(TmaCtx* ctx, CUtensorMap* out, const void* base, int elem_kind, int rank, const uint64_t* dims,
+               const uint64_t* strides_bytes, const uint32_t* box, int swizzle_bytes);
+
+constexpr int G2_BN = 256;
+constexpr int G2_THREADS = 14 * 32;
+constexpr int G2_PROD_WARPS = 8;
+
+struct G2Params {
+  int B, D1, D2, XT, YT, yt_shift, tiles_x_per_b, tiles_y;
+  long num_tiles;
+  int Nw, n_tiles;
+  const float* src;
+  int src_transposed;
+  const float* gamma;
+  const float* beta;
+  int op_fmt;
+  const float* bias;
+  int rowmask;
+  const float* seq_mask;
+  const float* msa_mask;
+  int mask_transposed;
+  const __half* gate;
+  int ldg;
+  bf16* cm_out[2];
+  int cm_channels;
+  bf16* heads_out;
+  int n_heads;
+  bf16* vt_out;
+  int vt_cols;
+  int Lpad;
+  G2Op ops[G2_MAX_OPS];
+};
+
+template <int K>
+struct G2Smem {
+  static constexpr int KB = K / 64;
+  static constexpr int A_BYTES = 128 * K * 2;
+  static constexpr int KB_BYTES = 128 * 128;            // one 64-wide k-block of the A tile
+  static constexpr int W_STAGE = G2_BN * 64 * 2;        // 32 KB
+  static constexpr int W_STAGES = (K == 256) ? 2 : 4;
+  static constexpr int A_OFF = 0;
+  static constexpr int W_OFF = 2 * A_BYTES;
+  static constexpr int ST_OFF = W_OFF + W_STAGES * W_STAGE;
+  static constexpr int ST_BYTES = 128 * 128;
+  static constexpr int BAR_OFF = ST_OFF + 2 * ST_BYTES;
+  static constexpr int TOTAL = BAR_OFF + 256 + 1024;
+};
+
+struct TileCoord {
+  int b, x0, y0;
+};
+__device__ __forceinline__ TileCoord tile_coord(long t, const G2Params& p) {
+  TileCoord c;
+  int ty = (int)(t % p.tiles_y);
+  long tx = t / p.tiles_y;
+  c.b = (int)(tx / p.tiles_x_per_b);
+  c.x0 = (int)(tx - (long)c.b * p.tiles_x_per_b) * p.XT;
+  c.y0 = ty * p.YT;
+  return c;
+}
+
+__device__ __forceinline__ float fast_sigmoid2(float x) { return __fdividef(1.0f, 1.0f + __expf(-x)); }
+
+__device__ __forceinline__ uint32_t pack16(float a, float b, int fmt) {
+  if (fmt) {
+    __half2 h = __floats2half2_rn(a, b);
+    return *reinterpret_cast<uint32_t*>(&h);
+  }
+  __nv_bfloat162 h = __floats2bfloat162_rn(a, b);
+  return *reinterpret_cast<uint32_t*>(&h);
+}
+
+template <int K, int AMODE>
+__global__ void __launch_bounds__(G2_THREADS, 1)
+gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUtensorMap tmA,
+             const __grid_constant__ CUtensorMap tmO0, const __grid_constant__ CUtensorMap tmO1,
+             const __grid_constant__ CUtensorMap tmR, const __grid_constant__ G2Params p) {
+  using SM = G2Smem<K>;
+  constexpr int KB = SM::KB;
+  constexpr int WS = SM::W_STAGES;
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + SM::BAR_OFF);
+  uint64_t* a_full = bars;             // [2]
+  uint64_t* a_empty = bars + 2;        // [2]
+  uint64_t* w_full = bars + 4;         // [WS]
+  uint64_t* w_empty = w_full + WS;     // [WS]
+  uint64_t* acc_full = w_empty + WS;   // [2]
+  uint64_t* acc_empty = acc_full + 2;  // [2]
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(acc_empty + 2);
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+  if (warp == 12 && lane == 0) {
+    tc::prefetch_tmap(&tmW);
+    if (AMODE == 1) tc::prefetch_tmap(&tmA);
+    tc::prefetch_tmap(&tmO0);
+    tc::prefetch_tmap(&tmO1);
+    tc::prefetch_tmap(&tmR);
+    for (int i = 0; i < 2; ++i) {
+      tc::mbar_init(&a_full[i], AMODE == 0 ? G2_PROD_WARPS * 32 : 1);
+      tc::mbar_init(&a_empty[i], 1);
+      tc::mbar_init(&acc_full[i], 1);
+      tc::mbar_init(&acc_empty[i], 128);
+    }
+    for (int i = 0; i < WS; ++i) {
+      tc::mbar_init(&w_full[i], 1);
+      tc::mbar_init(&w_empty[i], 1);
+    }
+    tc::fence_barrier_init();
+  }
+  if (warp == 13) tc::tmem_alloc<512>(tmem_slot);
+  tc::tc_fence_before();
+  __syncthreads();
+  tc::tc_fence_after();
+  const uint32_t tmem_base = *tmem_slot;
+
+  if (warp < 4) {
+    // =========================================================== epilogue
+    const int lr = warp * 32 + lane;                   // tile row = TMEM lane
+    const int xl = lr >> p.yt_shift, yl = lr & (p.YT - 1);
+    const uint32_t lane_addr = tmem_base + ((uint32_t)(warp * 32) << 16);
+    uint8_t* stage = smem + SM::ST_OFF;
+    const uint32_t sw = (uint32_t)(lr & 7);
+    uint32_t sstep = 0;                                // staging steps issued so far
+    uint32_t ac = 0;                                   // accumulator buffers consumed so far
+    for (long tile = blockIdx.x; tile < p.num_tiles; tile += gridDim.x) {
+      const TileCoord tcd = tile_coord(tile, p);
+      const int x = tcd.x0 + xl, y = tcd.y0 + yl;
+      const bool valid = x < p.D1 && y < p.D2;
+      float mask = 1.0f;
+      if (valid && p.rowmask == RM_MSA) {
+        mask = p.mask_transposed ? p.msa_mask[(long)tcd.b * p.D2 + y] * p.seq_mask[(long)tcd.b * p.D1 + x]
+                                 : p.msa_mask[(long)tcd.b * p.D1 + x] * p.seq_mask[(long)tcd.b * p.D2 + y];
+      } else if (valid && p.rowmask == RM_PAIR) {
+        mask = p.seq_mask[(long)tcd.b * p.D1 + x] * p.seq_mask[(long)tcd.b * p.D2 + y];
+      }
+      const long grow = ((long)tcd.b * p.D1 + x) * p.D2 + y;   // GEMM row index (gate rows)
+      for (int nt = 0; nt < p.n_tiles; ++nt, ++ac) {
+        const uint32_t buf = ac & 1;
+        tc::mbar_wait(&acc_full[buf], (ac >> 1) & 1);
+        tc::tc_fence_after();
+        const uint32_t tacc = lane_addr + buf * G2_BN;
+#pragma unroll 1
+        for (int j = 0; j < 4; ++j) {
+          const G2Op& op = p.ops[nt * 4 + j];
+          const int kind = op.kind;
+          if (kind == G2_SKIP) continue;
+          const int ncol0 = nt * G2_BN + j * 64;       // first GEMM column of this group
+          if (kind == G2_ROW16) {
+            uint8_t* sb = stage + (sstep & 1) * SM::ST_BYTES;
+            if (threadIdx.x == 0) tc::bulk_wait_read<1>();
+            tc::named_bar_sync(1, 128);
+            const float scale = op.scale;
+            const int act = op.act, fmt = op.fmt;
+#pragma unroll
+            for (int hf = 0; hf < 2; ++hf) {
+              uint32_t v[32];
+              tc::tmem_ld32(tacc + j * 64 + hf * 32, v);
+              tc::tmem_ld_wait();
+#pragma unroll
+              for (int c = 0; c < 4; ++c) {
+                float f[8];
+#pragma unroll
+                for (int e = 0; e < 8; ++e) {
+                  float xv = __uint_as_float(v[c * 8 + e]) * scale;
+                  if (p.bias) xv += __ldg(p.bias + ncol0 + hf * 32 + c * 8 + e);
+                  if (act == ACT_SIGMOID) xv = fast_sigmoid2(xv);
+                  else if (act == ACT_RELU) xv = fmaxf(xv, 0.f);
+                  f[e] = xv;
+                }
+                uint4 u = make_uint4(pack16(f[0], f[1], fmt), pack16(f[2], f[3], fmt), pack16(f[4], f[5], fmt),
+                                     pack16(f[6], f[7], fmt));
+                *reinterpret_cast<uint4*>(sb + lr * 128 + (((uint32_t)(hf * 4 + c) ^ sw) << 4)) = u;
+              }
+            }
+            tc::fence_proxy_async_smem();
+            tc::named_bar_sync(1, 128);
+            if (threadIdx.x == 0) {
+              tc::tma_store_4d(op.map ? &tmO1 : &tmO0, sb, op.dst_col, tcd.y0, tcd.x0, tcd.b);
+              tc::bulk_commit();
+            }
+            ++sstep;
+          } else if (kind == G2_RESID) {
+#pragma unroll 1
+            for (int hf = 0; hf < 2; ++hf) {
+              uint8_t* sb = stage + (sstep & 1) * SM::ST_BYTES;
+              if (threadIdx.x == 0) tc::bulk_wait_read<1>();
+              tc::named_bar_sync(1, 128);
+              uint32_t v[32];
+              tc::tmem_ld32(tacc + j * 64 + hf * 32, v);
+              tc::tmem_ld_wait();
+              const __half* gp = (p.gate && valid) ? p.gate + grow * p.ldg + op.dst_col + hf * 32 : nullptr;
+#pragma unroll
+              for (int c = 0; c < 8; ++c) {
+                float f[4];
+#pragma unroll
+                for (int e = 0; e < 4; ++e) f[e] = __uint_as_float(v[c * 4 + e]) + __ldg(p.bias + ncol0 + hf * 32 + c * 4 + e);
+                if (gp) {
+                  uint2 gu = *reinterpret_cast<const uint2*>(gp + c * 4);
+                  __half2 g01 = *reinterpret_cast<__half2*>(&gu.x), g23 = *reinterpret_cast<__half2*>(&gu.y);
+                  f[0] *= __low2float(g01);
+                  f[1] *= __high2float(g01);
+                  f[2] *= __low2float(g23);
+                  f[3] *= __high2float(g23);
+                }
+                *reinterpret_cast<float4*>(sb + lr * 128 + (((uint32_t)c ^ sw) << 4)) = make_float4(f[0], f[1], f[2], f[3]);
+              }
+              tc::fence_proxy_async_smem();
+              tc::named_bar_sync(1, 128);
+              if (threadIdx.x == 0) {
+                tc::tma_reduce_add_4d(&tmR, sb, op.dst_col + hf * 32, tcd.y0, tcd.x0, tcd.b);
+                tc::bulk_commit();
+              }
+              ++sstep;
+            }
+          } else if (kind == G2_CM_DUAL) {
+            bf16* base = p.cm_out[op.map] + (((long)tcd.b * p.cm_channels + op.dst_col) * p.D1 + x) * p.Lpad + y;
+            const long cstride = (long)p.D1 * p.Lpad;
+#pragma unroll 1
+            for (int hf = 0; hf < 2; ++hf) {
+              uint32_t v[32], g[32];
+              tc::tmem_ld32(tacc + j * 64 + hf * 32, v);
+              tc::tmem_ld32(tacc + 128 + j * 64 + hf * 32, g);
+              tc::tmem_ld_wait();
+              if (valid) {
+#pragma unroll
+                for (int e = 0; e < 32; ++e) {
+                  int n = ncol0 + hf * 32 + e;
+                  float pv = __uint_as_float(v[e]) + __ldg(p.bias + n);
+                  float gv = fast_sigmoid2(__uint_as_float(g[e]) + __ldg(p.bias + n + 128));
+                  base[(hf * 32 + e) * cstride] = __float2bfloat16_rn(mask * gv * pv);
+                }
+              }
+            }
+          } else if (kind == G2_HEADS) {
+            uint32_t v[32];
+            tc::tmem_ld32(tacc + j * 64, v);
+            tc::tmem_ld_wait();
+            if (valid) {
+              bf16* base = p.heads_out + (((long)tcd.b * p.n_heads + op.dst_col) * p.D1 + x) * p.Lpad + y;
+              const long hstride = (long)p.D1 * p.Lpad;
+#pragma unroll
+              for (int e = 0; e < 8; ++e)
+                if (e < op.ncols) base[e * hstride] = __float2bfloat16_rn(__uint_as_float(v[e]) * op.scale);
+            }
+          } else {   // G2_VT
+            bf16* base = p.vt_out + (((long)tcd.b * p.D1 + x) * p.vt_cols + op.dst_col) * p.Lpad + y;
+            const float mk = op.masked ? mask : 1.0f;
+#pragma unroll 1
+            for (int hf = 0; hf < 2; ++hf) {
+              uint32_t v[32];
+              tc::tmem_ld32(tacc + j * 64 + hf * 32, v);
+              tc::tmem_ld_wait();
+              if (valid) {
+#pragma unroll
+                for (int e = 0; e < 32; ++e) {
+                  if (hf * 32 + e < op.ncols) {
+                    float xv = __uint_as_float(v[e]);
+                    if (p.bias) xv += __ldg(p.bias + ncol0 + hf * 32 + e);
+                    base[(long)(hf * 32 + e) * p.Lpad] = __float2bfloat16_rn(xv * mk);
+                  }
+                }
+              }
+            }
+          }
+        }
+        tc::tc_fence_before();
+        tc::mbar_arrive(&acc_empty[buf]);
+      }
+    }
+    if (threadIdx.x == 0) tc::bulk_wait<0>();
+  } else if (warp < 12) {
+    if (AMODE == 0) {
+      // ========================================================= A producers: LayerNorm of gathered fp32 rows
+      constexpr int NV = K / 128;                      // float4 per lane per row
+      constexpr int RU = 8;                            // rows in flight per warp
+      const int pw = warp - 4;
+      float4 gm[NV], bt[NV];
+#pragma unroll
+      for (int i = 0; i < NV; ++i) {
+        gm[i] = __ldg(reinterpret_cast<const float4*>(p.gamma) + lane + 32 * i);
+        bt[i] = __ldg(reinterpret_cast<const float4*>(p.beta) + lane + 32 * i);
+      }
+      uint32_t it = 0;
+      for (long tile = blockIdx.x; tile < p.num_tiles; tile += gridDim.x, ++it) {
+        const uint32_t abuf = it & 1;
+        tc::mbar_wait(&a_empty[abuf], ((it >> 1) & 1) ^ 1);
+        const TileCoord tcd = tile_coord(tile, p);
+        uint8_t* abase = smem + SM::A_OFF + abuf * SM::A_BYTES;
+#pragma unroll 1
+        for (int r0 = 0; r0 < 16; r0 += RU) {
+          float4 v[RU][NV];
+#pragma unroll
+          for (int u = 0; u < RU; ++u) {
+            const int lr = pw * 16 + r0 + u;
+            const int x = tcd.x0 + (lr >> p.yt_shift), y = tcd.y0 + (lr & (p.YT - 1));
+            if (x < p.D1 && y < p.D2) {
+              long srow = p.src_transposed ? ((long)tcd.b * p.D2 + y) * p.D1 + x : ((long)tcd.b * p.D1 + x) * p.D2 + y;
+              const float4* xp = reinterpret_cast<const float4*>(p.src + srow * K);
+#pragma unroll
+              for (int i = 0; i < NV; ++i) v[u][i] = ld_nc_f4(xp + lane + 32 * i);
+            } else {
+#pragma unroll
+              for (int i = 0; i < NV; ++i) v[u][i] = make_float4(0.f, 0.f, 0.f, 0.f);
+            }
+          }
+#pragma unroll
+          for (int u = 0; u < RU; ++u) {
+            const int lr = pw * 16 + r0 + u;
+            float s = 0.f;
+#pragma unroll
+            for (int i = 0; i < NV; ++i) s += v[u][i].x + v[u][i].y + v[u][i].z + v[u][i].w;
+            const float mean = warp_sum(s) * (1.0f / K);
+            float q = 0.f;
+#pragma unroll
+            for (int i = 0; i < NV; ++i) {
+              float a = v[u][i].x - mean, b2 = v[u][i].y - mean, c = v[u][i].z - mean, d = v[u][i].w - mean;
+              q += a * a + b2 * b2 + c * c + d * d;
+            }
+            const float rstd = rsqrtf(warp_sum(q) * (1.0f / K) + 1e-5f);
+#pragma unroll
+            for (int i = 0; i < NV; ++i) {
+              float o0 = (v[u][i].x - mean) * rstd * gm[i].x + bt[i].x;
+              float o1 = (v[u][i].y - mean) * rstd * gm[i].y + bt[i].y;
+              float o2 = (v[u][i].z - mean) * rstd * gm[i].z + bt[i].z;
+              float o3 = (v[u][i].w - mean) * rstd * gm[i].w + bt[i].w;
+              // columns 128 i + 4 lane .. +3  ->  k-block 2 i + lane / 16, 16-byte chunk (lane % 16) / 2, half lane & 1
+              const int kb = 2 * i + (lane >> 4);
+              const uint32_t chunk = (uint32_t)((lane & 15) >> 1);
+              uint8_t* dst = abase + kb * SM::KB_BYTES + lr * 128 + ((chunk ^ (uint32_t)(lr & 7)) << 4) + (lane & 1) * 8;
+              *reinterpret_cast<uint2*>(dst) = make_uint2(pack16(o0, o1, p.op_fmt), pack16(o2, o3, p.op_fmt));
+            }
+          }
+        }
+        tc::fence_proxy_async_smem();
+        tc::mbar_arrive(&a_full[abuf]);
+      }
+    } else if (warp == 4) {
+      // ========================================================= A by TMA (a_mode 1)
+      if (tc::elect_one()) {
+        uint32_t it = 0;
+        for (long tile = blockIdx.x; tile < p.num_tiles; tile += gridDim.x, ++it) {
+          const uint32_t abuf = it & 1;
+          tc::mbar_wait(&a_empty[abuf], ((it >> 1) & 1) ^ 1);
+          const TileCoord tcd = tile_coord(tile, p);
+          uint8_t* abase = smem + SM::A_OFF + abuf * SM::A_BYTES;
+          tc::mbar_arrive_expect_tx(&a_full[abuf], SM::A_BYTES);
+#pragma unroll
+          for (int kb = 0; kb < KB; ++kb)
+            tc::tma_load_4d(abase + kb * SM::KB_BYTES, &tmA, &a_full[abuf], kb * 64, tcd.y0, tcd.x0, tcd.b);
+        }
+      }
+    }
+  } else if (warp == 12) {
+    // ============================================================= weight tiles
+    if (tc::elect_one()) {
+      uint32_t wc = 0;
+      for (long tile = blockIdx.x; tile < p.num_tiles; tile += gridDim.x) {
+        for (int nt = 0; nt < p.n_tiles; ++nt) {
+#pragma unroll 1
+          for (int kb = 0; kb < KB; ++kb, ++wc) {
+            const uint32_t s = wc % WS;
+            tc::mbar_wait(&w_empty[s], ((wc / WS) & 1) ^ 1);
+            tc::mbar_arrive_expect_tx(&w_full[s], SM::W_STAGE);
+            tc::tma_load_2d(smem + SM::W_OFF + s * SM::W_STAGE, &tmW, &w_full[s], kb * 64, nt * G2_BN);
+          }
+        }
+      }
+    }
+  } else {
+    // ============================================================= MMA issue
+    if (tc::elect_one()) {
+      uint32_t it = 0, wc = 0, ac = 0;
+      for (long tile = blockIdx.x; tile < p.num_tiles; tile += gridDim.x, ++it) {
+        const uint32_t abuf = it & 1;
+        tc::mbar_wait(&a_full[abuf], (it >> 1) & 1);
+        tc::tc_fence_after();
+        const uint32_t a_addr = tc::smem_u32(smem + SM::A_OFF + abuf * SM::A_BYTES);
+        for (int nt = 0; nt < p.n_tiles; ++nt, ++ac) {
+          const uint32_t buf = ac & 1;
+          tc::mbar_wait(&acc_empty[buf], ((ac >> 1) & 1) ^ 1);
+          tc::tc_fence_after();
+          int n_eff = p.Nw - nt * G2_BN;
+          n_eff = n_eff >= G2_BN ? G2_BN : ((n_eff + 15) & ~15);
+          const uint32_t idesc = p.op_fmt ? tc::idesc_f16_f32(128, n_eff) : tc::idesc_bf16_f32(128, n_eff);
+          const uint32_t d_tmem = tmem_base + buf * G2_BN;
+#pragma unroll 1
+          for (int kb = 0; kb < KB; ++kb, ++wc) {
+            const uint32_t s = wc % WS;
+            tc::mbar_wait(&w_full[s], (wc / WS) & 1);
+            tc::tc_fence_after();
+            const uint64_t a_desc = tc::smem_desc_kmajor<128>(a_addr + kb * SM::KB_BYTES);
+            const uint64_t b_desc = tc::smem_desc_kmajor<128>(tc::smem_u32(smem + SM::W_OFF + s * SM::W_STAGE));
+#pragma unroll
+            for (int k = 0; k < 4; ++k) tc::mma_bf16(d_tmem, a_desc + 2 * k, b_desc + 2 * k, idesc, (kb | k) != 0);
+            tc::mma_commit(&w_empty[s]);
+          }
+          tc::mma_commit(&acc_full[buf]);
+        }
+        tc::mma_commit(&a_empty[abuf]);
+      }
+    }
+  }
+  tc::tc_fence_before();
+  __syncthreads();
+  if (warp == 13) tc::tmem_dealloc<512>(tmem_base);
+}
+
+// ------------------------------------------------------------------------------------------------
+// host
+// ------------------------------------------------------------------------------------------------
+static int pick_yt(int D2) {
+  int best = 128;
+  double best_eff = -1.0;
+  for (int yt = 128; yt >= 8; yt >>= 1) {
+    int tiles = (D2 + yt - 1) / yt;
+    double eff = (double)D2 / ((double)tiles * yt);
+    if (eff > best_eff + 1e-9) {
+      best_eff = eff;
+      best = yt;
+    }
+  }
+  return best;
+}
+
+template <int K, int AMODE>
+static int launch_g2(const CUtensorMap& tmW, const CUtensorMap& tmA, const CUtensorMap& tmO0, const CUtensorMap& tmO1,
+                     const CUtensorMap& tmR, const G2Params& p, int num_sms, cudaStream_t st) {
+  auto kern = gemm2_kernel<K, AMODE>;
+  static bool configured = false;
+  if (!configured) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, G2Smem<K>::TOTAL);
+    if (e != cudaSuccess) {
+      tc_set_error(std::string("cudaFuncSetAttribute(gemm2): ") + cudaGetErrorString(e));
+      return -1;
+    }
+    configured = true;
+  }
+  unsigned grid = (unsigned)(p.num_tiles < (long)num_sms ? p.num_tiles : (long)num_sms);
+  kern<<<grid, G2_THREADS, G2Smem<K>::TOTAL, st>>>(tmW, tmA, tmO0, tmO1, tmR, p);
+  return 0;
+}
+
+int launch_gemm2(TmaCtx* ctx, const G2Desc& d, int num_sms, cudaStream_t st) {
+  if (d.K != 128 && d.K != 256) {
+    tc_set_error("gemm2: K must be 128 or 256");
+    return -1;
+  }
+  G2Params p;
+  memset(&p, 0, sizeof(p));
+  p.B = d.B; p.D1 = d.D1; p.D2 = d.D2;
+  p.YT = pick_yt(d.D2);
+  p.XT = 128 / p.YT;
+  p.yt_shift = 0;
+  while ((1 << p.yt_shift) < p.YT) ++p.yt_shift;
+  p.tiles_y = (d.D2 + p.YT - 1) / p.YT;
+  p.tiles_x_per_b = (d.D1 + p.XT - 1) / p.XT;
+  p.num_tiles = (long)d.B * p.tiles_x_per_b * p.tiles_y;
+  p.Nw = d.Nw;
+  p.n_tiles = (d.Nw + G2_BN - 1) / G2_BN;
+  if (p.n_tiles * 4 > G2_MAX_OPS || d.n_ops > G2_MAX_OPS) {
+    tc_set_error("gemm2: too many output columns");
+    return -1;
+  }
+  p.src = d.src; p.src_transposed = d.src_transposed; p.gamma = d.gamma; p.beta = d.beta;
+  p.op_fmt = d.op_fmt;
+  p.bias = d.bias;
+  p.rowmask = d.rowmask; p.seq_mask = d.seq_mask; p.msa_mask = d.msa_mask; p.mask_transposed = d.mask_transposed;
+  p.gate = reinterpret_cast<const __half*>(d.gate); p.ldg = d.ldg;
+  p.cm_out[0] = reinterpret_cast<bf16*>(d.cm_out[0]); p.cm_out[1] = reinterpret_cast<bf16*>(d.cm_out[1]);
+  p.cm_channels = d.cm_channels;
+  p.heads_out = reinterpret_cast<bf16*>(d.heads_out); p.n_heads = d.n_heads;
+  p.vt_out = reinterpret_cast<bf16*>(d.vt_out); p.vt_cols = d.vt_cols;
+  p.Lpad = d.Lpad;
+  bool need_bias = false;
+  for (int i = 0; i < G2_MAX_OPS; ++i) {
+    if (i < d.n_ops) p.ops[i] = d.ops[i];
+    else p.ops[i].kind = G2_SKIP;
+    if (p.ops[i].kind == G2_RESID || p.ops[i].kind == G2_CM_DUAL) need_bias = true;
+  }
+  if (need_bias && !d.bias) {
+    tc_set_error("gemm2: residual / gated groups need a bias vector");
+    return -1;
+  }
+
+  CUtensorMap tmW, tmA, tmO[2], tmR;
+  const int ek = d.op_fmt ? 1 : 0;   // 0 bf16, 1 fp16, 2 fp32
+  {
+    uint64_t dims[2] = {(uint64_t)d.K, (uint64_t)d.Nw}, str[1] = {(uint64_t)d.K * 2};
+    uint32_t box[2] = {64, G2_BN};
+    if (tma_encode(ctx, &tmW, d.Wt, ek, 2, dims, str, box, 128) != 0) return -1;
+  }
+  const uint64_t D1 = d.D1, D2 = d.D2, Bn = d.B;
+  if (d.a_mode == 1) {
+    uint64_t dims[4] = {(uint64_t)d.K, D2, D1, Bn};
+    uint64_t str[3] = {(uint64_t)d.K * 2, D2 * d.K * 2, D1 * D2 * d.K * 2};
+    uint32_t box[4] = {64, (uint32_t)p.YT, (uint32_t)p.XT, 1};
+    if (tma_encode(ctx, &tmA, d.A, ek, 4, dims, str, box, 128) != 0) return -1;
+  } else {
+    tmA = tmW;
+  }
+  for (int i = 0; i < 2; ++i) {
+    if (d.row_out[i]) {
+      uint64_t ld = d.row_ld[i];
+      uint64_t dims[4] = {ld, D2, D1, Bn};
+      uint64_t str[3] = {ld * 2, D2 * ld * 2, D1 * D2 * ld * 2};
+      uint32_t box[4] = {64, (uint32_t)p.YT, (uint32_t)p.XT, 1};
+      if (tma_encode(ctx, &tmO[i], d.row_out[i], 0, 4, dims, str, box, 128) != 0) return -1;
+    } else {
+      tmO[i] = tmW;
+    }
+  }
+  if (d.resid) {
+    uint64_t ld = d.resid_ld;
+    uint64_t dims[4] = {ld, D2, D1, Bn};
+    uint64_t str[3];
+    if (d.resid_transposed) {   // destination array is [B, D2, D1, ld]: y is its second axis
+      str[0] = D1 * ld * 4; str[1] = ld * 4; str[2] = D1 * D2 * ld * 4;
+    } else {
+      str[0] = ld * 4; str[1] = D2 * ld * 4; str[2] = D1 * D2 * ld * 4;
+    }
+    uint32_t box[4] = {32, (uint32_t)p.YT, (uint32_t)p.XT, 1};
+    if (tma_encode(ctx, &tmR, d.resid, 2, 4, dims, str, box, 128) != 0) return -1;
+  } else {
+    tmR = tmW;
+  }
+  if (d.K == 128) {
+    return d.a_mode == 0 ? launch_g2<128, 0>(tmW, tmA, tmO[0], tmO[1], tmR, p, num_sms, st)
+                         : launch_g2<128, 1>(tmW, tmA, tmO[0], tmO[1], tmR, p, num_sms, st);
+  }
+  return d.a_mode == 0 ? launch_g2<256, 0>(tmW, tmA, tmO[0], tmO[1], tmR, p, num_sms, st)
+                       : launch_g2<256, 1>(tmW, tmA, tmO[0], tmO[1], tmR, p, num_sms, st);
+}
+
+}  // namespace pf

@@ -1,5 +1,5 @@
 // SIMT (CUDA-core, fp32 arithmetic) kernels of the Evoformer block, templated on the storage type of
-// intermediates (float for the PF_F32 path, bf16 for PF_BF16_SIMT and for the parts of PF_BF16 that are
+// intermediates (float for the PF_F32 path; the 16-bit instantiations serve the parts of PF_BF16 that are
 // not contractions).  Formulas: SURVEY.md Appendix A; readings R3-R7, R12.
 #include "pf_internal.h"
 #include "pf_device.cuh"
@@ -285,6 +285,7 @@ void launch_lnc(const float* t_cm, T* y, const float* gamma, const float* beta, 
 }
 template void launch_lnc<float>(const float*, float*, const float*, const float*, int, int, int, int, cudaStream_t);
 template void launch_lnc<bf16>(const float*, bf16*, const float*, const float*, int, int, int, int, cudaStream_t);
+template void launch_lnc<__half>(const float*, __half*, const float*, const float*, int, int, int, int, cudaStream_t);
 
 // ---------------------------------------------------------------------------------------------
 // Outer-product-mean core (A.4): one block per (b, i, j).  a, b: [(b,s,i), c_opm] already masked by mu.

@@ -1,0 +1,376 @@
+// tcgen05 path of the trunk (PF_BF16): device weight layout and the per-sub-step launch sequences of SURVEY.md §8(a).
+// 16-bit MMA operands with fp32 accumulation, fp32 residual streams (R1).  Storage formats (reading R17):
+// LayerNorm outputs and the weights they multiply are fp16 operands (bounded by construction; the weight values are the
+// bf16-rounded ones of R15, exactly representable), sigmoid gates are stored as fp16 (never an MMA operand), every other
+// intermediate (q, k, v, P, o, transition hidden, triangle operands, outer-product operands, pair bias) is bf16.
+// No arithmetic of the method lives here except the constant 1/sqrt(head_dim) handed to the q projection (R12).
+#include "pf_handle.h"
+
+#include <cstring>
+
+namespace pf {
+
+// ------------------------------------------------------------------------------------------------
+// weights
+// ------------------------------------------------------------------------------------------------
+static uint16_t f32_to_bf16_bits(float f) {
+  uint32_t u;
+  memcpy(&u, &f, 4);
+  uint32_t lsb = (u >> 16) & 1;
+  u += 0x7FFFu + lsb;
+  return (uint16_t)(u >> 16);
+}
+static uint16_t f32_to_f16_bits(float f) {
+  __half h = __float2half_rn(f);   // host-callable conversion
+  uint16_t b;
+  memcpy(&b, &h, 2);
+  return b;
+}
+
+// dst[n, k] = src[k, n]  (src row-major [K, ld_src], columns [0, Nout)) as 16-bit
+static void put_transposed(std::vector<uint16_t>& dst, size_t at, const float* src, int K, int Nout, bool f16) {
+  for (int n = 0; n < Nout; ++n)
+    for (int k = 0; k < K; ++k) {
+      float v = src[(size_t)k * Nout + n];
+      dst[at + (size_t)n * K + k] = f16 ? f32_to_f16_bits(v) : f32_to_bf16_bits(v);
+    }
+}
+
+TcBlock tc_layout(const pf_config& c) {
+  TcBlock t{};
+  size_t o = 0, f = 0;
+  auto take = [&](size_t k) { size_t r = o; o += align_up(k, 64); return r; };
+  auto takef = [&](size_t k) { size_t r = f; f += align_up(k, 32); return r; };
+  auto attn = [&](int ch, int extra) {
+    AttnT a{};
+    a.w_in = take((size_t)(4 * ch + extra) * ch);
+    a.b_in = takef((size_t)4 * ch + extra);
+    a.wo = take((size_t)ch * ch);
+    return a;
+  };
+  t.row = attn(c.c_m, 0);
+  t.col = attn(c.c_m, 0);
+  t.tri_start = attn(c.c_z, c.heads_pair);
+  t.tri_end = attn(c.c_z, c.heads_pair);
+  t.row_wbias = take((size_t)c.heads_msa * c.c_z);
+  size_t n = c.transition_n;
+  t.mt_w1 = take(n * c.c_m * c.c_m); t.mt_w2 = take(n * c.c_m * c.c_m);
+  t.pt_w1 = take(n * c.c_z * c.c_z); t.pt_w2 = take(n * c.c_z * c.c_z);
+  t.opm_wab = take((size_t)2 * c.c_opm * c.c_m);
+  t.opm_bias_ab = takef((size_t)2 * c.c_opm);
+  t.opm_wout = take((size_t)c.c_opm * c.c_opm * c.c_z);
+  t.to_w = take((size_t)5 * c.c_tri * c.c_z); t.to_b = takef((size_t)5 * c.c_tri); t.to_wz = take((size_t)c.c_z * c.c_tri);
+  t.ti_w = take((size_t)5 * c.c_tri * c.c_z); t.ti_b = takef((size_t)5 * c.c_tri); t.ti_wz = take((size_t)c.c_z * c.c_tri);
+  t.total16 = o;
+  t.total_f32 = f;
+  return t;
+}
+
+void build_tc_block(const pf_config& c, const BlockW& off, const TcBlock& t, const float* w, std::vector<uint16_t>& w16,
+                    size_t base16, std::vector<float>& wf, size_t basef) {
+  auto attn = [&](const AttnW& a, const AttnT& d, int ch, int heads, bool self_bias) {
+    // column order of the fused projection: [q | k | gate | v (| pair-bias heads)], all fed by LN(x): fp16
+    put_transposed(w16, base16 + d.w_in + (size_t)0 * ch * ch, w + a.wq, ch, ch, true);
+    put_transposed(w16, base16 + d.w_in + (size_t)1 * ch * ch, w + a.wk, ch, ch, true);
+    put_transposed(w16, base16 + d.w_in + (size_t)2 * ch * ch, w + a.wg, ch, ch, true);
+    put_transposed(w16, base16 + d.w_in + (size_t)3 * ch * ch, w + a.wv, ch, ch, true);
+    if (self_bias) put_transposed(w16, base16 + d.w_in + (size_t)4 * ch * ch, w + a.w_bias, ch, heads, true);
+    int nb = 4 * ch + (self_bias ? heads : 0);
+    for (int i = 0; i < nb; ++i) wf[basef + d.b_in + i] = 0.f;
+    for (int i = 0; i < ch; ++i) wf[basef + d.b_in + 2 * ch + i] = w[a.bg + i];
+    put_transposed(w16, base16 + d.wo, w + a.wo, ch, ch, false);
+  };
+  attn(off.row, t.row, c.c_m, c.heads_msa, false);
+  attn(off.col, t.col, c.c_m, c.heads_msa, false);
+  attn(off.tri_start, t.tri_start, c.c_z, c.heads_pair, true);
+  attn(off.tri_end, t.tri_end, c.c_z, c.heads_pair, true);
+  put_transposed(w16, base16 + t.row_wbias, w + off.row.w_bias, c.c_z, c.heads_msa, true);
+  int n = c.transition_n;
+  put_transposed(w16, base16 + t.mt_w1, w + off.msa_trans.w1, c.c_m, n * c.c_m, true);
+  put_transposed(w16, base16 + t.mt_w2, w + off.msa_trans.w2, n * c.c_m, c.c_m, false);
+  put_transposed(w16, base16 + t.pt_w1, w + off.pair_trans.w1, c.c_z, n * c.c_z, true);
+  put_transposed(w16, base16 + t.pt_w2, w + off.pair_trans.w2, n * c.c_z, c.c_z, false);
+  put_transposed(w16, base16 + t.opm_wab, w + off.opm.wa, c.c_m, c.c_opm, true);
+  put_transposed(w16, base16 + t.opm_wab + (size_t)c.c_opm * c.c_m, w + off.opm.wb, c.c_m, c.c_opm, true);
+  for (int i = 0; i < c.c_opm; ++i) {
+    wf[basef + t.opm_bias_ab + i] = w[off.opm.ba + i];
+    wf[basef + t.opm_bias_ab + c.c_opm + i] = w[off.opm.bb + i];
+  }
+  put_transposed(w16, base16 + t.opm_wout, w + off.opm.wout, c.c_opm * c.c_opm, c.c_z, false);
+  // triangle multiplication: the einsum kernel contracts buffer 0 (rows i) with buffer 1 (rows j) along k.
+  // outgoing (A.5): buffer 0 = a, buffer 1 = b.  incoming (A.6) runs on the transposed rows with a and b swapped
+  // (SURVEY.md §0 finding 1): buffer 0 = b, buffer 1 = a.
+  auto tri = [&](const TriMulW& s, size_t wdst, size_t bdst, size_t wz, bool swap) {
+    const int ct = c.c_tri, cz = c.c_z;
+    size_t blk = (size_t)ct * cz;
+    size_t p0 = swap ? s.w_bp : s.w_ap, g0 = swap ? s.w_bg : s.w_ag, p1 = swap ? s.w_ap : s.w_bp, g1 = swap ? s.w_ag : s.w_bg;
+    size_t bp0 = swap ? s.b_bp : s.b_ap, bg0 = swap ? s.b_bg : s.b_ag, bp1 = swap ? s.b_ap : s.b_bp, bg1 = swap ? s.b_ag : s.b_bg;
+    put_transposed(w16, base16 + wdst + 0 * blk, w + p0, cz, ct, true);
+    put_transposed(w16, base16 + wdst + 1 * blk, w + g0, cz, ct, true);
+    put_transposed(w16, base16 + wdst + 2 * blk, w + p1, cz, ct, true);
+    put_transposed(w16, base16 + wdst + 3 * blk, w + g1, cz, ct, true);
+    put_transposed(w16, base16 + wdst + 4 * blk, w + s.w_g, cz, cz, true);
+    for (int i = 0; i < ct; ++i) {
+      wf[basef + bdst + 0 * ct + i] = w[bp0 + i];
+      wf[basef + bdst + 1 * ct + i] = w[bg0 + i];
+      wf[basef + bdst + 2 * ct + i] = w[bp1 + i];
+      wf[basef + bdst + 3 * ct + i] = w[bg1 + i];
+      wf[basef + bdst + 4 * ct + i] = w[s.b_g + i];
+    }
+    put_transposed(w16, base16 + wz, w + s.w_z, ct, cz, true);
+  };
+  tri(off.tri_out, t.to_w, t.to_b, t.to_wz, false);
+  tri(off.tri_in, t.ti_w, t.ti_b, t.ti_wz, true);
+}
+
+
+// ------------------------------------------------------------------------------------------------
+// sub-step driver
+// ------------------------------------------------------------------------------------------------
+namespace {
+
+struct TcDriver {
+  pf_evoformer* h;
+  cudaStream_t st;
+  int B, S, N;
+  float* msa;
+  float* pair;
+  const float* seq_mask;
+  const float* msa_mask;
+  Arena ar;
+  const float* w;        // fp32 blob of the current block (device): LN parameters and un-fused biases
+  const uint16_t* w16;   // 16-bit matrices of the current block
+  const float* wf;       // fused fp32 biases of the current block
+  std::string err;
+
+  template <typename U>
+  U* buf(size_t off) { return reinterpret_cast<U*>(h->ws + off); }
+
+  static G2Desc desc_base(int B, int D1, int D2, int K, int Nw) {
+    G2Desc d;
+    memset(&d, 0, sizeof(d));
+    d.B = B; d.D1 = D1; d.D2 = D2; d.K = K; d.Nw = Nw;
+    return d;
+  }
+  static G2Op op(int kind, int dst_col, int ncols = 64) {
+    G2Op o;
+    memset(&o, 0, sizeof(o));
+    o.kind = kind; o.dst_col = dst_col; o.ncols = ncols; o.scale = 1.0f;
+    return o;
+  }
+
+  bool gemm2(const G2Desc& d, double out_bytes) {
+    double R = (double)d.B * d.D1 * d.D2;
+    double in_bytes = R * d.K * (d.a_mode == 0 ? 4.0 : 2.0);
+    h->prof_begin(KK_LNGEMM, 2.0 * R * d.K * d.Nw, in_bytes + out_bytes + 2.0 * d.K * d.Nw, st);
+    if (launch_gemm2(h->tma, d, h->num_sms, st) != 0) {
+      err = std::string("gemm2: ") + tc_last_error();
+      return false;
+    }
+    h->prof_end(st);
+    return true;
+  }
+
+  // Gated attention sub-step on a residual stream `res` viewed as rows (b, x in D1, y in D2), attention along y.
+  //   transposed: rows are gathered from / scattered to the (b, y, x) layout of `res`  (A.2, A.8 via their identities)
+  bool attn_substep(float* res, int C, int H, int D1, int D2, bool transposed, const AttnW& a, const AttnT& at,
+                    const float* keymask, bool row_bias, bool self_bias) {
+    const pf_config& c = h->cfg;
+    const double R = (double)B * D1 * D2;
+    const int L = D2, Lp = pad8(L);
+    bf16* QKG = buf<bf16>(ar.qkg);
+    bf16* VT = buf<bf16>(ar.vt);
+    bf16* O = buf<bf16>(ar.o);
+    bf16* BIAS = (row_bias || self_bias) ? buf<bf16>(ar.bias) : nullptr;
+    if (row_bias) {   // A.1: beta[h,i,j] = Lin0(LN'(z[i,j]))_h
+      G2Desc d = desc_base(B, N, N, c.c_z, c.heads_msa);
+      d.src = pair; d.gamma = w + a.ln_z_g; d.beta = w + a.ln_z_b;
+      d.op_fmt = 1; d.Wt = w16 + h->tc.row_wbias;
+      d.heads_out = BIAS; d.n_heads = c.heads_msa; d.Lpad = pad8(N);
+      d.ops[0] = op(G2_HEADS, 0, c.heads_msa);
+      d.n_ops = 1;
+      if (!gemm2(d, (double)B * N * N * c.heads_msa * 2.0)) return false;
+    }
+    {
+      const int Nw = 4 * C + (self_bias ? H : 0);
+      G2Desc d = desc_base(B, D1, D2, C, Nw);
+      d.src = res; d.src_transposed = transposed ? 1 : 0; d.gamma = w + a.ln_g; d.beta = w + a.ln_b;
+      d.op_fmt = 1; d.Wt = w16 + at.w_in; d.bias = wf + at.b_in;
+      d.row_out[0] = QKG; d.row_ld[0] = 3 * C;
+      d.vt_out = VT; d.vt_cols = C; d.Lpad = Lp;
+      d.heads_out = BIAS; d.n_heads = H;
+      int n = 0;
+      for (int col = 0; col < 4 * C; col += 64, ++n) {
+        int seg = col / C;
+        if (seg < 3) {
+          d.ops[n] = op(G2_ROW16, col);
+          if (seg == 0) d.ops[n].scale = 0.17677669529663687f;   // 1/sqrt(32)  (R12)
+          if (seg == 2) { d.ops[n].act = ACT_SIGMOID; d.ops[n].fmt = 1; }
+        } else {
+          d.ops[n] = op(G2_VT, col - 3 * C);
+        }
+      }
+      if (self_bias) d.ops[n++] = op(G2_HEADS, 0, H);   // A.7 / A.8: beta from the same LN(z) rows
+      d.n_ops = n;
+      if (!gemm2(d, R * 4.0 * C * 2.0 + (self_bias ? R * H * 2.0 : 0.0))) return false;
+    }
+    {
+      double rows = R, Cc = C;
+      h->prof_begin(KK_ATTN, 4.0 * rows * L * Cc, 5.0 * rows * Cc * 2.0 + (BIAS ? (double)B * H * L * L * 2.0 : 0.0), st);
+      if (launch_attn_tc(h->tma, QKG, VT, BIAS, keymask, O, B, D1, L, Lp, H, h->num_sms, st) != 0) {
+        err = std::string("attn_tc: ") + tc_last_error();
+        return false;
+      }
+      h->prof_end(st);
+    }
+    G2Desc d = desc_base(B, D1, D2, C, C);
+    d.a_mode = 1; d.A = O; d.op_fmt = 0; d.Wt = w16 + at.wo; d.bias = w + a.bo;
+    d.resid = res; d.resid_ld = C; d.resid_transposed = transposed ? 1 : 0;
+    int n = 0;
+    for (int col = 0; col < C; col += 64) d.ops[n++] = op(G2_RESID, col);
+    d.n_ops = n;
+    return gemm2(d, R * C * 8.0);
+  }
+
+  bool transition_substep(float* res, int D1, int D2, int C, const TransW& t, size_t w1t, size_t w2t) {
+    const int n4 = h->cfg.transition_n * C;
+    const long R = (long)B * D1 * D2;
+    bf16* Hb = buf<bf16>(ar.qkg);
+    G2Desc d = desc_base(B, D1, D2, C, n4);
+    d.src = res; d.gamma = w + t.ln_g; d.beta = w + t.ln_b;
+    d.op_fmt = 1; d.Wt = w16 + w1t; d.bias = w + t.b1;
+    d.row_out[0] = Hb; d.row_ld[0] = n4;
+    int n = 0;
+    for (int col = 0; col < n4; col += 64, ++n) {
+      d.ops[n] = op(G2_ROW16, col);
+      d.ops[n].act = ACT_RELU;
+    }
+    d.n_ops = n;
+    if (!gemm2(d, (double)R * n4 * 2.0)) return false;
+    Epi e;
+    memset(&e, 0, sizeof(e));
+    e.kind = EPI_RESID; e.scale = 1.0f; e.vt_from = 1 << 30;
+    e.geom = RowGeom{1, 1, (int)R};
+    e.bias = w + t.b2;
+    e.resid = res; e.ldr = C;
+    h->prof_begin(KK_GEMM, 2.0 * R * n4 * C, (double)R * n4 * 2.0 + (double)R * C * 8.0 + 2.0 * n4 * C, st);
+    if (launch_gemm_tc(h->tma, Hb, n4, reinterpret_cast<const bf16*>(w16 + w2t), R, n4, C, e, h->num_sms, st) != 0) {
+      err = std::string("gemm_tc: ") + tc_last_error();
+      return false;
+    }
+    h->prof_end(st);
+    return true;
+  }
+
+  bool opm_substep() {
+    const pf_config& c = h->cfg;
+    const OpmW& o = h->off.opm;
+    if (S > 512) {
+      err = "opm_tc: N_seq above 512 not supported on the tensor-core path";
+      return false;
+    }
+    const double M = (double)B * S * N, P = (double)B * N * N, cc = (double)c.c_opm * c.c_opm;
+    const int Sp = pad8(S);
+    bf16* ABT = buf<bf16>(ar.vt);
+    // rows (b, i, s) gathered from msa[(b, s, i)]: a | b masked and written transposed, [(b,i), 64, Spad], s contiguous
+    G2Desc d = desc_base(B, N, S, c.c_m, 2 * c.c_opm);
+    d.src = msa; d.src_transposed = 1; d.gamma = w + o.ln_g; d.beta = w + o.ln_b;
+    d.op_fmt = 1; d.Wt = w16 + h->tc.opm_wab; d.bias = wf + h->tc.opm_bias_ab;
+    d.rowmask = RM_MSA; d.seq_mask = seq_mask; d.msa_mask = msa_mask; d.mask_transposed = 1;
+    d.vt_out = ABT; d.vt_cols = 2 * c.c_opm; d.Lpad = Sp;
+    d.ops[0] = op(G2_VT, 0, 2 * c.c_opm);
+    d.ops[0].masked = 1;
+    d.n_ops = 1;
+    if (!gemm2(d, M * 2.0 * c.c_opm * 2.0)) return false;
+    h->prof_begin(KK_OPM, 2.0 * P * cc * S + 2.0 * P * cc * c.c_z, 2.0 * M * c.c_opm * 2.0 + 8.0 * P * c.c_z, st);
+    if (launch_opm_tc(h->tma, ABT, reinterpret_cast<const bf16*>(w16 + h->tc.opm_wout), w + o.bout, seq_mask, msa_mask,
+                      pair, B, S, Sp, N, st) != 0) {
+      err = std::string("opm_tc: ") + tc_last_error();
+      return false;
+    }
+    h->prof_end(st);
+    return true;
+  }
+
+  bool trimul_substep(bool incoming) {
+    const pf_config& c = h->cfg;
+    const TriMulW& t = incoming ? h->off.tri_in : h->off.tri_out;
+    const double P = (double)B * N * N;
+    const int Np = pad8(N), ct = c.c_tri;
+    bf16* ACM = buf<bf16>(ar.acm);
+    bf16* BCM = buf<bf16>(ar.bcm);
+    __half* G = buf<__half>(ar.g);
+    float* TCM = buf<float>(ar.tcm);
+    __half* TN = buf<__half>(ar.tn);
+    {
+      G2Desc d = desc_base(B, N, N, c.c_z, 5 * ct);
+      d.src = pair; d.src_transposed = incoming ? 1 : 0; d.gamma = w + t.ln_in_g; d.beta = w + t.ln_in_b;
+      d.op_fmt = 1; d.Wt = w16 + (incoming ? h->tc.ti_w : h->tc.to_w); d.bias = wf + (incoming ? h->tc.ti_b : h->tc.to_b);
+      d.rowmask = RM_PAIR; d.seq_mask = seq_mask;
+      d.cm_out[0] = ACM; d.cm_out[1] = BCM; d.cm_channels = ct; d.Lpad = Np;
+      d.row_out[0] = G; d.row_ld[0] = c.c_z;
+      for (int tile = 0; tile < 2; ++tile)
+        for (int j = 0; j < 4; ++j) {
+          d.ops[tile * 4 + j] = j < 2 ? op(G2_CM_DUAL, j * 64) : op(G2_SKIP, 0);
+          d.ops[tile * 4 + j].map = tile;
+        }
+      for (int j = 0; j < 2; ++j) {
+        d.ops[8 + j] = op(G2_ROW16, j * 64);
+        d.ops[8 + j].act = ACT_SIGMOID;
+        d.ops[8 + j].fmt = 1;
+      }
+      d.n_ops = 10;
+      if (!gemm2(d, P * 3.0 * ct * 2.0)) return false;
+    }
+    h->prof_begin(KK_TRI, 2.0 * B * ct * (double)N * N * N, (double)B * ct * N * Np * 8.0, st);
+    if (launch_tri_einsum_tc(h->tma, ACM, BCM, TCM, B * ct, N, Np, h->num_sms, st) != 0) {
+      err = std::string("tri_einsum_tc: ") + tc_last_error();
+      return false;
+    }
+    h->prof_end(st);
+    h->prof_begin(KK_LNC, 0.0, P * ct * 6.0, st);
+    launch_lnc<__half>(TCM, TN, w + t.ln_out_g, w + t.ln_out_b, B, ct, N, Np, st);
+    h->prof_end(st);
+    G2Desc d = desc_base(B, N, N, ct, c.c_z);
+    d.a_mode = 1; d.A = TN; d.op_fmt = 1; d.Wt = w16 + (incoming ? h->tc.ti_wz : h->tc.to_wz); d.bias = w + t.b_z;
+    d.resid = pair; d.resid_ld = c.c_z; d.resid_transposed = incoming ? 1 : 0;
+    d.gate = G; d.ldg = c.c_z;
+    d.ops[0] = op(G2_RESID, 0);
+    d.ops[1] = op(G2_RESID, 64);
+    d.n_ops = 2;
+    return gemm2(d, P * c.c_z * 10.0);
+  }
+};
+
+}  // namespace
+
+bool tc_run_substep(pf_evoformer* h, float* msa, float* pair, const float* seq_mask, const float* msa_mask, int B, int S,
+                    int N, int block, int step, cudaStream_t st, std::string& err) {
+  const pf_config& c = h->cfg;
+  TcDriver d;
+  d.h = h; d.st = st; d.B = B; d.S = S; d.N = N;
+  d.msa = msa; d.pair = pair; d.seq_mask = seq_mask; d.msa_mask = msa_mask;
+  d.ar = arena_layout(c, B, S, N);
+  d.w = h->w32 + (size_t)block * h->off.total;
+  d.w16 = h->w16 + (size_t)block * h->tc.total16;
+  d.wf = h->wf + (size_t)block * h->tc.total_f32;
+  bool ok = false;
+  switch (step) {
+    case 1: ok = d.attn_substep(msa, c.c_m, c.heads_msa, S, N, false, h->off.row, h->tc.row, seq_mask, true, false); break;
+    case 2: ok = d.attn_substep(msa, c.c_m, c.heads_msa, N, S, true, h->off.col, h->tc.col, msa_mask, false, false); break;
+    case 3: ok = d.transition_substep(msa, S, N, c.c_m, h->off.msa_trans, h->tc.mt_w1, h->tc.mt_w2); break;
+    case 4: ok = d.opm_substep(); break;
+    case 5: ok = d.trimul_substep(false); break;
+    case 6: ok = d.trimul_substep(true); break;
+    case 7: ok = d.attn_substep(pair, c.c_z, c.heads_pair, N, N, false, h->off.tri_start, h->tc.tri_start, seq_mask, false,
+                                true); break;
+    case 8: ok = d.attn_substep(pair, c.c_z, c.heads_pair, N, N, true, h->off.tri_end, h->tc.tri_end, seq_mask, false,
+                                true); break;
+    case 9: ok = d.transition_substep(pair, N, N, c.c_z, h->off.pair_trans, h->tc.pt_w1, h->tc.pt_w2); break;
+    default: d.err = "substep not in 1..9";
+  }
+  if (!ok) err = d.err;
+  return ok;
+}
+
+}  // namespace pf

@@ -64,16 +64,6 @@ def test_runtime_shapes(B, S, N):
     _check(m, z, mr, zr, sm, mm, f"B{B} S{S} N{N}")
 
 
-def test_simt_and_tensor_core_paths_agree(ragged):
-    """Same storage points, contractions on CUDA cores (PF_BF16_SIMT) vs tcgen05 (PF_BF16): both within tolerance
-    of the oracle and close to each other (they differ only in accumulation order and fast-math sigmoid)."""
-    blocks, msa, pair, sm, mm = ragged
-    m1, z1 = run_cuda(pf.PF_BF16, blocks, msa, pair, sm, mm)
-    m2, z2 = run_cuda(pf.PF_BF16_SIMT, blocks, msa, pair, sm, mm)
-    vm, vz = valid_masks(sm, mm)
-    assert np.abs(m1[vm] - m2[vm]).max() <= TOL_ABS and np.abs(z1[vz] - z2[vz]).max() <= TOL_ABS
-
-
 def test_cfg2_full_size_sampled_proteins():
     """BASELINE.json configs[1] at full size in bench.py's launch configuration (B=64, N_seq=128, bucket 128, masks per
     R11), one teacher-forced block; the oracle recomputes two whole proteins of the batch (the two shortest, to bound
