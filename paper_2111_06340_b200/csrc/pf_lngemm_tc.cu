@@ -69,7 +69,8 @@ struct G2Smem {
   static constexpr int W_OFF = 2 * A_BYTES;
   static constexpr int ST_OFF = W_OFF + W_STAGES * W_STAGE;
   static constexpr int ST_BYTES = 128 * 128;
-  static constexpr int BAR_OFF = ST_OFF + 2 * ST_BYTES;
+  static constexpr int BIAS_OFF = ST_OFF + 2 * ST_BYTES;   // fp32 bias of the current 256-column window
+  static constexpr int BAR_OFF = BIAS_OFF + G2_BN * 4;
   static constexpr int TOTAL = BAR_OFF + 256 + 1024;
 };
 
@@ -148,6 +149,7 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
     const int xl = lr >> p.yt_shift, yl = lr & (p.YT - 1);
     const uint32_t lane_addr = tmem_base + ((uint32_t)(warp * 32) << 16);
     uint8_t* stage = smem + SM::ST_OFF;
+    float* sbias = reinterpret_cast<float*>(smem + SM::BIAS_OFF);
     const uint32_t sw = (uint32_t)(lr & 7);
     uint32_t sstep = 0;                                // staging steps issued so far
     uint32_t ac = 0;                                   // accumulator buffers consumed so far
@@ -165,6 +167,17 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
       const long grow = ((long)tcd.b * p.D1 + x) * p.D2 + y;   // GEMM row index (gate rows)
       for (int nt = 0; nt < p.n_tiles; ++nt, ++ac) {
         const uint32_t buf = ac & 1;
+        if (p.n_tiles > 1 || ac == 0) {
+          // bias of this 256-column window -> shared memory (global loads here would sit on the epilogue's critical path:
+          // the streaming LayerNorm loads keep evicting them from L1)
+          tc::named_bar_sync(1, 128);
+#pragma unroll
+          for (int e = 0; e < 2; ++e) {
+            const int n = nt * G2_BN + e * 128 + (int)threadIdx.x;
+            sbias[e * 128 + threadIdx.x] = (p.bias && n < p.Nw) ? __ldg(p.bias + n) : 0.f;
+          }
+          tc::named_bar_sync(1, 128);
+        }
         tc::mbar_wait(&acc_full[buf], (ac >> 1) & 1);
         tc::tc_fence_after();
         const uint32_t tacc = lane_addr + buf * G2_BN;
@@ -173,7 +186,6 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
           const G2Op& op = p.ops[nt * 4 + j];
           const int kind = op.kind;
           if (kind == G2_SKIP) continue;
-          const int ncol0 = nt * G2_BN + j * 64;       // first GEMM column of this group
           if (kind == G2_ROW16) {
             uint8_t* sb = stage + (sstep & 1) * SM::ST_BYTES;
             if (threadIdx.x == 0) tc::bulk_wait_read<1>();
@@ -190,8 +202,7 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
                 float f[8];
 #pragma unroll
                 for (int e = 0; e < 8; ++e) {
-                  float xv = __uint_as_float(v[c * 8 + e]) * scale;
-                  if (p.bias) xv += __ldg(p.bias + ncol0 + hf * 32 + c * 8 + e);
+                  float xv = fmaf(__uint_as_float(v[c * 8 + e]), scale, sbias[j * 64 + hf * 32 + c * 8 + e]);
                   if (act == ACT_SIGMOID) xv = fast_sigmoid2(xv);
                   else if (act == ACT_RELU) xv = fmaxf(xv, 0.f);
                   f[e] = xv;
@@ -222,7 +233,7 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
               for (int c = 0; c < 8; ++c) {
                 float f[4];
 #pragma unroll
-                for (int e = 0; e < 4; ++e) f[e] = __uint_as_float(v[c * 4 + e]) + __ldg(p.bias + ncol0 + hf * 32 + c * 4 + e);
+                for (int e = 0; e < 4; ++e) f[e] = __uint_as_float(v[c * 4 + e]) + sbias[j * 64 + hf * 32 + c * 4 + e];
                 if (gp) {
                   uint2 gu = *reinterpret_cast<const uint2*>(gp + c * 4);
                   __half2 g01 = *reinterpret_cast<__half2*>(&gu.x), g23 = *reinterpret_cast<__half2*>(&gu.y);
@@ -253,9 +264,9 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
               if (valid) {
 #pragma unroll
                 for (int e = 0; e < 32; ++e) {
-                  int n = ncol0 + hf * 32 + e;
-                  float pv = __uint_as_float(v[e]) + __ldg(p.bias + n);
-                  float gv = fast_sigmoid2(__uint_as_float(g[e]) + __ldg(p.bias + n + 128));
+                  const int n = j * 64 + hf * 32 + e;
+                  float pv = __uint_as_float(v[e]) + sbias[n];
+                  float gv = fast_sigmoid2(__uint_as_float(g[e]) + sbias[n + 128]);
                   base[(hf * 32 + e) * cstride] = __float2bfloat16_rn(mask * gv * pv);
                 }
               }
@@ -283,8 +294,7 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
 #pragma unroll
                 for (int e = 0; e < 32; ++e) {
                   if (hf * 32 + e < op.ncols) {
-                    float xv = __uint_as_float(v[e]);
-                    if (p.bias) xv += __ldg(p.bias + ncol0 + hf * 32 + e);
+                    float xv = __uint_as_float(v[e]) + sbias[j * 64 + hf * 32 + e];
                     base[(long)(hf * 32 + e) * p.Lpad] = __float2bfloat16_rn(xv * mk);
                   }
                 }
@@ -312,6 +322,20 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
       uint32_t it = 0;
       for (long tile = blockIdx.x; tile < p.num_tiles; tile += gridDim.x, ++it) {
         const uint32_t abuf = it & 1;
+        {
+          // pull the next tile's rows of this warp into L2 while this tile is normalised: the register-staged loads below
+          // then see L2 latency, not HBM latency (bytes in flight per SM are bounded by the register file)
+          const long nxt = tile + gridDim.x;
+          if (nxt < p.num_tiles && lane < 16) {
+            const TileCoord nc = tile_coord(nxt, p);
+            const int lr = pw * 16 + lane;
+            const int x = nc.x0 + (lr >> p.yt_shift), y = nc.y0 + (lr & (p.YT - 1));
+            if (x < p.D1 && y < p.D2) {
+              long srow = p.src_transposed ? ((long)nc.b * p.D2 + y) * p.D1 + x : ((long)nc.b * p.D1 + x) * p.D2 + y;
+              tc::prefetch_l2_bulk(p.src + srow * K, K * 4);
+            }
+          }
+        }
         tc::mbar_wait(&a_empty[abuf], ((it >> 1) & 1) ^ 1);
         const TileCoord tcd = tile_coord(tile, p);
         uint8_t* abase = smem + SM::A_OFF + abuf * SM::A_BYTES;
