@@ -44,7 +44,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQK, const __grid_constant__
                bf16* __restrict__ o, int R, int L, int H, int has_bias) {
   using SM = AttnSmem;
   extern __shared__ uint8_t smem_raw[];
-  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+  uint8_t* smem = tc::align_smem_1024(smem_raw);
   float* mterm = reinterpret_cast<float*>(smem + SM::MASK_OFF);
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem + SM::BAR_OFF);
   uint64_t* q_full = bars;                 // 1

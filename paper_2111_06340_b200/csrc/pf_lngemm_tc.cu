@@ -6,13 +6,17 @@
 // followed by per-64-column epilogue groups (G2Op): scaled / biased / activated 16-bit row-major stores, gated channel-major
 // triangle operands, pair-bias heads, transposed V / outer-product operands, or "residual += (acc + bias) * gate".
 //
-// One persistent CTA per SM, 14 warps:
-//   warps 0-3   epilogue: tcgen05.ld their TMEM lane quarter -> registers -> 128B-swizzled shared-memory staging tile ->
-//               one TMA store (16-bit outputs) or one TMA reduce-add (fp32 residual, the add happens at L2) per 128 x 128 B box
-//   warps 4-11  A producers (a_mode 0): warp-per-row LayerNorm with 128-bit loads and warp-shuffle statistics, several rows in
+// One persistent CTA per SM, 18 warps:
+//   warps 0-7   epilogue, two teams of four warps (team t takes the 64-column groups j with j % 2 == t, so one team's TMEM
+//               loads / barriers hide behind the other's arithmetic): tcgen05.ld their TMEM lane quarter -> registers ->
+//               shared-memory staging tile (one per team) -> ONE TMA store per group: row-major 16-bit (128B swizzle),
+//               transposed 16-bit (V^T / outer-product operands, channel-major triangle operands, pair-bias heads: the
+//               tile is written to shared memory already transposed, the box is {y, ...}) or a TMA reduce-add into the fp32
+//               residual (the add happens at L2)
+//   warps 8-15  A producers (a_mode 0): warp-per-row LayerNorm with 128-bit loads and warp-shuffle statistics, several rows in
 //               flight per warp, result written as fp16/bf16 straight into the UMMA K-major 128B-swizzle layout
-//   warp 12     TMA: weight tiles [256 x 64] through a ring (and the A tile itself in a_mode 1, issued by warp 4)
-//   warp 13     TMEM allocation + the single MMA-issuing thread
+//   warp 16     TMA: weight tiles [256 x 64] through a ring (and the A tile itself in a_mode 1, issued by warp 8)
+//   warp 17     TMEM allocation + the single MMA-issuing thread
 // The A tile (128 rows x K) stays resident while all N tiles are swept, A is double buffered (the LayerNorm of tile t+1
 // overlaps the MMAs / epilogue of tile t) and so is the 128 x 256 fp32 accumulator in TMEM (2 x 256 columns).
 // A tile covers XT x YT rows so that every output — also a transposed residual — is one 4-D TMA box {cols, YT, XT, 1}.
@@ -21,6 +25,7 @@
 #include "pf_tc.cuh"
 
 #include <cuda_fp16.h>
+#include <cstdlib>
 #include <string>
 
 namespace pf {
@@ -29,7 +34,8 @@ int tma_encode(TmaCtx* ctx, CUtensorMap* out, const void* base, int elem_kind, i
                const uint64_t* strides_bytes, const uint32_t* box, int swizzle_bytes);
 
 constexpr int G2_BN = 256;
-constexpr int G2_THREADS = 14 * 32;
+constexpr int G2_THREADS = 18 * 32;
+constexpr int G2_EPI_WARPS = 8;
 constexpr int G2_PROD_WARPS = 8;
 
 struct G2Params {
@@ -55,6 +61,7 @@ struct G2Params {
   bf16* vt_out;
   int vt_cols;
   int Lpad;
+  int debug;
   G2Op ops[G2_MAX_OPS];
 };
 
@@ -71,7 +78,7 @@ struct G2Smem {
   static constexpr int ST_BYTES = 128 * 128;
   static constexpr int BIAS_OFF = ST_OFF + 2 * ST_BYTES;   // fp32 bias of the current 256-column window
   static constexpr int BAR_OFF = BIAS_OFF + G2_BN * 4;
-  static constexpr int TOTAL = BAR_OFF + 256 + 1024;
+  static constexpr int TOTAL = BAR_OFF + 192 + 1024;
 };
 
 struct TileCoord {
@@ -98,16 +105,46 @@ __device__ __forceinline__ uint32_t pack16(float a, float b, int fmt) {
   return *reinterpret_cast<uint32_t*>(&h);
 }
 
+
+// One 64-column row-major 16-bit output group of one tile row: TMEM -> (scale, bias, activation) -> 128B-swizzled staging row.
+template <int ACT, int FMT>
+__device__ __forceinline__ void g2_row16_group(uint32_t taddr, uint8_t* srow, const float* bias64, float scale, uint32_t sw) {
+#pragma unroll
+  for (int hf = 0; hf < 2; ++hf) {
+    uint32_t v[32];
+    tc::tmem_ld32(taddr + hf * 32, v);
+    tc::tmem_ld_wait();
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {
+      const float4 b0 = *reinterpret_cast<const float4*>(bias64 + hf * 32 + c * 8);
+      const float4 b1 = *reinterpret_cast<const float4*>(bias64 + hf * 32 + c * 8 + 4);
+      const float bb[8] = {b0.x, b0.y, b0.z, b0.w, b1.x, b1.y, b1.z, b1.w};
+      float f[8];
+#pragma unroll
+      for (int e = 0; e < 8; ++e) {
+        float xv = fmaf(__uint_as_float(v[c * 8 + e]), scale, bb[e]);
+        if (ACT == ACT_SIGMOID) xv = fast_sigmoid2(xv);
+        else if (ACT == ACT_RELU) xv = fmaxf(xv, 0.f);
+        f[e] = xv;
+      }
+      uint4 u = make_uint4(pack16(f[0], f[1], FMT), pack16(f[2], f[3], FMT), pack16(f[4], f[5], FMT),
+                           pack16(f[6], f[7], FMT));
+      *reinterpret_cast<uint4*>(srow + (((uint32_t)(hf * 4 + c) ^ sw) << 4)) = u;
+    }
+  }
+}
+
 template <int K, int AMODE>
 __global__ void __launch_bounds__(G2_THREADS, 1)
 gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUtensorMap tmA,
-             const __grid_constant__ CUtensorMap tmO0, const __grid_constant__ CUtensorMap tmO1,
+             const __grid_constant__ CUtensorMap tmO0, const __grid_constant__ CUtensorMap tmT0,
+             const __grid_constant__ CUtensorMap tmT1, const __grid_constant__ CUtensorMap tmH,
              const __grid_constant__ CUtensorMap tmR, const __grid_constant__ G2Params p) {
   using SM = G2Smem<K>;
   constexpr int KB = SM::KB;
   constexpr int WS = SM::W_STAGES;
   extern __shared__ uint8_t smem_raw[];
-  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+  uint8_t* smem = tc::align_smem_1024(smem_raw);
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem + SM::BAR_OFF);
   uint64_t* a_full = bars;             // [2]
   uint64_t* a_empty = bars + 2;        // [2]
@@ -119,17 +156,19 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
-  if (warp == 12 && lane == 0) {
+  if (warp == 16 && lane == 0) {
     tc::prefetch_tmap(&tmW);
     if (AMODE == 1) tc::prefetch_tmap(&tmA);
     tc::prefetch_tmap(&tmO0);
-    tc::prefetch_tmap(&tmO1);
+    tc::prefetch_tmap(&tmT0);
+    tc::prefetch_tmap(&tmT1);
+    tc::prefetch_tmap(&tmH);
     tc::prefetch_tmap(&tmR);
     for (int i = 0; i < 2; ++i) {
       tc::mbar_init(&a_full[i], AMODE == 0 ? G2_PROD_WARPS * 32 : 1);
       tc::mbar_init(&a_empty[i], 1);
       tc::mbar_init(&acc_full[i], 1);
-      tc::mbar_init(&acc_empty[i], 128);
+      tc::mbar_init(&acc_empty[i], G2_EPI_WARPS * 32);
     }
     for (int i = 0; i < WS; ++i) {
       tc::mbar_init(&w_full[i], 1);
@@ -137,21 +176,24 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
     }
     tc::fence_barrier_init();
   }
-  if (warp == 13) tc::tmem_alloc<512>(tmem_slot);
+  if (warp == 17) tc::tmem_alloc<512>(tmem_slot);
   tc::tc_fence_before();
   __syncthreads();
   tc::tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
 
-  if (warp < 4) {
-    // =========================================================== epilogue
-    const int lr = warp * 32 + lane;                   // tile row = TMEM lane
+  if (warp < G2_EPI_WARPS) {
+    // =========================================================== epilogue (two teams of four warps)
+    const int team = warp >> 2, quarter = warp & 3;
+    const int lr = quarter * 32 + lane;                // tile row = TMEM lane
+    const bool leader = (threadIdx.x & 127) == 0;
+    const int bar_id = 1 + team;
     const int xl = lr >> p.yt_shift, yl = lr & (p.YT - 1);
-    const uint32_t lane_addr = tmem_base + ((uint32_t)(warp * 32) << 16);
-    uint8_t* stage = smem + SM::ST_OFF;
+    const uint32_t lane_addr = tmem_base + ((uint32_t)(quarter * 32) << 16);
+    uint8_t* sb = smem + SM::ST_OFF + team * SM::ST_BYTES;   // this team's staging tile
+    bf16* sb16 = reinterpret_cast<bf16*>(sb);
     float* sbias = reinterpret_cast<float*>(smem + SM::BIAS_OFF);
     const uint32_t sw = (uint32_t)(lr & 7);
-    uint32_t sstep = 0;                                // staging steps issued so far
     uint32_t ac = 0;                                   // accumulator buffers consumed so far
     for (long tile = blockIdx.x; tile < p.num_tiles; tile += gridDim.x) {
       const TileCoord tcd = tile_coord(tile, p);
@@ -170,61 +212,50 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
         if (p.n_tiles > 1 || ac == 0) {
           // bias of this 256-column window -> shared memory (global loads here would sit on the epilogue's critical path:
           // the streaming LayerNorm loads keep evicting them from L1)
-          tc::named_bar_sync(1, 128);
-#pragma unroll
-          for (int e = 0; e < 2; ++e) {
-            const int n = nt * G2_BN + e * 128 + (int)threadIdx.x;
-            sbias[e * 128 + threadIdx.x] = (p.bias && n < p.Nw) ? __ldg(p.bias + n) : 0.f;
-          }
-          tc::named_bar_sync(1, 128);
+          tc::named_bar_sync(3, G2_EPI_WARPS * 32);
+          const int n = nt * G2_BN + (int)threadIdx.x;
+          sbias[threadIdx.x] = (p.bias && n < p.Nw) ? __ldg(p.bias + n) : 0.f;
+          tc::named_bar_sync(3, G2_EPI_WARPS * 32);
         }
         tc::mbar_wait(&acc_full[buf], (ac >> 1) & 1);
         tc::tc_fence_after();
         const uint32_t tacc = lane_addr + buf * G2_BN;
 #pragma unroll 1
-        for (int j = 0; j < 4; ++j) {
+        for (int j = team; j < 4; j += 2) {
           const G2Op& op = p.ops[nt * 4 + j];
           const int kind = op.kind;
           if (kind == G2_SKIP) continue;
+          if (kind == G2_ROW16 && (p.debug & 4)) continue;
           if (kind == G2_ROW16) {
-            uint8_t* sb = stage + (sstep & 1) * SM::ST_BYTES;
-            if (threadIdx.x == 0) tc::bulk_wait_read<1>();
-            tc::named_bar_sync(1, 128);
-            const float scale = op.scale;
-            const int act = op.act, fmt = op.fmt;
-#pragma unroll
-            for (int hf = 0; hf < 2; ++hf) {
-              uint32_t v[32];
-              tc::tmem_ld32(tacc + j * 64 + hf * 32, v);
-              tc::tmem_ld_wait();
-#pragma unroll
-              for (int c = 0; c < 4; ++c) {
-                float f[8];
-#pragma unroll
-                for (int e = 0; e < 8; ++e) {
-                  float xv = fmaf(__uint_as_float(v[c * 8 + e]), scale, sbias[j * 64 + hf * 32 + c * 8 + e]);
-                  if (act == ACT_SIGMOID) xv = fast_sigmoid2(xv);
-                  else if (act == ACT_RELU) xv = fmaxf(xv, 0.f);
-                  f[e] = xv;
-                }
-                uint4 u = make_uint4(pack16(f[0], f[1], fmt), pack16(f[2], f[3], fmt), pack16(f[4], f[5], fmt),
-                                     pack16(f[6], f[7], fmt));
-                *reinterpret_cast<uint4*>(sb + lr * 128 + (((uint32_t)(hf * 4 + c) ^ sw) << 4)) = u;
+            if (leader) tc::bulk_wait_read<0>();
+            tc::named_bar_sync(bar_id, 128);
+            {
+              const float scale = op.scale;
+              const uint32_t ta = tacc + j * 64;
+              uint8_t* srow = sb + lr * 128;
+              const float* b64 = sbias + j * 64;
+              if (op.act == ACT_SIGMOID) {
+                if (op.fmt) g2_row16_group<ACT_SIGMOID, 1>(ta, srow, b64, scale, sw);
+                else g2_row16_group<ACT_SIGMOID, 0>(ta, srow, b64, scale, sw);
+              } else if (op.act == ACT_RELU) {
+                if (op.fmt) g2_row16_group<ACT_RELU, 1>(ta, srow, b64, scale, sw);
+                else g2_row16_group<ACT_RELU, 0>(ta, srow, b64, scale, sw);
+              } else {
+                if (op.fmt) g2_row16_group<ACT_NONE, 1>(ta, srow, b64, scale, sw);
+                else g2_row16_group<ACT_NONE, 0>(ta, srow, b64, scale, sw);
               }
             }
             tc::fence_proxy_async_smem();
-            tc::named_bar_sync(1, 128);
-            if (threadIdx.x == 0) {
-              tc::tma_store_4d(op.map ? &tmO1 : &tmO0, sb, op.dst_col, tcd.y0, tcd.x0, tcd.b);
+            tc::named_bar_sync(bar_id, 128);
+            if (leader && !(p.debug & 1)) {
+              tc::tma_store_4d(&tmO0, sb, op.dst_col, tcd.y0, tcd.x0, tcd.b);
               tc::bulk_commit();
             }
-            ++sstep;
           } else if (kind == G2_RESID) {
 #pragma unroll 1
             for (int hf = 0; hf < 2; ++hf) {
-              uint8_t* sb = stage + (sstep & 1) * SM::ST_BYTES;
-              if (threadIdx.x == 0) tc::bulk_wait_read<1>();
-              tc::named_bar_sync(1, 128);
+              if (leader) tc::bulk_wait_read<0>();
+              tc::named_bar_sync(bar_id, 128);
               uint32_t v[32];
               tc::tmem_ld32(tacc + j * 64 + hf * 32, v);
               tc::tmem_ld_wait();
@@ -245,60 +276,75 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
                 *reinterpret_cast<float4*>(sb + lr * 128 + (((uint32_t)c ^ sw) << 4)) = make_float4(f[0], f[1], f[2], f[3]);
               }
               tc::fence_proxy_async_smem();
-              tc::named_bar_sync(1, 128);
-              if (threadIdx.x == 0) {
+              tc::named_bar_sync(bar_id, 128);
+              if (leader) {
                 tc::tma_reduce_add_4d(&tmR, sb, op.dst_col + hf * 32, tcd.y0, tcd.x0, tcd.b);
                 tc::bulk_commit();
               }
-              ++sstep;
             }
           } else if (kind == G2_CM_DUAL) {
-            bf16* base = p.cm_out[op.map] + (((long)tcd.b * p.cm_channels + op.dst_col) * p.D1 + x) * p.Lpad + y;
-            const long cstride = (long)p.D1 * p.Lpad;
+            // 64 channels of a gated, masked triangle operand, channel-major: staging tile [channel][x][y] (2-byte stores of
+            // consecutive lanes are consecutive in shared memory), one TMA store with box {YT, XT, 64, 1}
+            if (leader) tc::bulk_wait_read<0>();
+            tc::named_bar_sync(bar_id, 128);
 #pragma unroll 1
             for (int hf = 0; hf < 2; ++hf) {
               uint32_t v[32], g[32];
               tc::tmem_ld32(tacc + j * 64 + hf * 32, v);
               tc::tmem_ld32(tacc + 128 + j * 64 + hf * 32, g);
               tc::tmem_ld_wait();
-              if (valid) {
 #pragma unroll
-                for (int e = 0; e < 32; ++e) {
-                  const int n = j * 64 + hf * 32 + e;
-                  float pv = __uint_as_float(v[e]) + sbias[n];
-                  float gv = fast_sigmoid2(__uint_as_float(g[e]) + sbias[n + 128]);
-                  base[(hf * 32 + e) * cstride] = __float2bfloat16_rn(mask * gv * pv);
-                }
+              for (int e = 0; e < 32; ++e) {
+                const int n = j * 64 + hf * 32 + e;
+                float pv = __uint_as_float(v[e]) + sbias[n];
+                float gv = fast_sigmoid2(__uint_as_float(g[e]) + sbias[n + 128]);
+                sb16[(hf * 32 + e) * 128 + lr] = __float2bfloat16_rn(mask * gv * pv);
               }
             }
+            tc::fence_proxy_async_smem();
+            tc::named_bar_sync(bar_id, 128);
+            if (leader) {
+              tc::tma_store_4d(op.map ? &tmT1 : &tmT0, sb, tcd.y0, tcd.x0, op.dst_col, tcd.b);
+              tc::bulk_commit();
+            }
           } else if (kind == G2_HEADS) {
+            // pair-bias heads [b, head, x, y]: staging tile [head][x][y], box {YT, XT, n_heads, 1}
+            if (leader) tc::bulk_wait_read<0>();
+            tc::named_bar_sync(bar_id, 128);
             uint32_t v[32];
             tc::tmem_ld32(tacc + j * 64, v);
             tc::tmem_ld_wait();
-            if (valid) {
-              bf16* base = p.heads_out + (((long)tcd.b * p.n_heads + op.dst_col) * p.D1 + x) * p.Lpad + y;
-              const long hstride = (long)p.D1 * p.Lpad;
 #pragma unroll
-              for (int e = 0; e < 8; ++e)
-                if (e < op.ncols) base[e * hstride] = __float2bfloat16_rn(__uint_as_float(v[e]) * op.scale);
+            for (int e = 0; e < 8; ++e)
+              if (e < op.ncols) sb16[e * 128 + lr] = __float2bfloat16_rn(__uint_as_float(v[e]) * op.scale);
+            tc::fence_proxy_async_smem();
+            tc::named_bar_sync(bar_id, 128);
+            if (leader) {
+              tc::tma_store_4d(&tmH, sb, tcd.y0, tcd.x0, op.dst_col, tcd.b);
+              tc::bulk_commit();
             }
           } else {   // G2_VT
-            bf16* base = p.vt_out + (((long)tcd.b * p.D1 + x) * p.vt_cols + op.dst_col) * p.Lpad + y;
+            // 64 columns written transposed, [(b, x), column, y]: staging tile [x][column][y], box {YT, 64, XT, 1}
+            if (leader) tc::bulk_wait_read<0>();
+            tc::named_bar_sync(bar_id, 128);
             const float mk = op.masked ? mask : 1.0f;
+            bf16* dst = sb16 + ((long)xl * 64 << p.yt_shift) + yl;
 #pragma unroll 1
             for (int hf = 0; hf < 2; ++hf) {
               uint32_t v[32];
               tc::tmem_ld32(tacc + j * 64 + hf * 32, v);
               tc::tmem_ld_wait();
-              if (valid) {
 #pragma unroll
-                for (int e = 0; e < 32; ++e) {
-                  if (hf * 32 + e < op.ncols) {
-                    float xv = __uint_as_float(v[e]) + sbias[j * 64 + hf * 32 + e];
-                    base[(long)(hf * 32 + e) * p.Lpad] = __float2bfloat16_rn(xv * mk);
-                  }
-                }
+              for (int e = 0; e < 32; ++e) {
+                float xv = __uint_as_float(v[e]) + sbias[j * 64 + hf * 32 + e];
+                dst[(hf * 32 + e) << p.yt_shift] = __float2bfloat16_rn(xv * mk);
               }
+            }
+            tc::fence_proxy_async_smem();
+            tc::named_bar_sync(bar_id, 128);
+            if (leader) {
+              tc::tma_store_4d(&tmT0, sb, tcd.y0, op.dst_col, tcd.x0, tcd.b);
+              tc::bulk_commit();
             }
           }
         }
@@ -306,13 +352,13 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
         tc::mbar_arrive(&acc_empty[buf]);
       }
     }
-    if (threadIdx.x == 0) tc::bulk_wait<0>();
-  } else if (warp < 12) {
+    if (leader) tc::bulk_wait<0>();
+  } else if (warp < 16) {
     if (AMODE == 0) {
       // ========================================================= A producers: LayerNorm of gathered fp32 rows
       constexpr int NV = K / 128;                      // float4 per lane per row
-      constexpr int RU = 8;                            // rows in flight per warp
-      const int pw = warp - 4;
+      constexpr int RU = (K == 256) ? 4 : 8;           // rows in flight per warp
+      const int pw = warp - 8;
       float4 gm[NV], bt[NV];
 #pragma unroll
       for (int i = 0; i < NV; ++i) {
@@ -346,7 +392,7 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
           for (int u = 0; u < RU; ++u) {
             const int lr = pw * 16 + r0 + u;
             const int x = tcd.x0 + (lr >> p.yt_shift), y = tcd.y0 + (lr & (p.YT - 1));
-            if (x < p.D1 && y < p.D2) {
+            if (x < p.D1 && y < p.D2 && !(p.debug & 2)) {
               long srow = p.src_transposed ? ((long)tcd.b * p.D2 + y) * p.D1 + x : ((long)tcd.b * p.D1 + x) * p.D2 + y;
               const float4* xp = reinterpret_cast<const float4*>(p.src + srow * K);
 #pragma unroll
@@ -380,14 +426,14 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
               const int kb = 2 * i + (lane >> 4);
               const uint32_t chunk = (uint32_t)((lane & 15) >> 1);
               uint8_t* dst = abase + kb * SM::KB_BYTES + lr * 128 + ((chunk ^ (uint32_t)(lr & 7)) << 4) + (lane & 1) * 8;
-              *reinterpret_cast<uint2*>(dst) = make_uint2(pack16(o0, o1, p.op_fmt), pack16(o2, o3, p.op_fmt));
+              *reinterpret_cast<uint2*>(dst) = make_uint2(pack16(o0, o1, 1), pack16(o2, o3, 1));   // LN outputs are fp16 operands (R17)
             }
           }
         }
         tc::fence_proxy_async_smem();
         tc::mbar_arrive(&a_full[abuf]);
       }
-    } else if (warp == 4) {
+    } else if (warp == 8) {
       // ========================================================= A by TMA (a_mode 1)
       if (tc::elect_one()) {
         uint32_t it = 0;
@@ -403,7 +449,7 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
         }
       }
     }
-  } else if (warp == 12) {
+  } else if (warp == 16) {
     // ============================================================= weight tiles
     if (tc::elect_one()) {
       uint32_t wc = 0;
@@ -455,7 +501,7 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
   }
   tc::tc_fence_before();
   __syncthreads();
-  if (warp == 13) tc::tmem_dealloc<512>(tmem_base);
+  if (warp == 17) tc::tmem_dealloc<512>(tmem_base);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -476,8 +522,9 @@ static int pick_yt(int D2) {
 }
 
 template <int K, int AMODE>
-static int launch_g2(const CUtensorMap& tmW, const CUtensorMap& tmA, const CUtensorMap& tmO0, const CUtensorMap& tmO1,
-                     const CUtensorMap& tmR, const G2Params& p, int num_sms, cudaStream_t st) {
+static int launch_g2(const CUtensorMap& tmW, const CUtensorMap& tmA, const CUtensorMap& tmO0, const CUtensorMap& tmT0,
+                     const CUtensorMap& tmT1, const CUtensorMap& tmH, const CUtensorMap& tmR, const G2Params& p, int num_sms,
+                     cudaStream_t st) {
   auto kern = gemm2_kernel<K, AMODE>;
   static bool configured = false;
   if (!configured) {
@@ -489,7 +536,7 @@ static int launch_g2(const CUtensorMap& tmW, const CUtensorMap& tmA, const CUten
     configured = true;
   }
   unsigned grid = (unsigned)(p.num_tiles < (long)num_sms ? p.num_tiles : (long)num_sms);
-  kern<<<grid, G2_THREADS, G2Smem<K>::TOTAL, st>>>(tmW, tmA, tmO0, tmO1, tmR, p);
+  kern<<<grid, G2_THREADS, G2Smem<K>::TOTAL, st>>>(tmW, tmA, tmO0, tmT0, tmT1, tmH, tmR, p);
   return 0;
 }
 
@@ -524,43 +571,74 @@ int launch_gemm2(TmaCtx* ctx, const G2Desc& d, int num_sms, cudaStream_t st) {
   p.heads_out = reinterpret_cast<bf16*>(d.heads_out); p.n_heads = d.n_heads;
   p.vt_out = reinterpret_cast<bf16*>(d.vt_out); p.vt_cols = d.vt_cols;
   p.Lpad = d.Lpad;
+  { const char* dbg = getenv("PF_G2_DEBUG"); p.debug = dbg ? atoi(dbg) : 0; }
   bool need_bias = false;
   for (int i = 0; i < G2_MAX_OPS; ++i) {
     if (i < d.n_ops) p.ops[i] = d.ops[i];
     else p.ops[i].kind = G2_SKIP;
     if (p.ops[i].kind == G2_RESID || p.ops[i].kind == G2_CM_DUAL) need_bias = true;
   }
+  if (d.a_mode == 0 && d.op_fmt != 1) {
+    tc_set_error("gemm2: LayerNorm-fed GEMMs use fp16 operands");
+    return -1;
+  }
   if (need_bias && !d.bias) {
     tc_set_error("gemm2: residual / gated groups need a bias vector");
     return -1;
   }
 
-  CUtensorMap tmW, tmA, tmO[2], tmR;
+  CUtensorMap tmW, tmA, tmO0, tmT[2], tmH, tmR;
   const int ek = d.op_fmt ? 1 : 0;   // 0 bf16, 1 fp16, 2 fp32
   {
     uint64_t dims[2] = {(uint64_t)d.K, (uint64_t)d.Nw}, str[1] = {(uint64_t)d.K * 2};
     uint32_t box[2] = {64, G2_BN};
     if (tma_encode(ctx, &tmW, d.Wt, ek, 2, dims, str, box, 128) != 0) return -1;
   }
-  const uint64_t D1 = d.D1, D2 = d.D2, Bn = d.B;
+  const uint64_t D1 = d.D1, D2 = d.D2, Bn = d.B, Lp = d.Lpad;
+  const uint32_t YT = (uint32_t)p.YT, XT = (uint32_t)p.XT;
   if (d.a_mode == 1) {
     uint64_t dims[4] = {(uint64_t)d.K, D2, D1, Bn};
     uint64_t str[3] = {(uint64_t)d.K * 2, D2 * d.K * 2, D1 * D2 * d.K * 2};
-    uint32_t box[4] = {64, (uint32_t)p.YT, (uint32_t)p.XT, 1};
+    uint32_t box[4] = {64, YT, XT, 1};
     if (tma_encode(ctx, &tmA, d.A, ek, 4, dims, str, box, 128) != 0) return -1;
   } else {
     tmA = tmW;
   }
+  if (d.row_out[0]) {
+    uint64_t ld = d.row_ld[0];
+    uint64_t dims[4] = {ld, D2, D1, Bn};
+    uint64_t str[3] = {ld * 2, D2 * ld * 2, D1 * D2 * ld * 2};
+    uint32_t box[4] = {64, YT, XT, 1};
+    if (tma_encode(ctx, &tmO0, d.row_out[0], 0, 4, dims, str, box, 128) != 0) return -1;
+  } else {
+    tmO0 = tmW;
+  }
+  tmT[0] = tmT[1] = tmH = tmW;
+  if (d.vt_out && d.cm_out[0]) {
+    tc_set_error("gemm2: transposed-column and channel-major outputs cannot be combined");
+    return -1;
+  }
+  if (d.vt_out) {   // [(b, x), column, y] with row pitch Lpad: dims {y, column, x, b}
+    uint64_t vc = d.vt_cols;
+    uint64_t dims[4] = {D2, vc, D1, Bn};
+    uint64_t str[3] = {Lp * 2, vc * Lp * 2, D1 * vc * Lp * 2};
+    uint32_t box[4] = {YT, 64, XT, 1};
+    if (tma_encode(ctx, &tmT[0], d.vt_out, 0, 4, dims, str, box, 0) != 0) return -1;
+  }
   for (int i = 0; i < 2; ++i) {
-    if (d.row_out[i]) {
-      uint64_t ld = d.row_ld[i];
-      uint64_t dims[4] = {ld, D2, D1, Bn};
-      uint64_t str[3] = {ld * 2, D2 * ld * 2, D1 * D2 * ld * 2};
-      uint32_t box[4] = {64, (uint32_t)p.YT, (uint32_t)p.XT, 1};
-      if (tma_encode(ctx, &tmO[i], d.row_out[i], 0, 4, dims, str, box, 128) != 0) return -1;
-    } else {
-      tmO[i] = tmW;
-    }
+    if (!d.cm_out[i]) continue;   // [(b, channel), x, y] with row pitch Lpad: dims {y, x, channel, b}
+    uint64_t ch = d.cm_channels;
+    uint64_t dims[4] = {D2, D1, ch, Bn};
+    uint64_t str[3] = {Lp * 2, D1 * Lp * 2, ch * D1 * Lp * 2};
+    uint32_t box[4] = {YT, XT, 64, 1};
+    if (tma_encode(ctx, &tmT[i], d.cm_out[i], 0, 4, dims, str, box, 0) != 0) return -1;
+  }
+  if (d.heads_out) {   // [(b, head), x, y] with row pitch Lpad
+    uint64_t nh = d.n_heads;
+    uint64_t dims[4] = {D2, D1, nh, Bn};
+    uint64_t str[3] = {Lp * 2, D1 * Lp * 2, nh * D1 * Lp * 2};
+    uint32_t box[4] = {YT, XT, (uint32_t)d.n_heads, 1};
+    if (tma_encode(ctx, &tmH, d.heads_out, 0, 4, dims, str, box, 0) != 0) return -1;
   }
   if (d.resid) {
     uint64_t ld = d.resid_ld;
@@ -577,11 +655,11 @@ int launch_gemm2(TmaCtx* ctx, const G2Desc& d, int num_sms, cudaStream_t st) {
     tmR = tmW;
   }
   if (d.K == 128) {
-    return d.a_mode == 0 ? launch_g2<128, 0>(tmW, tmA, tmO[0], tmO[1], tmR, p, num_sms, st)
-                         : launch_g2<128, 1>(tmW, tmA, tmO[0], tmO[1], tmR, p, num_sms, st);
+    return d.a_mode == 0 ? launch_g2<128, 0>(tmW, tmA, tmO0, tmT[0], tmT[1], tmH, tmR, p, num_sms, st)
+                         : launch_g2<128, 1>(tmW, tmA, tmO0, tmT[0], tmT[1], tmH, tmR, p, num_sms, st);
   }
-  return d.a_mode == 0 ? launch_g2<256, 0>(tmW, tmA, tmO[0], tmO[1], tmR, p, num_sms, st)
-                       : launch_g2<256, 1>(tmW, tmA, tmO[0], tmO[1], tmR, p, num_sms, st);
+  return d.a_mode == 0 ? launch_g2<256, 0>(tmW, tmA, tmO0, tmT[0], tmT[1], tmH, tmR, p, num_sms, st)
+                       : launch_g2<256, 1>(tmW, tmA, tmO0, tmT[0], tmT[1], tmH, tmR, p, num_sms, st);
 }
 
 }  // namespace pf

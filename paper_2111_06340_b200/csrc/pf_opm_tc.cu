@@ -41,7 +41,7 @@ opm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ C
               const float* __restrict__ msa_mask, float* __restrict__ z, int S, int N) {
   using SM = OpmSmem;
   extern __shared__ uint8_t smem_raw[];
-  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+  uint8_t* smem = tc::align_smem_1024(smem_raw);
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem + SM::BAR_OFF);
   uint64_t* b_full = bars;
   uint64_t* a_full = bars + 1;                    // [OP_A_STAGES]

@@ -12,6 +12,12 @@ namespace tc {
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
+// 1024-byte aligned start of the dynamic shared memory window (the swizzled TMA / UMMA layouts need it).  Pointer
+// arithmetic on the __shared__ array keeps the address space known to the compiler (LDS / STS, not generic LD / ST).
+__device__ __forceinline__ uint8_t* align_smem_1024(uint8_t* raw) {
+  return raw + ((1024u - (smem_u32(raw) & 1023u)) & 1023u);
+}
+
 __device__ __forceinline__ bool elect_one() {
   uint32_t pred = 0;
   asm volatile(

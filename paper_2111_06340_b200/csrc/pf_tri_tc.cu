@@ -22,7 +22,7 @@ __global__ void __launch_bounds__(TRI_THREADS, 2)
 tri_einsum_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
                      float* __restrict__ t, int N, int Npad) {
   extern __shared__ uint8_t smem_raw[];
-  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+  uint8_t* smem = tc::align_smem_1024(smem_raw);
   uint64_t* full = reinterpret_cast<uint64_t*>(smem + TRI_BAR_OFF);
   uint64_t* empty = full + TRI_STAGES;
   uint64_t* tmem_full = empty + TRI_STAGES;
