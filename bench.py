@@ -219,7 +219,7 @@ def cpu_baseline(wl, wl_name, budget_s=25.0):
 # the CUDA path
 # ------------------------------------------------------------------------------------------------
 KIND_BOUND = {"gemm": "tensor", "attn_core": "tensor", "tri_einsum": "tensor", "opm_core": "tensor",
-              "ln_rows": "hbm", "ln_channels": "hbm", "ln_gemm": "hbm"}
+              "ln_rows": "hbm", "ln_channels": "hbm", "ln_gemm": "hbm", "transition": "tensor"}
 
 
 def roofline_from_profile(prof, peaks, n_steps):

@@ -126,6 +126,9 @@ struct G2Desc {
   int n_ops;
 };
 int launch_gemm2(TmaCtx* ctx, const G2Desc& d, int num_sms, cudaStream_t st);
+// fused transition (pf_trans_tc.cu): res[R, C] += relu(LN(res) W1 + b1) W2 + b2; w1t fp16 [4C, C], w2t bf16 [C, 4C]
+int launch_transition_tc(TmaCtx* ctx, float* res, long R, int C, const float* gamma, const float* beta, const void* w1t,
+                         const float* b1, const void* w2t, const float* b2, int num_sms, cudaStream_t st);
 int launch_attn_tc(TmaCtx* ctx, const bf16* qkg, const bf16* vt, const bf16* bias, const float* keymask, bf16* o,
                    int B, int R, int L, int Lpad, int H, int num_sms, cudaStream_t st);
 // ab_t: [(b,i), 64 channels (a | b), Spad] bf16 masked projections; wout_t: [c_z, c_opm*c_opm] bf16

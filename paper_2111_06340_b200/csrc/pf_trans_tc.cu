@@ -1,0 +1,436 @@
+// Fused transition on tcgen05 tensor cores (sm_100a) — SURVEY.md App. A.3 (MSA, C = 256) and A.9 (pair, C = 128):
+//     res[r, :] += relu(LayerNorm(res[r, :]) W1 + b1) W2 + b2,      W1: C -> 4C,  W2: 4C -> C
+// (north_star: "MSA and pair transitions fused with their residual adds"; §8(a) rows 3 / 9: "hidden stays on-chip").
+// The 4C-wide hidden activation never reaches HBM: per 128-row tile it is produced 128 columns at a time into TMEM
+// (GEMM1), rectified by the epilogue warps into a bf16 K-major shared-memory tile, and immediately consumed as the A
+// operand of GEMM2, which accumulates the C output columns in TMEM over the 4C/128 chunks.  HBM traffic per row is one
+// fp32 read and one fp32 reduce-add of C values (the algorithmic minimum 8C bytes + the L2-resident weights).
+//
+// One persistent CTA per SM, 18 warps:
+//   warps 0-7   epilogue, two teams of four warps.  E1(chunk): team t rectifies columns [64t, 64t+64) of the hidden chunk
+//               (TMEM -> +b1 -> relu -> bf16 -> k-block t of the A2 tile, UMMA 128B-swizzle layout).  E2(tile): the C output
+//               columns + b2 in 32-column fp32 boxes through staging tiles (the idle A2 buffers) -> TMA reduce-add into the
+//               residual (the add happens at L2).
+//   warps 8-15  LayerNorm producers: warp-per-row, 128-bit loads, warp-shuffle statistics, fp16 result straight into the
+//               UMMA K-major 128B-swizzle layout (A1); the next tile's rows are pulled into L2 by a bulk prefetch.
+//   warp 16     TMA: [128 x 64] weight tiles of W1^T / W2^T through one ring, in the order the MMA thread consumes them
+//   warp 17     TMEM allocation + the single MMA-issuing thread.  Issue order per tile: G1(0), G1(1), G2(0), G1(2), G2(1),
+//               ... so the rectification of chunk c overlaps GEMM1 of chunk c+1 (hidden accumulator double-buffered in TMEM).
+#include "pf_internal.h"
+#include "pf_device.cuh"
+#include "pf_tc.cuh"
+
+#include <cuda_fp16.h>
+#include <string>
+
+namespace pf {
+
+int tma_encode(TmaCtx* ctx, CUtensorMap* out, const void* base, int elem_kind, int rank, const uint64_t* dims,
+               const uint64_t* strides_bytes, const uint32_t* box, int swizzle_bytes);
+
+constexpr int TR_THREADS = 18 * 32;
+constexpr int TR_EPI_WARPS = 8;
+constexpr int TR_PROD_WARPS = 8;
+constexpr int TR_HC = 128;              // hidden columns per chunk
+
+template <int C>
+struct TrSmem {
+  static constexpr int KB1 = C / 64;                       // k-blocks of GEMM1 (K = C)
+  static constexpr int NH = C / 128;                       // 128-column halves of the output
+  static constexpr int A1_BUFS = (C == 128) ? 2 : 1;
+  static constexpr int A1_BYTES = 128 * C * 2;
+  static constexpr int KB_BYTES = 128 * 128;               // one [128 x 64] 16-bit k-block
+  static constexpr int A2_BYTES = 2 * KB_BYTES;            // hidden chunk [128 x 128] bf16
+  static constexpr int W_STAGE = KB_BYTES;                 // [128 rows x 64 k] 16-bit
+  static constexpr int W_STAGES = 5;
+  static constexpr int A1_OFF = 0;
+  static constexpr int A2_OFF = A1_OFF + A1_BUFS * A1_BYTES;
+  static constexpr int W_OFF = A2_OFF + 2 * A2_BYTES;
+  static constexpr int B1_OFF = W_OFF + W_STAGES * W_STAGE;   // fp32 b1 [4C]
+  static constexpr int B2_OFF = B1_OFF + 4 * C * 4;           // fp32 b2 [C]
+  static constexpr int BAR_OFF = B2_OFF + C * 4;
+  static constexpr int TOTAL = BAR_OFF + 256 + 1024;
+  static constexpr int TMEM_ACC2 = 256;                    // acc1[2] at columns 0 / 128, acc2 at [256, 256 + C)
+};
+
+struct TrParams {
+  const float* res;       // [R, C] fp32 residual (read for the LayerNorm; updated through the tensor map)
+  const float* gamma;
+  const float* beta;
+  const float* b1;        // [4C]
+  const float* b2;        // [C]
+  long R;
+  long num_tiles;
+};
+
+__device__ __forceinline__ uint32_t tr_pack_bf16(float a, float b) {
+  __nv_bfloat162 h = __floats2bfloat162_rn(a, b);
+  return *reinterpret_cast<uint32_t*>(&h);
+}
+__device__ __forceinline__ uint32_t tr_pack_f16(float a, float b) {
+  __half2 h = __floats2half2_rn(a, b);
+  return *reinterpret_cast<uint32_t*>(&h);
+}
+
+template <int C>
+__global__ void __launch_bounds__(TR_THREADS, 1)
+transition_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constant__ CUtensorMap tmW2,
+                  const __grid_constant__ CUtensorMap tmR, const __grid_constant__ TrParams p) {
+  using SM = TrSmem<C>;
+  constexpr int KB1 = SM::KB1, NH = SM::NH, WS = SM::W_STAGES, A1B = SM::A1_BUFS;
+  constexpr int NC = 4 * C / TR_HC;                        // hidden chunks per tile
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = tc::align_smem_1024(smem_raw);
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + SM::BAR_OFF);
+  uint64_t* a1_full = bars;                // [2]
+  uint64_t* a1_empty = bars + 2;           // [2]
+  uint64_t* w_full = bars + 4;             // [WS]
+  uint64_t* w_empty = w_full + WS;         // [WS]
+  uint64_t* acc1_full = w_empty + WS;      // [2]
+  uint64_t* acc1_empty = acc1_full + 2;    // [2]
+  uint64_t* a2_full = acc1_empty + 2;      // [2]
+  uint64_t* a2_empty = a2_full + 2;        // [2]
+  uint64_t* acc2_full = a2_empty + 2;      // 1
+  uint64_t* acc2_empty = acc2_full + 1;    // 1
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(acc2_empty + 1);
+  float* sb1 = reinterpret_cast<float*>(smem + SM::B1_OFF);
+  float* sb2 = reinterpret_cast<float*>(smem + SM::B2_OFF);
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+  if (warp == 16 && lane == 0) {
+    tc::prefetch_tmap(&tmW1);
+    tc::prefetch_tmap(&tmW2);
+    tc::prefetch_tmap(&tmR);
+    for (int i = 0; i < 2; ++i) {
+      tc::mbar_init(&a1_full[i], TR_PROD_WARPS * 32);
+      tc::mbar_init(&a1_empty[i], 1);
+      tc::mbar_init(&acc1_full[i], 1);
+      tc::mbar_init(&acc1_empty[i], TR_EPI_WARPS * 32);
+      tc::mbar_init(&a2_full[i], TR_EPI_WARPS * 32);
+      tc::mbar_init(&a2_empty[i], 1);
+    }
+    for (int i = 0; i < WS; ++i) {
+      tc::mbar_init(&w_full[i], 1);
+      tc::mbar_init(&w_empty[i], 1);
+    }
+    tc::mbar_init(acc2_full, 1);
+    tc::mbar_init(acc2_empty, TR_EPI_WARPS * 32);
+    tc::fence_barrier_init();
+  }
+  if (warp == 17) tc::tmem_alloc<512>(tmem_slot);
+  for (int i = threadIdx.x; i < 4 * C; i += TR_THREADS) sb1[i] = __ldg(p.b1 + i);
+  for (int i = threadIdx.x; i < C; i += TR_THREADS) sb2[i] = __ldg(p.b2 + i);
+  tc::tc_fence_before();
+  __syncthreads();
+  tc::tc_fence_after();
+  const uint32_t tmem_base = *tmem_slot;
+
+  if (warp < TR_EPI_WARPS) {
+    // =========================================================== epilogue (two teams of four warps)
+    const int team = warp >> 2, quarter = warp & 3;
+    const int lr = quarter * 32 + lane;                // tile row = TMEM lane
+    const bool leader = (threadIdx.x & 127) == 0;
+    const int bar_id = 1 + team;
+    const uint32_t lane_addr = tmem_base + ((uint32_t)(quarter * 32) << 16);
+    const uint32_t sw = (uint32_t)(lr & 7);
+    uint32_t cc = 0;                                   // hidden chunks consumed so far (all tiles)
+    uint32_t it = 0;
+    for (long tile = blockIdx.x; tile < p.num_tiles; tile += gridDim.x, ++it) {
+#pragma unroll 1
+      for (int c = 0; c < NC; ++c, ++cc) {
+        const uint32_t buf = cc & 1, ph = (cc >> 1) & 1;
+        tc::mbar_wait(&acc1_full[buf], ph);
+        tc::tc_fence_after();
+        tc::mbar_wait(&a2_empty[buf], ph ^ 1);         // GEMM2 of the chunk two steps back has read this A2 buffer
+        if (c < 2) {
+          // the previous tile's E2 staged its output in this A2 buffer: its TMA reads must be complete
+          if (leader) tc::bulk_wait_read<0>();
+          tc::named_bar_sync(bar_id, 128);
+        }
+        uint8_t* arow = smem + SM::A2_OFF + buf * SM::A2_BYTES + team * SM::KB_BYTES + lr * 128;
+        const float* bb = sb1 + c * TR_HC + team * 64;
+        const uint32_t ta = lane_addr + buf * TR_HC + team * 64;
+#pragma unroll
+        for (int hf = 0; hf < 2; ++hf) {
+          uint32_t v[32];
+          tc::tmem_ld32(ta + hf * 32, v);
+          tc::tmem_ld_wait();
+#pragma unroll
+          for (int q = 0; q < 4; ++q) {
+            const float4 b0 = *reinterpret_cast<const float4*>(bb + hf * 32 + q * 8);
+            const float4 b1v = *reinterpret_cast<const float4*>(bb + hf * 32 + q * 8 + 4);
+            uint4 u;
+            u.x = tr_pack_bf16(fmaxf(__uint_as_float(v[q * 8 + 0]) + b0.x, 0.f), fmaxf(__uint_as_float(v[q * 8 + 1]) + b0.y, 0.f));
+            u.y = tr_pack_bf16(fmaxf(__uint_as_float(v[q * 8 + 2]) + b0.z, 0.f), fmaxf(__uint_as_float(v[q * 8 + 3]) + b0.w, 0.f));
+            u.z = tr_pack_bf16(fmaxf(__uint_as_float(v[q * 8 + 4]) + b1v.x, 0.f), fmaxf(__uint_as_float(v[q * 8 + 5]) + b1v.y, 0.f));
+            u.w = tr_pack_bf16(fmaxf(__uint_as_float(v[q * 8 + 6]) + b1v.z, 0.f), fmaxf(__uint_as_float(v[q * 8 + 7]) + b1v.w, 0.f));
+            *reinterpret_cast<uint4*>(arow + (((uint32_t)(hf * 4 + q) ^ sw) << 4)) = u;
+          }
+        }
+        tc::tc_fence_before();
+        tc::mbar_arrive(&acc1_empty[buf]);
+        tc::fence_proxy_async_smem();
+        tc::mbar_arrive(&a2_full[buf]);
+      }
+      // ---- E2: output columns + b2 -> fp32 staging (this team's A2 buffer, two 16 KB boxes) -> TMA reduce-add
+      tc::mbar_wait(acc2_full, it & 1);                // all GEMM2 of this tile complete: acc2 final, A2 buffers idle
+      tc::tc_fence_after();
+      // staging boxes: k-block `team` of both A2 buffers — the region only this team writes in E1, so the team leader's
+      // own bulk-group bookkeeping covers every reuse
+      uint8_t* stage = smem + SM::A2_OFF + team * SM::KB_BYTES;
+      int nbox = 0;
+#pragma unroll 1
+      for (int bx = team; bx < C / 32; bx += 2, ++nbox) {
+        uint8_t* sb = stage + (nbox & 1) * SM::A2_BYTES;
+        if (nbox >= 2) {
+          if (leader) tc::bulk_wait_read<1>();
+          tc::named_bar_sync(bar_id, 128);
+        }
+        uint32_t v[32];
+        tc::tmem_ld32(lane_addr + SM::TMEM_ACC2 + bx * 32, v);
+        tc::tmem_ld_wait();
+#pragma unroll
+        for (int q = 0; q < 8; ++q) {
+          const float4 b = *reinterpret_cast<const float4*>(sb2 + bx * 32 + q * 4);
+          *reinterpret_cast<float4*>(sb + lr * 128 + (((uint32_t)q ^ sw) << 4)) =
+              make_float4(__uint_as_float(v[q * 4 + 0]) + b.x, __uint_as_float(v[q * 4 + 1]) + b.y,
+                          __uint_as_float(v[q * 4 + 2]) + b.z, __uint_as_float(v[q * 4 + 3]) + b.w);
+        }
+        tc::fence_proxy_async_smem();
+        tc::named_bar_sync(bar_id, 128);
+        if (leader) {
+          tc::tma_reduce_add_2d(&tmR, sb, bx * 32, (int)(tile * 128));
+          tc::bulk_commit();
+        }
+      }
+      tc::tc_fence_before();
+      tc::mbar_arrive(acc2_empty);
+    }
+    if (leader) tc::bulk_wait<0>();
+  } else if (warp < 16) {
+    // ============================================================= A1 producers: LayerNorm of fp32 rows
+    constexpr int NV = C / 128;                        // float4 per lane per row
+    constexpr int RU = (C == 256) ? 4 : 8;             // rows in flight per warp
+    const int pw = warp - 8;
+    float4 gm[NV], bt[NV];
+#pragma unroll
+    for (int i = 0; i < NV; ++i) {
+      gm[i] = __ldg(reinterpret_cast<const float4*>(p.gamma) + lane + 32 * i);
+      bt[i] = __ldg(reinterpret_cast<const float4*>(p.beta) + lane + 32 * i);
+    }
+    uint32_t it = 0;
+    for (long tile = blockIdx.x; tile < p.num_tiles; tile += gridDim.x, ++it) {
+      const uint32_t abuf = it % A1B;
+      {
+        const long nxt = tile + gridDim.x;             // next tile's 16 rows of this warp -> L2
+        const long r0 = nxt * 128 + pw * 16;
+        if (nxt < p.num_tiles && lane == 0 && r0 < p.R) {
+          long n = p.R - r0 < 16 ? p.R - r0 : 16;
+          tc::prefetch_l2_bulk(p.res + r0 * C, (uint32_t)(n * C * 4));
+        }
+      }
+      tc::mbar_wait(&a1_empty[abuf], ((it / A1B) & 1) ^ 1);
+      uint8_t* abase = smem + SM::A1_OFF + abuf * SM::A1_BYTES;
+#pragma unroll 1
+      for (int r0 = 0; r0 < 16; r0 += RU) {
+        float4 v[RU][NV];
+#pragma unroll
+        for (int u = 0; u < RU; ++u) {
+          const int lr = pw * 16 + r0 + u;
+          const long r = tile * 128 + lr;
+          if (r < p.R) {
+            const float4* xp = reinterpret_cast<const float4*>(p.res + r * C);
+#pragma unroll
+            for (int i = 0; i < NV; ++i) v[u][i] = ld_nc_f4(xp + lane + 32 * i);
+          } else {
+#pragma unroll
+            for (int i = 0; i < NV; ++i) v[u][i] = make_float4(0.f, 0.f, 0.f, 0.f);
+          }
+        }
+#pragma unroll
+        for (int u = 0; u < RU; ++u) {
+          const int lr = pw * 16 + r0 + u;
+          float s = 0.f;
+#pragma unroll
+          for (int i = 0; i < NV; ++i) s += v[u][i].x + v[u][i].y + v[u][i].z + v[u][i].w;
+          const float mean = warp_sum(s) * (1.0f / C);
+          float q = 0.f;
+#pragma unroll
+          for (int i = 0; i < NV; ++i) {
+            float a = v[u][i].x - mean, b2 = v[u][i].y - mean, c = v[u][i].z - mean, d = v[u][i].w - mean;
+            q += a * a + b2 * b2 + c * c + d * d;
+          }
+          const float rstd = rsqrtf(warp_sum(q) * (1.0f / C) + 1e-5f);
+#pragma unroll
+          for (int i = 0; i < NV; ++i) {
+            float o0 = (v[u][i].x - mean) * rstd * gm[i].x + bt[i].x;
+            float o1 = (v[u][i].y - mean) * rstd * gm[i].y + bt[i].y;
+            float o2 = (v[u][i].z - mean) * rstd * gm[i].z + bt[i].z;
+            float o3 = (v[u][i].w - mean) * rstd * gm[i].w + bt[i].w;
+            // columns 128 i + 4 lane .. +3  ->  k-block 2 i + lane / 16, 16-byte chunk (lane % 16) / 2, half lane & 1
+            const int kb = 2 * i + (lane >> 4);
+            const uint32_t chunk = (uint32_t)((lane & 15) >> 1);
+            uint8_t* dst = abase + kb * SM::KB_BYTES + lr * 128 + ((chunk ^ (uint32_t)(lr & 7)) << 4) + (lane & 1) * 8;
+            *reinterpret_cast<uint2*>(dst) = make_uint2(tr_pack_f16(o0, o1), tr_pack_f16(o2, o3));   // fp16 operand (R17)
+          }
+        }
+      }
+      tc::fence_proxy_async_smem();
+      tc::mbar_arrive(&a1_full[abuf]);
+    }
+  } else if (warp == 16) {
+    // ============================================================= weight tiles, in the MMA thread's consumption order
+    if (tc::elect_one()) {
+      uint32_t wc = 0;
+      auto load = [&](const CUtensorMap* m, int k0, int row0) {
+        const uint32_t s = wc % WS;
+        tc::mbar_wait(&w_empty[s], ((wc / WS) & 1) ^ 1);
+        tc::mbar_arrive_expect_tx(&w_full[s], SM::W_STAGE);
+        tc::tma_load_2d(smem + SM::W_OFF + s * SM::W_STAGE, m, &w_full[s], k0, row0);
+        ++wc;
+      };
+      auto g1 = [&](int c) {   // W1^T [4C, C]: rows = hidden columns of the chunk
+        for (int kb = 0; kb < KB1; ++kb) load(&tmW1, kb * 64, c * TR_HC);
+      };
+      auto g2 = [&](int c) {   // W2^T [C, 4C]: rows = output columns, k = hidden columns of the chunk
+        for (int kb = 0; kb < 2; ++kb)
+          for (int nh = 0; nh < NH; ++nh) load(&tmW2, c * TR_HC + kb * 64, nh * 128);
+      };
+      for (long tile = blockIdx.x; tile < p.num_tiles; tile += gridDim.x) {
+        g1(0);
+        for (int c = 1; c < NC; ++c) {
+          g1(c);
+          g2(c - 1);
+        }
+        g2(NC - 1);
+      }
+    }
+  } else {
+    // ============================================================= MMA issue
+    if (tc::elect_one()) {
+      constexpr uint32_t idesc1 = tc::idesc_f16_f32(128, 128);    // GEMM1: fp16 LayerNorm output x fp16 W1
+      constexpr uint32_t idesc2 = tc::idesc_bf16_f32(128, 128);   // GEMM2: bf16 hidden x bf16 W2
+      uint32_t wc = 0, c1 = 0, c2 = 0, it = 0;
+      const uint32_t acc2 = tmem_base + SM::TMEM_ACC2;
+      for (long tile = blockIdx.x; tile < p.num_tiles; tile += gridDim.x, ++it) {
+        const uint32_t abuf = it % A1B;
+        const uint32_t a1_addr = tc::smem_u32(smem + SM::A1_OFF + abuf * SM::A1_BYTES);
+        auto gemm1 = [&](int c) {
+          const uint32_t buf = c1 & 1;
+          tc::mbar_wait(&acc1_empty[buf], ((c1 >> 1) & 1) ^ 1);
+          tc::tc_fence_after();
+          const uint32_t d = tmem_base + buf * TR_HC;
+#pragma unroll 1
+          for (int kb = 0; kb < KB1; ++kb, ++wc) {
+            const uint32_t s = wc % WS;
+            tc::mbar_wait(&w_full[s], (wc / WS) & 1);
+            tc::tc_fence_after();
+            const uint64_t a_desc = tc::smem_desc_kmajor<128>(a1_addr + kb * SM::KB_BYTES);
+            const uint64_t b_desc = tc::smem_desc_kmajor<128>(tc::smem_u32(smem + SM::W_OFF + s * SM::W_STAGE));
+#pragma unroll
+            for (int k = 0; k < 4; ++k) tc::mma_bf16(d, a_desc + 2 * k, b_desc + 2 * k, idesc1, (kb | k) != 0);
+            tc::mma_commit(&w_empty[s]);
+          }
+          tc::mma_commit(&acc1_full[buf]);
+          ++c1;
+          (void)c;
+        };
+        auto gemm2 = [&](int c) {
+          const uint32_t buf = c2 & 1;
+          tc::mbar_wait(&a2_full[buf], (c2 >> 1) & 1);
+          tc::tc_fence_after();
+          const uint32_t a2_addr = tc::smem_u32(smem + SM::A2_OFF + buf * SM::A2_BYTES);
+#pragma unroll 1
+          for (int kb = 0; kb < 2; ++kb) {
+            const uint64_t a_desc = tc::smem_desc_kmajor<128>(a2_addr + kb * SM::KB_BYTES);
+#pragma unroll 1
+            for (int nh = 0; nh < NH; ++nh, ++wc) {
+              const uint32_t s = wc % WS;
+              tc::mbar_wait(&w_full[s], (wc / WS) & 1);
+              tc::tc_fence_after();
+              const uint64_t b_desc = tc::smem_desc_kmajor<128>(tc::smem_u32(smem + SM::W_OFF + s * SM::W_STAGE));
+#pragma unroll
+              for (int k = 0; k < 4; ++k)
+                tc::mma_bf16(acc2 + nh * 128, a_desc + 2 * k, b_desc + 2 * k, idesc2, (c | kb | k) != 0);
+              tc::mma_commit(&w_empty[s]);
+            }
+          }
+          tc::mma_commit(&a2_empty[buf]);
+          ++c2;
+        };
+        tc::mbar_wait(&a1_full[abuf], (it / A1B) & 1);
+        tc::tc_fence_after();
+        gemm1(0);
+        for (int c = 1; c < NC; ++c) {
+          gemm1(c);
+          if (c == NC - 1) tc::mma_commit(&a1_empty[abuf]);   // every GEMM1 of this tile has been issued: A1 is free when they finish
+          if (c == 1) {
+            // acc2 of the previous tile must have been drained by E2 before the first GEMM2 overwrites it
+            tc::mbar_wait(acc2_empty, (it & 1) ^ 1);
+            tc::tc_fence_after();
+          }
+          gemm2(c - 1);
+        }
+        gemm2(NC - 1);
+        tc::mma_commit(acc2_full);
+      }
+    }
+  }
+  tc::tc_fence_before();
+  __syncthreads();
+  if (warp == 17) tc::tmem_dealloc<512>(tmem_base);
+}
+
+// ------------------------------------------------------------------------------------------------
+// host
+// ------------------------------------------------------------------------------------------------
+template <int C>
+static int launch_tr(const CUtensorMap& tmW1, const CUtensorMap& tmW2, const CUtensorMap& tmR, const TrParams& p, int num_sms,
+                     cudaStream_t st) {
+  auto kern = transition_kernel<C>;
+  static bool configured = false;
+  if (!configured) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, TrSmem<C>::TOTAL);
+    if (e != cudaSuccess) {
+      tc_set_error(std::string("cudaFuncSetAttribute(transition): ") + cudaGetErrorString(e));
+      return -1;
+    }
+    configured = true;
+  }
+  unsigned grid = (unsigned)(p.num_tiles < (long)num_sms ? p.num_tiles : (long)num_sms);
+  kern<<<grid, TR_THREADS, TrSmem<C>::TOTAL, st>>>(tmW1, tmW2, tmR, p);
+  return 0;
+}
+
+// w1t: fp16 [4C, C] (K = C contiguous); w2t: bf16 [C, 4C] (K = 4C contiguous); res: fp32 [R, C] updated in place.
+int launch_transition_tc(TmaCtx* ctx, float* res, long R, int C, const float* gamma, const float* beta, const void* w1t,
+                         const float* b1, const void* w2t, const float* b2, int num_sms, cudaStream_t st) {
+  if (C != 128 && C != 256) {
+    tc_set_error("transition_tc: C must be 128 or 256");
+    return -1;
+  }
+  TrParams p;
+  p.res = res; p.gamma = gamma; p.beta = beta; p.b1 = b1; p.b2 = b2;
+  p.R = R;
+  p.num_tiles = (R + 127) / 128;
+  CUtensorMap tmW1, tmW2, tmR;
+  {
+    uint64_t dims[2] = {(uint64_t)C, (uint64_t)4 * C}, str[1] = {(uint64_t)C * 2};
+    uint32_t box[2] = {64, 128};
+    if (tma_encode(ctx, &tmW1, w1t, 1, 2, dims, str, box, 128) != 0) return -1;
+  }
+  {
+    uint64_t dims[2] = {(uint64_t)4 * C, (uint64_t)C}, str[1] = {(uint64_t)4 * C * 2};
+    uint32_t box[2] = {64, 128};
+    if (tma_encode(ctx, &tmW2, w2t, 0, 2, dims, str, box, 128) != 0) return -1;
+  }
+  {
+    uint64_t dims[2] = {(uint64_t)C, (uint64_t)R}, str[1] = {(uint64_t)C * 4};
+    uint32_t box[2] = {32, 128};
+    if (tma_encode(ctx, &tmR, res, 2, 2, dims, str, box, 128) != 0) return -1;
+  }
+  return C == 128 ? launch_tr<128>(tmW1, tmW2, tmR, p, num_sms, st) : launch_tr<256>(tmW1, tmW2, tmR, p, num_sms, st);
+}
+
+}  // namespace pf

@@ -232,30 +232,13 @@ struct TcDriver {
     return gemm2(d, R * C * 8.0);
   }
 
+  // A.3 / A.9: one fused kernel, the 4C-wide hidden activation stays on chip
   bool transition_substep(float* res, int D1, int D2, int C, const TransW& t, size_t w1t, size_t w2t) {
-    const int n4 = h->cfg.transition_n * C;
-    const long R = (long)B * D1 * D2;
-    bf16* Hb = buf<bf16>(ar.qkg);
-    G2Desc d = desc_base(B, D1, D2, C, n4);
-    d.src = res; d.gamma = w + t.ln_g; d.beta = w + t.ln_b;
-    d.op_fmt = 1; d.Wt = w16 + w1t; d.bias = w + t.b1;
-    d.row_out[0] = Hb; d.row_ld[0] = n4;
-    int n = 0;
-    for (int col = 0; col < n4; col += 64, ++n) {
-      d.ops[n] = op(G2_ROW16, col);
-      d.ops[n].act = ACT_RELU;
-    }
-    d.n_ops = n;
-    if (!gemm2(d, (double)R * n4 * 2.0)) return false;
-    Epi e;
-    memset(&e, 0, sizeof(e));
-    e.kind = EPI_RESID; e.scale = 1.0f; e.vt_from = 1 << 30;
-    e.geom = RowGeom{1, 1, (int)R};
-    e.bias = w + t.b2;
-    e.resid = res; e.ldr = C;
-    h->prof_begin(KK_GEMM, 2.0 * R * n4 * C, (double)R * n4 * 2.0 + (double)R * C * 8.0 + 2.0 * n4 * C, st);
-    if (launch_gemm_tc(h->tma, Hb, n4, reinterpret_cast<const bf16*>(w16 + w2t), R, n4, C, e, h->num_sms, st) != 0) {
-      err = std::string("gemm_tc: ") + tc_last_error();
+    const double R = (double)B * D1 * D2, n4 = (double)h->cfg.transition_n * C;
+    h->prof_begin(KK_TRANS, 4.0 * R * n4 * C, R * C * 8.0 + 4.0 * n4 * C, st);
+    if (launch_transition_tc(h->tma, res, (long)B * D1 * D2, C, w + t.ln_g, w + t.ln_b, w16 + w1t, w + t.b1, w16 + w2t,
+                             w + t.b2, h->num_sms, st) != 0) {
+      err = std::string("transition_tc: ") + tc_last_error();
       return false;
     }
     h->prof_end(st);
