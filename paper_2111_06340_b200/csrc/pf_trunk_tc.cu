@@ -3,7 +3,8 @@
 // LayerNorm outputs and the weights they multiply are fp16 operands (bounded by construction; the weight values are the
 // bf16-rounded ones of R15, exactly representable), sigmoid gates are stored as fp16 (never an MMA operand), every other
 // intermediate (q, k, v, P, o, transition hidden, triangle operands, outer-product operands, pair bias) is bf16.
-// No arithmetic of the method lives here except the constant 1/sqrt(head_dim) handed to the q projection (R12).
+// No arithmetic of the method lives here except two constants handed to the projection epilogues: log2(e)/sqrt(head_dim) on q
+// (R12) and log2(e) on the pair bias, so that the attention kernel's softmax runs in the exp2 domain.
 #include "pf_handle.h"
 
 #include <cstring>
@@ -129,6 +130,8 @@ void build_tc_block(const pf_config& c, const BlockW& off, const TcBlock& t, con
 // ------------------------------------------------------------------------------------------------
 namespace {
 
+constexpr float kLog2e = 1.4426950408889634f;
+
 struct TcDriver {
   pf_evoformer* h;
   cudaStream_t st;
@@ -188,6 +191,7 @@ struct TcDriver {
       d.op_fmt = 1; d.Wt = w16 + h->tc.row_wbias;
       d.heads_out = BIAS; d.n_heads = c.heads_msa; d.Lpad = pad8(N);
       d.ops[0] = op(G2_HEADS, 0, c.heads_msa);
+      d.ops[0].scale = kLog2e;
       d.n_ops = 1;
       if (!gemm2(d, (double)B * N * N * c.heads_msa * 2.0)) return false;
     }
@@ -204,13 +208,16 @@ struct TcDriver {
         int seg = col / C;
         if (seg < 3) {
           d.ops[n] = op(G2_ROW16, col);
-          if (seg == 0) d.ops[n].scale = 0.17677669529663687f;   // 1/sqrt(32)  (R12)
+          if (seg == 0) d.ops[n].scale = 0.17677669529663687f * kLog2e;   // log2(e)/sqrt(32)  (R12)
           if (seg == 2) { d.ops[n].act = ACT_SIGMOID; d.ops[n].fmt = 1; }
         } else {
           d.ops[n] = op(G2_VT, col - 3 * C);
         }
       }
-      if (self_bias) d.ops[n++] = op(G2_HEADS, 0, H);   // A.7 / A.8: beta from the same LN(z) rows
+      if (self_bias) {   // A.7 / A.8: beta from the same LN(z) rows
+        d.ops[n] = op(G2_HEADS, 0, H);
+        d.ops[n++].scale = kLog2e;
+      }
       d.n_ops = n;
       if (!gemm2(d, R * 4.0 * C * 2.0 + (self_bias ? R * H * 2.0 : 0.0))) return false;
     }
