@@ -94,7 +94,25 @@ __device__ __forceinline__ TileCoord tile_coord(long t, const G2Params& p) {
   return c;
 }
 
-__device__ __forceinline__ float fast_sigmoid2(float x) { return __fdividef(1.0f, 1.0f + __expf(-x)); }
+// sigmoid through the two MUFU approximations (ex2, rcp), flush-to-zero: 4 instructions, ~1e-6 relative error
+__device__ __forceinline__ float fast_sigmoid2(float x) {
+  float e, r;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(x * -1.4426950408889634f));
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(1.0f + e));
+  return r;
+}
+// 32 consecutive fp32 values from shared memory into registers (eight 128-bit loads).  Epilogue groups fetch their bias this
+// way BEFORE the arithmetic: a shared-memory load placed between the staging stores could not be moved across them.
+__device__ __forceinline__ void lds32(const float* src, float (&dst)[32]) {
+#pragma unroll
+  for (int q = 0; q < 8; ++q) {
+    const float4 t = *reinterpret_cast<const float4*>(src + q * 4);
+    dst[q * 4 + 0] = t.x;
+    dst[q * 4 + 1] = t.y;
+    dst[q * 4 + 2] = t.z;
+    dst[q * 4 + 3] = t.w;
+  }
+}
 
 __device__ __forceinline__ uint32_t pack16(float a, float b, int fmt) {
   if (fmt) {
@@ -112,25 +130,27 @@ __device__ __forceinline__ void g2_row16_group(uint32_t taddr, uint8_t* srow, co
 #pragma unroll
   for (int hf = 0; hf < 2; ++hf) {
     uint32_t v[32];
+    float bb[32];
     tc::tmem_ld32(taddr + hf * 32, v);
+    lds32(bias64 + hf * 32, bb);
     tc::tmem_ld_wait();
+    uint32_t pk[16];
 #pragma unroll
-    for (int c = 0; c < 4; ++c) {
-      const float4 b0 = *reinterpret_cast<const float4*>(bias64 + hf * 32 + c * 8);
-      const float4 b1 = *reinterpret_cast<const float4*>(bias64 + hf * 32 + c * 8 + 4);
-      const float bb[8] = {b0.x, b0.y, b0.z, b0.w, b1.x, b1.y, b1.z, b1.w};
-      float f[8];
-#pragma unroll
-      for (int e = 0; e < 8; ++e) {
-        float xv = fmaf(__uint_as_float(v[c * 8 + e]), scale, bb[e]);
-        if (ACT == ACT_SIGMOID) xv = fast_sigmoid2(xv);
-        else if (ACT == ACT_RELU) xv = fmaxf(xv, 0.f);
-        f[e] = xv;
+    for (int e = 0; e < 32; e += 2) {
+      float x0 = fmaf(__uint_as_float(v[e]), scale, bb[e]), x1 = fmaf(__uint_as_float(v[e + 1]), scale, bb[e + 1]);
+      if (ACT == ACT_SIGMOID) {
+        x0 = fast_sigmoid2(x0);
+        x1 = fast_sigmoid2(x1);
+      } else if (ACT == ACT_RELU) {
+        x0 = fmaxf(x0, 0.f);
+        x1 = fmaxf(x1, 0.f);
       }
-      uint4 u = make_uint4(pack16(f[0], f[1], FMT), pack16(f[2], f[3], FMT), pack16(f[4], f[5], FMT),
-                           pack16(f[6], f[7], FMT));
-      *reinterpret_cast<uint4*>(srow + (((uint32_t)(hf * 4 + c) ^ sw) << 4)) = u;
+      pk[e >> 1] = pack16(x0, x1, FMT);
     }
+#pragma unroll
+    for (int c = 0; c < 4; ++c)
+      *reinterpret_cast<uint4*>(srow + (((uint32_t)(hf * 4 + c) ^ sw) << 4)) =
+          make_uint4(pk[c * 4], pk[c * 4 + 1], pk[c * 4 + 2], pk[c * 4 + 3]);
   }
 }
 
@@ -257,24 +277,35 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
               if (leader) tc::bulk_wait_read<0>();
               tc::named_bar_sync(bar_id, 128);
               uint32_t v[32];
+              float bb[32];
               tc::tmem_ld32(tacc + j * 64 + hf * 32, v);
-              tc::tmem_ld_wait();
+              lds32(sbias + j * 64 + hf * 32, bb);
               const __half* gp = (p.gate && valid) ? p.gate + grow * p.ldg + op.dst_col + hf * 32 : nullptr;
+              uint4 gu[4];
+              if (gp) {
 #pragma unroll
-              for (int c = 0; c < 8; ++c) {
-                float f[4];
-#pragma unroll
-                for (int e = 0; e < 4; ++e) f[e] = __uint_as_float(v[c * 4 + e]) + sbias[j * 64 + hf * 32 + c * 4 + e];
-                if (gp) {
-                  uint2 gu = *reinterpret_cast<const uint2*>(gp + c * 4);
-                  __half2 g01 = *reinterpret_cast<__half2*>(&gu.x), g23 = *reinterpret_cast<__half2*>(&gu.y);
-                  f[0] *= __low2float(g01);
-                  f[1] *= __high2float(g01);
-                  f[2] *= __low2float(g23);
-                  f[3] *= __high2float(g23);
-                }
-                *reinterpret_cast<float4*>(sb + lr * 128 + (((uint32_t)c ^ sw) << 4)) = make_float4(f[0], f[1], f[2], f[3]);
+                for (int c = 0; c < 4; ++c) gu[c] = *reinterpret_cast<const uint4*>(gp + c * 8);
               }
+              tc::tmem_ld_wait();
+              float f[32];
+#pragma unroll
+              for (int e = 0; e < 32; ++e) f[e] = __uint_as_float(v[e]) + bb[e];
+              if (gp) {
+#pragma unroll
+                for (int c = 0; c < 4; ++c) {
+                  const uint32_t gw[4] = {gu[c].x, gu[c].y, gu[c].z, gu[c].w};
+#pragma unroll
+                  for (int e = 0; e < 4; ++e) {
+                    const __half2 g2 = *reinterpret_cast<const __half2*>(&gw[e]);
+                    f[c * 8 + 2 * e] *= __low2float(g2);
+                    f[c * 8 + 2 * e + 1] *= __high2float(g2);
+                  }
+                }
+              }
+#pragma unroll
+              for (int c = 0; c < 8; ++c)
+                *reinterpret_cast<float4*>(sb + lr * 128 + (((uint32_t)c ^ sw) << 4)) =
+                    make_float4(f[c * 4], f[c * 4 + 1], f[c * 4 + 2], f[c * 4 + 3]);
               tc::fence_proxy_async_smem();
               tc::named_bar_sync(bar_id, 128);
               if (leader) {
@@ -290,16 +321,21 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
 #pragma unroll 1
             for (int hf = 0; hf < 2; ++hf) {
               uint32_t v[32], g[32];
+              float bp[32], bg[32];
               tc::tmem_ld32(tacc + j * 64 + hf * 32, v);
               tc::tmem_ld32(tacc + 128 + j * 64 + hf * 32, g);
+              lds32(sbias + j * 64 + hf * 32, bp);
+              lds32(sbias + 128 + j * 64 + hf * 32, bg);
               tc::tmem_ld_wait();
+              bf16 r[32];
 #pragma unroll
               for (int e = 0; e < 32; ++e) {
-                const int n = j * 64 + hf * 32 + e;
-                float pv = __uint_as_float(v[e]) + sbias[n];
-                float gv = fast_sigmoid2(__uint_as_float(g[e]) + sbias[n + 128]);
-                sb16[(hf * 32 + e) * 128 + lr] = __float2bfloat16_rn(mask * gv * pv);
+                const float pv = __uint_as_float(v[e]) + bp[e];
+                const float gv = fast_sigmoid2(__uint_as_float(g[e]) + bg[e]);
+                r[e] = __float2bfloat16_rn(mask * gv * pv);
               }
+#pragma unroll
+              for (int e = 0; e < 32; ++e) sb16[(hf * 32 + e) * 128 + lr] = r[e];
             }
             tc::fence_proxy_async_smem();
             tc::named_bar_sync(bar_id, 128);
@@ -332,13 +368,15 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
 #pragma unroll 1
             for (int hf = 0; hf < 2; ++hf) {
               uint32_t v[32];
+              float bb[32];
               tc::tmem_ld32(tacc + j * 64 + hf * 32, v);
+              lds32(sbias + j * 64 + hf * 32, bb);
               tc::tmem_ld_wait();
+              bf16 r[32];
 #pragma unroll
-              for (int e = 0; e < 32; ++e) {
-                float xv = __uint_as_float(v[e]) + sbias[j * 64 + hf * 32 + e];
-                dst[(hf * 32 + e) << p.yt_shift] = __float2bfloat16_rn(xv * mk);
-              }
+              for (int e = 0; e < 32; ++e) r[e] = __float2bfloat16_rn((__uint_as_float(v[e]) + bb[e]) * mk);
+#pragma unroll
+              for (int e = 0; e < 32; ++e) dst[(hf * 32 + e) << p.yt_shift] = r[e];
             }
             tc::fence_proxy_async_smem();
             tc::named_bar_sync(bar_id, 128);

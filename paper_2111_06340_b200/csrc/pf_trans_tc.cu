@@ -154,19 +154,25 @@ transition_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constan
 #pragma unroll
         for (int hf = 0; hf < 2; ++hf) {
           uint32_t v[32];
+          float b1r[32];
           tc::tmem_ld32(ta + hf * 32, v);
-          tc::tmem_ld_wait();
 #pragma unroll
-          for (int q = 0; q < 4; ++q) {
-            const float4 b0 = *reinterpret_cast<const float4*>(bb + hf * 32 + q * 8);
-            const float4 b1v = *reinterpret_cast<const float4*>(bb + hf * 32 + q * 8 + 4);
-            uint4 u;
-            u.x = tr_pack_bf16(fmaxf(__uint_as_float(v[q * 8 + 0]) + b0.x, 0.f), fmaxf(__uint_as_float(v[q * 8 + 1]) + b0.y, 0.f));
-            u.y = tr_pack_bf16(fmaxf(__uint_as_float(v[q * 8 + 2]) + b0.z, 0.f), fmaxf(__uint_as_float(v[q * 8 + 3]) + b0.w, 0.f));
-            u.z = tr_pack_bf16(fmaxf(__uint_as_float(v[q * 8 + 4]) + b1v.x, 0.f), fmaxf(__uint_as_float(v[q * 8 + 5]) + b1v.y, 0.f));
-            u.w = tr_pack_bf16(fmaxf(__uint_as_float(v[q * 8 + 6]) + b1v.z, 0.f), fmaxf(__uint_as_float(v[q * 8 + 7]) + b1v.w, 0.f));
-            *reinterpret_cast<uint4*>(arow + (((uint32_t)(hf * 4 + q) ^ sw) << 4)) = u;
+          for (int q = 0; q < 8; ++q) {   // bias to registers first: a shared load between the stores below could not move
+            const float4 t = *reinterpret_cast<const float4*>(bb + hf * 32 + q * 4);
+            b1r[q * 4 + 0] = t.x;
+            b1r[q * 4 + 1] = t.y;
+            b1r[q * 4 + 2] = t.z;
+            b1r[q * 4 + 3] = t.w;
           }
+          tc::tmem_ld_wait();
+          uint32_t pk[16];
+#pragma unroll
+          for (int e = 0; e < 32; e += 2)
+            pk[e >> 1] = tr_pack_bf16(fmaxf(__uint_as_float(v[e]) + b1r[e], 0.f), fmaxf(__uint_as_float(v[e + 1]) + b1r[e + 1], 0.f));
+#pragma unroll
+          for (int q = 0; q < 4; ++q)
+            *reinterpret_cast<uint4*>(arow + (((uint32_t)(hf * 4 + q) ^ sw) << 4)) =
+                make_uint4(pk[q * 4], pk[q * 4 + 1], pk[q * 4 + 2], pk[q * 4 + 3]);
         }
         tc::tc_fence_before();
         tc::mbar_arrive(&acc1_empty[buf]);
@@ -188,15 +194,22 @@ transition_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constan
           tc::named_bar_sync(bar_id, 128);
         }
         uint32_t v[32];
+        float b2r[32];
         tc::tmem_ld32(lane_addr + SM::TMEM_ACC2 + bx * 32, v);
-        tc::tmem_ld_wait();
 #pragma unroll
         for (int q = 0; q < 8; ++q) {
-          const float4 b = *reinterpret_cast<const float4*>(sb2 + bx * 32 + q * 4);
-          *reinterpret_cast<float4*>(sb + lr * 128 + (((uint32_t)q ^ sw) << 4)) =
-              make_float4(__uint_as_float(v[q * 4 + 0]) + b.x, __uint_as_float(v[q * 4 + 1]) + b.y,
-                          __uint_as_float(v[q * 4 + 2]) + b.z, __uint_as_float(v[q * 4 + 3]) + b.w);
+          const float4 t = *reinterpret_cast<const float4*>(sb2 + bx * 32 + q * 4);
+          b2r[q * 4 + 0] = t.x;
+          b2r[q * 4 + 1] = t.y;
+          b2r[q * 4 + 2] = t.z;
+          b2r[q * 4 + 3] = t.w;
         }
+        tc::tmem_ld_wait();
+#pragma unroll
+        for (int q = 0; q < 8; ++q)
+          *reinterpret_cast<float4*>(sb + lr * 128 + (((uint32_t)q ^ sw) << 4)) =
+              make_float4(__uint_as_float(v[q * 4 + 0]) + b2r[q * 4 + 0], __uint_as_float(v[q * 4 + 1]) + b2r[q * 4 + 1],
+                          __uint_as_float(v[q * 4 + 2]) + b2r[q * 4 + 2], __uint_as_float(v[q * 4 + 3]) + b2r[q * 4 + 3]);
         tc::fence_proxy_async_smem();
         tc::named_bar_sync(bar_id, 128);
         if (leader) {
