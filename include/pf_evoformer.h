@@ -132,6 +132,15 @@ pf_status pf_sched_add(pf_sched_t* s, int protein_id, int length);
 int pf_sched_next_batch(pf_sched_t* s, int* ids_out, int* lengths_out, int cap, int* bucket_out);
 /* Footprint model used for batching: residual streams + workspace, bytes per protein. */
 size_t pf_sched_bytes_per_protein(int bucket, int S);
+/* Cost of one protein for load balancing: GEMM FLOPs of one Evoformer block at its bucket (SURVEY.md §8(d) F(S,N)). */
+double pf_sched_cost(int bucket, int S);
+/* Multi-GPU is replicas only (PAPER.md:190 runs independent single-GPU tasks, PAPER.md:260 lists
+ * multi-GPU inference as future work): this call shards the PROTEIN LIST, there is no data-path collective.
+ * lengths[n], ascending buckets[n_buckets] (host ints) -> rank_out[n] in [0, world): longest-processing-time-first over
+ * pf_sched_cost, ties to the lowest rank; deterministic, so every rank computes the same assignment without talking.
+ * Errors: INVALID_ARG (null, world < 1, buckets not ascending), SHAPE (a length outside [1, largest bucket]). */
+pf_status pf_sched_partition(const int* lengths, int n, const int* buckets, int n_buckets, int S, int world,
+                             int* rank_out);
 void pf_sched_destroy(pf_sched_t* s);
 
 #ifdef __cplusplus

@@ -26,7 +26,7 @@ EXPORTED_SYMBOLS = (
     "pf_evoformer_forward_host", "pf_evoformer_workspace_bytes", "pf_evoformer_last_launch_count",
     "pf_evoformer_set_profiling", "pf_evoformer_profile_kinds", "pf_evoformer_profile_name",
     "pf_evoformer_get_profile", "pf_evoformer_destroy", "pf_last_error", "pf_sched_create", "pf_sched_add", "pf_sched_next_batch",
-    "pf_sched_bytes_per_protein", "pf_sched_destroy",
+    "pf_sched_bytes_per_protein", "pf_sched_cost", "pf_sched_partition", "pf_sched_destroy",
 )
 
 
@@ -87,6 +87,10 @@ def lib() -> ctypes.CDLL:
         L.pf_sched_next_batch.argtypes = [c_void_p, POINTER(c_int), POINTER(c_int), c_int, POINTER(c_int)]
         L.pf_sched_bytes_per_protein.restype = c_size_t
         L.pf_sched_bytes_per_protein.argtypes = [c_int, c_int]
+        L.pf_sched_cost.restype = ctypes.c_double
+        L.pf_sched_cost.argtypes = [c_int, c_int]
+        L.pf_sched_partition.restype = c_int
+        L.pf_sched_partition.argtypes = [POINTER(c_int), c_int, POINTER(c_int), c_int, c_int, c_int, POINTER(c_int)]
         L.pf_sched_destroy.restype = None
         L.pf_sched_destroy.argtypes = [c_void_p]
         _lib = L
@@ -226,3 +230,19 @@ class Scheduler:
 
 def bytes_per_protein(bucket: int, S: int) -> int:
     return int(lib().pf_sched_bytes_per_protein(bucket, S))
+
+
+def sched_cost(bucket: int, S: int) -> float:
+    return float(lib().pf_sched_cost(bucket, S))
+
+
+def partition(lengths, buckets, S: int, world: int):
+    """pf_sched_partition: rank of every protein (replicas-only multi-GPU: the protein LIST is sharded, no collective)."""
+    n = len(lengths)
+    la = (c_int * max(n, 1))(*[int(x) for x in lengths])
+    ba = (c_int * len(buckets))(*[int(b) for b in buckets])
+    out = (c_int * max(n, 1))()
+    st = lib().pf_sched_partition(la, n, ba, len(buckets), S, world, out)
+    if st != PF_OK:
+        raise PfError(st, "pf_sched_partition")
+    return [int(out[i]) for i in range(n)]

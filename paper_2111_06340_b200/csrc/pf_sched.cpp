@@ -71,4 +71,36 @@ extern "C" int pf_sched_next_batch(pf_sched_t* s, int* ids_out, int* lengths_out
   return n;
 }
 
+// Per-protein cost model for list sharding: GEMM FLOPs of one Evoformer block at the protein's bucket (SURVEY.md §8(d)
+// F(S, N) with the AlphaFold dims); only ratios matter.
+extern "C" double pf_sched_cost(int bucket, int S) {
+  const double N = bucket, s = S, cm = 256, cz = 128, co = 32, hm = 8, hz = 4;
+  return 36 * s * N * cm * cm + 4 * s * N * N * cm + 4 * N * s * s * cm + 4 * s * N * cm * co + 2 * s * N * N * co * co +
+         2 * N * N * co * co * cz + 60 * N * N * cz * cz + 12 * N * N * N * cz + 2 * N * N * cz * hm + 4 * N * N * cz * hz;
+}
+
+// Replicas-only multi-GPU (independent single-GPU tasks, no communication): assign every
+// protein to one of `world` ranks, longest-processing-time first over pf_sched_cost of its bucket, ties to the lowest rank.
+extern "C" pf_status pf_sched_partition(const int* lengths, int n, const int* buckets, int n_buckets, int S, int world,
+                                        int* rank_out) {
+  if (!lengths || !buckets || !rank_out || n < 0 || n_buckets < 1 || S < 1 || world < 1) return PF_ERR_INVALID_ARG;
+  for (int i = 0; i < n_buckets; ++i)
+    if (buckets[i] < 1 || (i && buckets[i] <= buckets[i - 1])) return PF_ERR_INVALID_ARG;
+  std::vector<int> order(n);
+  std::vector<double> cost(n);
+  for (int i = 0; i < n; ++i) {
+    if (lengths[i] < 1 || lengths[i] > buckets[n_buckets - 1]) return PF_ERR_SHAPE;
+    order[i] = i;
+    cost[i] = pf_sched_cost(*std::lower_bound(buckets, buckets + n_buckets, lengths[i]), S);
+  }
+  std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return cost[a] > cost[b]; });
+  std::vector<double> load(world, 0.0);
+  for (int i : order) {
+    int r = (int)(std::min_element(load.begin(), load.end()) - load.begin());
+    rank_out[i] = r;
+    load[r] += cost[i];
+  }
+  return PF_OK;
+}
+
 extern "C" void pf_sched_destroy(pf_sched_t* s) { delete s; }
