@@ -25,7 +25,6 @@
 #include "pf_tc.cuh"
 
 #include <cuda_fp16.h>
-#include <cstdlib>
 #include <string>
 
 namespace pf {
@@ -61,7 +60,6 @@ struct G2Params {
   bf16* vt_out;
   int vt_cols;
   int Lpad;
-  int debug;
   G2Op ops[G2_MAX_OPS];
 };
 
@@ -245,7 +243,6 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
           const G2Op& op = p.ops[nt * 4 + j];
           const int kind = op.kind;
           if (kind == G2_SKIP) continue;
-          if (kind == G2_ROW16 && (p.debug & 4)) continue;
           if (kind == G2_ROW16) {
             if (leader) tc::bulk_wait_read<0>();
             tc::named_bar_sync(bar_id, 128);
@@ -267,7 +264,7 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
             }
             tc::fence_proxy_async_smem();
             tc::named_bar_sync(bar_id, 128);
-            if (leader && !(p.debug & 1)) {
+            if (leader) {
               tc::tma_store_4d(&tmO0, sb, op.dst_col, tcd.y0, tcd.x0, tcd.b);
               tc::bulk_commit();
             }
@@ -430,7 +427,7 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
           for (int u = 0; u < RU; ++u) {
             const int lr = pw * 16 + r0 + u;
             const int x = tcd.x0 + (lr >> p.yt_shift), y = tcd.y0 + (lr & (p.YT - 1));
-            if (x < p.D1 && y < p.D2 && !(p.debug & 2)) {
+            if (x < p.D1 && y < p.D2) {
               long srow = p.src_transposed ? ((long)tcd.b * p.D2 + y) * p.D1 + x : ((long)tcd.b * p.D1 + x) * p.D2 + y;
               const float4* xp = reinterpret_cast<const float4*>(p.src + srow * K);
 #pragma unroll
@@ -609,7 +606,6 @@ int launch_gemm2(TmaCtx* ctx, const G2Desc& d, int num_sms, cudaStream_t st) {
   p.heads_out = reinterpret_cast<bf16*>(d.heads_out); p.n_heads = d.n_heads;
   p.vt_out = reinterpret_cast<bf16*>(d.vt_out); p.vt_cols = d.vt_cols;
   p.Lpad = d.Lpad;
-  { const char* dbg = getenv("PF_G2_DEBUG"); p.debug = dbg ? atoi(dbg) : 0; }
   bool need_bias = false;
   for (int i = 0; i < G2_MAX_OPS; ++i) {
     if (i < d.n_ops) p.ops[i] = d.ops[i];
