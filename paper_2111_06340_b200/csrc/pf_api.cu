@@ -88,7 +88,7 @@ extern "C" size_t pf_evoformer_block_floats(const pf_config* cfg) {
   return block_offsets(*cfg).total;
 }
 
-static const char* const kKindNames[KK_COUNT] = {"ln_rows", "gemm", "attn_core", "tri_einsum", "ln_channels", "opm_core", "ln_gemm", "transition"};
+static const char* const kKindNames[KK_COUNT] = {"ln_rows", "gemm", "attn_core", "tri_einsum", "ln_channels", "opm_core", "ln_gemm", "transition", "mask_flags"};
 
 
 Arena pf::arena_layout(const pf_config& c, int B, int S, int N) {
@@ -112,6 +112,17 @@ Arena pf::arena_layout(const pf_config& c, int B, int S, int N) {
   a.tn = take(P * c.c_tri * es);
   a.oa = take(M * c.c_opm * es);
   a.ob = take(M * c.c_opm * es);
+  a.f_msa = take((size_t)g2_num_tiles(B, S, N));
+  a.f_msat = take((size_t)g2_num_tiles(B, N, S));
+  a.f_pair = take((size_t)g2_num_tiles(B, N, N));
+  a.f_msa_lin = take((M + 127) / 128);
+  a.f_pair_lin = take((P + 127) / 128);
+  a.kt_seq = take((size_t)B * 4);
+  a.kt_msa = take((size_t)B * 4);
+  a.rl_row = take((size_t)B * S * 8);
+  a.rl_col = take((size_t)B * N * 8);
+  a.rl_tri = take((size_t)B * N * 8);
+  a.rl_count = take(3 * 4);
   a.total = o;
   return a;
 }
@@ -447,6 +458,8 @@ static pf_status check_and_grow(pf_evoformer* h, const float* msa, const float* 
       return fail(PF_ERR_ALLOC, "cudaMalloc workspace");
     }
     h->ws_bytes = need;
+    // masked tiles are skipped (pf_flags.cu): what they would have written must still be finite
+    if (cudaMemset(h->ws, 0, need) != cudaSuccess) return fail(PF_ERR_CUDA, "cudaMemset workspace");
   }
   return PF_OK;
 }
@@ -461,6 +474,8 @@ static pf_status dispatch(pf_evoformer* h, float* msa, float* pair, const float*
   d.msa = msa; d.pair = pair; d.seq_mask = sm; d.msa_mask = mm;
   d.ar = arena_layout(h->cfg, B, S, N);
   h->launches = 0;
+  if (h->cfg.dtype == PF_BF16 && block1 > block0 && !tc_prepare_flags(h, sm, mm, B, S, N, st))
+    return fail(PF_ERR_CUDA, "mask flags launch failed");
   for (int blk = block0; blk < block1; ++blk)
     for (int step = step0; step <= step1; ++step) {
       bool ok = (h->cfg.dtype == PF_F32) ? d.run_substep(blk, step)

@@ -47,8 +47,15 @@ struct AttnParams {
   const float* keymask;
   bf16* o;
   int R, L, H, QT, n_kt, has_bias, stages, stage_bytes;
-  long units;
+  const int2* rows;        // device list {b*R + r, key tiles to visit} of the rows with an unmasked query (pf_flags.cu)
+  const int* n_rows;       // device scalar: its length
 };
+
+// Work unit u -> (row entry, head, query tile); the row entry is a plain load (no data-dependent branch), so every role
+// fetches the NEXT unit's entry at the top of the current unit and the load latency is off its critical path.
+__device__ __forceinline__ int2 attn_row_entry(int u, int units, const AttnParams& p) {
+  return u < units ? __ldg(p.rows + u / (p.QT * p.H)) : make_int2(0, 0);
+}
 
 __device__ __forceinline__ float ex2_approx(float x) {
   float y;
@@ -107,11 +114,12 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQK, const __grid_constant__
     if (tc::elect_one()) {
       const uint32_t stage_tx = SM::K_BYTES + SM::V_BYTES + (p.has_bias ? SM::B_BYTES : 0);
       uint32_t uc = 0, i = 0;
-      for (long u = blockIdx.x; u < p.units; u += gridDim.x, ++uc) {
-        const int qt = (int)(u % p.QT);
-        const long bh = u / p.QT;
-        const int h = (int)(bh % p.H);
-        const int br = (int)(bh / p.H);
+      const int units = *p.n_rows * p.H * p.QT;
+      int2 ent = attn_row_entry((int)blockIdx.x, units, p);
+      for (int u = blockIdx.x; u < units; u += (int)gridDim.x, ++uc) {
+        const int2 ent_next = attn_row_entry(u + (int)gridDim.x, units, p);
+        const int br = ent.x, n_kt = min(ent.y, p.n_kt);
+        const int qt = u % p.QT, h = (u / p.QT) % p.H;
         const int b = br / p.R;
         const int i0 = qt * AT_BQ;
         const uint32_t qb = uc & 1;
@@ -120,7 +128,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQK, const __grid_constant__
         uint8_t* qs = smem + SM::Q_OFF + qb * SM::Q_BYTES;
         tc::tma_load_3d(qs, &tmQK, &q_full[qb], h * 32, i0, br);            // box {32, 64, 1} twice: rows i0.., i0+64..
         tc::tma_load_3d(qs + 64 * 64, &tmQK, &q_full[qb], h * 32, i0 + 64, br);
-        for (int kt = 0; kt < p.n_kt; ++kt, ++i) {
+        for (int kt = 0; kt < n_kt; ++kt, ++i) {
           const uint32_t s = i % ST;
           tc::mbar_wait(&kv_empty[s], ((i / ST) & 1) ^ 1);
           uint8_t* st = smem + SM::STAGE_OFF + s * p.stage_bytes;
@@ -129,6 +137,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQK, const __grid_constant__
           tc::tma_load_2d(st + SM::K_BYTES, &tmV, &kv_full[s], kt * AT_BK, (br * p.H + h) * 32);
           if (p.has_bias) tc::tma_load_3d(st + SM::K_BYTES + SM::V_BYTES, &tmBias, &kv_full[s], kt * AT_BK, i0, b * p.H + h);
         }
+        ent = ent_next;
       }
     }
   } else if (warp == 5) {
@@ -137,37 +146,52 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQK, const __grid_constant__
       constexpr uint32_t idesc_s = tc::idesc_bf16_f32(AT_BQ, AT_BK);
       constexpr uint32_t idesc_o = tc::idesc_bf16_f32(AT_BQ, 32);
       const uint64_t p_desc = tc::smem_desc_kmajor<128>(tc::smem_u32(smem + SM::P_OFF));
-      const long my_units = p.units > (long)blockIdx.x ? (p.units - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
-      const long total = my_units * p.n_kt;
-      // S(j) = Q K^T for step j = (unit j / n_kt, key tile j % n_kt)
-      auto issue_s = [&](long j) {
-        const long uc = j / p.n_kt;
-        const int kt = (int)(j - uc * p.n_kt);
-        const uint32_t qb = (uint32_t)uc & 1, s = (uint32_t)(j % ST);
-        if (kt == 0) {
-          tc::mbar_wait(&q_full[qb], (uint32_t)(uc >> 1) & 1);
+      // issue side: S(j) = Q K^T for the next (unit, key tile); consume side: P(i) V.  j runs one step ahead of i.
+      const int units = *p.n_rows * p.H * p.QT;
+      int cu = blockIdx.x, ckt = 0;
+      int2 ent = attn_row_entry(cu, units, p), ent_next = make_int2(0, 0);
+      int cn = min(ent.y, p.n_kt);
+      uint32_t cuc = 0, j = 0, i = 0;
+      auto issue_s = [&]() -> bool {
+        if (cu >= units) return false;
+        const uint32_t qb = cuc & 1, s = j % ST;
+        if (ckt == 0) {
+          ent_next = attn_row_entry(cu + (int)gridDim.x, units, p);   // used when this unit's last S has been issued
+          tc::mbar_wait(&q_full[qb], (cuc >> 1) & 1);
         }
-        tc::mbar_wait(&kv_full[s], (uint32_t)(j / ST) & 1);
+        tc::mbar_wait(&kv_full[s], (j / ST) & 1);
         tc::tc_fence_after();
         const uint64_t q_desc = tc::smem_desc_kmajor<64>(tc::smem_u32(smem + SM::Q_OFF + qb * SM::Q_BYTES));
         const uint64_t k_desc = tc::smem_desc_kmajor<64>(tc::smem_u32(smem + SM::STAGE_OFF + s * p.stage_bytes));
-        const uint32_t d = tmem_S + ((uint32_t)j & 1) * AT_BK;
+        const uint32_t d = tmem_S + (j & 1) * AT_BK;
         tc::mma_bf16(d, q_desc, k_desc, idesc_s, false);
         tc::mma_bf16(d, q_desc + 2, k_desc + 2, idesc_s, true);
         tc::mma_commit(&s_full[j & 1]);
-        if (kt == p.n_kt - 1) tc::mma_commit(&q_empty[qb]);
+        if (ckt == cn - 1) {
+          tc::mma_commit(&q_empty[qb]);
+          cu += (int)gridDim.x;
+          cn = min(ent_next.y, p.n_kt);
+          ckt = 0;
+          ++cuc;
+        } else {
+          ++ckt;
+        }
+        ++j;
+        return true;
       };
-      if (total > 0) issue_s(0);
-      for (long i = 0; i < total; ++i) {
-        if (i + 1 < total) issue_s(i + 1);       // S(i-1) was drained before P(i-1) arrived, so its buffer is free
-        const uint32_t s = (uint32_t)(i % ST);
-        tc::mbar_wait(p_full, (uint32_t)i & 1);
-        tc::tc_fence_after();
-        const uint64_t v_desc = tc::smem_desc_kmajor<128>(tc::smem_u32(smem + SM::STAGE_OFF + s * p.stage_bytes + SM::K_BYTES));
+      if (issue_s()) {
+        while (true) {
+          issue_s();                               // S(i-1) was drained before P(i-1) arrived, so its buffer is free
+          const uint32_t s = i % ST;
+          tc::mbar_wait(p_full, i & 1);
+          tc::tc_fence_after();
+          const uint64_t v_desc = tc::smem_desc_kmajor<128>(tc::smem_u32(smem + SM::STAGE_OFF + s * p.stage_bytes + SM::K_BYTES));
 #pragma unroll
-        for (int k = 0; k < AT_BK / 16; ++k) tc::mma_bf16(tmem_O, p_desc + 2 * k, v_desc + 2 * k, idesc_o, k != 0);
-        tc::mma_commit(o_full);
-        tc::mma_commit(&kv_empty[s]);
+          for (int k = 0; k < AT_BK / 16; ++k) tc::mma_bf16(tmem_O, p_desc + 2 * k, v_desc + 2 * k, idesc_o, k != 0);
+          tc::mma_commit(o_full);
+          tc::mma_commit(&kv_empty[s]);
+          if (++i == j) break;
+        }
       }
     }
   } else {
@@ -178,11 +202,12 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQK, const __grid_constant__
     int cur_b = -1;
     uint32_t tile_masked = 0;                    // bit kt: key tile kt holds a masked / out-of-range key
     uint32_t i = 0;                              // pipeline step (all units)
-    for (long u = blockIdx.x; u < p.units; u += gridDim.x) {
-      const int qt = (int)(u % p.QT);
-      const long bh = u / p.QT;
-      const int h = (int)(bh % p.H);
-      const int br = (int)(bh / p.H);
+    const int units = *p.n_rows * p.H * p.QT;
+    int2 ent = attn_row_entry((int)blockIdx.x, units, p);
+    for (int u = blockIdx.x; u < units; u += (int)gridDim.x) {
+      const int2 ent_next = attn_row_entry(u + (int)gridDim.x, units, p);
+      const int br = ent.x, n_kt = min(ent.y, p.n_kt);
+      const int qt = u % p.QT, h = (u / p.QT) % p.H;
       const int b = br / p.R;
       const int qi = qt * AT_BQ + row;
       if (b != cur_b) {
@@ -213,7 +238,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQK, const __grid_constant__
       float oacc[32];
 #pragma unroll
       for (int d = 0; d < 32; ++d) oacc[d] = 0.f;
-      for (int kt = 0; kt < p.n_kt; ++kt, ++i) {
+      for (int kt = 0; kt < n_kt; ++kt, ++i) {
         const uint32_t s = i % ST;
         const uint8_t* bias_t = smem + SM::STAGE_OFF + s * p.stage_bytes + SM::K_BYTES + SM::V_BYTES;
         if (p.has_bias) tc::mbar_wait(&kv_full[s], (i / ST) & 1);
@@ -319,6 +344,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQK, const __grid_constant__
           *reinterpret_cast<uint4*>(op + d * 8) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
         }
       }
+      ent = ent_next;
     }
   }
   tc::tc_fence_before();
@@ -327,7 +353,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQK, const __grid_constant__
 }
 
 int launch_attn_tc(TmaCtx* ctx, const bf16* qkg, const bf16* vt, const bf16* bias, const float* keymask, bf16* o, int B,
-                   int R, int L, int Lpad, int H, int num_sms, cudaStream_t st) {
+                   int R, int L, int Lpad, int H, const void* rows, const int* n_rows, int num_sms, cudaStream_t st) {
   if (L > AT_MAXKEYS) {
     tc_set_error("attn_tc: key length above 1024 not supported");
     return -1;
@@ -368,9 +394,15 @@ int launch_attn_tc(TmaCtx* ctx, const bf16* qkg, const bf16* vt, const bf16* bia
   p.has_bias = bias ? 1 : 0;
   p.stage_bytes = AttnSmem::K_BYTES + AttnSmem::V_BYTES + (bias ? AttnSmem::B_BYTES : 0);
   p.stages = bias ? 3 : AttnSmem::MAX_STAGES;
-  p.units = (long)B * R * H * p.QT;
+  const long units = (long)B * R * H * p.QT;      // upper bound (all rows active)
+  if (units >= (1L << 31) - 4096) {
+    tc_set_error("attn_tc: too many work units");
+    return -1;
+  }
+  p.rows = reinterpret_cast<const int2*>(rows);
+  p.n_rows = n_rows;
   const long max_ctas = 2L * num_sms;
-  unsigned grid = (unsigned)(p.units < max_ctas ? p.units : max_ctas);
+  unsigned grid = (unsigned)(units < max_ctas ? units : max_ctas);
   attn_tc_kernel<<<grid, AT_THREADS, AttnSmem::TOTAL, st>>>(tmQK, tmV, tmB, p);
   return 0;
 }

@@ -53,13 +53,18 @@ TcBlock tc_layout(const pf_config& c);
 void build_tc_block(const pf_config& c, const BlockW& off, const TcBlock& t, const float* w, std::vector<uint16_t>& w16,
                     size_t base16, std::vector<float>& wf, size_t basef);
 
-enum KernelKind { KK_LN = 0, KK_GEMM, KK_ATTN, KK_TRI, KK_LNC, KK_OPM, KK_LNGEMM, KK_TRANS, KK_COUNT };
+enum KernelKind { KK_LN = 0, KK_GEMM, KK_ATTN, KK_TRI, KK_LNC, KK_OPM, KK_LNGEMM, KK_TRANS, KK_FLAGS, KK_COUNT };
 
 inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 inline int pad8(int v) { return (v + 7) / 8 * 8; }
 
 struct Arena {
-  size_t x, qkg, vt, o, bias, acm, bcm, g, tcm, tn, oa, ob, total;
+  size_t x, qkg, vt, o, bias, acm, bcm, g, tcm, tn, oa, ob;
+  // mask-derived work flags (pf_flags.cu): active-tile bytes per row geometry, key-tile counts per protein
+  size_t f_msa, f_msat, f_pair, f_msa_lin, f_pair_lin, kt_seq, kt_msa;
+  // compacted attention row lists {row, key tiles} + their lengths: row attention (b,s), column attention (b,i), triangle (b,i)
+  size_t rl_row, rl_col, rl_tri, rl_count;
+  size_t total;
 };
 Arena arena_layout(const pf_config& c, int B, int S, int N);
 
@@ -108,6 +113,8 @@ struct pf_evoformer {
 
 namespace pf {
 // tcgen05 path: one sub-step (1..9) of block `block`; returns false and sets err on failure.
+// mask-derived work flags for one forward call (launched once, before the first block)
+bool tc_prepare_flags(pf_evoformer* h, const float* seq_mask, const float* msa_mask, int B, int S, int N, cudaStream_t st);
 bool tc_run_substep(pf_evoformer* h, float* msa, float* pair, const float* seq_mask, const float* msa_mask, int B, int S,
                     int N, int block, int step, cudaStream_t st, std::string& err);
 }  // namespace pf

@@ -92,6 +92,24 @@ struct G2Op {
   int masked;    // VT: multiply by the row mask
 };
 constexpr int G2_MAX_OPS = 20;
+// tile height along y for a [B, D1, D2] row grid: the power of two in [8, 128] that wastes the fewest rows (ties: largest)
+inline int g2_pick_yt(int D2) {
+  int best = 128;
+  double best_eff = -1.0;
+  for (int yt = 128; yt >= 8; yt >>= 1) {
+    int tiles = (D2 + yt - 1) / yt;
+    double eff = (double)D2 / ((double)tiles * yt);
+    if (eff > best_eff + 1e-9) {
+      best_eff = eff;
+      best = yt;
+    }
+  }
+  return best;
+}
+inline long g2_num_tiles(int B, int D1, int D2) {
+  const int yt = g2_pick_yt(D2), xt = 128 / yt;
+  return (long)B * ((D1 + xt - 1) / xt) * ((D2 + yt - 1) / yt);
+}
 struct G2Desc {
   int B, D1, D2;            // row geometry
   int K, Nw;                // K in {128, 256}; Nw = rows of Wt (GEMM columns including gate partners)
@@ -124,13 +142,22 @@ struct G2Desc {
   int Lpad;
   G2Op ops[G2_MAX_OPS];
   int n_ops;
+  const unsigned char* tile_active;   // optional [num_tiles]: 0 = every row of the tile is masked, skip it (pf_flags.cu)
 };
 int launch_gemm2(TmaCtx* ctx, const G2Desc& d, int num_sms, cudaStream_t st);
 // fused transition (pf_trans_tc.cu): res[R, C] += relu(LN(res) W1 + b1) W2 + b2; w1t fp16 [4C, C], w2t bf16 [C, 4C]
 int launch_transition_tc(TmaCtx* ctx, float* res, long R, int C, const float* gamma, const float* beta, const void* w1t,
-                         const float* b1, const void* w2t, const float* b2, int num_sms, cudaStream_t st);
+                         const float* b1, const void* w2t, const float* b2, const unsigned char* tile_active, int num_sms,
+                         cudaStream_t st);
+// rows: device list of int2 {b*R + r, key tiles to visit} of the rows to process, *n_rows its length (pf_flags.cu
+// launch_row_list): rows all of whose queries are masked are not in it, key tiles past the last unmasked key are not visited
 int launch_attn_tc(TmaCtx* ctx, const bf16* qkg, const bf16* vt, const bf16* bias, const float* keymask, bf16* o,
-                   int B, int R, int L, int Lpad, int H, int num_sms, cudaStream_t st);
+                   int B, int R, int L, int Lpad, int H, const void* rows, const int* n_rows, int num_sms, cudaStream_t st);
+void launch_row_list(const float* rowmask, const int* key_tiles, int B, int R, void* rows, int* n_rows, cudaStream_t st);
+// pf_flags.cu
+void launch_tile_flags(const float* seq_mask, const float* msa_mask, int kind, int B, int D1, int D2, int XT, int YT,
+                       unsigned char* flags, long num_tiles, cudaStream_t st);
+void launch_key_tiles(const float* mask, int B, int L, int* key_tiles, cudaStream_t st);
 // ab_t: [(b,i), 64 channels (a | b), Spad] bf16 masked projections; wout_t: [c_z, c_opm*c_opm] bf16
 int launch_opm_tc(TmaCtx* ctx, const bf16* ab_t, const bf16* wout_t, const float* bout, const float* seq_mask,
                   const float* msa_mask, float* z, int B, int S, int Spad, int N, cudaStream_t st);

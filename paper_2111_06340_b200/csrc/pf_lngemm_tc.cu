@@ -60,6 +60,7 @@ struct G2Params {
   bf16* vt_out;
   int vt_cols;
   int Lpad;
+  const unsigned char* tile_active;
   G2Op ops[G2_MAX_OPS];
 };
 
@@ -82,6 +83,7 @@ struct G2Smem {
 struct TileCoord {
   int b, x0, y0;
 };
+__device__ __forceinline__ bool tile_on(long t, const G2Params& p) { return !p.tile_active || p.tile_active[t] != 0; }
 __device__ __forceinline__ TileCoord tile_coord(long t, const G2Params& p) {
   TileCoord c;
   int ty = (int)(t % p.tiles_y);
@@ -214,6 +216,7 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
     const uint32_t sw = (uint32_t)(lr & 7);
     uint32_t ac = 0;                                   // accumulator buffers consumed so far
     for (long tile = blockIdx.x; tile < p.num_tiles; tile += gridDim.x) {
+      if (!tile_on(tile, p)) continue;
       const TileCoord tcd = tile_coord(tile, p);
       const int x = tcd.x0 + xl, y = tcd.y0 + yl;
       const bool valid = x < p.D1 && y < p.D2;
@@ -401,13 +404,14 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
         bt[i] = __ldg(reinterpret_cast<const float4*>(p.beta) + lane + 32 * i);
       }
       uint32_t it = 0;
-      for (long tile = blockIdx.x; tile < p.num_tiles; tile += gridDim.x, ++it) {
+      for (long tile = blockIdx.x; tile < p.num_tiles; tile += gridDim.x) {
+        if (!tile_on(tile, p)) continue;
         const uint32_t abuf = it & 1;
         {
           // pull the next tile's rows of this warp into L2 while this tile is normalised: the register-staged loads below
           // then see L2 latency, not HBM latency (bytes in flight per SM are bounded by the register file)
           const long nxt = tile + gridDim.x;
-          if (nxt < p.num_tiles && lane < 16) {
+          if (nxt < p.num_tiles && lane < 16 && tile_on(nxt, p)) {
             const TileCoord nc = tile_coord(nxt, p);
             const int lr = pw * 16 + lane;
             const int x = nc.x0 + (lr >> p.yt_shift), y = nc.y0 + (lr & (p.YT - 1));
@@ -467,12 +471,14 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
         }
         tc::fence_proxy_async_smem();
         tc::mbar_arrive(&a_full[abuf]);
+        ++it;
       }
     } else if (warp == 8) {
       // ========================================================= A by TMA (a_mode 1)
       if (tc::elect_one()) {
         uint32_t it = 0;
-        for (long tile = blockIdx.x; tile < p.num_tiles; tile += gridDim.x, ++it) {
+        for (long tile = blockIdx.x; tile < p.num_tiles; tile += gridDim.x) {
+          if (!tile_on(tile, p)) continue;
           const uint32_t abuf = it & 1;
           tc::mbar_wait(&a_empty[abuf], ((it >> 1) & 1) ^ 1);
           const TileCoord tcd = tile_coord(tile, p);
@@ -481,6 +487,7 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
 #pragma unroll
           for (int kb = 0; kb < KB; ++kb)
             tc::tma_load_4d(abase + kb * SM::KB_BYTES, &tmA, &a_full[abuf], kb * 64, tcd.y0, tcd.x0, tcd.b);
+          ++it;
         }
       }
     }
@@ -489,6 +496,7 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
     if (tc::elect_one()) {
       uint32_t wc = 0;
       for (long tile = blockIdx.x; tile < p.num_tiles; tile += gridDim.x) {
+        if (!tile_on(tile, p)) continue;
         for (int nt = 0; nt < p.n_tiles; ++nt) {
 #pragma unroll 1
           for (int kb = 0; kb < KB; ++kb, ++wc) {
@@ -504,7 +512,8 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
     // ============================================================= MMA issue
     if (tc::elect_one()) {
       uint32_t it = 0, wc = 0, ac = 0;
-      for (long tile = blockIdx.x; tile < p.num_tiles; tile += gridDim.x, ++it) {
+      for (long tile = blockIdx.x; tile < p.num_tiles; tile += gridDim.x) {
+        if (!tile_on(tile, p)) continue;
         const uint32_t abuf = it & 1;
         tc::mbar_wait(&a_full[abuf], (it >> 1) & 1);
         tc::tc_fence_after();
@@ -531,6 +540,7 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
           tc::mma_commit(&acc_full[buf]);
         }
         tc::mma_commit(&a_empty[abuf]);
+        ++it;
       }
     }
   }
@@ -542,20 +552,6 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
 // ------------------------------------------------------------------------------------------------
 // host
 // ------------------------------------------------------------------------------------------------
-static int pick_yt(int D2) {
-  int best = 128;
-  double best_eff = -1.0;
-  for (int yt = 128; yt >= 8; yt >>= 1) {
-    int tiles = (D2 + yt - 1) / yt;
-    double eff = (double)D2 / ((double)tiles * yt);
-    if (eff > best_eff + 1e-9) {
-      best_eff = eff;
-      best = yt;
-    }
-  }
-  return best;
-}
-
 template <int K, int AMODE>
 static int launch_g2(const CUtensorMap& tmW, const CUtensorMap& tmA, const CUtensorMap& tmO0, const CUtensorMap& tmT0,
                      const CUtensorMap& tmT1, const CUtensorMap& tmH, const CUtensorMap& tmR, const G2Params& p, int num_sms,
@@ -583,7 +579,7 @@ int launch_gemm2(TmaCtx* ctx, const G2Desc& d, int num_sms, cudaStream_t st) {
   G2Params p;
   memset(&p, 0, sizeof(p));
   p.B = d.B; p.D1 = d.D1; p.D2 = d.D2;
-  p.YT = pick_yt(d.D2);
+  p.YT = g2_pick_yt(d.D2);
   p.XT = 128 / p.YT;
   p.yt_shift = 0;
   while ((1 << p.yt_shift) < p.YT) ++p.yt_shift;
@@ -606,6 +602,7 @@ int launch_gemm2(TmaCtx* ctx, const G2Desc& d, int num_sms, cudaStream_t st) {
   p.heads_out = reinterpret_cast<bf16*>(d.heads_out); p.n_heads = d.n_heads;
   p.vt_out = reinterpret_cast<bf16*>(d.vt_out); p.vt_cols = d.vt_cols;
   p.Lpad = d.Lpad;
+  p.tile_active = d.tile_active;
   bool need_bias = false;
   for (int i = 0; i < G2_MAX_OPS; ++i) {
     if (i < d.n_ops) p.ops[i] = d.ops[i];

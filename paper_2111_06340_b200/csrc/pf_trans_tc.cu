@@ -61,7 +61,10 @@ struct TrParams {
   const float* b2;        // [C]
   long R;
   long num_tiles;
+  const unsigned char* tile_active;   // optional: 0 = every row of the 128-row tile is masked, skip it
 };
+
+__device__ __forceinline__ bool tr_tile_on(long t, const TrParams& p) { return !p.tile_active || p.tile_active[t] != 0; }
 
 __device__ __forceinline__ uint32_t tr_pack_bf16(float a, float b) {
   __nv_bfloat162 h = __floats2bfloat162_rn(a, b);
@@ -136,7 +139,8 @@ transition_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constan
     const uint32_t sw = (uint32_t)(lr & 7);
     uint32_t cc = 0;                                   // hidden chunks consumed so far (all tiles)
     uint32_t it = 0;
-    for (long tile = blockIdx.x; tile < p.num_tiles; tile += gridDim.x, ++it) {
+    for (long tile = blockIdx.x; tile < p.num_tiles; tile += gridDim.x) {
+      if (!tr_tile_on(tile, p)) continue;
 #pragma unroll 1
       for (int c = 0; c < NC; ++c, ++cc) {
         const uint32_t buf = cc & 1, ph = (cc >> 1) & 1;
@@ -219,6 +223,7 @@ transition_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constan
       }
       tc::tc_fence_before();
       tc::mbar_arrive(acc2_empty);
+      ++it;
     }
     if (leader) tc::bulk_wait<0>();
   } else if (warp < 16) {
@@ -233,12 +238,13 @@ transition_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constan
       bt[i] = __ldg(reinterpret_cast<const float4*>(p.beta) + lane + 32 * i);
     }
     uint32_t it = 0;
-    for (long tile = blockIdx.x; tile < p.num_tiles; tile += gridDim.x, ++it) {
+    for (long tile = blockIdx.x; tile < p.num_tiles; tile += gridDim.x) {
+      if (!tr_tile_on(tile, p)) continue;
       const uint32_t abuf = it % A1B;
       {
         const long nxt = tile + gridDim.x;             // next tile's 16 rows of this warp -> L2
         const long r0 = nxt * 128 + pw * 16;
-        if (nxt < p.num_tiles && lane == 0 && r0 < p.R) {
+        if (nxt < p.num_tiles && lane == 0 && r0 < p.R && tr_tile_on(nxt, p)) {
           long n = p.R - r0 < 16 ? p.R - r0 : 16;
           tc::prefetch_l2_bulk(p.res + r0 * C, (uint32_t)(n * C * 4));
         }
@@ -291,6 +297,7 @@ transition_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constan
       }
       tc::fence_proxy_async_smem();
       tc::mbar_arrive(&a1_full[abuf]);
+      ++it;
     }
   } else if (warp == 16) {
     // ============================================================= weight tiles, in the MMA thread's consumption order
@@ -311,6 +318,7 @@ transition_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constan
           for (int nh = 0; nh < NH; ++nh) load(&tmW2, c * TR_HC + kb * 64, nh * 128);
       };
       for (long tile = blockIdx.x; tile < p.num_tiles; tile += gridDim.x) {
+        if (!tr_tile_on(tile, p)) continue;
         g1(0);
         for (int c = 1; c < NC; ++c) {
           g1(c);
@@ -326,7 +334,8 @@ transition_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constan
       constexpr uint32_t idesc2 = tc::idesc_bf16_f32(128, 128);   // GEMM2: bf16 hidden x bf16 W2
       uint32_t wc = 0, c1 = 0, c2 = 0, it = 0;
       const uint32_t acc2 = tmem_base + SM::TMEM_ACC2;
-      for (long tile = blockIdx.x; tile < p.num_tiles; tile += gridDim.x, ++it) {
+      for (long tile = blockIdx.x; tile < p.num_tiles; tile += gridDim.x) {
+      if (!tr_tile_on(tile, p)) continue;
         const uint32_t abuf = it % A1B;
         const uint32_t a1_addr = tc::smem_u32(smem + SM::A1_OFF + abuf * SM::A1_BYTES);
         auto gemm1 = [&](int c) {
@@ -387,6 +396,7 @@ transition_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constan
         }
         gemm2(NC - 1);
         tc::mma_commit(acc2_full);
+        ++it;
       }
     }
   }
@@ -418,7 +428,8 @@ static int launch_tr(const CUtensorMap& tmW1, const CUtensorMap& tmW2, const CUt
 
 // w1t: fp16 [4C, C] (K = C contiguous); w2t: bf16 [C, 4C] (K = 4C contiguous); res: fp32 [R, C] updated in place.
 int launch_transition_tc(TmaCtx* ctx, float* res, long R, int C, const float* gamma, const float* beta, const void* w1t,
-                         const float* b1, const void* w2t, const float* b2, int num_sms, cudaStream_t st) {
+                         const float* b1, const void* w2t, const float* b2, const unsigned char* tile_active, int num_sms,
+                         cudaStream_t st) {
   if (C != 128 && C != 256) {
     tc_set_error("transition_tc: C must be 128 or 256");
     return -1;
@@ -427,6 +438,7 @@ int launch_transition_tc(TmaCtx* ctx, float* res, long R, int C, const float* ga
   p.res = res; p.gamma = gamma; p.beta = beta; p.b1 = b1; p.b2 = b2;
   p.R = R;
   p.num_tiles = (R + 127) / 128;
+  p.tile_active = tile_active;
   CUtensorMap tmW1, tmW2, tmR;
   {
     uint64_t dims[2] = {(uint64_t)C, (uint64_t)4 * C}, str[1] = {(uint64_t)C * 2};

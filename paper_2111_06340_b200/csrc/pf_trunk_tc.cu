@@ -148,6 +148,7 @@ struct TcDriver {
 
   template <typename U>
   U* buf(size_t off) { return reinterpret_cast<U*>(h->ws + off); }
+  const unsigned char* flags(size_t off) { return reinterpret_cast<const unsigned char*>(h->ws + off); }
 
   static G2Desc desc_base(int B, int D1, int D2, int K, int Nw) {
     G2Desc d;
@@ -176,8 +177,9 @@ struct TcDriver {
 
   // Gated attention sub-step on a residual stream `res` viewed as rows (b, x in D1, y in D2), attention along y.
   //   transposed: rows are gathered from / scattered to the (b, y, x) layout of `res`  (A.2, A.8 via their identities)
+  //   f_rows: active-tile flags of this row geometry; rl_off / rl_idx: the compacted row list of this attention (pf_flags.cu)
   bool attn_substep(float* res, int C, int H, int D1, int D2, bool transposed, const AttnW& a, const AttnT& at,
-                    const float* keymask, bool row_bias, bool self_bias) {
+                    const float* keymask, bool row_bias, bool self_bias, size_t f_rows, size_t rl_off, int rl_idx) {
     const pf_config& c = h->cfg;
     const double R = (double)B * D1 * D2;
     const int L = D2, Lp = pad8(L);
@@ -193,6 +195,7 @@ struct TcDriver {
       d.ops[0] = op(G2_HEADS, 0, c.heads_msa);
       d.ops[0].scale = kLog2e;
       d.n_ops = 1;
+      d.tile_active = flags(ar.f_pair);
       if (!gemm2(d, (double)B * N * N * c.heads_msa * 2.0)) return false;
     }
     {
@@ -219,12 +222,14 @@ struct TcDriver {
         d.ops[n++].scale = kLog2e;
       }
       d.n_ops = n;
+      d.tile_active = flags(f_rows);
       if (!gemm2(d, R * 4.0 * C * 2.0 + (self_bias ? R * H * 2.0 : 0.0))) return false;
     }
     {
       double rows = R, Cc = C;
       h->prof_begin(KK_ATTN, 4.0 * rows * L * Cc, 5.0 * rows * Cc * 2.0 + (BIAS ? (double)B * H * L * L * 2.0 : 0.0), st);
-      if (launch_attn_tc(h->tma, QKG, VT, BIAS, keymask, O, B, D1, L, Lp, H, h->num_sms, st) != 0) {
+      if (launch_attn_tc(h->tma, QKG, VT, BIAS, keymask, O, B, D1, L, Lp, H, h->ws + rl_off, buf<int>(ar.rl_count) + rl_idx,
+                         h->num_sms, st) != 0) {
         err = std::string("attn_tc: ") + tc_last_error();
         return false;
       }
@@ -236,15 +241,16 @@ struct TcDriver {
     int n = 0;
     for (int col = 0; col < C; col += 64) d.ops[n++] = op(G2_RESID, col);
     d.n_ops = n;
+    d.tile_active = flags(f_rows);
     return gemm2(d, R * C * 8.0);
   }
 
   // A.3 / A.9: one fused kernel, the 4C-wide hidden activation stays on chip
-  bool transition_substep(float* res, int D1, int D2, int C, const TransW& t, size_t w1t, size_t w2t) {
+  bool transition_substep(float* res, int D1, int D2, int C, const TransW& t, size_t w1t, size_t w2t, size_t f_lin) {
     const double R = (double)B * D1 * D2, n4 = (double)h->cfg.transition_n * C;
     h->prof_begin(KK_TRANS, 4.0 * R * n4 * C, R * C * 8.0 + 4.0 * n4 * C, st);
     if (launch_transition_tc(h->tma, res, (long)B * D1 * D2, C, w + t.ln_g, w + t.ln_b, w16 + w1t, w + t.b1, w16 + w2t,
-                             w + t.b2, h->num_sms, st) != 0) {
+                             w + t.b2, flags(f_lin), h->num_sms, st) != 0) {
       err = std::string("transition_tc: ") + tc_last_error();
       return false;
     }
@@ -271,6 +277,7 @@ struct TcDriver {
     d.ops[0] = op(G2_VT, 0, 2 * c.c_opm);
     d.ops[0].masked = 1;
     d.n_ops = 1;
+    d.tile_active = flags(ar.f_msat);
     if (!gemm2(d, M * 2.0 * c.c_opm * 2.0)) return false;
     h->prof_begin(KK_OPM, 2.0 * P * cc * S + 2.0 * P * cc * c.c_z, 2.0 * M * c.c_opm * 2.0 + 8.0 * P * c.c_z, st);
     if (launch_opm_tc(h->tma, ABT, reinterpret_cast<const bf16*>(w16 + h->tc.opm_wout), w + o.bout, seq_mask, msa_mask,
@@ -310,6 +317,7 @@ struct TcDriver {
         d.ops[8 + j].fmt = 1;
       }
       d.n_ops = 10;
+      d.tile_active = flags(ar.f_pair);
       if (!gemm2(d, P * 3.0 * ct * 2.0)) return false;
     }
     h->prof_begin(KK_TRI, 2.0 * B * ct * (double)N * N * N, (double)B * ct * N * Np * 8.0, st);
@@ -328,11 +336,41 @@ struct TcDriver {
     d.ops[0] = op(G2_RESID, 0);
     d.ops[1] = op(G2_RESID, 64);
     d.n_ops = 2;
+    d.tile_active = flags(ar.f_pair);
     return gemm2(d, P * c.c_z * 10.0);
   }
 };
 
 }  // namespace
+
+bool tc_prepare_flags(pf_evoformer* h, const float* seq_mask, const float* msa_mask, int B, int S, int N, cudaStream_t st) {
+  const Arena ar = arena_layout(h->cfg, B, S, N);
+  auto fl = [&](size_t off) { return reinterpret_cast<unsigned char*>(h->ws + off); };
+  const long M = (long)B * S * N, P = (long)B * N * N;
+  h->prof_begin(KK_FLAGS, 0.0, 0.0, st);
+  {
+    const int yt = g2_pick_yt(N);
+    launch_tile_flags(seq_mask, msa_mask, 0, B, S, N, 128 / yt, yt, fl(ar.f_msa), g2_num_tiles(B, S, N), st);
+    launch_tile_flags(seq_mask, msa_mask, 2, B, N, N, 128 / yt, yt, fl(ar.f_pair), g2_num_tiles(B, N, N), st);
+  }
+  {
+    const int yt = g2_pick_yt(S);
+    launch_tile_flags(seq_mask, msa_mask, 1, B, N, S, 128 / yt, yt, fl(ar.f_msat), g2_num_tiles(B, N, S), st);
+  }
+  launch_tile_flags(seq_mask, msa_mask, 0, B, S, N, 0, 0, fl(ar.f_msa_lin), (M + 127) / 128, st);
+  launch_tile_flags(seq_mask, msa_mask, 2, B, N, N, 0, 0, fl(ar.f_pair_lin), (P + 127) / 128, st);
+  launch_key_tiles(seq_mask, B, N, reinterpret_cast<int*>(h->ws + ar.kt_seq), st);
+  launch_key_tiles(msa_mask, B, S, reinterpret_cast<int*>(h->ws + ar.kt_msa), st);
+  int* kt_seq = reinterpret_cast<int*>(h->ws + ar.kt_seq);
+  int* kt_msa = reinterpret_cast<int*>(h->ws + ar.kt_msa);
+  int* cnt = reinterpret_cast<int*>(h->ws + ar.rl_count);
+  launch_row_list(msa_mask, kt_seq, B, S, h->ws + ar.rl_row, cnt + 0, st);   // row attention: rows (b, s), keys = residues
+  launch_row_list(seq_mask, kt_msa, B, N, h->ws + ar.rl_col, cnt + 1, st);   // column attention: rows (b, i), keys = sequences
+  launch_row_list(seq_mask, kt_seq, B, N, h->ws + ar.rl_tri, cnt + 2, st);   // triangle attention: rows (b, i), keys = residues
+  h->prof_end(st);
+  h->launches += 9;   // prof_begin counted one of the ten
+  return cudaGetLastError() == cudaSuccess;
+}
 
 bool tc_run_substep(pf_evoformer* h, float* msa, float* pair, const float* seq_mask, const float* msa_mask, int B, int S,
                     int N, int block, int step, cudaStream_t st, std::string& err) {
@@ -346,17 +384,19 @@ bool tc_run_substep(pf_evoformer* h, float* msa, float* pair, const float* seq_m
   d.wf = h->wf + (size_t)block * h->tc.total_f32;
   bool ok = false;
   switch (step) {
-    case 1: ok = d.attn_substep(msa, c.c_m, c.heads_msa, S, N, false, h->off.row, h->tc.row, seq_mask, true, false); break;
-    case 2: ok = d.attn_substep(msa, c.c_m, c.heads_msa, N, S, true, h->off.col, h->tc.col, msa_mask, false, false); break;
-    case 3: ok = d.transition_substep(msa, S, N, c.c_m, h->off.msa_trans, h->tc.mt_w1, h->tc.mt_w2); break;
+    case 1: ok = d.attn_substep(msa, c.c_m, c.heads_msa, S, N, false, h->off.row, h->tc.row, seq_mask, true, false, d.ar.f_msa,
+                                d.ar.rl_row, 0); break;
+    case 2: ok = d.attn_substep(msa, c.c_m, c.heads_msa, N, S, true, h->off.col, h->tc.col, msa_mask, false, false, d.ar.f_msat,
+                                d.ar.rl_col, 1); break;
+    case 3: ok = d.transition_substep(msa, S, N, c.c_m, h->off.msa_trans, h->tc.mt_w1, h->tc.mt_w2, d.ar.f_msa_lin); break;
     case 4: ok = d.opm_substep(); break;
     case 5: ok = d.trimul_substep(false); break;
     case 6: ok = d.trimul_substep(true); break;
     case 7: ok = d.attn_substep(pair, c.c_z, c.heads_pair, N, N, false, h->off.tri_start, h->tc.tri_start, seq_mask, false,
-                                true); break;
+                                true, d.ar.f_pair, d.ar.rl_tri, 2); break;
     case 8: ok = d.attn_substep(pair, c.c_z, c.heads_pair, N, N, true, h->off.tri_end, h->tc.tri_end, seq_mask, false,
-                                true); break;
-    case 9: ok = d.transition_substep(pair, N, N, c.c_z, h->off.pair_trans, h->tc.pt_w1, h->tc.pt_w2); break;
+                                true, d.ar.f_pair, d.ar.rl_tri, 2); break;
+    case 9: ok = d.transition_substep(pair, N, N, c.c_z, h->off.pair_trans, h->tc.pt_w1, h->tc.pt_w2, d.ar.f_pair_lin); break;
     default: d.err = "substep not in 1..9";
   }
   if (!ok) err = d.err;
