@@ -408,7 +408,7 @@ struct Driver {
     launch_tri_einsum_simt<T>(ACM, BCM, TCM, B * c.c_tri, N, Np, st);
     pe();
     pb(KK_LNC, 0.0, (double)P * c.c_tri * 8.0);
-    launch_lnc<T>(TCM, TN, w + t.ln_out_g, w + t.ln_out_b, B, c.c_tri, N, Np, st);
+    launch_lnc<T>(TCM, TN, w + t.ln_out_g, w + t.ln_out_b, nullptr, B, c.c_tri, N, Np, st);
     pe();
     Epi e = epi_base(EPI_RESID, g);
     e.bias = w + t.b_z;

@@ -90,6 +90,13 @@ struct pf_evoformer {
   std::vector<ProfRec> prof;
   std::vector<cudaEvent_t> ev_pool;
   size_t ev_used = 0;
+  // Fractions of the nominal (padded) work the mask-derived skipping leaves, computed on the host from the masks while
+  // profiling is on, so that the per-launch FLOP / byte tags count executed work only.  1.0 when not profiling.
+  struct WorkFrac {
+    double msa = 1, msat = 1, pair = 1, msa_lin = 1, pair_lin = 1;   // active 128-row tiles per geometry
+    double attn_row = 1, attn_col = 1, attn_tri = 1;                 // visited (row, key tile) pairs
+    double opm = 1, tri_k = 1, lnc = 1;                              // active j pairs, visited k-blocks, unpadded rows i
+  } frac;
   cudaEvent_t next_event() {
     if (ev_used == ev_pool.size()) {
       cudaEvent_t e;

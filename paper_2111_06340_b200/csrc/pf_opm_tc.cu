@@ -40,6 +40,13 @@ opm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ C
               const __grid_constant__ CUtensorMap tmW, const float* __restrict__ bout, const float* __restrict__ seq_mask,
               const float* __restrict__ msa_mask, float* __restrict__ z, int S, int N) {
   using SM = OpmSmem;
+  {
+    // both residues j of this CTA padded: every output is at a masked position (uniform over the CTA: exit before any setup)
+    const int jj = blockIdx.x * OP_BJ, bb = blockIdx.z;
+    bool any = false;
+    for (int e = 0; e < OP_BJ; ++e) any = any || (jj + e < N && seq_mask[(long)bb * N + jj + e] > 0.5f);
+    if (!any) return;
+  }
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = tc::align_smem_1024(smem_raw);
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem + SM::BAR_OFF);

@@ -249,9 +249,10 @@ template void launch_tri_einsum_simt<bf16>(const bf16*, const bf16*, float*, int
 template <typename T>
 __global__ void __launch_bounds__(256) lnc_kernel(const float* __restrict__ t, T* __restrict__ y,
                                                   const float* __restrict__ gamma, const float* __restrict__ beta,
-                                                  int C, int N, int Npad) {
+                                                  const float* __restrict__ seq_mask, int C, int N, int Npad) {
   extern __shared__ float tile[];   // [C][33]
   int j0 = blockIdx.x * 32, i = blockIdx.y, b = blockIdx.z;
+  if (seq_mask && seq_mask[(long)b * N + i] < 0.5f) return;   // padded row i: every output of it is at a masked position
   int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   for (int c = warp; c < C; c += 8) {
     int j = j0 + lane;
@@ -278,14 +279,14 @@ __global__ void __launch_bounds__(256) lnc_kernel(const float* __restrict__ t, T
 }
 
 template <typename T>
-void launch_lnc(const float* t_cm, T* y, const float* gamma, const float* beta, int B, int C, int N, int Npad,
-                cudaStream_t st) {
+void launch_lnc(const float* t_cm, T* y, const float* gamma, const float* beta, const float* seq_mask, int B, int C, int N,
+                int Npad, cudaStream_t st) {
   dim3 grid((N + 31) / 32, N, B);
-  lnc_kernel<T><<<grid, 256, C * 33 * sizeof(float), st>>>(t_cm, y, gamma, beta, C, N, Npad);
+  lnc_kernel<T><<<grid, 256, C * 33 * sizeof(float), st>>>(t_cm, y, gamma, beta, seq_mask, C, N, Npad);
 }
-template void launch_lnc<float>(const float*, float*, const float*, const float*, int, int, int, int, cudaStream_t);
-template void launch_lnc<bf16>(const float*, bf16*, const float*, const float*, int, int, int, int, cudaStream_t);
-template void launch_lnc<__half>(const float*, __half*, const float*, const float*, int, int, int, int, cudaStream_t);
+template void launch_lnc<float>(const float*, float*, const float*, const float*, const float*, int, int, int, int, cudaStream_t);
+template void launch_lnc<bf16>(const float*, bf16*, const float*, const float*, const float*, int, int, int, int, cudaStream_t);
+template void launch_lnc<__half>(const float*, __half*, const float*, const float*, const float*, int, int, int, int, cudaStream_t);
 
 // ---------------------------------------------------------------------------------------------
 // Outer-product-mean core (A.4): one block per (b, i, j).  a, b: [(b,s,i), c_opm] already masked by mu.

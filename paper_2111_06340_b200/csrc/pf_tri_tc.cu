@@ -20,7 +20,7 @@ constexpr int TRI_SMEM = TRI_BAR_OFF + 256 + 1024;
 
 __global__ void __launch_bounds__(TRI_THREADS, 2)
 tri_einsum_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
-                     float* __restrict__ t, int N, int Npad) {
+                     float* __restrict__ t, int N, int Npad, const int* __restrict__ key_tiles, int channels) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = tc::align_smem_1024(smem_raw);
   uint64_t* full = reinterpret_cast<uint64_t*>(smem + TRI_BAR_OFF);
@@ -29,7 +29,8 @@ tri_einsum_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(tmem_full + 1);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int j0 = blockIdx.x * TRI_BN, i0 = blockIdx.y * TRI_BM, bc = blockIdx.z;
-  const int num_kb = (N + TRI_BK - 1) / TRI_BK;
+  int num_kb = (N + TRI_BK - 1) / TRI_BK;
+  if (key_tiles) num_kb = min(num_kb, key_tiles[bc / channels]);   // operands are exactly zero at masked residues k
 
   if (warp == 0 && lane == 0) {
     tc::prefetch_tmap(&tmA);
@@ -102,7 +103,7 @@ tri_einsum_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
 }
 
 int launch_tri_einsum_tc(TmaCtx* ctx, const bf16* a_cm, const bf16* b_cm, float* t_cm, int batch, int N, int Npad,
-                         int num_sms, cudaStream_t st) {
+                         const int* key_tiles, int channels, int num_sms, cudaStream_t st) {
   (void)num_sms;
   CUtensorMap tmA, tmB;
   uint64_t d[3] = {(uint64_t)N, (uint64_t)N, (uint64_t)batch}, s[2] = {(uint64_t)Npad, (uint64_t)N * Npad};
@@ -119,7 +120,7 @@ int launch_tri_einsum_tc(TmaCtx* ctx, const bf16* a_cm, const bf16* b_cm, float*
     configured = true;
   }
   dim3 grid((N + TRI_BN - 1) / TRI_BN, (N + TRI_BM - 1) / TRI_BM, batch);
-  tri_einsum_tc_kernel<<<grid, TRI_THREADS, TRI_SMEM, st>>>(tmA, tmB, t_cm, N, Npad);
+  tri_einsum_tc_kernel<<<grid, TRI_THREADS, TRI_SMEM, st>>>(tmA, tmB, t_cm, N, Npad, key_tiles, channels);
   return 0;
 }
 

@@ -7,7 +7,9 @@
 // (R12) and log2(e) on the pair bias, so that the attention kernel's softmax runs in the exp2 domain.
 #include "pf_handle.h"
 
+#include <algorithm>
 #include <cstring>
+#include <vector>
 
 namespace pf {
 
@@ -163,8 +165,10 @@ struct TcDriver {
     return o;
   }
 
-  bool gemm2(const G2Desc& d, double out_bytes) {
-    double R = (double)d.B * d.D1 * d.D2;
+  // frac: share of the row tiles that is executed (mask-derived skipping), applied to the FLOP / byte tags
+  bool gemm2(const G2Desc& d, double out_bytes, double frac) {
+    double R = (double)d.B * d.D1 * d.D2 * frac;
+    out_bytes *= frac;
     double in_bytes = R * d.K * (d.a_mode == 0 ? 4.0 : 2.0);
     h->prof_begin(KK_LNGEMM, 2.0 * R * d.K * d.Nw, in_bytes + out_bytes + 2.0 * d.K * d.Nw, st);
     if (launch_gemm2(h->tma, d, h->num_sms, st) != 0) {
@@ -180,6 +184,8 @@ struct TcDriver {
   //   f_rows: active-tile flags of this row geometry; rl_off / rl_idx: the compacted row list of this attention (pf_flags.cu)
   bool attn_substep(float* res, int C, int H, int D1, int D2, bool transposed, const AttnW& a, const AttnT& at,
                     const float* keymask, bool row_bias, bool self_bias, size_t f_rows, size_t rl_off, int rl_idx) {
+    const double f_frac = rl_idx == 0 ? h->frac.msa : rl_idx == 1 ? h->frac.msat : h->frac.pair;
+    const double a_frac = rl_idx == 0 ? h->frac.attn_row : rl_idx == 1 ? h->frac.attn_col : h->frac.attn_tri;
     const pf_config& c = h->cfg;
     const double R = (double)B * D1 * D2;
     const int L = D2, Lp = pad8(L);
@@ -196,7 +202,7 @@ struct TcDriver {
       d.ops[0].scale = kLog2e;
       d.n_ops = 1;
       d.tile_active = flags(ar.f_pair);
-      if (!gemm2(d, (double)B * N * N * c.heads_msa * 2.0)) return false;
+      if (!gemm2(d, (double)B * N * N * c.heads_msa * 2.0, h->frac.pair)) return false;
     }
     {
       const int Nw = 4 * C + (self_bias ? H : 0);
@@ -223,11 +229,12 @@ struct TcDriver {
       }
       d.n_ops = n;
       d.tile_active = flags(f_rows);
-      if (!gemm2(d, R * 4.0 * C * 2.0 + (self_bias ? R * H * 2.0 : 0.0))) return false;
+      if (!gemm2(d, R * 4.0 * C * 2.0 + (self_bias ? R * H * 2.0 : 0.0), f_frac)) return false;
     }
     {
       double rows = R, Cc = C;
-      h->prof_begin(KK_ATTN, 4.0 * rows * L * Cc, 5.0 * rows * Cc * 2.0 + (BIAS ? (double)B * H * L * L * 2.0 : 0.0), st);
+      h->prof_begin(KK_ATTN, 4.0 * rows * L * Cc * a_frac,
+                    (5.0 * rows * Cc * 2.0 + (BIAS ? (double)B * H * L * L * 2.0 : 0.0)) * a_frac, st);
       if (launch_attn_tc(h->tma, QKG, VT, BIAS, keymask, O, B, D1, L, Lp, H, h->ws + rl_off, buf<int>(ar.rl_count) + rl_idx,
                          h->num_sms, st) != 0) {
         err = std::string("attn_tc: ") + tc_last_error();
@@ -242,12 +249,13 @@ struct TcDriver {
     for (int col = 0; col < C; col += 64) d.ops[n++] = op(G2_RESID, col);
     d.n_ops = n;
     d.tile_active = flags(f_rows);
-    return gemm2(d, R * C * 8.0);
+    return gemm2(d, R * C * 8.0, f_frac);
   }
 
   // A.3 / A.9: one fused kernel, the 4C-wide hidden activation stays on chip
   bool transition_substep(float* res, int D1, int D2, int C, const TransW& t, size_t w1t, size_t w2t, size_t f_lin) {
-    const double R = (double)B * D1 * D2, n4 = (double)h->cfg.transition_n * C;
+    const double R = (double)B * D1 * D2 * (C == h->cfg.c_m ? h->frac.msa_lin : h->frac.pair_lin);
+    const double n4 = (double)h->cfg.transition_n * C;
     h->prof_begin(KK_TRANS, 4.0 * R * n4 * C, R * C * 8.0 + 4.0 * n4 * C, st);
     if (launch_transition_tc(h->tma, res, (long)B * D1 * D2, C, w + t.ln_g, w + t.ln_b, w16 + w1t, w + t.b1, w16 + w2t,
                              w + t.b2, flags(f_lin), h->num_sms, st) != 0) {
@@ -278,8 +286,9 @@ struct TcDriver {
     d.ops[0].masked = 1;
     d.n_ops = 1;
     d.tile_active = flags(ar.f_msat);
-    if (!gemm2(d, M * 2.0 * c.c_opm * 2.0)) return false;
-    h->prof_begin(KK_OPM, 2.0 * P * cc * S + 2.0 * P * cc * c.c_z, 2.0 * M * c.c_opm * 2.0 + 8.0 * P * c.c_z, st);
+    if (!gemm2(d, M * 2.0 * c.c_opm * 2.0, h->frac.msat)) return false;
+    h->prof_begin(KK_OPM, (2.0 * P * cc * S + 2.0 * P * cc * c.c_z) * h->frac.opm,
+                  (2.0 * M * c.c_opm * 2.0 + 8.0 * P * c.c_z) * h->frac.opm, st);
     if (launch_opm_tc(h->tma, ABT, reinterpret_cast<const bf16*>(w16 + h->tc.opm_wout), w + o.bout, seq_mask, msa_mask,
                       pair, B, S, Sp, N, st) != 0) {
       err = std::string("opm_tc: ") + tc_last_error();
@@ -318,16 +327,17 @@ struct TcDriver {
       }
       d.n_ops = 10;
       d.tile_active = flags(ar.f_pair);
-      if (!gemm2(d, P * 3.0 * ct * 2.0)) return false;
+      if (!gemm2(d, P * 3.0 * ct * 2.0, h->frac.pair)) return false;
     }
-    h->prof_begin(KK_TRI, 2.0 * B * ct * (double)N * N * N, (double)B * ct * N * Np * 8.0, st);
-    if (launch_tri_einsum_tc(h->tma, ACM, BCM, TCM, B * ct, N, Np, h->num_sms, st) != 0) {
+    h->prof_begin(KK_TRI, 2.0 * B * ct * (double)N * N * N * h->frac.tri_k,
+                  (double)B * ct * N * Np * (4.0 * h->frac.tri_k + 4.0), st);
+    if (launch_tri_einsum_tc(h->tma, ACM, BCM, TCM, B * ct, N, Np, buf<int>(ar.kt_seq), ct, h->num_sms, st) != 0) {
       err = std::string("tri_einsum_tc: ") + tc_last_error();
       return false;
     }
     h->prof_end(st);
-    h->prof_begin(KK_LNC, 0.0, P * ct * 6.0, st);
-    launch_lnc<__half>(TCM, TN, w + t.ln_out_g, w + t.ln_out_b, B, ct, N, Np, st);
+    h->prof_begin(KK_LNC, 0.0, P * ct * 6.0 * h->frac.lnc, st);
+    launch_lnc<__half>(TCM, TN, w + t.ln_out_g, w + t.ln_out_b, seq_mask, B, ct, N, Np, st);
     h->prof_end(st);
     G2Desc d = desc_base(B, N, N, ct, c.c_z);
     d.a_mode = 1; d.A = TN; d.op_fmt = 1; d.Wt = w16 + (incoming ? h->tc.ti_wz : h->tc.to_wz); d.bias = w + t.b_z;
@@ -337,13 +347,96 @@ struct TcDriver {
     d.ops[1] = op(G2_RESID, 64);
     d.n_ops = 2;
     d.tile_active = flags(ar.f_pair);
-    return gemm2(d, P * c.c_z * 10.0);
+    return gemm2(d, P * c.c_z * 10.0, h->frac.pair);
   }
 };
 
 }  // namespace
 
+// Host restatement of the skipping rules of pf_flags.cu, used only while profiling to scale the FLOP / byte tags.
+static void host_work_fractions(pf_evoformer* h, const std::vector<float>& sg, const std::vector<float>& rho, int B, int S,
+                                int N) {
+  auto act = [&](int kind, int b, int x, int y, int D1, int D2) {
+    const float mx = (kind == 0 ? rho : sg)[(size_t)b * D1 + x], my = (kind == 1 ? rho : sg)[(size_t)b * D2 + y];
+    return mx * my > 0.5f;
+  };
+  auto tiles2d = [&](int kind, int D1, int D2) {
+    const int yt = g2_pick_yt(D2), xt = 128 / yt;
+    long on = 0, all = 0;
+    for (int b = 0; b < B; ++b)
+      for (int x0 = 0; x0 < D1; x0 += xt)
+        for (int y0 = 0; y0 < D2; y0 += yt, ++all) {
+          bool any = false;
+          for (int x = x0; x < x0 + xt && x < D1 && !any; ++x)
+            for (int y = y0; y < y0 + yt && y < D2 && !any; ++y) any = act(kind, b, x, y, D1, D2);
+          on += any;
+        }
+    return all ? (double)on / all : 1.0;
+  };
+  auto tiles_lin = [&](int kind, int D1, int D2) {
+    const long R = (long)B * D1 * D2, per = (long)D1 * D2;
+    long on = 0, all = 0;
+    for (long t0 = 0; t0 < R; t0 += 128, ++all) {
+      bool any = false;
+      for (long r = t0; r < t0 + 128 && r < R && !any; ++r) {
+        const int b = (int)(r / per), rem = (int)(r % per);
+        any = act(kind, b, rem / D2, rem % D2, D1, D2);
+      }
+      on += any;
+    }
+    return all ? (double)on / all : 1.0;
+  };
+  auto key_tiles = [&](const std::vector<float>& m, int b, int L) {
+    int last = 0;
+    for (int j = 0; j < L; ++j)
+      if (m[(size_t)b * L + j] > 0.5f) last = j;
+    return last / 64 + 1;
+  };
+  auto attn = [&](const std::vector<float>& rowm, int R, const std::vector<float>& keym, int L) {
+    const int nkt = (L + 63) / 64;
+    double on = 0;
+    for (int b = 0; b < B; ++b) {
+      const int kt = std::min(nkt, key_tiles(keym, b, L));
+      for (int r = 0; r < R; ++r)
+        if (rowm[(size_t)b * R + r] > 0.5f) on += kt;
+    }
+    return on / ((double)B * R * nkt);
+  };
+  pf_evoformer::WorkFrac f;
+  f.msa = tiles2d(0, S, N);
+  f.msat = tiles2d(1, N, S);
+  f.pair = tiles2d(2, N, N);
+  f.msa_lin = tiles_lin(0, S, N);
+  f.pair_lin = tiles_lin(2, N, N);
+  f.attn_row = attn(rho, S, sg, N);
+  f.attn_col = attn(sg, N, rho, S);
+  f.attn_tri = attn(sg, N, sg, N);
+  {
+    long on = 0, all = 0, rows = 0;
+    double kb = 0;
+    const int nkb = (N + 63) / 64;
+    for (int b = 0; b < B; ++b) {
+      for (int j = 0; j < N; j += 2, ++all) on += sg[(size_t)b * N + j] > 0.5f || (j + 1 < N && sg[(size_t)b * N + j + 1] > 0.5f);
+      for (int i = 0; i < N; ++i) rows += sg[(size_t)b * N + i] > 0.5f;
+      kb += std::min(nkb, key_tiles(sg, b, N));
+    }
+    f.opm = (double)on / all;
+    f.lnc = (double)rows / ((double)B * N);
+    f.tri_k = kb / ((double)B * nkb);
+  }
+  h->frac = f;
+}
+
 bool tc_prepare_flags(pf_evoformer* h, const float* seq_mask, const float* msa_mask, int B, int S, int N, cudaStream_t st) {
+  h->frac = pf_evoformer::WorkFrac();
+  if (h->prof_on) {
+    std::vector<float> sg((size_t)B * N), rho((size_t)B * S);
+    if (cudaMemcpyAsync(sg.data(), seq_mask, sg.size() * 4, cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+        cudaMemcpyAsync(rho.data(), msa_mask, rho.size() * 4, cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+        cudaStreamSynchronize(st) != cudaSuccess)
+      return false;
+    host_work_fractions(h, sg, rho, B, S, N);
+  }
   const Arena ar = arena_layout(h->cfg, B, S, N);
   auto fl = [&](size_t off) { return reinterpret_cast<unsigned char*>(h->ws + off); };
   const long M = (long)B * S * N, P = (long)B * N * N;
