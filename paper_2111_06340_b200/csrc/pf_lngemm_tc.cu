@@ -407,25 +407,28 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
       for (long tile = blockIdx.x; tile < p.num_tiles; tile += gridDim.x) {
         if (!tile_on(tile, p)) continue;
         const uint32_t abuf = it & 1;
-        {
-          // pull the next tile's rows of this warp into L2 while this tile is normalised: the register-staged loads below
-          // then see L2 latency, not HBM latency (bytes in flight per SM are bounded by the register file)
-          const long nxt = tile + gridDim.x;
-          if (nxt < p.num_tiles && lane < 16 && tile_on(nxt, p)) {
-            const TileCoord nc = tile_coord(nxt, p);
-            const int lr = pw * 16 + lane;
-            const int x = nc.x0 + (lr >> p.yt_shift), y = nc.y0 + (lr & (p.YT - 1));
-            if (x < p.D1 && y < p.D2) {
-              long srow = p.src_transposed ? ((long)nc.b * p.D2 + y) * p.D1 + x : ((long)nc.b * p.D1 + x) * p.D2 + y;
-              tc::prefetch_l2_bulk(p.src + srow * K, K * 4);
-            }
-          }
-        }
+        // Short-distance L2 prefetch: while a batch of RU rows is normalised, the next batch of this warp (the first batch of
+        // the next active tile after the last one) is pulled into L2, so the register-staged loads see L2 latency, not HBM
+        // latency (bytes in flight per SM are bounded by the register file).  A whole tile ahead was too far: with the
+        // output stream passing through L2 in between, a third of the prefetched lines were evicted before use.
+        const long nxt = tile + gridDim.x;
+        const bool nxt_on = nxt < p.num_tiles && tile_on(nxt, p);
+        const TileCoord ncd = tile_coord(nxt_on ? nxt : tile, p);
         tc::mbar_wait(&a_empty[abuf], ((it >> 1) & 1) ^ 1);
         const TileCoord tcd = tile_coord(tile, p);
         uint8_t* abase = smem + SM::A_OFF + abuf * SM::A_BYTES;
 #pragma unroll 1
         for (int r0 = 0; r0 < 16; r0 += RU) {
+          if (lane < RU && (r0 + RU < 16 || nxt_on)) {
+            const bool same = r0 + RU < 16;
+            const TileCoord& pc = same ? tcd : ncd;
+            const int lr = pw * 16 + (same ? r0 + RU : 0) + lane;
+            const int x = pc.x0 + (lr >> p.yt_shift), y = pc.y0 + (lr & (p.YT - 1));
+            if (x < p.D1 && y < p.D2) {
+              long srow = p.src_transposed ? ((long)pc.b * p.D2 + y) * p.D1 + x : ((long)pc.b * p.D1 + x) * p.D2 + y;
+              tc::prefetch_l2_bulk(p.src + srow * K, K * 4);
+            }
+          }
           float4 v[RU][NV];
 #pragma unroll
           for (int u = 0; u < RU; ++u) {
