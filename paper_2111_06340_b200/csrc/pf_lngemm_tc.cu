@@ -70,12 +70,13 @@ struct G2Smem {
   static constexpr int A_BYTES = 128 * K * 2;
   static constexpr int KB_BYTES = 128 * 128;            // one 64-wide k-block of the A tile
   static constexpr int W_STAGE = G2_BN * 64 * 2;        // 32 KB
-  static constexpr int W_STAGES = (K == 256) ? 2 : 4;
+  static constexpr int W_STAGES = 2;
+  static constexpr int ST_PER_TEAM = (K == 256) ? 1 : 2;   // staging tiles per epilogue team (K = 256 has no room for two)
   static constexpr int A_OFF = 0;
   static constexpr int W_OFF = 2 * A_BYTES;
   static constexpr int ST_OFF = W_OFF + W_STAGES * W_STAGE;
   static constexpr int ST_BYTES = 128 * 128;
-  static constexpr int BIAS_OFF = ST_OFF + 2 * ST_BYTES;   // fp32 bias of the current 256-column window
+  static constexpr int BIAS_OFF = ST_OFF + 2 * ST_PER_TEAM * ST_BYTES;   // fp32 bias of the current 256-column window
   static constexpr int BAR_OFF = BIAS_OFF + G2_BN * 4;
   static constexpr int TOTAL = BAR_OFF + 192 + 1024;
 };
@@ -210,7 +211,10 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
     const int bar_id = 1 + team;
     const int xl = lr >> p.yt_shift, yl = lr & (p.YT - 1);
     const uint32_t lane_addr = tmem_base + ((uint32_t)(quarter * 32) << 16);
-    uint8_t* sb = smem + SM::ST_OFF + team * SM::ST_BYTES;   // this team's staging tile
+    constexpr int NST = SM::ST_PER_TEAM;
+    uint8_t* const sb_team = smem + SM::ST_OFF + team * NST * SM::ST_BYTES;   // this team's staging tile(s)
+    uint32_t gcnt = 0;                                  // staging steps of this team so far
+    uint8_t* sb = sb_team;
     bf16* sb16 = reinterpret_cast<bf16*>(sb);
     float* sbias = reinterpret_cast<float*>(smem + SM::BIAS_OFF);
     const uint32_t sw = (uint32_t)(lr & 7);
@@ -247,7 +251,9 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
           const int kind = op.kind;
           if (kind == G2_SKIP) continue;
           if (kind == G2_ROW16) {
-            if (leader) tc::bulk_wait_read<0>();
+            sb = sb_team + (gcnt++ % NST) * SM::ST_BYTES;
+            sb16 = reinterpret_cast<bf16*>(sb);
+            if (leader) tc::bulk_wait_read<NST - 1>();
             tc::named_bar_sync(bar_id, 128);
             {
               const float scale = op.scale;
@@ -274,7 +280,9 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
           } else if (kind == G2_RESID) {
 #pragma unroll 1
             for (int hf = 0; hf < 2; ++hf) {
-              if (leader) tc::bulk_wait_read<0>();
+              sb = sb_team + (gcnt++ % NST) * SM::ST_BYTES;
+            sb16 = reinterpret_cast<bf16*>(sb);
+            if (leader) tc::bulk_wait_read<NST - 1>();
               tc::named_bar_sync(bar_id, 128);
               uint32_t v[32];
               float bb[32];
@@ -316,7 +324,9 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
           } else if (kind == G2_CM_DUAL) {
             // 64 channels of a gated, masked triangle operand, channel-major: staging tile [channel][x][y] (2-byte stores of
             // consecutive lanes are consecutive in shared memory), one TMA store with box {YT, XT, 64, 1}
-            if (leader) tc::bulk_wait_read<0>();
+            sb = sb_team + (gcnt++ % NST) * SM::ST_BYTES;
+            sb16 = reinterpret_cast<bf16*>(sb);
+            if (leader) tc::bulk_wait_read<NST - 1>();
             tc::named_bar_sync(bar_id, 128);
 #pragma unroll 1
             for (int hf = 0; hf < 2; ++hf) {
@@ -345,7 +355,9 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
             }
           } else if (kind == G2_HEADS) {
             // pair-bias heads [b, head, x, y]: staging tile [head][x][y], box {YT, XT, n_heads, 1}
-            if (leader) tc::bulk_wait_read<0>();
+            sb = sb_team + (gcnt++ % NST) * SM::ST_BYTES;
+            sb16 = reinterpret_cast<bf16*>(sb);
+            if (leader) tc::bulk_wait_read<NST - 1>();
             tc::named_bar_sync(bar_id, 128);
             uint32_t v[32];
             tc::tmem_ld32(tacc + j * 64, v);
@@ -361,7 +373,9 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
             }
           } else {   // G2_VT
             // 64 columns written transposed, [(b, x), column, y]: staging tile [x][column][y], box {YT, 64, XT, 1}
-            if (leader) tc::bulk_wait_read<0>();
+            sb = sb_team + (gcnt++ % NST) * SM::ST_BYTES;
+            sb16 = reinterpret_cast<bf16*>(sb);
+            if (leader) tc::bulk_wait_read<NST - 1>();
             tc::named_bar_sync(bar_id, 128);
             const float mk = op.masked ? mask : 1.0f;
             bf16* dst = sb16 + ((long)xl * 64 << p.yt_shift) + yl;
