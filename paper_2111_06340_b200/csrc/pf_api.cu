@@ -117,6 +117,8 @@ Arena pf::arena_layout(const pf_config& c, int B, int S, int N) {
   a.f_pair = take((size_t)g2_num_tiles(B, N, N));
   a.f_msa_lin = take((M + 127) / 128);
   a.f_pair_lin = take((P + 127) / 128);
+  a.f_pair_x = take((size_t)g2_num_tiles(B, N, N));
+  a.f_msat_x = take((size_t)g2_num_tiles(B, N, S));
   a.kt_seq = take((size_t)B * 4);
   a.kt_msa = take((size_t)B * 4);
   a.rl_row = take((size_t)B * S * 8);

@@ -3,14 +3,19 @@
 // (padded residues, masked MSA rows) produces only outputs at masked positions, which are unspecified (R3) and enter
 // every later sum with an exactly-zero weight.  Such tiles / units are skipped; what they would have written stays at
 // the (finite: the workspace is zero-filled at allocation) value it had.  Key tiles past the last unmasked key are
-// skipped as well (exact: their softmax weights are exactly 0).
+// skipped as well (exact: their softmax weights are exactly 0).  Exception: operands that are contracted over a masked
+// index without a softmax (triangle einsum over k, outer product over s) must be exactly zero there, so their projection
+// tiles are skipped only when the KEPT index is padded (kind 3).
 #include "pf_internal.h"
 
 namespace pf {
 
 // kind: 0 rows (b, s=x, i=y) of the MSA: rho_x sigma_y | 1 rows (b, i=x, s=y): sigma_x rho_y | 2 pair rows: sigma_x sigma_y
+//       3 rows (b, i=x, y) whose y index is CONTRACTED later (k of the triangle einsum, s of the outer product): only a
+//         padded residue x makes the row skippable; entries at masked y must be written (as exact zeros)
 __device__ __forceinline__ bool row_active(const float* seq_mask, const float* msa_mask, int kind, int b, int x, int y, int D1,
                                            int D2) {
+  if (kind == 3) return seq_mask[(long)b * D1 + x] > 0.5f;
   const float mx = (kind == 0 ? msa_mask : seq_mask)[(long)b * D1 + x];
   const float my = (kind == 1 ? msa_mask : seq_mask)[(long)b * D2 + y];
   return mx * my > 0.5f;

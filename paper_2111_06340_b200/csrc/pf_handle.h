@@ -61,7 +61,7 @@ inline int pad8(int v) { return (v + 7) / 8 * 8; }
 struct Arena {
   size_t x, qkg, vt, o, bias, acm, bcm, g, tcm, tn, oa, ob;
   // mask-derived work flags (pf_flags.cu): active-tile bytes per row geometry, key-tile counts per protein
-  size_t f_msa, f_msat, f_pair, f_msa_lin, f_pair_lin, kt_seq, kt_msa;
+  size_t f_msa, f_msat, f_pair, f_msa_lin, f_pair_lin, f_pair_x, f_msat_x, kt_seq, kt_msa;
   // compacted attention row lists {row, key tiles} + their lengths: row attention (b,s), column attention (b,i), triangle (b,i)
   size_t rl_row, rl_col, rl_tri, rl_count;
   size_t total;
@@ -93,7 +93,7 @@ struct pf_evoformer {
   // Fractions of the nominal (padded) work the mask-derived skipping leaves, computed on the host from the masks while
   // profiling is on, so that the per-launch FLOP / byte tags count executed work only.  1.0 when not profiling.
   struct WorkFrac {
-    double msa = 1, msat = 1, pair = 1, msa_lin = 1, pair_lin = 1;   // active 128-row tiles per geometry
+    double msa = 1, msat = 1, pair = 1, msa_lin = 1, pair_lin = 1, pair_x = 1, msat_x = 1;   // active 128-row tiles per geometry
     double attn_row = 1, attn_col = 1, attn_tri = 1;                 // visited (row, key tile) pairs
     double opm = 1, tri_k = 1, lnc = 1;                              // active j pairs, visited k-blocks, unpadded rows i
   } frac;

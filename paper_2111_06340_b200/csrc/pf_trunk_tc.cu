@@ -285,8 +285,8 @@ struct TcDriver {
     d.ops[0] = op(G2_VT, 0, 2 * c.c_opm);
     d.ops[0].masked = 1;
     d.n_ops = 1;
-    d.tile_active = flags(ar.f_msat);
-    if (!gemm2(d, M * 2.0 * c.c_opm * 2.0, h->frac.msat)) return false;
+    d.tile_active = flags(ar.f_msat_x);   // a, b are summed over s: masked s must be written as zeros
+    if (!gemm2(d, M * 2.0 * c.c_opm * 2.0, h->frac.msat_x)) return false;
     h->prof_begin(KK_OPM, (2.0 * P * cc * S + 2.0 * P * cc * c.c_z) * h->frac.opm,
                   (2.0 * M * c.c_opm * 2.0 + 8.0 * P * c.c_z) * h->frac.opm, st);
     if (launch_opm_tc(h->tma, ABT, reinterpret_cast<const bf16*>(w16 + h->tc.opm_wout), w + o.bout, seq_mask, msa_mask,
@@ -326,8 +326,8 @@ struct TcDriver {
         d.ops[8 + j].fmt = 1;
       }
       d.n_ops = 10;
-      d.tile_active = flags(ar.f_pair);
-      if (!gemm2(d, P * 3.0 * ct * 2.0, h->frac.pair)) return false;
+      d.tile_active = flags(ar.f_pair_x);   // a, b are summed over k: masked k must be written as zeros
+      if (!gemm2(d, P * 3.0 * ct * 2.0, h->frac.pair_x)) return false;
     }
     h->prof_begin(KK_TRI, 2.0 * B * ct * (double)N * N * N * h->frac.tri_k,
                   (double)B * ct * N * Np * (4.0 * h->frac.tri_k + 4.0), st);
@@ -357,6 +357,7 @@ struct TcDriver {
 static void host_work_fractions(pf_evoformer* h, const std::vector<float>& sg, const std::vector<float>& rho, int B, int S,
                                 int N) {
   auto act = [&](int kind, int b, int x, int y, int D1, int D2) {
+    if (kind == 3) return sg[(size_t)b * D1 + x] > 0.5f;
     const float mx = (kind == 0 ? rho : sg)[(size_t)b * D1 + x], my = (kind == 1 ? rho : sg)[(size_t)b * D2 + y];
     return mx * my > 0.5f;
   };
@@ -406,6 +407,8 @@ static void host_work_fractions(pf_evoformer* h, const std::vector<float>& sg, c
   f.msa = tiles2d(0, S, N);
   f.msat = tiles2d(1, N, S);
   f.pair = tiles2d(2, N, N);
+  f.pair_x = tiles2d(3, N, N);
+  f.msat_x = tiles2d(3, N, S);
   f.msa_lin = tiles_lin(0, S, N);
   f.pair_lin = tiles_lin(2, N, N);
   f.attn_row = attn(rho, S, sg, N);
@@ -445,10 +448,12 @@ bool tc_prepare_flags(pf_evoformer* h, const float* seq_mask, const float* msa_m
     const int yt = g2_pick_yt(N);
     launch_tile_flags(seq_mask, msa_mask, 0, B, S, N, 128 / yt, yt, fl(ar.f_msa), g2_num_tiles(B, S, N), st);
     launch_tile_flags(seq_mask, msa_mask, 2, B, N, N, 128 / yt, yt, fl(ar.f_pair), g2_num_tiles(B, N, N), st);
+    launch_tile_flags(seq_mask, msa_mask, 3, B, N, N, 128 / yt, yt, fl(ar.f_pair_x), g2_num_tiles(B, N, N), st);
   }
   {
     const int yt = g2_pick_yt(S);
     launch_tile_flags(seq_mask, msa_mask, 1, B, N, S, 128 / yt, yt, fl(ar.f_msat), g2_num_tiles(B, N, S), st);
+    launch_tile_flags(seq_mask, msa_mask, 3, B, N, S, 128 / yt, yt, fl(ar.f_msat_x), g2_num_tiles(B, N, S), st);
   }
   launch_tile_flags(seq_mask, msa_mask, 0, B, S, N, 0, 0, fl(ar.f_msa_lin), (M + 127) / 128, st);
   launch_tile_flags(seq_mask, msa_mask, 2, B, N, N, 0, 0, fl(ar.f_pair_lin), (P + 127) / 128, st);
@@ -461,7 +466,7 @@ bool tc_prepare_flags(pf_evoformer* h, const float* seq_mask, const float* msa_m
   launch_row_list(seq_mask, kt_msa, B, N, h->ws + ar.rl_col, cnt + 1, st);   // column attention: rows (b, i), keys = sequences
   launch_row_list(seq_mask, kt_seq, B, N, h->ws + ar.rl_tri, cnt + 2, st);   // triangle attention: rows (b, i), keys = residues
   h->prof_end(st);
-  h->launches += 9;   // prof_begin counted one of the ten
+  h->launches += 11;   // prof_begin counted one of the twelve
   return cudaGetLastError() == cudaSuccess;
 }
 

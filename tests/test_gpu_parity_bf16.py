@@ -64,6 +64,48 @@ def test_runtime_shapes(B, S, N):
     _check(m, z, mr, zr, sm, mm, f"B{B} S{S} N{N}")
 
 
+def test_medium_protein_many_tiles():
+    """A medium single protein with full masks plus one with a padded tail: N_res = 200 (two 128-query tiles, four 64-key
+    tiles, row tiles of every geometry), N_seq = 96, one teacher-forced block checked element by element."""
+    B, S, N = 2, 96, 200
+    blocks = ps.make_weights(21, 1, bf16_weights=True)
+    msa, pair, sm, mm = ps.make_inputs(22, B, S, N, lengths=[200, 131], msa_mask_frac_max=0.2)
+    m, z = run_cuda(pf.PF_BF16, blocks, msa, pair, sm, mm)
+    mr, zr = run_oracle(blocks, msa, pair, sm, mm)
+    assert np.isfinite(m).all() and np.isfinite(z).all()
+    _check(m, z, mr, zr, sm, mm, "medium protein")
+
+
+@pytest.mark.parametrize("Np,Sp", [(140, 40), (192, 24), (128, 33)])
+def test_masked_work_is_skipped_not_needed(Np, Sp):
+    """Skipping of fully masked tiles / rows / key tiles (pf_flags.cu) must not change unmasked outputs: the same proteins
+    embedded in a larger padded problem (bucket Np, N_seq Sp), with different garbage in the padding, give the same unmasked
+    outputs up to the rounding of a different tile decomposition.  Run as ONE block so that later sub-steps see the stale
+    workspace contents earlier sub-steps left at skipped positions (operands contracted over a masked index must be
+    exact zeros there: this test failed before the kind-3 flags of pf_flags.cu)."""
+    blocks = ps.make_weights(31, 1, bf16_weights=True)
+    msa, pair, sm, mm = ps.make_inputs(32, 2, 24, 70, lengths=[70, 40], msa_mask_frac_max=0.3)
+    m1, z1 = run_cuda(pf.PF_BF16, blocks, msa, pair, sm, mm)
+    r = ps.rng(33, 1)
+    msa2 = (3.0 * r.standard_normal((2, Sp, Np, 256))).astype(np.float32)
+    pair2 = (3.0 * r.standard_normal((2, Np, Np, 128))).astype(np.float32)
+    msa2[:, :24, :70] = msa
+    pair2[:, :70, :70] = pair
+    sm2 = np.zeros((2, Np), np.float32)
+    sm2[:, :70] = sm
+    mm2 = np.zeros((2, Sp), np.float32)
+    mm2[:, :24] = mm
+    m2, z2 = run_cuda(pf.PF_BF16, blocks, msa2, pair2, sm2, mm2)
+    assert np.isfinite(m2).all() and np.isfinite(z2).all()
+    vm, vz = valid_masks(sm, mm)
+    em, rm = errors(m2[:, :24, :70], m1, vm)
+    ez, rz = errors(z2[:, :70, :70], z1, vz)
+    print(f"embedding: m max-abs {em:.3e} mean-rel {rm:.3e}; z max-abs {ez:.3e} mean-rel {rz:.3e}")
+    assert em <= TOL_ABS and ez <= TOL_ABS and rm <= TOL_REL and rz <= TOL_REL
+    mr, zr = run_oracle(blocks, msa, pair, sm, mm)
+    _check(m2[:, :24, :70], z2[:, :70, :70], mr, zr, sm, mm, "embedded vs oracle")
+
+
 def test_cfg2_full_size_sampled_proteins():
     """BASELINE.json configs[1] at full size in bench.py's launch configuration (B=64, N_seq=128, bucket 128, masks per
     R11), one teacher-forced block; the oracle recomputes two whole proteins of the batch (the two shortest, to bound
