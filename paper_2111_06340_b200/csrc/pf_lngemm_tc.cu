@@ -38,7 +38,7 @@ constexpr int G2_EPI_WARPS = 8;
 constexpr int G2_PROD_WARPS = 8;
 
 struct G2Params {
-  int B, D1, D2, XT, YT, yt_shift, tiles_x_per_b, tiles_y;
+  int B, D1, D2, XT, YT, yt_shift, ytw_shift, tiles_x_per_b, tiles_y;
   long num_tiles;
   int Nw, n_tiles;
   const float* src;
@@ -75,7 +75,8 @@ struct G2Smem {
   static constexpr int A_OFF = 0;
   static constexpr int W_OFF = 2 * A_BYTES;
   static constexpr int ST_OFF = W_OFF + W_STAGES * W_STAGE;
-  static constexpr int ST_BYTES = 128 * 128;
+  static constexpr int ST_BYTES = 128 * 128;            // per team of four warps; each warp owns a quarter (32 rows x 128 B)
+  static constexpr int STW_BYTES = 32 * 128;
   static constexpr int BIAS_OFF = ST_OFF + 2 * ST_PER_TEAM * ST_BYTES;   // fp32 bias of the current 256-column window
   static constexpr int BAR_OFF = BIAS_OFF + G2_BN * 4;
   static constexpr int TOTAL = BAR_OFF + 192 + 1024;
@@ -204,16 +205,19 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
   const uint32_t tmem_base = *tmem_slot;
 
   if (warp < G2_EPI_WARPS) {
-    // =========================================================== epilogue (two teams of four warps)
+    // =========================================================== epilogue: eight free-running warps.  Warp w owns the 32 tile
+    // rows of TMEM lane quarter w % 4 and the 64-column groups j with j % 2 == w / 4; it stages its 32 x 128 B piece in its
+    // own shared-memory tile and issues its own TMA store, so no barrier couples it to any other warp.
     const int team = warp >> 2, quarter = warp & 3;
     const int lr = quarter * 32 + lane;                // tile row = TMEM lane
-    const bool leader = (threadIdx.x & 127) == 0;
-    const int bar_id = 1 + team;
+    const bool leader = lane == 0;
     const int xl = lr >> p.yt_shift, yl = lr & (p.YT - 1);
+    const int xw0 = (quarter * 32) >> p.yt_shift, yw0 = (quarter * 32) & (p.YT - 1);   // first row of this warp in the tile
+    const int xlw = lane >> p.ytw_shift, ylw = lane & ((1 << p.ytw_shift) - 1);         // this row inside the warp's box
     const uint32_t lane_addr = tmem_base + ((uint32_t)(quarter * 32) << 16);
     constexpr int NST = SM::ST_PER_TEAM;
-    uint8_t* const sb_team = smem + SM::ST_OFF + team * NST * SM::ST_BYTES;   // this team's staging tile(s)
-    uint32_t gcnt = 0;                                  // staging steps of this team so far
+    uint8_t* const sb_team = smem + SM::ST_OFF + (team * 4 + quarter) * NST * SM::STW_BYTES;   // this warp's staging tile(s)
+    uint32_t gcnt = 0;                                  // staging steps of this warp so far
     uint8_t* sb = sb_team;
     bf16* sb16 = reinterpret_cast<bf16*>(sb);
     float* sbias = reinterpret_cast<float*>(smem + SM::BIAS_OFF);
@@ -251,14 +255,14 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
           const int kind = op.kind;
           if (kind == G2_SKIP) continue;
           if (kind == G2_ROW16) {
-            sb = sb_team + (gcnt++ % NST) * SM::ST_BYTES;
+            sb = sb_team + (gcnt++ % NST) * SM::STW_BYTES;
             sb16 = reinterpret_cast<bf16*>(sb);
             if (leader) tc::bulk_wait_read<NST - 1>();
-            tc::named_bar_sync(bar_id, 128);
+            __syncwarp();
             {
               const float scale = op.scale;
               const uint32_t ta = tacc + j * 64;
-              uint8_t* srow = sb + lr * 128;
+              uint8_t* srow = sb + lane * 128;
               const float* b64 = sbias + j * 64;
               if (op.act == ACT_SIGMOID) {
                 if (op.fmt) g2_row16_group<ACT_SIGMOID, 1>(ta, srow, b64, scale, sw);
@@ -272,18 +276,18 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
               }
             }
             tc::fence_proxy_async_smem();
-            tc::named_bar_sync(bar_id, 128);
+            __syncwarp();
             if (leader) {
-              tc::tma_store_4d(&tmO0, sb, op.dst_col, tcd.y0, tcd.x0, tcd.b);
+              tc::tma_store_4d(&tmO0, sb, op.dst_col, tcd.y0 + yw0, tcd.x0 + xw0, tcd.b);
               tc::bulk_commit();
             }
           } else if (kind == G2_RESID) {
 #pragma unroll 1
             for (int hf = 0; hf < 2; ++hf) {
-              sb = sb_team + (gcnt++ % NST) * SM::ST_BYTES;
+              sb = sb_team + (gcnt++ % NST) * SM::STW_BYTES;
             sb16 = reinterpret_cast<bf16*>(sb);
             if (leader) tc::bulk_wait_read<NST - 1>();
-              tc::named_bar_sync(bar_id, 128);
+              __syncwarp();
               uint32_t v[32];
               float bb[32];
               tc::tmem_ld32(tacc + j * 64 + hf * 32, v);
@@ -312,22 +316,22 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
               }
 #pragma unroll
               for (int c = 0; c < 8; ++c)
-                *reinterpret_cast<float4*>(sb + lr * 128 + (((uint32_t)c ^ sw) << 4)) =
+                *reinterpret_cast<float4*>(sb + lane * 128 + (((uint32_t)c ^ sw) << 4)) =
                     make_float4(f[c * 4], f[c * 4 + 1], f[c * 4 + 2], f[c * 4 + 3]);
               tc::fence_proxy_async_smem();
-              tc::named_bar_sync(bar_id, 128);
+              __syncwarp();
               if (leader) {
-                tc::tma_reduce_add_4d(&tmR, sb, op.dst_col + hf * 32, tcd.y0, tcd.x0, tcd.b);
+                tc::tma_reduce_add_4d(&tmR, sb, op.dst_col + hf * 32, tcd.y0 + yw0, tcd.x0 + xw0, tcd.b);
                 tc::bulk_commit();
               }
             }
           } else if (kind == G2_CM_DUAL) {
             // 64 channels of a gated, masked triangle operand, channel-major: staging tile [channel][x][y] (2-byte stores of
             // consecutive lanes are consecutive in shared memory), one TMA store with box {YT, XT, 64, 1}
-            sb = sb_team + (gcnt++ % NST) * SM::ST_BYTES;
+            sb = sb_team + (gcnt++ % NST) * SM::STW_BYTES;
             sb16 = reinterpret_cast<bf16*>(sb);
             if (leader) tc::bulk_wait_read<NST - 1>();
-            tc::named_bar_sync(bar_id, 128);
+            __syncwarp();
 #pragma unroll 1
             for (int hf = 0; hf < 2; ++hf) {
               uint32_t v[32], g[32];
@@ -345,40 +349,40 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
                 r[e] = __float2bfloat16_rn(mask * gv * pv);
               }
 #pragma unroll
-              for (int e = 0; e < 32; ++e) sb16[(hf * 32 + e) * 128 + lr] = r[e];
+              for (int e = 0; e < 32; ++e) sb16[(hf * 32 + e) * 32 + lane] = r[e];
             }
             tc::fence_proxy_async_smem();
-            tc::named_bar_sync(bar_id, 128);
+            __syncwarp();
             if (leader) {
-              tc::tma_store_4d(op.map ? &tmT1 : &tmT0, sb, tcd.y0, tcd.x0, op.dst_col, tcd.b);
+              tc::tma_store_4d(op.map ? &tmT1 : &tmT0, sb, tcd.y0 + yw0, tcd.x0 + xw0, op.dst_col, tcd.b);
               tc::bulk_commit();
             }
           } else if (kind == G2_HEADS) {
             // pair-bias heads [b, head, x, y]: staging tile [head][x][y], box {YT, XT, n_heads, 1}
-            sb = sb_team + (gcnt++ % NST) * SM::ST_BYTES;
+            sb = sb_team + (gcnt++ % NST) * SM::STW_BYTES;
             sb16 = reinterpret_cast<bf16*>(sb);
             if (leader) tc::bulk_wait_read<NST - 1>();
-            tc::named_bar_sync(bar_id, 128);
+            __syncwarp();
             uint32_t v[32];
             tc::tmem_ld32(tacc + j * 64, v);
             tc::tmem_ld_wait();
 #pragma unroll
             for (int e = 0; e < 8; ++e)
-              if (e < op.ncols) sb16[e * 128 + lr] = __float2bfloat16_rn(__uint_as_float(v[e]) * op.scale);
+              if (e < op.ncols) sb16[e * 32 + lane] = __float2bfloat16_rn(__uint_as_float(v[e]) * op.scale);
             tc::fence_proxy_async_smem();
-            tc::named_bar_sync(bar_id, 128);
+            __syncwarp();
             if (leader) {
-              tc::tma_store_4d(&tmH, sb, tcd.y0, tcd.x0, op.dst_col, tcd.b);
+              tc::tma_store_4d(&tmH, sb, tcd.y0 + yw0, tcd.x0 + xw0, op.dst_col, tcd.b);
               tc::bulk_commit();
             }
           } else {   // G2_VT
             // 64 columns written transposed, [(b, x), column, y]: staging tile [x][column][y], box {YT, 64, XT, 1}
-            sb = sb_team + (gcnt++ % NST) * SM::ST_BYTES;
+            sb = sb_team + (gcnt++ % NST) * SM::STW_BYTES;
             sb16 = reinterpret_cast<bf16*>(sb);
             if (leader) tc::bulk_wait_read<NST - 1>();
-            tc::named_bar_sync(bar_id, 128);
+            __syncwarp();
             const float mk = op.masked ? mask : 1.0f;
-            bf16* dst = sb16 + ((long)xl * 64 << p.yt_shift) + yl;
+            bf16* dst = sb16 + ((xlw * 64) << p.ytw_shift) + ylw;
 #pragma unroll 1
             for (int hf = 0; hf < 2; ++hf) {
               uint32_t v[32];
@@ -390,12 +394,12 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
 #pragma unroll
               for (int e = 0; e < 32; ++e) r[e] = __float2bfloat16_rn((__uint_as_float(v[e]) + bb[e]) * mk);
 #pragma unroll
-              for (int e = 0; e < 32; ++e) dst[(hf * 32 + e) << p.yt_shift] = r[e];
+              for (int e = 0; e < 32; ++e) dst[(hf * 32 + e) << p.ytw_shift] = r[e];
             }
             tc::fence_proxy_async_smem();
-            tc::named_bar_sync(bar_id, 128);
+            __syncwarp();
             if (leader) {
-              tc::tma_store_4d(&tmT0, sb, tcd.y0, op.dst_col, tcd.x0, tcd.b);
+              tc::tma_store_4d(&tmT0, sb, tcd.y0 + yw0, op.dst_col, tcd.x0 + xw0, tcd.b);
               tc::bulk_commit();
             }
           }
@@ -644,6 +648,9 @@ int launch_gemm2(TmaCtx* ctx, const G2Desc& d, int num_sms, cudaStream_t st) {
   }
   const uint64_t D1 = d.D1, D2 = d.D2, Bn = d.B, Lp = d.Lpad;
   const uint32_t YT = (uint32_t)p.YT, XT = (uint32_t)p.XT;
+  const uint32_t YTW = YT < 32 ? YT : 32, XTW = 32 / YTW;   // the 32 rows one epilogue warp stores: YTW consecutive y of XTW x
+  p.ytw_shift = 0;
+  while ((1u << p.ytw_shift) < YTW) ++p.ytw_shift;
   if (d.a_mode == 1) {
     uint64_t dims[4] = {(uint64_t)d.K, D2, D1, Bn};
     uint64_t str[3] = {(uint64_t)d.K * 2, D2 * d.K * 2, D1 * D2 * d.K * 2};
@@ -656,7 +663,7 @@ int launch_gemm2(TmaCtx* ctx, const G2Desc& d, int num_sms, cudaStream_t st) {
     uint64_t ld = d.row_ld[0];
     uint64_t dims[4] = {ld, D2, D1, Bn};
     uint64_t str[3] = {ld * 2, D2 * ld * 2, D1 * D2 * ld * 2};
-    uint32_t box[4] = {64, YT, XT, 1};
+    uint32_t box[4] = {64, YTW, XTW, 1};
     if (tma_encode(ctx, &tmO0, d.row_out[0], 0, 4, dims, str, box, 128) != 0) return -1;
   } else {
     tmO0 = tmW;
@@ -670,7 +677,7 @@ int launch_gemm2(TmaCtx* ctx, const G2Desc& d, int num_sms, cudaStream_t st) {
     uint64_t vc = d.vt_cols;
     uint64_t dims[4] = {D2, vc, D1, Bn};
     uint64_t str[3] = {Lp * 2, vc * Lp * 2, D1 * vc * Lp * 2};
-    uint32_t box[4] = {YT, 64, XT, 1};
+    uint32_t box[4] = {YTW, 64, XTW, 1};
     if (tma_encode(ctx, &tmT[0], d.vt_out, 0, 4, dims, str, box, 0) != 0) return -1;
   }
   for (int i = 0; i < 2; ++i) {
@@ -678,14 +685,14 @@ int launch_gemm2(TmaCtx* ctx, const G2Desc& d, int num_sms, cudaStream_t st) {
     uint64_t ch = d.cm_channels;
     uint64_t dims[4] = {D2, D1, ch, Bn};
     uint64_t str[3] = {Lp * 2, D1 * Lp * 2, ch * D1 * Lp * 2};
-    uint32_t box[4] = {YT, XT, 64, 1};
+    uint32_t box[4] = {YTW, XTW, 64, 1};
     if (tma_encode(ctx, &tmT[i], d.cm_out[i], 0, 4, dims, str, box, 0) != 0) return -1;
   }
   if (d.heads_out) {   // [(b, head), x, y] with row pitch Lpad
     uint64_t nh = d.n_heads;
     uint64_t dims[4] = {D2, D1, nh, Bn};
     uint64_t str[3] = {Lp * 2, D1 * Lp * 2, nh * D1 * Lp * 2};
-    uint32_t box[4] = {YT, XT, (uint32_t)d.n_heads, 1};
+    uint32_t box[4] = {YTW, XTW, (uint32_t)d.n_heads, 1};
     if (tma_encode(ctx, &tmH, d.heads_out, 0, 4, dims, str, box, 0) != 0) return -1;
   }
   if (d.resid) {
@@ -697,7 +704,7 @@ int launch_gemm2(TmaCtx* ctx, const G2Desc& d, int num_sms, cudaStream_t st) {
     } else {
       str[0] = ld * 4; str[1] = D2 * ld * 4; str[2] = D1 * D2 * ld * 4;
     }
-    uint32_t box[4] = {32, (uint32_t)p.YT, (uint32_t)p.XT, 1};
+    uint32_t box[4] = {32, YTW, XTW, 1};
     if (tma_encode(ctx, &tmR, d.resid, 2, 4, dims, str, box, 128) != 0) return -1;
   } else {
     tmR = tmW;
