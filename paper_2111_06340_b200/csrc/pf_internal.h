@@ -122,6 +122,8 @@ struct G2Desc {
   int op_fmt;               // MMA operand format: 0 bf16, 1 fp16 (A and Wt alike)
   const void* Wt;           // [Nw, K] 16-bit, K contiguous
   const float* bias;        // [Nw] fp32 or null
+  int bias_lo, bias_n;      // columns [bias_lo, bias_lo + bias_n) may be non-zero (bias_n = 0: [bias_lo, Nw)); multiples of 64,
+                            // at most 256 (K = 256) / 768 (K = 128) columns: the kernel keeps this range in shared memory
   int rowmask;              // RowMaskKind, applied by CM_DUAL and masked VT groups
   const float* seq_mask;
   const float* msa_mask;

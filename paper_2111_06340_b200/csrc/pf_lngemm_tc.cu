@@ -61,6 +61,7 @@ struct G2Params {
   int vt_cols;
   int Lpad;
   const unsigned char* tile_active;
+  int bias_lo, bias_n;    // the bias table holds columns [bias_lo, bias_lo + bias_n); all other columns have zero bias
   G2Op ops[G2_MAX_OPS];
 };
 
@@ -77,8 +78,11 @@ struct G2Smem {
   static constexpr int ST_OFF = W_OFF + W_STAGES * W_STAGE;
   static constexpr int ST_BYTES = 128 * 128;            // per team of four warps; each warp owns a quarter (32 rows x 128 B)
   static constexpr int STW_BYTES = 32 * 128;
-  static constexpr int BIAS_OFF = ST_OFF + 2 * ST_PER_TEAM * ST_BYTES;   // fp32 bias of the current 256-column window
-  static constexpr int BAR_OFF = BIAS_OFF + G2_BN * 4;
+  // fp32 bias table, staged ONCE per CTA: columns [bias_lo, bias_lo + BIAS_FLOATS) of the bias vector, followed by 64 zeros
+  // that stand in for every 64-column group outside the table (q, k, v of the attention projections carry no bias)
+  static constexpr int BIAS_FLOATS = (K == 256) ? 256 : 768;
+  static constexpr int BIAS_OFF = ST_OFF + 2 * ST_PER_TEAM * ST_BYTES;
+  static constexpr int BAR_OFF = BIAS_OFF + (BIAS_FLOATS + 64) * 4;
   static constexpr int TOTAL = BAR_OFF + 192 + 1024;
 };
 
@@ -199,6 +203,8 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
     tc::fence_barrier_init();
   }
   if (warp == 17) tc::tmem_alloc<512>(tmem_slot);
+  for (int i = threadIdx.x; i < SM::BIAS_FLOATS + 64; i += G2_THREADS)
+    reinterpret_cast<float*>(smem + SM::BIAS_OFF)[i] = (p.bias && i < p.bias_n) ? __ldg(p.bias + p.bias_lo + i) : 0.f;
   tc::tc_fence_before();
   __syncthreads();
   tc::tc_fence_after();
@@ -220,7 +226,7 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
     uint32_t gcnt = 0;                                  // staging steps of this warp so far
     uint8_t* sb = sb_team;
     bf16* sb16 = reinterpret_cast<bf16*>(sb);
-    float* sbias = reinterpret_cast<float*>(smem + SM::BIAS_OFF);
+    const float* const sbias_tab = reinterpret_cast<const float*>(smem + SM::BIAS_OFF);
     const uint32_t sw = (uint32_t)(lr & 7);
     uint32_t ac = 0;                                   // accumulator buffers consumed so far
     for (long tile = blockIdx.x; tile < p.num_tiles; tile += gridDim.x) {
@@ -238,14 +244,6 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
       const long grow = ((long)tcd.b * p.D1 + x) * p.D2 + y;   // GEMM row index (gate rows)
       for (int nt = 0; nt < p.n_tiles; ++nt, ++ac) {
         const uint32_t buf = ac & 1;
-        if (p.n_tiles > 1 || ac == 0) {
-          // bias of this 256-column window -> shared memory (global loads here would sit on the epilogue's critical path:
-          // the streaming LayerNorm loads keep evicting them from L1)
-          tc::named_bar_sync(3, G2_EPI_WARPS * 32);
-          const int n = nt * G2_BN + (int)threadIdx.x;
-          sbias[threadIdx.x] = (p.bias && n < p.Nw) ? __ldg(p.bias + n) : 0.f;
-          tc::named_bar_sync(3, G2_EPI_WARPS * 32);
-        }
         tc::mbar_wait(&acc_full[buf], (ac >> 1) & 1);
         tc::tc_fence_after();
         const uint32_t tacc = lane_addr + buf * G2_BN;
@@ -254,6 +252,11 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
           const G2Op& op = p.ops[nt * 4 + j];
           const int kind = op.kind;
           if (kind == G2_SKIP) continue;
+          // this group's 64 bias values: inside the table, or the zero pad behind it
+          const int bcol = nt * G2_BN + j * 64 - p.bias_lo;
+          const float* const sbias = sbias_tab + ((bcol >= 0 && bcol + 64 <= p.bias_n) ? bcol : SM::BIAS_FLOATS);
+          const int bcol2 = bcol + 128;   // gate partner of a dual group
+          const float* const sbias2 = sbias_tab + ((bcol2 >= 0 && bcol2 + 64 <= p.bias_n) ? bcol2 : SM::BIAS_FLOATS);
           if (kind == G2_ROW16) {
             sb = sb_team + (gcnt++ % NST) * SM::STW_BYTES;
             sb16 = reinterpret_cast<bf16*>(sb);
@@ -263,7 +266,7 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
               const float scale = op.scale;
               const uint32_t ta = tacc + j * 64;
               uint8_t* srow = sb + lane * 128;
-              const float* b64 = sbias + j * 64;
+              const float* b64 = sbias;
               if (op.act == ACT_SIGMOID) {
                 if (op.fmt) g2_row16_group<ACT_SIGMOID, 1>(ta, srow, b64, scale, sw);
                 else g2_row16_group<ACT_SIGMOID, 0>(ta, srow, b64, scale, sw);
@@ -291,7 +294,7 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
               uint32_t v[32];
               float bb[32];
               tc::tmem_ld32(tacc + j * 64 + hf * 32, v);
-              lds32(sbias + j * 64 + hf * 32, bb);
+              lds32(sbias + hf * 32, bb);
               const __half* gp = (p.gate && valid) ? p.gate + grow * p.ldg + op.dst_col + hf * 32 : nullptr;
               uint4 gu[4];
               if (gp) {
@@ -338,8 +341,8 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
               float bp[32], bg[32];
               tc::tmem_ld32(tacc + j * 64 + hf * 32, v);
               tc::tmem_ld32(tacc + 128 + j * 64 + hf * 32, g);
-              lds32(sbias + j * 64 + hf * 32, bp);
-              lds32(sbias + 128 + j * 64 + hf * 32, bg);
+              lds32(sbias + hf * 32, bp);
+              lds32(sbias2 + hf * 32, bg);
               tc::tmem_ld_wait();
               bf16 r[32];
 #pragma unroll
@@ -388,7 +391,7 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
               uint32_t v[32];
               float bb[32];
               tc::tmem_ld32(tacc + j * 64 + hf * 32, v);
-              lds32(sbias + j * 64 + hf * 32, bb);
+              lds32(sbias + hf * 32, bb);
               tc::tmem_ld_wait();
               bf16 r[32];
 #pragma unroll
@@ -624,6 +627,15 @@ int launch_gemm2(TmaCtx* ctx, const G2Desc& d, int num_sms, cudaStream_t st) {
   p.vt_out = reinterpret_cast<bf16*>(d.vt_out); p.vt_cols = d.vt_cols;
   p.Lpad = d.Lpad;
   p.tile_active = d.tile_active;
+  p.bias_lo = d.bias_lo;
+  p.bias_n = d.bias ? (d.bias_n > 0 ? d.bias_n : d.Nw - d.bias_lo) : 0;
+  {
+    const int cap = d.K == 256 ? G2Smem<256>::BIAS_FLOATS : G2Smem<128>::BIAS_FLOATS;
+    if (p.bias_n > cap || (p.bias_lo & 63) || p.bias_lo < 0) {
+      tc_set_error("gemm2: bias range does not fit the shared-memory table (give bias_lo / bias_n, multiples of 64)");
+      return -1;
+    }
+  }
   bool need_bias = false;
   for (int i = 0; i < G2_MAX_OPS; ++i) {
     if (i < d.n_ops) p.ops[i] = d.ops[i];

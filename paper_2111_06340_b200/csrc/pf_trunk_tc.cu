@@ -209,6 +209,7 @@ struct TcDriver {
       G2Desc d = desc_base(B, D1, D2, C, Nw);
       d.src = res; d.src_transposed = transposed ? 1 : 0; d.gamma = w + a.ln_g; d.beta = w + a.ln_b;
       d.op_fmt = 1; d.Wt = w16 + at.w_in; d.bias = wf + at.b_in;
+      d.bias_lo = 2 * C; d.bias_n = C;   // only the gate columns carry a bias (R7)
       d.row_out[0] = QKG; d.row_ld[0] = 3 * C;
       d.vt_out = VT; d.vt_cols = C; d.Lpad = Lp;
       d.heads_out = BIAS; d.n_heads = H;
