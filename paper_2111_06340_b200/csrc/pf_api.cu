@@ -199,6 +199,11 @@ extern "C" void pf_evoformer_destroy(pf_evoformer_t* h) {
   cudaFree(h->wf);
   cudaFree(h->ws);
   cudaFree(h->stage);
+  if (h->h2d_stream) {
+    cudaStreamDestroy(h->h2d_stream);
+    cudaStreamDestroy(h->d2h_stream);
+    for (cudaEvent_t e : h->host_ev) cudaEventDestroy(e);
+  }
   if (h->tma) tma_ctx_destroy(h->tma);
   for (cudaEvent_t e : h->ev_pool) cudaEventDestroy(e);
   delete h;
@@ -531,14 +536,43 @@ extern "C" pf_status pf_evoformer_forward_host(pf_evoformer_t* h, float* msa_hos
   float* dz = reinterpret_cast<float*>(h->stage + align_up(nm, 256));
   float* ds = reinterpret_cast<float*>(h->stage + align_up(nm, 256) + align_up(nz, 256));
   float* dr = reinterpret_cast<float*>(h->stage + align_up(nm, 256) + align_up(nz, 256) + ns);
-  CUDA_TRY(cudaMemcpyAsync(dm, msa_host, nm, cudaMemcpyHostToDevice, st));
-  CUDA_TRY(cudaMemcpyAsync(dz, pair_host, nz, cudaMemcpyHostToDevice, st));
-  CUDA_TRY(cudaMemcpyAsync(ds, seq_mask_host, (size_t)B * N * 4, cudaMemcpyHostToDevice, st));
-  CUDA_TRY(cudaMemcpyAsync(dr, msa_mask_host, (size_t)B * S * 4, cudaMemcpyHostToDevice, st));
-  pf_status s = pf_evoformer_forward(h, dm, dz, ds, dr, B, S, N, n_blocks, stream);
-  if (s != PF_OK) return s;
-  CUDA_TRY(cudaMemcpyAsync(msa_host, dm, nm, cudaMemcpyDeviceToHost, st));
-  CUDA_TRY(cudaMemcpyAsync(pair_host, dz, nz, cudaMemcpyDeviceToHost, st));
+  // Proteins are independent, so the batch is pipelined in chunks: while chunk c is computed on the caller's stream, chunk
+  // c+1 is copied in and chunk c-1 is copied out on two copy streams (PCIe is full duplex).  Pageable host memory still
+  // works (the copies then serialise inside the driver).
+  if (!h->h2d_stream) {
+    CUDA_TRY(cudaStreamCreateWithFlags(&h->h2d_stream, cudaStreamNonBlocking));
+    CUDA_TRY(cudaStreamCreateWithFlags(&h->d2h_stream, cudaStreamNonBlocking));
+    for (auto& e : h->host_ev) CUDA_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+  }
+  const int n_chunks = B < 8 ? (B < 1 ? 1 : B) : 8;
+  const size_t pm = (size_t)S * N * h->cfg.c_m, pz = (size_t)N * N * h->cfg.c_z;   // floats per protein
+  CUDA_TRY(cudaEventRecord(h->host_ev[16], st));                  // earlier work on the caller's stream comes first
+  CUDA_TRY(cudaStreamWaitEvent(h->h2d_stream, h->host_ev[16], 0));
+  CUDA_TRY(cudaStreamWaitEvent(h->d2h_stream, h->host_ev[16], 0));
+  CUDA_TRY(cudaMemcpyAsync(ds, seq_mask_host, (size_t)B * N * 4, cudaMemcpyHostToDevice, h->h2d_stream));
+  CUDA_TRY(cudaMemcpyAsync(dr, msa_mask_host, (size_t)B * S * 4, cudaMemcpyHostToDevice, h->h2d_stream));
+  int b0 = 0;
+  for (int c = 0; c < n_chunks; ++c) {
+    const int bc = (B - b0 + (n_chunks - c) - 1) / (n_chunks - c);
+    CUDA_TRY(cudaMemcpyAsync(dm + b0 * pm, msa_host + b0 * pm, bc * pm * 4, cudaMemcpyHostToDevice, h->h2d_stream));
+    CUDA_TRY(cudaMemcpyAsync(dz + b0 * pz, pair_host + b0 * pz, bc * pz * 4, cudaMemcpyHostToDevice, h->h2d_stream));
+    CUDA_TRY(cudaEventRecord(h->host_ev[c], h->h2d_stream));
+    b0 += bc;
+  }
+  b0 = 0;
+  for (int c = 0; c < n_chunks; ++c) {
+    const int bc = (B - b0 + (n_chunks - c) - 1) / (n_chunks - c);
+    CUDA_TRY(cudaStreamWaitEvent(st, h->host_ev[c], 0));
+    pf_status s = pf_evoformer_forward(h, dm + b0 * pm, dz + b0 * pz, ds + (size_t)b0 * N, dr + (size_t)b0 * S, bc, S, N, n_blocks,
+                                       stream);
+    if (s != PF_OK) return s;
+    CUDA_TRY(cudaEventRecord(h->host_ev[8 + c], st));
+    CUDA_TRY(cudaStreamWaitEvent(h->d2h_stream, h->host_ev[8 + c], 0));
+    CUDA_TRY(cudaMemcpyAsync(msa_host + b0 * pm, dm + b0 * pm, bc * pm * 4, cudaMemcpyDeviceToHost, h->d2h_stream));
+    CUDA_TRY(cudaMemcpyAsync(pair_host + b0 * pz, dz + b0 * pz, bc * pz * 4, cudaMemcpyDeviceToHost, h->d2h_stream));
+    b0 += bc;
+  }
+  CUDA_TRY(cudaStreamSynchronize(h->d2h_stream));
   CUDA_TRY(cudaStreamSynchronize(st));
   return PF_OK;
 }

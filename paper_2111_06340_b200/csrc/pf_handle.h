@@ -81,6 +81,9 @@ struct pf_evoformer {
   size_t ws_bytes = 0;
   char* stage = nullptr;     // forward_host staging
   size_t stage_bytes = 0;
+  // forward_host pipelines the batch in chunks of proteins: copy-in stream, the caller's stream for compute, copy-out stream
+  cudaStream_t h2d_stream = nullptr, d2h_stream = nullptr;
+  cudaEvent_t host_ev[3 * 8] = {};   // per chunk: inputs landed, compute done, (spare)
   int num_sms = 148;
   long long launches = 0;
   pf::TmaCtx* tma = nullptr;

@@ -121,3 +121,23 @@ def test_cfg2_full_size_sampled_proteins():
         sl = slice(int(b), int(b) + 1)
         mr, zr = run_oracle(blocks, msa[sl], pair[sl], sm[sl], mm[sl])
         _check(m[sl], z[sl], mr, zr, sm[sl], mm[sl], f"cfg2 protein {int(b)} (len {int(lengths[b])})")
+
+
+@pytest.mark.parametrize("B", [1, 5, 11])
+def test_forward_host_pipelined_chunks_match_forward(B):
+    """pf_evoformer_forward_host pipelines the batch in chunks of proteins over copy streams: every protein must come back
+    exactly as from the device-resident call on the same batch (proteins are independent, so chunking changes nothing)."""
+    import torch
+    S, N = 12, 40
+    blocks = ps.make_weights(41, 2, bf16_weights=True)
+    lengths = ps.rng(42, B).integers(20, N + 1, size=B)
+    msa, pair, sm, mm = ps.make_inputs(43, B, S, N, lengths=lengths, msa_mask_frac_max=0.3)
+    valid_m, valid_z = valid_masks(sm, mm)
+    m, z = run_cuda(pf.PF_BF16, blocks, msa, pair, sm, mm)
+    h = pf.Evoformer(ps.pack_blob(blocks), pf.make_config(2, pf.PF_BF16))
+    mh = torch.from_numpy(msa.copy()).pin_memory()
+    zh = torch.from_numpy(pair.copy()).pin_memory()
+    h.forward_host(mh, zh, torch.from_numpy(sm).pin_memory(), torch.from_numpy(mm).pin_memory(), 2)
+    h.close()
+    assert np.isfinite(mh.numpy()).all() and np.isfinite(zh.numpy()).all()
+    assert np.array_equal(mh.numpy()[valid_m], m[valid_m]) and np.array_equal(zh.numpy()[valid_z], z[valid_z])
