@@ -23,6 +23,7 @@
 #include "pf_internal.h"
 #include "pf_device.cuh"
 #include "pf_tc.cuh"
+#include "pf_lnprod.cuh"
 
 #include <cuda_fp16.h>
 #include <string>
@@ -415,15 +416,17 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
   } else if (warp < 16) {
     if (AMODE == 0) {
       // ========================================================= A producers: LayerNorm of gathered fp32 rows
-      constexpr int NV = K / 128;                      // float4 per lane per row
-      constexpr int RU = (K == 256) ? 4 : 8;           // rows in flight per warp
+      using LN = LnProd<K>;
+      constexpr int RU = LN::ROWS;                     // rows per batch of this warp (4 at K = 256, 8 at K = 128)
       const int pw = warp - 8;
-      float4 gm[NV], bt[NV];
-#pragma unroll
-      for (int i = 0; i < NV; ++i) {
-        gm[i] = __ldg(reinterpret_cast<const float4*>(p.gamma) + lane + 32 * i);
-        bt[i] = __ldg(reinterpret_cast<const float4*>(p.beta) + lane + 32 * i);
-      }
+      LN ln;
+      ln.init(p.gamma, p.beta, lane);
+      auto src_row = [&](const TileCoord& c, int lr) -> const float* {
+        const int x = c.x0 + (lr >> p.yt_shift), y = c.y0 + (lr & (p.YT - 1));
+        if (x >= p.D1 || y >= p.D2) return nullptr;
+        const long srow = p.src_transposed ? ((long)c.b * p.D2 + y) * p.D1 + x : ((long)c.b * p.D1 + x) * p.D2 + y;
+        return p.src + srow * K;
+      };
       uint32_t it = 0;
       for (long tile = blockIdx.x; tile < p.num_tiles; tile += gridDim.x) {
         if (!tile_on(tile, p)) continue;
@@ -442,56 +445,17 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
         for (int r0 = 0; r0 < 16; r0 += RU) {
           if (lane < RU && (r0 + RU < 16 || nxt_on)) {
             const bool same = r0 + RU < 16;
-            const TileCoord& pc = same ? tcd : ncd;
-            const int lr = pw * 16 + (same ? r0 + RU : 0) + lane;
-            const int x = pc.x0 + (lr >> p.yt_shift), y = pc.y0 + (lr & (p.YT - 1));
-            if (x < p.D1 && y < p.D2) {
-              long srow = p.src_transposed ? ((long)pc.b * p.D2 + y) * p.D1 + x : ((long)pc.b * p.D1 + x) * p.D2 + y;
-              tc::prefetch_l2_bulk(p.src + srow * K, K * 4);
-            }
+            const float* rp = src_row(same ? tcd : ncd, pw * 16 + (same ? r0 + RU : 0) + lane);
+            if (rp) tc::prefetch_l2_bulk(rp, K * 4);
           }
-          float4 v[RU][NV];
+          const float* rp[LN::PASSES];
+          int lr[LN::PASSES];
 #pragma unroll
-          for (int u = 0; u < RU; ++u) {
-            const int lr = pw * 16 + r0 + u;
-            const int x = tcd.x0 + (lr >> p.yt_shift), y = tcd.y0 + (lr & (p.YT - 1));
-            if (x < p.D1 && y < p.D2) {
-              long srow = p.src_transposed ? ((long)tcd.b * p.D2 + y) * p.D1 + x : ((long)tcd.b * p.D1 + x) * p.D2 + y;
-              const float4* xp = reinterpret_cast<const float4*>(p.src + srow * K);
-#pragma unroll
-              for (int i = 0; i < NV; ++i) v[u][i] = ld_nc_f4(xp + lane + 32 * i);
-            } else {
-#pragma unroll
-              for (int i = 0; i < NV; ++i) v[u][i] = make_float4(0.f, 0.f, 0.f, 0.f);
-            }
+          for (int ps = 0; ps < LN::PASSES; ++ps) {
+            lr[ps] = pw * 16 + ln.row_of(r0, ps);
+            rp[ps] = src_row(tcd, lr[ps]);
           }
-#pragma unroll
-          for (int u = 0; u < RU; ++u) {
-            const int lr = pw * 16 + r0 + u;
-            float s = 0.f;
-#pragma unroll
-            for (int i = 0; i < NV; ++i) s += v[u][i].x + v[u][i].y + v[u][i].z + v[u][i].w;
-            const float mean = warp_sum(s) * (1.0f / K);
-            float q = 0.f;
-#pragma unroll
-            for (int i = 0; i < NV; ++i) {
-              float a = v[u][i].x - mean, b2 = v[u][i].y - mean, c = v[u][i].z - mean, d = v[u][i].w - mean;
-              q += a * a + b2 * b2 + c * c + d * d;
-            }
-            const float rstd = rsqrtf(warp_sum(q) * (1.0f / K) + 1e-5f);
-#pragma unroll
-            for (int i = 0; i < NV; ++i) {
-              float o0 = (v[u][i].x - mean) * rstd * gm[i].x + bt[i].x;
-              float o1 = (v[u][i].y - mean) * rstd * gm[i].y + bt[i].y;
-              float o2 = (v[u][i].z - mean) * rstd * gm[i].z + bt[i].z;
-              float o3 = (v[u][i].w - mean) * rstd * gm[i].w + bt[i].w;
-              // columns 128 i + 4 lane .. +3  ->  k-block 2 i + lane / 16, 16-byte chunk (lane % 16) / 2, half lane & 1
-              const int kb = 2 * i + (lane >> 4);
-              const uint32_t chunk = (uint32_t)((lane & 15) >> 1);
-              uint8_t* dst = abase + kb * SM::KB_BYTES + lr * 128 + ((chunk ^ (uint32_t)(lr & 7)) << 4) + (lane & 1) * 8;
-              *reinterpret_cast<uint2*>(dst) = make_uint2(pack16(o0, o1, 1), pack16(o2, o3, 1));   // LN outputs are fp16 operands (R17)
-            }
-          }
+          ln.run(rp, lr, abase);
         }
         tc::fence_proxy_async_smem();
         tc::mbar_arrive(&a_full[abuf]);

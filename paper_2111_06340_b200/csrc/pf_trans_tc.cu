@@ -19,6 +19,7 @@
 #include "pf_internal.h"
 #include "pf_device.cuh"
 #include "pf_tc.cuh"
+#include "pf_lnprod.cuh"
 
 #include <cuda_fp16.h>
 #include <string>
@@ -228,72 +229,38 @@ transition_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constan
     if (leader) tc::bulk_wait<0>();
   } else if (warp < 16) {
     // ============================================================= A1 producers: LayerNorm of fp32 rows
-    constexpr int NV = C / 128;                        // float4 per lane per row
-    constexpr int RU = (C == 256) ? 4 : 8;             // rows in flight per warp
+    using LN = LnProd<C>;
+    constexpr int RU = LN::ROWS;                       // rows per batch of this warp (4 at C = 256, 8 at C = 128)
     const int pw = warp - 8;
-    float4 gm[NV], bt[NV];
-#pragma unroll
-    for (int i = 0; i < NV; ++i) {
-      gm[i] = __ldg(reinterpret_cast<const float4*>(p.gamma) + lane + 32 * i);
-      bt[i] = __ldg(reinterpret_cast<const float4*>(p.beta) + lane + 32 * i);
-    }
+    LN ln;
+    ln.init(p.gamma, p.beta, lane);
     uint32_t it = 0;
     for (long tile = blockIdx.x; tile < p.num_tiles; tile += gridDim.x) {
       if (!tr_tile_on(tile, p)) continue;
       const uint32_t abuf = it % A1B;
-      {
-        const long nxt = tile + gridDim.x;             // next tile's 16 rows of this warp -> L2
-        const long r0 = nxt * 128 + pw * 16;
-        if (nxt < p.num_tiles && lane == 0 && r0 < p.R && tr_tile_on(nxt, p)) {
-          long n = p.R - r0 < 16 ? p.R - r0 : 16;
-          tc::prefetch_l2_bulk(p.res + r0 * C, (uint32_t)(n * C * 4));
-        }
-      }
+      const long nxt = tile + gridDim.x;
+      const bool nxt_on = nxt < p.num_tiles && tr_tile_on(nxt, p);
       tc::mbar_wait(&a1_empty[abuf], ((it / A1B) & 1) ^ 1);
       uint8_t* abase = smem + SM::A1_OFF + abuf * SM::A1_BYTES;
 #pragma unroll 1
       for (int r0 = 0; r0 < 16; r0 += RU) {
-        float4 v[RU][NV];
-#pragma unroll
-        for (int u = 0; u < RU; ++u) {
-          const int lr = pw * 16 + r0 + u;
-          const long r = tile * 128 + lr;
+        // short-distance L2 prefetch of this warp's next batch of rows (first batch of the next active tile after the last)
+        if (lane == 0 && (r0 + RU < 16 || nxt_on)) {
+          const long r = (r0 + RU < 16 ? tile : nxt) * 128 + pw * 16 + (r0 + RU < 16 ? r0 + RU : 0);
           if (r < p.R) {
-            const float4* xp = reinterpret_cast<const float4*>(p.res + r * C);
-#pragma unroll
-            for (int i = 0; i < NV; ++i) v[u][i] = ld_nc_f4(xp + lane + 32 * i);
-          } else {
-#pragma unroll
-            for (int i = 0; i < NV; ++i) v[u][i] = make_float4(0.f, 0.f, 0.f, 0.f);
+            const long n = p.R - r < RU ? p.R - r : RU;
+            tc::prefetch_l2_bulk(p.res + r * C, (uint32_t)(n * C * 4));
           }
         }
+        const float* rp[LN::PASSES];
+        int lr[LN::PASSES];
 #pragma unroll
-        for (int u = 0; u < RU; ++u) {
-          const int lr = pw * 16 + r0 + u;
-          float s = 0.f;
-#pragma unroll
-          for (int i = 0; i < NV; ++i) s += v[u][i].x + v[u][i].y + v[u][i].z + v[u][i].w;
-          const float mean = warp_sum(s) * (1.0f / C);
-          float q = 0.f;
-#pragma unroll
-          for (int i = 0; i < NV; ++i) {
-            float a = v[u][i].x - mean, b2 = v[u][i].y - mean, c = v[u][i].z - mean, d = v[u][i].w - mean;
-            q += a * a + b2 * b2 + c * c + d * d;
-          }
-          const float rstd = rsqrtf(warp_sum(q) * (1.0f / C) + 1e-5f);
-#pragma unroll
-          for (int i = 0; i < NV; ++i) {
-            float o0 = (v[u][i].x - mean) * rstd * gm[i].x + bt[i].x;
-            float o1 = (v[u][i].y - mean) * rstd * gm[i].y + bt[i].y;
-            float o2 = (v[u][i].z - mean) * rstd * gm[i].z + bt[i].z;
-            float o3 = (v[u][i].w - mean) * rstd * gm[i].w + bt[i].w;
-            // columns 128 i + 4 lane .. +3  ->  k-block 2 i + lane / 16, 16-byte chunk (lane % 16) / 2, half lane & 1
-            const int kb = 2 * i + (lane >> 4);
-            const uint32_t chunk = (uint32_t)((lane & 15) >> 1);
-            uint8_t* dst = abase + kb * SM::KB_BYTES + lr * 128 + ((chunk ^ (uint32_t)(lr & 7)) << 4) + (lane & 1) * 8;
-            *reinterpret_cast<uint2*>(dst) = make_uint2(tr_pack_f16(o0, o1), tr_pack_f16(o2, o3));   // fp16 operand (R17)
-          }
+        for (int ps = 0; ps < LN::PASSES; ++ps) {
+          lr[ps] = pw * 16 + ln.row_of(r0, ps);
+          const long r = tile * 128 + lr[ps];
+          rp[ps] = r < p.R ? p.res + r * C : nullptr;
         }
+        ln.run(rp, lr, abase);
       }
       tc::fence_proxy_async_smem();
       tc::mbar_arrive(&a1_full[abuf]);
