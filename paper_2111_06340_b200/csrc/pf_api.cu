@@ -1,5 +1,5 @@
 // C-ABI entry points and the block/trunk driver: sequences the nine sub-steps of SURVEY.md §8(a) over the
-// kernels of pf_simt.cu / pf_gemm_tc.cu / pf_attn_tc.cu.  No arithmetic of the method lives here except the
+// kernels of pf_simt.cu (fp32 path) and, through pf_trunk_tc.cu, the tcgen05 kernels (bf16 path).  No arithmetic of the method lives here except the
 // constant 1/sqrt(head_dim) handed to the q-projection epilogue (R12).
 #include "pf_handle.h"
 

@@ -68,15 +68,13 @@ template <typename T>
 void launch_opm_simt(const T* a, const T* b, const float* wout, const float* bout, const float* seq_mask,
                      const float* msa_mask, float* z, int B, int S, int N, int c_opm, int c_z, cudaStream_t st);
 
-// ---- tcgen05 kernels (bf16), pf_gemm_tc.cu / pf_attn_tc.cu ----
-// Weights Wt are bf16 [Nout, K] (K contiguous).  DUAL: Wt is [2*Nout_eff, K] = [Wp ; Wg] stacked per 128 columns.
+// ---- tcgen05 kernels (pf_tma.cu: TMA host side; pf_lngemm_tc.cu, pf_trans_tc.cu, pf_attn_tc.cu, pf_opm_tc.cu, pf_tri_tc.cu) ----
+// Weights Wt are 16-bit [Nout, K] (K contiguous).
 struct TmaCtx;   // holds the driver entry point for cuTensorMapEncodeTiled
 TmaCtx* tma_ctx_create();
 void tma_ctx_destroy(TmaCtx*);
 const char* tc_last_error();
 void tc_set_error(const std::string& s);
-int launch_gemm_tc(TmaCtx* ctx, const bf16* A, int lda, const bf16* Wt, long R, int K, int Nout, const Epi& epi,
-                   int num_sms, cudaStream_t st);
 // ---- persistent LN-fused projection GEMM (pf_lngemm_tc.cu) ----
 // Rows of the GEMM are (b, x in [0,D1), y in [0,D2)); one CTA tile = XT consecutive x times YT consecutive y (XT*YT = 128).
 // The 64-column groups of the output are described by G2Op: what is done to the accumulator and where it goes.
