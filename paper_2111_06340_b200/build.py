@@ -21,6 +21,10 @@ NVCC_FLAGS = [
 ]
 
 
+# extra nvcc flags for one-off experiments (e.g. -DPF_G2_TRACE); not used by any committed caller
+NVCC_FLAGS += os.environ.get("PF_NVCC_EXTRA", "").split()
+
+
 def sources():
     return sorted(os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".cu", ".cpp")))
 

@@ -33,6 +33,24 @@ namespace pf {
 int tma_encode(TmaCtx* ctx, CUtensorMap* out, const void* base, int elem_kind, int rank, const uint64_t* dims,
                const uint64_t* strides_bytes, const uint32_t* box, int swizzle_bytes);
 
+#ifdef PF_G2_TRACE
+// Timeline tracing of CTA 0 (experiments only; never defined in the product build): per traced thread a private slot of
+// (tag, clock64) pairs written with plain stores (no atomics: ~10 ns per event).
+__device__ unsigned long long g2_trace_buf[4 * 8192];
+#define G2_TRACE_DECL unsigned g2_trc = 0;
+#define G2_TRACE(slot, tag)                                                         \
+  do {                                                                              \
+    if (blockIdx.x == 0 && g2_trc < 4000) {                                         \
+      g2_trace_buf[(slot) * 8192 + 2 * g2_trc] = (tag);                             \
+      g2_trace_buf[(slot) * 8192 + 2 * g2_trc + 1] = (unsigned long long)clock64(); \
+      ++g2_trc;                                                                     \
+    }                                                                               \
+  } while (0)
+#else
+#define G2_TRACE_DECL
+#define G2_TRACE(slot, tag)
+#endif
+
 constexpr int G2_BN = 256;
 constexpr int G2_THREADS = 18 * 32;
 constexpr int G2_EPI_WARPS = 8;
@@ -101,12 +119,13 @@ __device__ __forceinline__ TileCoord tile_coord(long t, const G2Params& p) {
   return c;
 }
 
-// sigmoid through the two MUFU approximations (ex2, rcp), flush-to-zero: 4 instructions, ~1e-6 relative error
+// sigmoid(x) = 0.5 + 0.5 tanh(x / 2) with the MUFU tanh approximation: one MUFU and two FMA-pipe instructions per value
+// (the ex2 + rcp form costs two MUFU; the epilogue warps are the critical path of this kernel).  tanh.approx has a
+// relative error of ~2^-11, i.e. <= 2.5e-4 absolute on the gate, which is stored as fp16 (2^-11 relative) anyway.
 __device__ __forceinline__ float fast_sigmoid2(float x) {
-  float e, r;
-  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(x * -1.4426950408889634f));
-  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(1.0f + e));
-  return r;
+  float t;
+  asm("tanh.approx.f32 %0, %1;" : "=f"(t) : "f"(x * 0.5f));
+  return fmaf(t, 0.5f, 0.5f);
 }
 // 32 consecutive fp32 values from shared memory into registers (eight 128-bit loads).  Epilogue groups fetch their bias this
 // way BEFORE the arithmetic: a shared-memory load placed between the staging stores could not be moved across them.
@@ -182,6 +201,7 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(acc_empty + 2);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  G2_TRACE_DECL
 
   if (warp == 16 && lane == 0) {
     tc::prefetch_tmap(&tmW);
@@ -245,14 +265,20 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
       const long grow = ((long)tcd.b * p.D1 + x) * p.D2 + y;   // GEMM row index (gate rows)
       for (int nt = 0; nt < p.n_tiles; ++nt, ++ac) {
         const uint32_t buf = ac & 1;
+        // this warp's two groups of the window: their descriptors are fetched (indexed constant loads) BEFORE waiting for the
+        // accumulator, so that latency is off the critical path
+        const G2Op op_a = p.ops[nt * 4 + team], op_b = p.ops[nt * 4 + team + 2];
+        if (lane == 0 && quarter == 0) G2_TRACE(team, 0x100 + 0);
         tc::mbar_wait(&acc_full[buf], (ac >> 1) & 1);
         tc::tc_fence_after();
+        if (lane == 0 && quarter == 0) G2_TRACE(team, 0x100 + 1);
         const uint32_t tacc = lane_addr + buf * G2_BN;
 #pragma unroll 1
         for (int j = team; j < 4; j += 2) {
-          const G2Op& op = p.ops[nt * 4 + j];
+          const G2Op& op = (j == team) ? op_a : op_b;
           const int kind = op.kind;
           if (kind == G2_SKIP) continue;
+          if (lane == 0 && quarter == 0) G2_TRACE(team, 0x100 + 3);
           // this group's 64 bias values: inside the table, or the zero pad behind it
           const int bcol = nt * G2_BN + j * 64 - p.bias_lo;
           const float* const sbias = sbias_tab + ((bcol >= 0 && bcol + 64 <= p.bias_n) ? bcol : SM::BIAS_FLOATS);
@@ -261,8 +287,10 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
           if (kind == G2_ROW16) {
             sb = sb_team + (gcnt++ % NST) * SM::STW_BYTES;
             sb16 = reinterpret_cast<bf16*>(sb);
+            if (leader && quarter == 0) G2_TRACE(team, 0x120);
             if (leader) tc::bulk_wait_read<NST - 1>();
             __syncwarp();
+            if (leader && quarter == 0) G2_TRACE(team, 0x121);
             {
               const float scale = op.scale;
               const uint32_t ta = tacc + j * 64;
@@ -279,12 +307,15 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
                 else g2_row16_group<ACT_NONE, 0>(ta, srow, b64, scale, sw);
               }
             }
+            if (leader && quarter == 0) G2_TRACE(team, 0x122);
             tc::fence_proxy_async_smem();
             __syncwarp();
+            if (leader && quarter == 0) G2_TRACE(team, 0x123);
             if (leader) {
               tc::tma_store_4d(&tmO0, sb, op.dst_col, tcd.y0 + yw0, tcd.x0 + xw0, tcd.b);
               tc::bulk_commit();
             }
+            if (leader && quarter == 0) G2_TRACE(team, 0x124);
           } else if (kind == G2_RESID) {
 #pragma unroll 1
             for (int hf = 0; hf < 2; ++hf) {
@@ -410,6 +441,7 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
         }
         tc::tc_fence_before();
         tc::mbar_arrive(&acc_empty[buf]);
+        if (lane == 0 && quarter == 0) G2_TRACE(team, 0x100 + 2);
       }
     }
     if (leader) tc::bulk_wait<0>();
@@ -438,7 +470,9 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
         const long nxt = tile + gridDim.x;
         const bool nxt_on = nxt < p.num_tiles && tile_on(nxt, p);
         const TileCoord ncd = tile_coord(nxt_on ? nxt : tile, p);
+        if (lane == 0 && pw == 0) G2_TRACE(2, 0x200);
         tc::mbar_wait(&a_empty[abuf], ((it >> 1) & 1) ^ 1);
+        if (lane == 0 && pw == 0) G2_TRACE(2, 0x201);
         const TileCoord tcd = tile_coord(tile, p);
         uint8_t* abase = smem + SM::A_OFF + abuf * SM::A_BYTES;
 #pragma unroll 1
@@ -459,6 +493,7 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
         }
         tc::fence_proxy_async_smem();
         tc::mbar_arrive(&a_full[abuf]);
+        if (lane == 0 && pw == 0) G2_TRACE(2, 0x202);
         ++it;
       }
     } else if (warp == 8) {
@@ -503,13 +538,17 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
       for (long tile = blockIdx.x; tile < p.num_tiles; tile += gridDim.x) {
         if (!tile_on(tile, p)) continue;
         const uint32_t abuf = it & 1;
+        G2_TRACE(3, 0x300);
         tc::mbar_wait(&a_full[abuf], (it >> 1) & 1);
         tc::tc_fence_after();
+        G2_TRACE(3, 0x301);
         const uint32_t a_addr = tc::smem_u32(smem + SM::A_OFF + abuf * SM::A_BYTES);
         for (int nt = 0; nt < p.n_tiles; ++nt, ++ac) {
           const uint32_t buf = ac & 1;
+          G2_TRACE(3, 0x302);
           tc::mbar_wait(&acc_empty[buf], ((ac >> 1) & 1) ^ 1);
           tc::tc_fence_after();
+          G2_TRACE(3, 0x303);
           int n_eff = p.Nw - nt * G2_BN;
           n_eff = n_eff >= G2_BN ? G2_BN : ((n_eff + 15) & ~15);
           const uint32_t idesc = p.op_fmt ? tc::idesc_f16_f32(128, n_eff) : tc::idesc_bf16_f32(128, n_eff);
@@ -526,6 +565,7 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
             tc::mma_commit(&w_empty[s]);
           }
           tc::mma_commit(&acc_full[buf]);
+          G2_TRACE(3, 0x304);
         }
         tc::mma_commit(&a_empty[abuf]);
         ++it;
@@ -558,6 +598,18 @@ static int launch_g2(const CUtensorMap& tmW, const CUtensorMap& tmA, const CUten
   kern<<<grid, G2_THREADS, G2Smem<K>::TOTAL, st>>>(tmW, tmA, tmO0, tmT0, tmT1, tmH, tmR, p);
   return 0;
 }
+
+#ifdef PF_G2_TRACE
+extern "C" int pf_debug_g2_trace(unsigned long long* out, int reset) {
+  cudaDeviceSynchronize();
+  cudaMemcpyFromSymbol(out, g2_trace_buf, sizeof(g2_trace_buf));
+  if (reset) {
+    static unsigned long long zeros[4 * 8192];
+    cudaMemcpyToSymbol(g2_trace_buf, zeros, sizeof(zeros));
+  }
+  return 4 * 8192;
+}
+#endif
 
 int launch_gemm2(TmaCtx* ctx, const G2Desc& d, int num_sms, cudaStream_t st) {
   if (d.K != 128 && d.K != 256) {
