@@ -222,7 +222,7 @@ KIND_BOUND = {"gemm": "tensor", "attn_core": "tensor", "tri_einsum": "tensor", "
               "ln_rows": "hbm", "ln_channels": "hbm", "ln_gemm": "hbm", "transition": "tensor"}
 
 
-def roofline_from_profile(prof, peaks, n_steps):
+def roofline_from_profile(prof, peaks, n_steps, wl_name):
     """Dominant kernel kind (largest share of device time) -> roofline object; plus the per-kind table."""
     total_ms = sum(v["ms"] for v in prof.values()) or 1e-9
     table = {}
@@ -240,7 +240,7 @@ def roofline_from_profile(prof, peaks, n_steps):
     if os.path.exists(tp):
         try:
             with open(tp) as f:
-                traffic = json.load(f).get(top)
+                traffic = json.load(f).get(wl_name, {}).get(top)   # captured per workload (launch sizes differ)
         except Exception:
             traffic = None
     if bound == "tensor":
@@ -414,7 +414,7 @@ def run_ours(args, wl, wl_name):
     ms_per_step = ms / args.steps
     value = world * n_prot * args.steps / (ms * 1e-3)
     flops_step = ps.gemm_flops_per_block(S, N) * nb * B          # padded FLOPs: what the GPU executes
-    roof, table = roofline_from_profile(prof, peaks, n_prof)
+    roof, table = roofline_from_profile(prof, peaks, n_prof, wl_name)
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
