@@ -7,7 +7,9 @@
 // (b*r, h, 128-query tile), its key tiles of 64 are the pipeline steps, and steps run back to back across units:
 //   warp 4 (TMA)   Q (double buffered per unit) and per step {K 64x32 (64B swizzle), V^T 32x64, bias 128x64 (128B swizzle)}
 //                  through a ring, running ahead of the consumers by the ring depth
-//   warp 5 (MMA)   S(i+1) = Q K^T  (M=128 N=64 K=2x16, TMEM double buffered) is issued BEFORE waiting for P(i), so the
+//   warp 5 (MMA)   S(i+1) = Q K^T + bias I  (M=128 N=64; K=2x16 for Q K^T, then the bf16 pair-bias tile [128 x 64] times a
+//                  constant 64 x 64 identity, K=4x16: the tensor core adds the bias exactly (fp32 accumulation), so the softmax
+//                  warps never unpack it; TMEM double buffered) is issued BEFORE waiting for P(i), so the
 //                  tensor core works on the next logits while the softmax warps are busy; O_tile = P V (M=128 N=32 K=4x16)
 //   warps 0-3      thread-per-row online softmax in fp32 from tcgen05.ld (ex2.approx), P (bf16) -> smem in the UMMA
 //                  128B-swizzle layout; o_acc = o_acc * alpha + O_tile in registers; gate (prefetched at unit start) and 1/l
@@ -37,9 +39,12 @@ struct AttnSmem {
   static constexpr int B_BYTES = AT_BQ * 128;                      // 128 x 64 bf16: 16 KB
   static constexpr int POOL_BYTES = 72 * 1024;                     // 3 stages with a bias tile, 8 without (one is unused)
   static constexpr int MAX_STAGES = 8;
-  static constexpr int MASK_OFF = STAGE_OFF + POOL_BYTES;
-  static constexpr int BAR_OFF = MASK_OFF + AT_MAXKEYS * 4;
-  static constexpr int TOTAL = BAR_OFF + 256 + 1024;
+  static constexpr int ID_OFF = STAGE_OFF + POOL_BYTES;            // 64 x 64 bf16 identity, K-major 128B swizzle: 8 KB
+  static constexpr int MASK_OFF = ID_OFF + 64 * 128;               // one bit per key: 1 = masked or out of range
+  static constexpr int BAR_OFF = MASK_OFF + AT_MAXKEYS / 8;
+  // No alignment slack: two CTAs of 115,072 B fit one SM only without it.  The dynamic shared memory window of a kernel
+  // without static shared memory starts 1024-byte aligned; the kernel traps if it ever does not.
+  static constexpr int TOTAL = BAR_OFF + 256;
 };
 
 struct AttnParams {
@@ -68,8 +73,9 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQK, const __grid_constant__
                const __grid_constant__ CUtensorMap tmBias, const __grid_constant__ AttnParams p) {
   using SM = AttnSmem;
   extern __shared__ uint8_t smem_raw[];
-  uint8_t* smem = tc::align_smem_1024(smem_raw);
-  float* mterm = reinterpret_cast<float*>(smem + SM::MASK_OFF);
+  uint8_t* smem = smem_raw;
+  if (tc::smem_u32(smem_raw) & 1023u) __trap();
+  uint32_t* mbits = reinterpret_cast<uint32_t*>(smem + SM::MASK_OFF);
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem + SM::BAR_OFF);
   uint64_t* q_full = bars;                       // [2]
   uint64_t* q_empty = bars + 2;                  // [2]
@@ -103,6 +109,17 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQK, const __grid_constant__
     tc::fence_barrier_init();
   }
   if (warp == 5) tc::tmem_alloc<256>(tmem_slot);
+  if (p.has_bias) {
+    // identity operand of the bias MMA: element (j, k) of a K-major [64 x 64] bf16 tile, 1.0 on the diagonal
+    uint32_t* idw = reinterpret_cast<uint32_t*>(smem + SM::ID_OFF);
+    for (int i = threadIdx.x; i < 64 * 128 / 4; i += AT_THREADS) idw[i] = 0u;
+    __syncthreads();
+    if (threadIdx.x < 64) {
+      const int j = threadIdx.x;
+      *reinterpret_cast<uint16_t*>(smem + SM::ID_OFF + tc::swz_offset<128>(j, j >> 3) + (j & 7) * 2) = 0x3F80;
+    }
+    tc::fence_proxy_async_smem();
+  }
   tc::tc_fence_before();
   __syncthreads();
   tc::tc_fence_after();
@@ -146,6 +163,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQK, const __grid_constant__
       constexpr uint32_t idesc_s = tc::idesc_bf16_f32(AT_BQ, AT_BK);
       constexpr uint32_t idesc_o = tc::idesc_bf16_f32(AT_BQ, 32);
       const uint64_t p_desc = tc::smem_desc_kmajor<128>(tc::smem_u32(smem + SM::P_OFF));
+      const uint64_t id_desc = tc::smem_desc_kmajor<128>(tc::smem_u32(smem + SM::ID_OFF));
       // issue side: S(j) = Q K^T for the next (unit, key tile); consume side: P(i) V.  j runs one step ahead of i.
       const int units = *p.n_rows * p.H * p.QT;
       int cu = blockIdx.x, ckt = 0;
@@ -166,6 +184,12 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQK, const __grid_constant__
         const uint32_t d = tmem_S + (j & 1) * AT_BK;
         tc::mma_bf16(d, q_desc, k_desc, idesc_s, false);
         tc::mma_bf16(d, q_desc + 2, k_desc + 2, idesc_s, true);
+        if (p.has_bias) {   // S += bias I: the pair-bias tile of this stage as A operand, the identity as B
+          const uint64_t b_desc = tc::smem_desc_kmajor<128>(
+              tc::smem_u32(smem + SM::STAGE_OFF + s * p.stage_bytes + SM::K_BYTES + SM::V_BYTES));
+#pragma unroll
+          for (int k = 0; k < AT_BK / 16; ++k) tc::mma_bf16(d, b_desc + 2 * k, id_desc + 2 * k, idesc_s, true);
+        }
         tc::mma_commit(&s_full[j & 1]);
         if (ckt == cn - 1) {
           tc::mma_commit(&q_empty[qb]);
@@ -211,14 +235,17 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQK, const __grid_constant__
       const int b = br / p.R;
       const int qi = qt * AT_BQ + row;
       if (b != cur_b) {
-        // additive key mask in the exp2 domain: 0 for an unmasked key, -inf for a masked or out-of-range key (R3)
+        // key mask of this protein as one bit per key (1 = masked or out of range, R3) + one bit per key tile
         tc::named_bar_sync(1, 128);
         if (threadIdx.x == 0) *maskbits = 0;
         tc::named_bar_sync(1, 128);
         for (int j = threadIdx.x; j < p.n_kt * AT_BK; j += 128) {
           const bool keep = j < p.L && p.keymask[(long)b * p.L + j] > 0.5f;
-          mterm[j] = keep ? 0.f : -INFINITY;
-          if (!keep) atomicOr(maskbits, 1u << (j / AT_BK));
+          const uint32_t w = __ballot_sync(0xffffffffu, !keep);
+          if (lane == 0) {
+            mbits[j >> 5] = w;
+            if (w) atomicOr(maskbits, 1u << (j / AT_BK));
+          }
         }
         tc::named_bar_sync(1, 128);
         tile_masked = *maskbits;
@@ -239,40 +266,21 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQK, const __grid_constant__
 #pragma unroll
       for (int d = 0; d < 32; ++d) oacc[d] = 0.f;
       for (int kt = 0; kt < n_kt; ++kt, ++i) {
-        const uint32_t s = i % ST;
-        const uint8_t* bias_t = smem + SM::STAGE_OFF + s * p.stage_bytes + SM::K_BYTES + SM::V_BYTES;
-        if (p.has_bias) tc::mbar_wait(&kv_full[s], (i / ST) & 1);
         tc::mbar_wait(&s_full[i & 1], (i >> 1) & 1);
         tc::tc_fence_after();
         uint32_t sv[2][32];
         tc::tmem_ld32(tmem_S + lane_addr + (i & 1) * AT_BK, sv[0]);
         tc::tmem_ld32(tmem_S + lane_addr + (i & 1) * AT_BK + 32, sv[1]);
         tc::tmem_ld_wait();
-        float x[64];
-        if (p.has_bias) {
+        float x[64];   // logits in the exp2 domain; the pair bias was already added by the tensor core
 #pragma unroll
-          for (int c = 0; c < 8; ++c) {   // 8 keys per 16-byte bias chunk
-            const uint4 bu = *reinterpret_cast<const uint4*>(bias_t + tc::swz_offset<128>(row, c));
-            const uint32_t bw[4] = {bu.x, bu.y, bu.z, bu.w};
-#pragma unroll
-            for (int e = 0; e < 4; ++e) {
-              const int j = c * 8 + 2 * e;
-              x[j] = __uint_as_float(sv[j >> 5][j & 31]) + __uint_as_float(bw[e] << 16);
-              x[j + 1] = __uint_as_float(sv[j >> 5][(j + 1) & 31]) + __uint_as_float(bw[e] & 0xffff0000u);
-            }
-          }
-        } else {
-#pragma unroll
-          for (int j = 0; j < 64; ++j) x[j] = __uint_as_float(sv[j >> 5][j & 31]);
-        }
+        for (int j = 0; j < 64; ++j) x[j] = __uint_as_float(sv[j >> 5][j & 31]);
         if ((tile_masked >> kt) & 1) {
+          const uint32_t w0 = mbits[2 * kt], w1 = mbits[2 * kt + 1];
 #pragma unroll
-          for (int c = 0; c < 16; ++c) {
-            const float4 m4 = *reinterpret_cast<const float4*>(mterm + kt * AT_BK + c * 4);
-            x[c * 4 + 0] += m4.x;
-            x[c * 4 + 1] += m4.y;
-            x[c * 4 + 2] += m4.z;
-            x[c * 4 + 3] += m4.w;
+          for (int j = 0; j < 32; ++j) {
+            if ((w0 >> j) & 1) x[j] = -INFINITY;
+            if ((w1 >> j) & 1) x[32 + j] = -INFINITY;
           }
         }
         float mx0 = x[0], mx1 = x[1], mx2 = x[2], mx3 = x[3];
