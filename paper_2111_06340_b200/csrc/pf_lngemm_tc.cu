@@ -180,6 +180,34 @@ __device__ __forceinline__ void g2_row16_group(uint32_t taddr, uint8_t* srow, co
   }
 }
 
+// The same for a group without bias and activation (q, k of the attention projections): both TMEM loads are issued before
+// the single wait, and the arithmetic is one multiply (q: log2(e)/sqrt(d)) or nothing (k) per value before the conversion.
+template <int FMT>
+__device__ __forceinline__ void g2_row16_plain(uint32_t taddr, uint8_t* srow, float scale, uint32_t sw) {
+  uint32_t v[2][32];
+  tc::tmem_ld32(taddr, v[0]);
+  tc::tmem_ld32(taddr + 32, v[1]);
+  tc::tmem_ld_wait();
+  const bool scaled = scale != 1.0f;
+#pragma unroll
+  for (int hf = 0; hf < 2; ++hf) {
+    uint32_t pk[16];
+#pragma unroll
+    for (int e = 0; e < 32; e += 2) {
+      float x0 = __uint_as_float(v[hf][e]), x1 = __uint_as_float(v[hf][e + 1]);
+      if (scaled) {
+        x0 *= scale;
+        x1 *= scale;
+      }
+      pk[e >> 1] = pack16(x0, x1, FMT);
+    }
+#pragma unroll
+    for (int c = 0; c < 4; ++c)
+      *reinterpret_cast<uint4*>(srow + (((uint32_t)(hf * 4 + c) ^ sw) << 4)) =
+          make_uint4(pk[c * 4], pk[c * 4 + 1], pk[c * 4 + 2], pk[c * 4 + 3]);
+  }
+}
+
 template <int K, int AMODE>
 __global__ void __launch_bounds__(G2_THREADS, 1)
 gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUtensorMap tmA,
@@ -302,6 +330,9 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
               } else if (op.act == ACT_RELU) {
                 if (op.fmt) g2_row16_group<ACT_RELU, 1>(ta, srow, b64, scale, sw);
                 else g2_row16_group<ACT_RELU, 0>(ta, srow, b64, scale, sw);
+              } else if (b64 == sbias_tab + SM::BIAS_FLOATS) {   // no bias: the zero pad
+                if (op.fmt) g2_row16_plain<1>(ta, srow, scale, sw);
+                else g2_row16_plain<0>(ta, srow, scale, sw);
               } else {
                 if (op.fmt) g2_row16_group<ACT_NONE, 1>(ta, srow, b64, scale, sw);
                 else g2_row16_group<ACT_NONE, 0>(ta, srow, b64, scale, sw);
@@ -418,18 +449,30 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
             __syncwarp();
             const float mk = op.masked ? mask : 1.0f;
             bf16* dst = sb16 + ((xlw * 64) << p.ytw_shift) + ylw;
+            if (!op.masked && sbias == sbias_tab + SM::BIAS_FLOATS) {
+              // V^T of the attention projections: no bias, no mask -> convert and store only
 #pragma unroll 1
-            for (int hf = 0; hf < 2; ++hf) {
-              uint32_t v[32];
-              float bb[32];
-              tc::tmem_ld32(tacc + j * 64 + hf * 32, v);
-              lds32(sbias + hf * 32, bb);
-              tc::tmem_ld_wait();
-              bf16 r[32];
+              for (int hf = 0; hf < 2; ++hf) {
+                uint32_t v[32];
+                tc::tmem_ld32(tacc + j * 64 + hf * 32, v);
+                tc::tmem_ld_wait();
 #pragma unroll
-              for (int e = 0; e < 32; ++e) r[e] = __float2bfloat16_rn((__uint_as_float(v[e]) + bb[e]) * mk);
+                for (int e = 0; e < 32; ++e) dst[(hf * 32 + e) << p.ytw_shift] = __float2bfloat16_rn(__uint_as_float(v[e]));
+              }
+            } else {
+#pragma unroll 1
+              for (int hf = 0; hf < 2; ++hf) {
+                uint32_t v[32];
+                float bb[32];
+                tc::tmem_ld32(tacc + j * 64 + hf * 32, v);
+                lds32(sbias + hf * 32, bb);
+                tc::tmem_ld_wait();
+                bf16 r[32];
 #pragma unroll
-              for (int e = 0; e < 32; ++e) dst[(hf * 32 + e) << p.ytw_shift] = r[e];
+                for (int e = 0; e < 32; ++e) r[e] = __float2bfloat16_rn((__uint_as_float(v[e]) + bb[e]) * mk);
+#pragma unroll
+                for (int e = 0; e < 32; ++e) dst[(hf * 32 + e) << p.ytw_shift] = r[e];
+              }
             }
             tc::fence_proxy_async_smem();
             __syncwarp();
