@@ -78,7 +78,10 @@ void tc_set_error(const std::string& s);
 // ---- persistent LN-fused projection GEMM (pf_lngemm_tc.cu) ----
 // Rows of the GEMM are (b, x in [0,D1), y in [0,D2)); one CTA tile = XT consecutive x times YT consecutive y (XT*YT = 128).
 // The 64-column groups of the output are described by G2Op: what is done to the accumulator and where it goes.
-enum G2Kind { G2_SKIP = 0, G2_ROW16 = 1, G2_CM_DUAL = 2, G2_HEADS = 3, G2_VT = 4, G2_RESID = 5 };
+// G2_VTS: like G2_VT, but the half-window it belongs to is computed with the operand roles SWAPPED (weights as the M side,
+// the LayerNorm tile as the N side), so the accumulator already holds the transposed tile: TMEM lane = output column,
+// TMEM column = tile row.  Group j of a window covers half j / 2 and tile rows [64 (j % 2), +64); needs YT >= 64.
+enum G2Kind { G2_SKIP = 0, G2_ROW16 = 1, G2_CM_DUAL = 2, G2_HEADS = 3, G2_VT = 4, G2_RESID = 5, G2_VTS = 6 };
 struct G2Op {
   int kind;      // G2Kind
   int act;       // Act, applied after scale and bias (ROW16)
@@ -142,6 +145,7 @@ struct G2Desc {
   int Lpad;
   G2Op ops[G2_MAX_OPS];
   int n_ops;
+  unsigned swap_mask;       // bit (2 nt + h): the 128 columns of half h of window nt are computed operand-swapped (G2_VTS groups)
   const unsigned char* tile_active;   // optional [num_tiles]: 0 = every row of the tile is masked, skip it (pf_flags.cu)
 };
 int launch_gemm2(TmaCtx* ctx, const G2Desc& d, int num_sms, cudaStream_t st);

@@ -80,6 +80,7 @@ struct G2Params {
   int vt_cols;
   int Lpad;
   const unsigned char* tile_active;
+  unsigned swap_mask;
   int bias_lo, bias_n;    // the bias table holds columns [bias_lo, bias_lo + bias_n); all other columns have zero bias
   G2Op ops[G2_MAX_OPS];
 };
@@ -208,12 +209,45 @@ __device__ __forceinline__ void g2_row16_plain(uint32_t taddr, uint8_t* srow, fl
   }
 }
 
+// Sigmoid gate stored as fp16: the pre-activation is rounded to fp16 pairs first and the sigmoid is evaluated on the
+// pair, sigmoid(x) = 0.5 + 0.5 tanh(x / 2) with tanh.approx.f16x2 — one MUFU per TWO values and the result is already the
+// packed fp16 pair that is stored (per value: 1 FFMA + 2.5 half-rate-free packed ops instead of 4.5 fp32 ops + 1 MUFU).
+// The gate is a number in [0, 1] kept in fp16 anyway; the extra error of the fp16 evaluation is ~5e-4 absolute.
+template <int FMT>
+__device__ __forceinline__ void g2_row16_gate(uint32_t taddr, uint8_t* srow, const float* bias64, float scale, uint32_t sw) {
+  static_assert(FMT == 1, "the packed gate path stores fp16");
+  const __half2 half_h = __floats2half2_rn(0.5f, 0.5f);
+#pragma unroll
+  for (int hf = 0; hf < 2; ++hf) {
+    uint32_t v[32];
+    float bb[32];
+    tc::tmem_ld32(taddr + hf * 32, v);
+    lds32(bias64 + hf * 32, bb);
+    tc::tmem_ld_wait();
+    uint32_t pk[16];
+#pragma unroll
+    for (int e = 0; e < 32; e += 2) {
+      const float x0 = fmaf(__uint_as_float(v[e]), scale, bb[e]), x1 = fmaf(__uint_as_float(v[e + 1]), scale, bb[e + 1]);
+      __half2 h = __hmul2(__floats2half2_rn(x0, x1), half_h);
+      uint32_t hu = *reinterpret_cast<uint32_t*>(&h), tu;
+      asm("tanh.approx.f16x2 %0, %1;" : "=r"(tu) : "r"(hu));
+      __half2 r = __hfma2(*reinterpret_cast<__half2*>(&tu), half_h, half_h);
+      pk[e >> 1] = *reinterpret_cast<uint32_t*>(&r);
+    }
+#pragma unroll
+    for (int c = 0; c < 4; ++c)
+      *reinterpret_cast<uint4*>(srow + (((uint32_t)(hf * 4 + c) ^ sw) << 4)) =
+          make_uint4(pk[c * 4], pk[c * 4 + 1], pk[c * 4 + 2], pk[c * 4 + 3]);
+  }
+}
+
 template <int K, int AMODE>
 __global__ void __launch_bounds__(G2_THREADS, 1)
 gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUtensorMap tmA,
              const __grid_constant__ CUtensorMap tmO0, const __grid_constant__ CUtensorMap tmT0,
              const __grid_constant__ CUtensorMap tmT1, const __grid_constant__ CUtensorMap tmH,
-             const __grid_constant__ CUtensorMap tmR, const __grid_constant__ G2Params p) {
+             const __grid_constant__ CUtensorMap tmR, const __grid_constant__ CUtensorMap tmVS,
+             const __grid_constant__ G2Params p) {
   using SM = G2Smem<K>;
   constexpr int KB = SM::KB;
   constexpr int WS = SM::W_STAGES;
@@ -239,6 +273,7 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
     tc::prefetch_tmap(&tmT1);
     tc::prefetch_tmap(&tmH);
     tc::prefetch_tmap(&tmR);
+    tc::prefetch_tmap(&tmVS);
     for (int i = 0; i < 2; ++i) {
       tc::mbar_init(&a_full[i], AMODE == 0 ? G2_PROD_WARPS * 32 : 1);
       tc::mbar_init(&a_empty[i], 1);
@@ -325,7 +360,7 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
               uint8_t* srow = sb + lane * 128;
               const float* b64 = sbias;
               if (op.act == ACT_SIGMOID) {
-                if (op.fmt) g2_row16_group<ACT_SIGMOID, 1>(ta, srow, b64, scale, sw);
+                if (op.fmt) g2_row16_gate<1>(ta, srow, b64, scale, sw);
                 else g2_row16_group<ACT_SIGMOID, 0>(ta, srow, b64, scale, sw);
               } else if (op.act == ACT_RELU) {
                 if (op.fmt) g2_row16_group<ACT_RELU, 1>(ta, srow, b64, scale, sw);
@@ -439,6 +474,20 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
             __syncwarp();
             if (leader) {
               tc::tma_store_4d(&tmH, sb, tcd.y0 + yw0, tcd.x0 + xw0, op.dst_col, tcd.b);
+              tc::bulk_commit();
+            }
+          } else if (kind == G2_VTS) {
+            // operand-swapped half-window: this thread owns output column (channel) 32 quarter + lane of the half and reads 64
+            // consecutive tile rows from TMEM: convert, stage as a 128-byte row, one TMA store {64 y, 32 channels}
+            sb = sb_team + (gcnt++ % NST) * SM::STW_BYTES;
+            if (leader) tc::bulk_wait_read<NST - 1>();
+            __syncwarp();
+            g2_row16_plain<0>(tacc + j * 64, sb + lane * 128, 1.0f, sw);
+            tc::fence_proxy_async_smem();
+            __syncwarp();
+            if (leader) {
+              const int r0 = (j & 1) * 64;   // first tile row of this group
+              tc::tma_store_4d(&tmVS, sb, tcd.y0 + (r0 & (p.YT - 1)), op.dst_col + quarter * 32, tcd.x0 + (r0 >> p.yt_shift), tcd.b);
               tc::bulk_commit();
             }
           } else {   // G2_VT
@@ -596,15 +645,39 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
           n_eff = n_eff >= G2_BN ? G2_BN : ((n_eff + 15) & ~15);
           const uint32_t idesc = p.op_fmt ? tc::idesc_f16_f32(128, n_eff) : tc::idesc_bf16_f32(128, n_eff);
           const uint32_t d_tmem = tmem_base + buf * G2_BN;
+          const unsigned swp = (p.swap_mask >> (2 * nt)) & 3u;
+          // per 128-column half when a half of this window is operand-swapped
+          const int nh0 = n_eff < 128 ? n_eff : 128, nh1 = n_eff - 128;
+          const uint32_t idesc_sw = p.op_fmt ? tc::idesc_f16_f32(128, 128) : tc::idesc_bf16_f32(128, 128);
 #pragma unroll 1
           for (int kb = 0; kb < KB; ++kb, ++wc) {
             const uint32_t s = wc % WS;
             tc::mbar_wait(&w_full[s], (wc / WS) & 1);
             tc::tc_fence_after();
             const uint64_t a_desc = tc::smem_desc_kmajor<128>(a_addr + kb * SM::KB_BYTES);
-            const uint64_t b_desc = tc::smem_desc_kmajor<128>(tc::smem_u32(smem + SM::W_OFF + s * SM::W_STAGE));
+            const uint32_t w_addr = tc::smem_u32(smem + SM::W_OFF + s * SM::W_STAGE);
+            const uint64_t b_desc = tc::smem_desc_kmajor<128>(w_addr);
+            if (swp == 0) {
 #pragma unroll
-            for (int k = 0; k < 4; ++k) tc::mma_bf16(d_tmem, a_desc + 2 * k, b_desc + 2 * k, idesc, (kb | k) != 0);
+              for (int k = 0; k < 4; ++k) tc::mma_bf16(d_tmem, a_desc + 2 * k, b_desc + 2 * k, idesc, (kb | k) != 0);
+            } else {
+#pragma unroll 1
+              for (int hh = 0; hh < 2; ++hh) {
+                const int nh = hh ? nh1 : nh0;
+                if (nh <= 0) continue;
+                const uint64_t wh_desc = tc::smem_desc_kmajor<128>(w_addr + hh * (128 * 128));   // weight rows [128 hh, +128)
+                if ((swp >> hh) & 1) {   // D[out column, tile row] = W_half (M side) x A tile (N side)
+#pragma unroll
+                  for (int k = 0; k < 4; ++k)
+                    tc::mma_bf16(d_tmem + hh * 128, wh_desc + 2 * k, a_desc + 2 * k, idesc_sw, (kb | k) != 0);
+                } else {
+                  const uint32_t idh = p.op_fmt ? tc::idesc_f16_f32(128, nh) : tc::idesc_bf16_f32(128, nh);
+#pragma unroll
+                  for (int k = 0; k < 4; ++k)
+                    tc::mma_bf16(d_tmem + hh * 128, a_desc + 2 * k, wh_desc + 2 * k, idh, (kb | k) != 0);
+                }
+              }
+            }
             tc::mma_commit(&w_empty[s]);
           }
           tc::mma_commit(&acc_full[buf]);
@@ -625,8 +698,8 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
 // ------------------------------------------------------------------------------------------------
 template <int K, int AMODE>
 static int launch_g2(const CUtensorMap& tmW, const CUtensorMap& tmA, const CUtensorMap& tmO0, const CUtensorMap& tmT0,
-                     const CUtensorMap& tmT1, const CUtensorMap& tmH, const CUtensorMap& tmR, const G2Params& p, int num_sms,
-                     cudaStream_t st) {
+                     const CUtensorMap& tmT1, const CUtensorMap& tmH, const CUtensorMap& tmR, const CUtensorMap& tmVS,
+                     const G2Params& p, int num_sms, cudaStream_t st) {
   auto kern = gemm2_kernel<K, AMODE>;
   static bool configured = false;
   if (!configured) {
@@ -638,7 +711,7 @@ static int launch_g2(const CUtensorMap& tmW, const CUtensorMap& tmA, const CUten
     configured = true;
   }
   unsigned grid = (unsigned)(p.num_tiles < (long)num_sms ? p.num_tiles : (long)num_sms);
-  kern<<<grid, G2_THREADS, G2Smem<K>::TOTAL, st>>>(tmW, tmA, tmO0, tmT0, tmT1, tmH, tmR, p);
+  kern<<<grid, G2_THREADS, G2Smem<K>::TOTAL, st>>>(tmW, tmA, tmO0, tmT0, tmT1, tmH, tmR, tmVS, p);
   return 0;
 }
 
@@ -739,10 +812,23 @@ int launch_gemm2(TmaCtx* ctx, const G2Desc& d, int num_sms, cudaStream_t st) {
   } else {
     tmO0 = tmW;
   }
+  CUtensorMap tmVS = tmW;
   tmT[0] = tmT[1] = tmH = tmW;
   if (d.vt_out && d.cm_out[0]) {
     tc_set_error("gemm2: transposed-column and channel-major outputs cannot be combined");
     return -1;
+  }
+  p.swap_mask = d.swap_mask;
+  if (d.swap_mask) {
+    if (!d.vt_out || p.YT < 64) {
+      tc_set_error("gemm2: operand-swapped transposed outputs need vt_out and a tile of at least 64 consecutive y");
+      return -1;
+    }
+    uint64_t vc = d.vt_cols;
+    uint64_t dims[4] = {D2, vc, D1, Bn};
+    uint64_t str[3] = {Lp * 2, vc * Lp * 2, D1 * vc * Lp * 2};
+    uint32_t box[4] = {64, 32, 1, 1};
+    if (tma_encode(ctx, &tmVS, d.vt_out, 0, 4, dims, str, box, 128) != 0) return -1;
   }
   if (d.vt_out) {   // [(b, x), column, y] with row pitch Lpad: dims {y, column, x, b}
     uint64_t vc = d.vt_cols;
@@ -781,11 +867,11 @@ int launch_gemm2(TmaCtx* ctx, const G2Desc& d, int num_sms, cudaStream_t st) {
     tmR = tmW;
   }
   if (d.K == 128) {
-    return d.a_mode == 0 ? launch_g2<128, 0>(tmW, tmA, tmO0, tmT[0], tmT[1], tmH, tmR, p, num_sms, st)
-                         : launch_g2<128, 1>(tmW, tmA, tmO0, tmT[0], tmT[1], tmH, tmR, p, num_sms, st);
+    return d.a_mode == 0 ? launch_g2<128, 0>(tmW, tmA, tmO0, tmT[0], tmT[1], tmH, tmR, tmVS, p, num_sms, st)
+                         : launch_g2<128, 1>(tmW, tmA, tmO0, tmT[0], tmT[1], tmH, tmR, tmVS, p, num_sms, st);
   }
-  return d.a_mode == 0 ? launch_g2<256, 0>(tmW, tmA, tmO0, tmT[0], tmT[1], tmH, tmR, p, num_sms, st)
-                       : launch_g2<256, 1>(tmW, tmA, tmO0, tmT[0], tmT[1], tmH, tmR, p, num_sms, st);
+  return d.a_mode == 0 ? launch_g2<256, 0>(tmW, tmA, tmO0, tmT[0], tmT[1], tmH, tmR, tmVS, p, num_sms, st)
+                       : launch_g2<256, 1>(tmW, tmA, tmO0, tmT[0], tmT[1], tmH, tmR, tmVS, p, num_sms, st);
 }
 
 }  // namespace pf

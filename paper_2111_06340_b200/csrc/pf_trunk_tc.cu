@@ -220,6 +220,10 @@ struct TcDriver {
           d.ops[n] = op(G2_ROW16, col);
           if (seg == 0) d.ops[n].scale = 0.17677669529663687f * kLog2e;   // log2(e)/sqrt(32)  (R12)
           if (seg == 2) { d.ops[n].act = ACT_SIGMOID; d.ops[n].fmt = 1; }
+        } else if (g2_pick_yt(D2) >= 64) {
+          // V^T comes out of the MMA already transposed: the half-window holding these columns is computed operand-swapped
+          d.ops[n] = op(G2_VTS, ((col - 3 * C) / 128) * 128);
+          d.swap_mask |= 1u << (col / 128);
         } else {
           d.ops[n] = op(G2_VT, col - 3 * C);
         }
