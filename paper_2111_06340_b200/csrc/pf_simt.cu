@@ -278,9 +278,101 @@ __global__ void __launch_bounds__(256) lnc_kernel(const float* __restrict__ t, T
   }
 }
 
+// Streaming variant for C = 128 (the triangle hidden size): block = one (b, i) row x 64 consecutive j x 128 channels.
+// Warp w loads channels [16 w, 16 w + 16) as 256-byte rows (float2 per lane: positions 2 lane, 2 lane + 1), so every thread
+// holds 16 channels x 2 positions in registers; per-position statistics are the thread's partial sums combined across the
+// eight warps through shared memory (no shuffles); the normalised values are staged [position][channel] in shared memory
+// and leave as coalesced 16-byte stores.
+template <typename T>
+__global__ void __launch_bounds__(256) lnc128_kernel(const float* __restrict__ t, T* __restrict__ y,
+                                                     const float* __restrict__ gamma, const float* __restrict__ beta,
+                                                     const float* __restrict__ seq_mask, int N, int Npad) {
+  constexpr int C = 128, PJ = 64;
+  __shared__ float part[2][8][PJ];                       // [sum | sum of squares][warp][position]
+  constexpr int ROWP = C + 16 / (int)sizeof(T);           // row pitch: + 16 bytes, so the packed 16-byte stores of the 32
+                                                         // lanes (two rows apart) spread over the banks (2-way at worst)
+  __shared__ __align__(16) T stage[PJ][ROWP];
+  const int j0 = blockIdx.x * PJ, i = blockIdx.y, b = blockIdx.z;
+  if (seq_mask && seq_mask[(long)b * N + i] < 0.5f) return;   // padded row i: every output of it is at a masked position
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int j = j0 + 2 * lane;
+  float2 v[16];
+  const bool in = j < Npad;                              // Npad is even: a pair never straddles the padded row end
+#pragma unroll
+  for (int k = 0; k < 16; ++k) {
+    const int c = warp * 16 + k;
+    v[k] = in ? __ldg(reinterpret_cast<const float2*>(t + (((long)b * C + c) * N + i) * Npad + j)) : make_float2(0.f, 0.f);
+  }
+  float s0 = 0.f, s1 = 0.f;
+#pragma unroll
+  for (int k = 0; k < 16; ++k) {
+    s0 += v[k].x;
+    s1 += v[k].y;
+  }
+  part[0][warp][2 * lane] = s0;
+  part[0][warp][2 * lane + 1] = s1;
+  __syncthreads();
+  float m0 = 0.f, m1 = 0.f;
+#pragma unroll
+  for (int w = 0; w < 8; ++w) {
+    m0 += part[0][w][2 * lane];
+    m1 += part[0][w][2 * lane + 1];
+  }
+  m0 *= (1.0f / C);
+  m1 *= (1.0f / C);
+  float q0 = 0.f, q1 = 0.f;
+#pragma unroll
+  for (int k = 0; k < 16; ++k) {
+    const float d0 = v[k].x - m0, d1 = v[k].y - m1;
+    q0 += d0 * d0;
+    q1 += d1 * d1;
+  }
+  part[1][warp][2 * lane] = q0;
+  part[1][warp][2 * lane + 1] = q1;
+  __syncthreads();
+  float r0 = 0.f, r1 = 0.f;
+#pragma unroll
+  for (int w = 0; w < 8; ++w) {
+    r0 += part[1][w][2 * lane];
+    r1 += part[1][w][2 * lane + 1];
+  }
+  r0 = rsqrtf(r0 * (1.0f / C) + 1e-5f);
+  r1 = rsqrtf(r1 * (1.0f / C) + 1e-5f);
+  {
+    // this thread's 16 consecutive channels of its two positions: 16 * sizeof(T) contiguous bytes each, written as 16-byte packs
+    __align__(16) T o0[16], o1[16];
+#pragma unroll
+    for (int k = 0; k < 16; ++k) {
+      const int c = warp * 16 + k;
+      const float g = __ldg(gamma + c), be = __ldg(beta + c);
+      store1(&o0[k], (v[k].x - m0) * r0 * g + be);
+      store1(&o1[k], (v[k].y - m1) * r1 * g + be);
+    }
+    constexpr int NP = 16 * sizeof(T) / 16;              // 16-byte packs per position
+#pragma unroll
+    for (int q = 0; q < NP; ++q) {
+      reinterpret_cast<uint4*>(&stage[2 * lane][warp * 16])[q] = reinterpret_cast<const uint4*>(o0)[q];
+      reinterpret_cast<uint4*>(&stage[2 * lane + 1][warp * 16])[q] = reinterpret_cast<const uint4*>(o1)[q];
+    }
+  }
+  __syncthreads();
+  // PJ rows of C * sizeof(T) bytes, 16 bytes per thread and step
+  constexpr int CH = C * sizeof(T) / 16;                 // 16-byte chunks per position
+  for (int q = threadIdx.x; q < PJ * CH; q += 256) {
+    const int pj = q / CH, ch = q % CH;
+    if (j0 + pj < N)
+      reinterpret_cast<uint4*>(y + (((long)b * N + i) * N + j0 + pj) * C)[ch] = reinterpret_cast<const uint4*>(&stage[pj][0])[ch];
+  }
+}
+
 template <typename T>
 void launch_lnc(const float* t_cm, T* y, const float* gamma, const float* beta, const float* seq_mask, int B, int C, int N,
                 int Npad, cudaStream_t st) {
+  if (C == 128) {
+    dim3 grid((N + 63) / 64, N, B);
+    lnc128_kernel<T><<<grid, 256, 0, st>>>(t_cm, y, gamma, beta, seq_mask, N, Npad);
+    return;
+  }
   dim3 grid((N + 31) / 32, N, B);
   lnc_kernel<T><<<grid, 256, C * 33 * sizeof(float), st>>>(t_cm, y, gamma, beta, seq_mask, C, N, Npad);
 }
