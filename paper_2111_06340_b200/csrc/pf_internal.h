@@ -81,7 +81,9 @@ void tc_set_error(const std::string& s);
 // G2_VTS: like G2_VT, but the half-window it belongs to is computed with the operand roles SWAPPED (weights as the M side,
 // the LayerNorm tile as the N side), so the accumulator already holds the transposed tile: TMEM lane = output column,
 // TMEM column = tile row.  Group j of a window covers half j / 2 and tile rows [64 (j % 2), +64); needs YT >= 64.
-enum G2Kind { G2_SKIP = 0, G2_ROW16 = 1, G2_CM_DUAL = 2, G2_HEADS = 3, G2_VT = 4, G2_RESID = 5, G2_VTS = 6 };
+// G2_CMS: G2_CM_DUAL on a window whose two halves (p | gate) are both operand-swapped: lane = channel, the group j (0 or 1)
+// covers tile rows [64 j, +64); the row masks of the tile come from a small shared-memory table.
+enum G2Kind { G2_SKIP = 0, G2_ROW16 = 1, G2_CM_DUAL = 2, G2_HEADS = 3, G2_VT = 4, G2_RESID = 5, G2_VTS = 6, G2_CMS = 7 };
 struct G2Op {
   int kind;      // G2Kind
   int act;       // Act, applied after scale and bias (ROW16)

@@ -81,6 +81,7 @@ struct G2Params {
   int Lpad;
   const unsigned char* tile_active;
   unsigned swap_mask;
+  int has_cms;            // some group is G2_CMS: the epilogue warps publish the tile's row masks once per tile
   int bias_lo, bias_n;    // the bias table holds columns [bias_lo, bias_lo + bias_n); all other columns have zero bias
   G2Op ops[G2_MAX_OPS];
 };
@@ -102,7 +103,9 @@ struct G2Smem {
   // that stand in for every 64-column group outside the table (q, k, v of the attention projections carry no bias)
   static constexpr int BIAS_FLOATS = (K == 256) ? 256 : 768;
   static constexpr int BIAS_OFF = ST_OFF + 2 * ST_PER_TEAM * ST_BYTES;
-  static constexpr int BAR_OFF = BIAS_OFF + (BIAS_FLOATS + 64) * 4;
+  static constexpr int RM_OFF = BIAS_OFF + (BIAS_FLOATS + 64) * 4;   // row masks of the current tile, two buffers (G2_CMS)
+  static constexpr int RM_BYTES = (K == 128) ? 2 * 128 * 4 : 0;     // only the K = 128 kernels have operand-swapped gated groups
+  static constexpr int BAR_OFF = RM_OFF + RM_BYTES;
   static constexpr int TOTAL = BAR_OFF + 192 + 1024;
 };
 
@@ -313,6 +316,7 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
     const float* const sbias_tab = reinterpret_cast<const float*>(smem + SM::BIAS_OFF);
     const uint32_t sw = (uint32_t)(lr & 7);
     uint32_t ac = 0;                                   // accumulator buffers consumed so far
+    uint32_t tcount = 0;                               // tiles processed so far
     for (long tile = blockIdx.x; tile < p.num_tiles; tile += gridDim.x) {
       if (!tile_on(tile, p)) continue;
       const TileCoord tcd = tile_coord(tile, p);
@@ -326,6 +330,14 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
         mask = p.seq_mask[(long)tcd.b * p.D1 + x] * p.seq_mask[(long)tcd.b * p.D2 + y];
       }
       const long grow = ((long)tcd.b * p.D1 + x) * p.D2 + y;   // GEMM row index (gate rows)
+      float* rmask = reinterpret_cast<float*>(smem + SM::RM_OFF) + (tcount & 1) * 128;
+      if (SM::RM_BYTES && p.has_cms) {
+        // operand-swapped gated groups index the row mask by TMEM column: publish this tile's 128 masks (the buffer of two
+        // tiles ago is free: every warp passed the previous tile's barrier after its last read of it)
+        if (team == 0) rmask[lr] = valid ? mask : 0.f;
+        tc::named_bar_sync(3, G2_EPI_WARPS * 32);
+      }
+      ++tcount;
       for (int nt = 0; nt < p.n_tiles; ++nt, ++ac) {
         const uint32_t buf = ac & 1;
         // this warp's two groups of the window: their descriptors are fetched (indexed constant loads) BEFORE waiting for the
@@ -474,6 +486,43 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
             __syncwarp();
             if (leader) {
               tc::tma_store_4d(&tmH, sb, tcd.y0 + yw0, tcd.x0 + xw0, op.dst_col, tcd.b);
+              tc::bulk_commit();
+            }
+          } else if (kind == G2_CMS) {
+            // gated, masked triangle operand out of two operand-swapped halves (p | gate): this thread owns channel
+            // 32 quarter + lane and the 64 tile rows [64 j, +64) -> 128-byte staging row -> TMA store {64 y, 1 x, 32 channels}
+            sb = sb_team + (gcnt++ % NST) * SM::STW_BYTES;
+            const int ch = quarter * 32 + lane;
+            const int wcol = nt * G2_BN - p.bias_lo;   // the whole window's bias is in the table (checked by the launcher)
+            const float bpv = sbias_tab[wcol + ch], bgv = sbias_tab[wcol + 128 + ch];
+            if (leader) tc::bulk_wait_read<NST - 1>();
+            __syncwarp();
+#pragma unroll 1
+            for (int hf = 0; hf < 2; ++hf) {
+              uint32_t v[32], g[32];
+              float mk[32];
+              tc::tmem_ld32(tacc + j * 64 + hf * 32, v);
+              tc::tmem_ld32(tacc + 128 + j * 64 + hf * 32, g);
+              lds32(rmask + j * 64 + hf * 32, mk);
+              tc::tmem_ld_wait();
+              uint32_t pk[16];
+#pragma unroll
+              for (int e = 0; e < 32; e += 2) {
+                const float o0 = mk[e] * fast_sigmoid2(__uint_as_float(g[e]) + bgv) * (__uint_as_float(v[e]) + bpv);
+                const float o1 = mk[e + 1] * fast_sigmoid2(__uint_as_float(g[e + 1]) + bgv) * (__uint_as_float(v[e + 1]) + bpv);
+                pk[e >> 1] = pack16(o0, o1, 0);
+              }
+#pragma unroll
+              for (int c = 0; c < 4; ++c)
+                *reinterpret_cast<uint4*>(sb + lane * 128 + (((uint32_t)(hf * 4 + c) ^ sw) << 4)) =
+                    make_uint4(pk[c * 4], pk[c * 4 + 1], pk[c * 4 + 2], pk[c * 4 + 3]);
+            }
+            tc::fence_proxy_async_smem();
+            __syncwarp();
+            if (leader) {
+              const int r0 = j * 64;   // first tile row of this group
+              tc::tma_store_4d(op.map ? &tmT1 : &tmT0, sb, tcd.y0 + (r0 & (p.YT - 1)), tcd.x0 + (r0 >> p.yt_shift),
+                               op.dst_col + quarter * 32, tcd.b);
               tc::bulk_commit();
             }
           } else if (kind == G2_VTS) {
@@ -769,10 +818,12 @@ int launch_gemm2(TmaCtx* ctx, const G2Desc& d, int num_sms, cudaStream_t st) {
     }
   }
   bool need_bias = false;
+  p.has_cms = 0;
   for (int i = 0; i < G2_MAX_OPS; ++i) {
     if (i < d.n_ops) p.ops[i] = d.ops[i];
     else p.ops[i].kind = G2_SKIP;
-    if (p.ops[i].kind == G2_RESID || p.ops[i].kind == G2_CM_DUAL) need_bias = true;
+    if (p.ops[i].kind == G2_CMS) p.has_cms = 1;
+    if (p.ops[i].kind == G2_RESID || p.ops[i].kind == G2_CM_DUAL || p.ops[i].kind == G2_CMS) need_bias = true;
   }
   if (d.a_mode == 0 && d.op_fmt != 1) {
     tc_set_error("gemm2: LayerNorm-fed GEMMs use fp16 operands");
@@ -819,7 +870,11 @@ int launch_gemm2(TmaCtx* ctx, const G2Desc& d, int num_sms, cudaStream_t st) {
     return -1;
   }
   p.swap_mask = d.swap_mask;
-  if (d.swap_mask) {
+  if (p.has_cms && (d.K != 128 || p.YT < 64 || !d.cm_out[0] || d.bias_lo != 0 || d.Nw > G2Smem<128>::BIAS_FLOATS)) {
+    tc_set_error("gemm2: operand-swapped gated groups need K = 128, YT >= 64, cm_out and the whole bias in the table");
+    return -1;
+  }
+  if (d.swap_mask && !p.has_cms) {
     if (!d.vt_out || p.YT < 64) {
       tc_set_error("gemm2: operand-swapped transposed outputs need vt_out and a tile of at least 64 consecutive y");
       return -1;
@@ -843,7 +898,8 @@ int launch_gemm2(TmaCtx* ctx, const G2Desc& d, int num_sms, cudaStream_t st) {
     uint64_t dims[4] = {D2, D1, ch, Bn};
     uint64_t str[3] = {Lp * 2, D1 * Lp * 2, ch * D1 * Lp * 2};
     uint32_t box[4] = {YTW, XTW, 64, 1};
-    if (tma_encode(ctx, &tmT[i], d.cm_out[i], 0, 4, dims, str, box, 0) != 0) return -1;
+    uint32_t box_s[4] = {64, 1, 32, 1};   // operand-swapped groups: 128-byte rows of 64 y per channel, 128B swizzle
+    if (tma_encode(ctx, &tmT[i], d.cm_out[i], 0, 4, dims, str, p.has_cms ? box_s : box, p.has_cms ? 128 : 0) != 0) return -1;
   }
   if (d.heads_out) {   // [(b, head), x, y] with row pitch Lpad
     uint64_t nh = d.n_heads;

@@ -322,7 +322,13 @@ struct TcDriver {
       d.row_out[0] = G; d.row_ld[0] = c.c_z;
       for (int tile = 0; tile < 2; ++tile)
         for (int j = 0; j < 4; ++j) {
-          d.ops[tile * 4 + j] = j < 2 ? op(G2_CM_DUAL, j * 64) : op(G2_SKIP, 0);
+          if (g2_pick_yt(N) >= 64) {
+            // both halves (p | gate) of the window are computed operand-swapped: the gated operand leaves the MMA channel-major
+            d.ops[tile * 4 + j] = j < 2 ? op(G2_CMS, 0) : op(G2_SKIP, 0);
+            d.swap_mask |= 3u << (2 * tile);
+          } else {
+            d.ops[tile * 4 + j] = j < 2 ? op(G2_CM_DUAL, j * 64) : op(G2_SKIP, 0);
+          }
           d.ops[tile * 4 + j].map = tile;
         }
       for (int j = 0; j < 2; ++j) {
