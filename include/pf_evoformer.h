@@ -75,7 +75,12 @@ pf_status pf_evoformer_create(pf_evoformer_t** out, const float* weights_host, s
  * Sub-step order inside a block: 1 row attention with pair bias (A.1), 2 column attention
  * (A.2), 3 MSA transition (A.3), 4 outer-product-mean (A.4, reads the updated msa), 5/6 triangle
  * multiplication outgoing/incoming (A.5/A.6), 7/8 triangle attention starting/ending node (A.7/A.8),
- * 9 pair transition (A.9). */
+ * 9 pair transition (A.9).
+ * Limits (PF_ERR_SHAPE / PF_ERR_CUDA with a message otherwise): B*S <= 65535 and B*N <= 65535; on the PF_BF16 path also
+ * N <= 1024 and S <= 1024 (keys per attention row) and S <= 512 (outer-product-mean contraction length).
+ * Masked work: on the PF_BF16 path 128-row tiles, attention rows and key tiles whose outputs all lie at masked positions are
+ * skipped (outputs there are unspecified but finite, as stated above); unmasked outputs do not depend on what the masked
+ * positions of msa / pair contain. */
 pf_status pf_evoformer_forward(pf_evoformer_t* h, float* msa_dev, float* pair_dev,
                                const float* seq_mask_dev, const float* msa_mask_dev,
                                int B, int S, int N, int n_blocks, void* cuda_stream);
