@@ -53,9 +53,12 @@ def test_block(ragged):
     _check(m, z, mr, zr, sm, mm, "block")
 
 
-@pytest.mark.parametrize("B,S,N", [(1, 1, 9), (3, 17, 50), (1, 3, 129), (2, 130, 33)])
+@pytest.mark.parametrize("B,S,N", [(1, 1, 9), (3, 17, 50), (1, 3, 129), (2, 130, 33),
+                                   (2, 20, 64), (1, 40, 96), (2, 9, 48), (1, 64, 256)])
 def test_runtime_shapes(B, S, N):
-    """One binary, many shapes (H11): sizes that are not multiples of any tile, S=1, keys spanning two key tiles."""
+    """One binary, many shapes (H11): sizes that are not multiples of any tile, S=1, keys spanning two key tiles, and row
+    tiles of every height (N = 64 / 96 / 48 / 256 -> 64 / 32 / 16 / 128 consecutive y per tile: the operand-swapped, TMA-staged
+    and fallback store paths of the projection GEMM)."""
     blocks = ps.make_weights(8, 1, bf16_weights=True)
     lengths = ps.rng(B * 1000 + N, 7).integers(max(1, N // 2), N + 1, size=B)
     msa, pair, sm, mm = ps.make_inputs(9, B, S, N, lengths=lengths, msa_mask_frac_max=0.4)
