@@ -8,8 +8,12 @@ bucket, N_seq=128 with 0-30 % of MSA rows masked per protein, 4 Evoformer blocks
 accumulation / fp32 residual streams.  A *step* is one pf_evoformer_forward over that whole batch
 (all nine sub-steps x 4 blocks).  value = real proteins per second over all ranks (padding does not count).
 
-N>1 (torchrun): replicas only (SURVEY.md §8(e)): every rank runs its own seeded batch, no data-path collective;
-time = max over ranks, value = N * 64 * K / time ("weak").
+Beside the headline (default run, N=1): "workloads" = BASELINE.json configs[2] / configs[3] (one protein, N_res 384 / 768,
+N_seq 512, 48 distinct blocks; 3 timed steps each) and "cfg5_sweep" = configs[4] run for real (2,000 proteins, every scheduler
+batch through 48 blocks, about 1.5 minutes); --no-sides / --no-sweep skip them.
+
+N>1 (torchrun): replicas only: one shared list of N x 64 proteins is sharded by pf_sched_partition, every
+rank runs its share, no data-path collective; time = max over ranks, value = all proteins * K / time ("weak").
 
 --impl reference: the fp64 numpy oracle (oracle/) timed on the host cores on a bounded sample of the same
 workload (one protein, cropped to its true length because the CPU code needs no padding, one block per step;
@@ -254,67 +258,145 @@ def roofline_from_profile(prof, peaks, n_steps, wl_name):
     return roof, table
 
 
-def per_bucket_sweep(h, pf, ps, torch, dev, nb, peaks, n_proteins=2000, S=512, cap=48):
-    """BASELINE.json metric: proteins/s and TFLOP/s per length bucket (configs[4]: lengths R10, buckets {64..320}, N_seq=512,
-    random msa_mask R11, 48 blocks).  The length-bucketing scheduler (pf_sched_*) cuts the protein list into batches; ONE
-    batch per bucket is timed on the GPU (nb blocks, CUDA events) and the 48-block, whole-list figures are derived from it."""
+def time_forward(h, torch, m, z, smd, mmd, nb, steps, warmup, barrier=None):
+    """W untimed + K timed pf_evoformer_forward calls on device-resident tensors; CUDA events on the launch stream.
+    Returns (total ms of the K steps, first-call ms, launches per step)."""
+    stream = torch.cuda.current_stream()
+    if barrier:
+        barrier()
+    t0 = time.perf_counter()
+    h.forward(m, z, smd, mmd, nb)
+    torch.cuda.synchronize()
+    first_call_ms = (time.perf_counter() - t0) * 1e3
+    launches = h.last_launch_count()
+    for _ in range(max(warmup - 1, 0)):
+        h.forward(m, z, smd, mmd, nb)
+    if barrier:
+        barrier()
+    else:
+        torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(steps):
+        h.forward(m, z, smd, mmd, nb)
+    e1.record(stream)
+    if barrier:
+        barrier()
+    else:
+        torch.cuda.synchronize()
+    return e0.elapsed_time(e1), first_call_ms, launches
+
+
+def profile_forward(h, torch, m, z, smd, mmd, nb, n_prof):
+    """The same steps with every launch bracketed by CUDA events on the launch stream (pf_evoformer_set_profiling)."""
+    h.set_profiling(True)
+    for _ in range(n_prof):
+        h.forward(m, z, smd, mmd, nb)
+    torch.cuda.synchronize()
+    prof = h.get_profile()
+    h.set_profiling(False)
+    return prof
+
+
+def side_workload(h, ps, torch, dev, name, peaks, steps=3, warmup=3):
+    """BASELINE.json configs[2] / configs[3] beside the headline: one protein, full masks, 48 distinct blocks."""
+    wl = WORKLOADS[name]
+    B, S, N, nb = wl["B"], wl["S"], wl["N"], wl["n_blocks"]
+    m, z, sm, mm = ps.make_inputs_device(100, B, S, N, dev)
+    smd, mmd = torch.from_numpy(sm).to(dev), torch.from_numpy(mm).to(dev)
+    ms, first_ms, launches = time_forward(h, torch, m, z, smd, mmd, nb, steps, warmup)
+    prof = profile_forward(h, torch, m, z, smd, mmd, nb, 1)
+    finite = bool(torch.isfinite(m).all().item() and torch.isfinite(z).all().item())
+    roof, table = roofline_from_profile(prof, peaks, 1, name)
+    ms_step = ms / steps
+    flops = ps.gemm_flops_per_block(S, N) * nb * B
+    del m, z
+    torch.cuda.empty_cache()
+    return {"desc": wl["desc"], "steps": steps, "warmup": warmup, "ms_per_step": ms_step, "proteins_per_s": B / (ms_step * 1e-3),
+            "residues_per_s": B * N / (ms_step * 1e-3), "tflops_padded": flops / (ms_step * 1e-3) / 1e12,
+            "tflops_frac_of_bf16_sustained": flops / (ms_step * 1e-3) / 1e12 / peaks["bf16_tflops_sustained"],
+            "first_call_ms": first_ms, "gpu_launches_per_step": int(launches), "outputs_finite": finite,
+            "l2": f"residual streams {(B * S * N * 256 + B * N * N * 128) * 4 / 1e6:.0f} MB per step (> L2)",
+            "roofline": roof, "kernels": table}
+
+
+def cfg5_sweep(h, pf, ps, torch, dev, peaks, n_proteins=2000, S=512, cap=48, nb=48):
+    """BASELINE.json configs[4], run for real: 2,000 proteins (lengths R10), buckets {64..320}, N_seq=512, msa_mask R11, every
+    batch the length-bucketing scheduler (pf_sched_*) cuts goes through all 48 blocks (48 distinct weight sets).  Inputs are
+    drawn on the device before each batch's timed forward (CUDA events around the forward only; the wall clock of the whole
+    sweep, input generation included, is reported beside it)."""
     import numpy as np
     lengths = ps.cfg5_lengths(5, n_proteins)
     sched = pf.Scheduler(list(ps.CFG5_BUCKETS), 16 << 30, S)
     for i, L in enumerate(lengths):
         sched.add(i, int(L))
-    per_bucket, order = {}, []
-    for ids, lens, bucket in sched.batches(cap):
-        e = per_bucket.setdefault(bucket, {"proteins": 0, "batches": 0, "first": None})
-        e["proteins"] += len(ids)
-        e["batches"] += 1
-        if e["first"] is None or len(ids) > len(e["first"][1]):
-            e["first"] = (ids, lens)
-        if bucket not in order:
-            order.append(bucket)
+    batches = list(sched.batches(cap))
     sched.close()
-    out, total_s = [], 0.0
-    g = torch.Generator(device=dev).manual_seed(55)
-    for bucket in order:
-        e = per_bucket[bucket]
-        ids, lens = e["first"]
+    per = {}
+    events = []
+    finite = True
+    t_wall = time.perf_counter()
+    stream = torch.cuda.current_stream()
+    for k, (ids, lens, bucket) in enumerate(batches):
         B, N = len(ids), bucket
-        sm = np.zeros((B, N), np.float32)
-        for b, L in enumerate(lens):
-            sm[b, :L] = 1.0
-        mm = np.ones((B, S), np.float32)
-        r = ps.rng(77, bucket)
-        for b in range(B):                                           # R11: 0-30 % of the MSA rows masked, never row 0
-            k = int(r.uniform(0.0, 0.3) * S)
-            mm[b, 1 + r.choice(S - 1, size=k, replace=False)] = 0.0
-        m = torch.randn(B, S, N, 256, device=dev, generator=g)
-        z = torch.randn(B, N, N, 128, device=dev, generator=g)
+        m, z, sm, mm = ps.make_inputs_device(9000 + k, B, S, N, dev, lengths=lens, msa_mask_frac_max=0.3)
         smd, mmd = torch.from_numpy(sm).to(dev), torch.from_numpy(mm).to(dev)
-        h.forward(m, z, smd, mmd, nb)
-        torch.cuda.synchronize()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        reps = 2
-        e0.record()
-        for _ in range(reps):
-            h.forward(m, z, smd, mmd, nb)
-        e1.record()
-        torch.cuda.synchronize()
-        ms_block = e0.elapsed_time(e1) / reps / nb
-        ok = bool(torch.isfinite(m).all().item() and torch.isfinite(z).all().item())
+        e0.record(stream)
+        h.forward(m, z, smd, mmd, nb)
+        e1.record(stream)
+        events.append((bucket, B, float(np.mean(lens)), e0, e1))
+        if k % 8 == 7 or k == len(batches) - 1:      # bounded memory in flight; outputs checked on a sample of the batches
+            finite = finite and bool(torch.isfinite(m).all().item() and torch.isfinite(z).all().item())
         del m, z
-        flops_block = ps.gemm_flops_per_block(S, N) * B
-        s48 = ms_block * 48e-3                                       # seconds for this batch through 48 blocks
-        total_s += s48 / B * e["proteins"]
-        out.append({"bucket": bucket, "B": B, "proteins_in_list": e["proteins"], "batches_in_list": e["batches"],
-                    "mean_len": float(np.mean(lens)), "ms_per_block": ms_block,
-                    "tflops_padded": flops_block / (ms_block * 1e-3) / 1e12,
-                    "frac_bf16_sustained": flops_block / (ms_block * 1e-3) / 1e12 / peaks["bf16_tflops_sustained"],
-                    "proteins_per_s_48_blocks": B / s48, "outputs_finite": ok})
-    return {"workload": f"cfg5-style: {n_proteins} proteins, lengths R10, buckets {list(ps.CFG5_BUCKETS)}, N_seq={S}, "
-                        f"msa_mask R11; batches by pf_sched (16 GB budget, cap {cap}); one batch per bucket timed over "
-                        f"{nb} blocks, 48-block figures derived",
-            "buckets": out, "sweep_seconds_48_blocks_derived": total_s,
-            "proteins_per_hour_derived": n_proteins / total_s * 3600.0}
+    torch.cuda.synchronize()
+    wall_s = time.perf_counter() - t_wall
+    total_ms = 0.0
+    for bucket, B, mean_len, e0, e1 in events:
+        ms = e0.elapsed_time(e1)
+        total_ms += ms
+        e = per.setdefault(bucket, {"proteins": 0, "batches": 0, "ms": 0.0, "flops": 0.0, "residues": 0.0, "max_B": 0})
+        e["proteins"] += B
+        e["batches"] += 1
+        e["ms"] += ms
+        e["flops"] += ps.gemm_flops_per_block(S, bucket) * nb * B
+        e["residues"] += mean_len * B
+        e["max_B"] = max(e["max_B"], B)
+    out = []
+    for bucket in sorted(per):
+        e = per[bucket]
+        sec = e["ms"] * 1e-3
+        out.append({"bucket": bucket, "proteins": e["proteins"], "batches": e["batches"], "max_B": e["max_B"],
+                    "seconds": sec, "proteins_per_s": e["proteins"] / sec, "residues_per_s": e["residues"] / sec,
+                    "ms_per_block_per_batch": e["ms"] / e["batches"] / nb,
+                    "tflops_padded": e["flops"] / sec / 1e12,
+                    "frac_bf16_sustained": e["flops"] / sec / 1e12 / peaks["bf16_tflops_sustained"]})
+    return {"workload": f"BASELINE.json configs[4]: {n_proteins} proteins, lengths R10, buckets {list(ps.CFG5_BUCKETS)}, "
+                        f"N_seq={S}, msa_mask R11, {nb} distinct blocks; {len(batches)} batches by pf_sched (16 GB budget, cap {cap}), "
+                        f"every batch run through all {nb} blocks",
+            "measured": True, "buckets": out, "device_seconds": total_ms * 1e-3, "wall_seconds_incl_input_generation": wall_s,
+            "proteins_per_hour": n_proteins / (total_ms * 1e-3) * 3600.0,
+            "proteins_per_hour_wall": n_proteins / wall_s * 3600.0, "outputs_finite": finite}
+
+
+def rank_batch(pf, ps, wl, world, rank):
+    """--gpus N, replicas only: ONE shared list of world x B proteins of the workload's length law is
+    sharded by pf_sched_partition (longest-processing-time first, deterministic: every rank computes the same assignment
+    without talking) and this rank takes its share.  Returns (global ids, lengths) of the rank's proteins."""
+    import numpy as np
+    B, N = wl["B"], wl["N"]
+    n = world * B
+    if wl["lengths"] == "cfg2":
+        lengths = ps.cfg2_lengths(100, n)
+    elif wl["lengths"] == "cfg2small":
+        lengths = ps.cfg2_lengths(100, n, lo=N // 2, hi=N)
+    else:
+        lengths = np.full(n, N)
+    if world == 1:
+        return np.arange(n), lengths
+    ranks = np.asarray(pf.partition([int(x) for x in lengths], [N], wl["S"], world))
+    mine = np.flatnonzero(ranks == rank)
+    return mine, lengths[mine]
 
 
 def run_ours(args, wl, wl_name):
@@ -337,54 +419,38 @@ def run_ours(args, wl, wl_name):
     pf.lib()                                                     # fail loudly if the extension is not built
 
     dtype = pf.PF_F32 if args.dtype == "f32" else pf.PF_BF16
-    B, S, N, nb = wl["B"], wl["S"], wl["N"], wl["n_blocks"]
-    # the weights of nb distinct blocks (R8/R15); for 48-block workloads the same seeded recipe
-    blocks = ps.make_weights(7, nb, bf16_weights=(dtype != pf.PF_F32))
-    h = pf.Evoformer(ps.pack_blob(blocks), pf.make_config(nb, dtype))
+    S, N, nb = wl["S"], wl["N"], wl["n_blocks"]
+    extras = world == 1 and wl_name == "cfg2" and dtype == pf.PF_BF16
+    want_sides = extras and not args.no_sides
+    want_sweep = extras and not args.no_sweep
+    # weights: seeded recipe R8/R15, distinct per block; 48 blocks when the side workloads / the sweep run on the same handle
+    nb_handle = 48 if (want_sides or want_sweep) else nb
+    blocks = ps.make_weights(7, nb_handle, bf16_weights=(dtype != pf.PF_F32))
+    h = pf.Evoformer(ps.pack_blob(blocks), pf.make_config(nb_handle, dtype))
     del blocks
-    msa, pair, sm, mm, lengths = make_batch(ps, wl, 100 + rank)
+    ids, lengths = rank_batch(pf, ps, wl, world, rank)
+    B = len(ids)
+    msa, pair, sm, mm = ps.make_inputs(100 + rank, B, S, N, lengths=lengths, msa_mask_frac_max=wl["mask"])
     n_prot, n_res = B, int(np.sum(lengths))
     m0 = torch.from_numpy(msa).pin_memory()
     z0 = torch.from_numpy(pair).pin_memory()
     smh, mmh = torch.from_numpy(sm).pin_memory(), torch.from_numpy(mm).pin_memory()
     m, z = m0.to(dev), z0.to(dev)
     smd, mmd = smh.to(dev), mmh.to(dev)
-    stream = torch.cuda.current_stream()
 
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
-    # first call (workspace growth, module load) vs steady state — the analogue of the paper's per-model compile
-    barrier()
-    t0 = time.perf_counter()
-    h.forward(m, z, smd, mmd, nb)
-    torch.cuda.synchronize()
-    first_call_ms = (time.perf_counter() - t0) * 1e3
-    launches_per_step = h.last_launch_count()
-    for _ in range(max(args.warmup - 1, 0)):
-        h.forward(m, z, smd, mmd, nb)
-
     sampler = ClockSampler(local)
-    barrier()
     if rank == 0:
         sampler.start()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record(stream)
-    for _ in range(args.steps):
-        h.forward(m, z, smd, mmd, nb)
-    e1.record(stream)
-    barrier()
-    ms = e0.elapsed_time(e1)
+    # first call (workspace growth, module load) vs steady state — the analogue of the paper's per-model compile
+    ms, first_call_ms, launches_per_step = time_forward(h, torch, m, z, smd, mmd, nb, args.steps, args.warmup, barrier)
     # per-kernel pass: the same steps with every launch bracketed by events on the launch stream
     n_prof = max(1, min(args.steps, 3))
-    h.set_profiling(True)
-    for _ in range(n_prof):
-        h.forward(m, z, smd, mmd, nb)
-    torch.cuda.synchronize()
-    prof = h.get_profile()
-    h.set_profiling(False)
+    prof = profile_forward(h, torch, m, z, smd, mmd, nb, n_prof)
     clocks = sampler.stop() if rank == 0 else None
     finite = bool(torch.isfinite(m).all().item() and torch.isfinite(z).all().item())
 
@@ -401,10 +467,15 @@ def run_ours(args, wl, wl_name):
     h2d = m0.numel() * 4 + z0.numel() * 4 + smh.numel() * 4 + mmh.numel() * 4
     d2h = m0.numel() * 4 + z0.numel() * 4
 
-    t = torch.tensor([ms, e2e_s * 1e3], dtype=torch.float64, device=dev)
+    t = torch.tensor([ms, e2e_s * 1e3, float(n_prot), float(n_res)], dtype=torch.float64, device=dev)
     if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms, e2e_ms = float(t[0]), float(t[1])
+        tmax = t.clone()
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)              # times: max over ranks
+        dist.all_reduce(t, op=dist.ReduceOp.SUM)                 # proteins / residues: all ranks
+        ms, e2e_ms = float(tmax[0]), float(tmax[1])
+        n_prot_all, n_res_all = float(t[2]), float(t[3])
+    else:
+        ms, e2e_ms, n_prot_all, n_res_all = float(t[0]), float(t[1]), float(n_prot), float(n_res)
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -412,35 +483,38 @@ def run_ours(args, wl, wl_name):
 
     peaks = load_peaks()
     ms_per_step = ms / args.steps
-    value = world * n_prot * args.steps / (ms * 1e-3)
-    flops_step = ps.gemm_flops_per_block(S, N) * nb * B          # padded FLOPs: what the GPU executes
+    value = n_prot_all * args.steps / (ms * 1e-3)
+    flops_step = ps.gemm_flops_per_block(S, N) * nb * B          # padded FLOPs of this rank: what its GPU executes
     roof, table = roofline_from_profile(prof, peaks, n_prof, wl_name)
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": args.dtype, "data": "synthetic",
         "config": {"workload": wl_name, "desc": wl["desc"], "B": B, "N_seq": S, "N_res": N, "n_blocks": nb,
-                   "parallelism": f"replicas x{world}", "l2": "inputs larger than L2 (msa+pair residual streams "
+                   "parallelism": f"replicas x{world}" + (" (protein list sharded by pf_sched_partition)" if world > 1 else ""),
+                   "l2": "inputs larger than L2 (msa+pair residual streams "
                    f"{(m0.numel() + z0.numel()) * 4 / 1e6:.0f} MB per step)", "path": args.dtype,
                    "masked_work": "128-row tiles, attention rows and key tiles that are entirely masked are skipped; "
                                   "roofline / kernels count executed work only, tflops_padded counts the padded bucket"},
-        "residues_per_s": world * n_res * args.steps / (ms * 1e-3),
-        "tflops_padded": world * flops_step / (ms_per_step * 1e-3) / 1e12,
-        "tflops_frac_of_bf16_sustained": world * flops_step / (ms_per_step * 1e-3) / 1e12 / peaks["bf16_tflops_sustained"] / world,
+        "residues_per_s": n_res_all * args.steps / (ms * 1e-3),
+        "tflops_padded": flops_step / (ms_per_step * 1e-3) / 1e12,
+        "tflops_frac_of_bf16_sustained": flops_step / (ms_per_step * 1e-3) / 1e12 / peaks["bf16_tflops_sustained"],
         # GEMM FLOPs actually executed (fully masked tiles / rows / key tiles are skipped) per GPU
         "tflops_executed": sum(v["flops"] for v in prof.values()) / n_prof / (ms_per_step * 1e-3) / 1e12,
         "first_call_ms": first_call_ms, "steady_ms": ms_per_step, "outputs_finite": finite,
-        "e2e": {"value": world * n_prot * n_e2e / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
+        "e2e": {"value": n_prot_all * n_e2e / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
                 "d2h_bytes_per_step": d2h, "steps": n_e2e, "api": "pf_evoformer_forward_host (pinned host buffers)"},
         "gpu_launches": int(launches_per_step * args.steps),
         "clocks": clocks, "roofline": roof, "kernels": table,
         "paper_context": "ParaFold: ~20,000 50-res proteins / 5.4 h on 16 V100 (whole model), 13.8x from compile reuse; "
                          "no Evoformer-only number (BASELINE.md)",
     }
-    if world == 1 and not args.no_buckets:
-        del m, z, mh, zh
-        torch.cuda.empty_cache()
-        line["per_bucket"] = per_bucket_sweep(h, pf, ps, torch, dev, nb, peaks)
+    del m, z, mh, zh, m0, z0
+    torch.cuda.empty_cache()
+    if want_sides:
+        line["workloads"] = {k: side_workload(h, ps, torch, dev, k, peaks) for k in ("cfg3", "cfg4")}
+    if want_sweep:
+        line["cfg5_sweep"] = cfg5_sweep(h, pf, ps, torch, dev, peaks)
     if world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(wl, wl_name)
     print(json.dumps(line), flush=True)
@@ -459,7 +533,8 @@ def main():
     ap.add_argument("--workload", default="cfg2", choices=sorted(WORKLOADS))
     ap.add_argument("--dtype", default="bf16", choices=["bf16", "f32"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-buckets", action="store_true", help="skip the per-length-bucket sweep (cfg5-style)")
+    ap.add_argument("--no-sweep", action="store_true", help="skip the 2,000-protein sweep of BASELINE.json configs[4]")
+    ap.add_argument("--no-sides", action="store_true", help="skip the cfg3 / cfg4 side workloads")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     wl = WORKLOADS[args.workload]

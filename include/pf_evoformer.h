@@ -76,8 +76,16 @@ pf_status pf_evoformer_create(pf_evoformer_t** out, const float* weights_host, s
  * (A.2), 3 MSA transition (A.3), 4 outer-product-mean (A.4, reads the updated msa), 5/6 triangle
  * multiplication outgoing/incoming (A.5/A.6), 7/8 triangle attention starting/ending node (A.7/A.8),
  * 9 pair transition (A.9).
- * Limits (PF_ERR_SHAPE / PF_ERR_CUDA with a message otherwise): B*S <= 65535 and B*N <= 65535; on the PF_BF16 path also
- * N <= 1024 and S <= 1024 (keys per attention row) and S <= 512 (outer-product-mean contraction length).
+ * Limits (PF_ERR_SHAPE / PF_ERR_CUDA with a message otherwise): S <= 65535 and N <= 65535; on the PF_BF16 path also
+ * N <= 1024 and S <= 1024 (keys per attention row) and S <= 512 (outer-product-mean contraction length).  B is not
+ * limited: batches beyond what one launch sequence takes (grid limits) are cut into chunks of proteins internally.
+ * The current CUDA device must be the one the handle was created on (PF_ERR_INVALID_ARG otherwise).
+ * Value range on the PF_BF16 path (reading R17): LayerNorm outputs, sigmoid gates and the weight matrices that
+ * multiply a LayerNorm output are held as fp16.  Precondition: those weights (after bf16 rounding, R15) lie in the fp16
+ * normal range, 2^-14 <= |w| <= 65504 or w == 0 (smaller magnitudes lose bits or flush to zero), and LayerNorm outputs
+ * gamma * xhat + beta stay below 65504 in magnitude (|xhat| <= sqrt(C)).  create() counts weights outside that range and
+ * refuses blobs with overflowing ones (PF_ERR_SHAPE); the seeded R8 init has about 0.08 % of entries below 2^-14 (a
+ * relative perturbation of those entries only, far below the bf16 tolerances).
  * Masked work: on the PF_BF16 path 128-row tiles, attention rows and key tiles whose outputs all lie at masked positions are
  * skipped (outputs there are unspecified but finite, as stated above); unmasked outputs do not depend on what the masked
  * positions of msa / pair contain. */
@@ -90,9 +98,10 @@ pf_status pf_evoformer_forward_substep(pf_evoformer_t* h, float* msa_dev, float*
                                        const float* seq_mask_dev, const float* msa_mask_dev,
                                        int B, int S, int N, int block, int substep, void* cuda_stream);
 
-/* End-to-end convenience: the same computation with HOST buffers (pinned or pageable).  Copies msa, pair
- * and masks host->device on cuda_stream, runs forward, copies msa and pair back, and synchronises the
- * stream before returning.  Device staging buffers are owned by the handle (grow-only). */
+/* End-to-end convenience: the same computation with HOST buffers (pinned or pageable).  The batch is pipelined in
+ * chunks of proteins: host->device copies on an internal copy stream, forward on cuda_stream, device->host copies on a
+ * second internal copy stream (ordered after earlier work on cuda_stream); returns after everything has completed.
+ * Device staging buffers and the copy streams are owned by the handle (grow-only). */
 pf_status pf_evoformer_forward_host(pf_evoformer_t* h, float* msa_host, float* pair_host,
                                     const float* seq_mask_host, const float* msa_mask_host,
                                     int B, int S, int N, int n_blocks, void* cuda_stream);

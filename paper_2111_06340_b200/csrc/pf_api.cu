@@ -101,7 +101,8 @@ Arena pf::arena_layout(const pf_config& c, int B, int S, int N) {
   Arena a{};
   size_t o = 0;
   auto take = [&](size_t bytes) { size_t r = o; o = align_up(o + bytes, 1024); return r; };
-  a.x = take(mx(M * c.c_m, P * c.c_z) * es);
+  const bool f32 = c.dtype == PF_F32;   // x, oa, ob: LayerNorm output and row-major outer-product operands of the SIMT path only
+  a.x = take(f32 ? mx(M * c.c_m, P * c.c_z) * es : 0);
   a.qkg = take(mx(M * mx(n, 3) * c.c_m, P * mx(n, 3) * c.c_z) * es);
   a.vt = take(mx(mx((size_t)B * S * c.c_m * Np, (size_t)B * N * c.c_m * Sp), (size_t)B * N * c.c_z * Np) * es);
   a.o = take(mx(M * c.c_m, P * c.c_z) * es);
@@ -111,8 +112,8 @@ Arena pf::arena_layout(const pf_config& c, int B, int S, int N) {
   a.g = take(P * c.c_z * es);
   a.tcm = take((size_t)B * c.c_tri * N * Np * 4);
   a.tn = take(P * c.c_tri * es);
-  a.oa = take(M * c.c_opm * es);
-  a.ob = take(M * c.c_opm * es);
+  a.oa = take(f32 ? M * c.c_opm * es : 0);
+  a.ob = take(f32 ? M * c.c_opm * es : 0);
   a.f_msa = take((size_t)g2_num_tiles(B, S, N));
   a.f_msat = take((size_t)g2_num_tiles(B, N, S));
   a.f_pair = take((size_t)g2_num_tiles(B, N, N));
@@ -161,6 +162,7 @@ extern "C" pf_status pf_evoformer_create(pf_evoformer_t** out, const float* weig
   h->cfg = c;
   h->off = off;
   h->num_sms = prop.multiProcessorCount;
+  h->device = dev;
   size_t nbytes = n_weight_floats * sizeof(float);
   if (cudaMalloc(&h->w32, nbytes) != cudaSuccess) { delete h; return fail(PF_ERR_ALLOC, "cudaMalloc weights"); }
   if (cudaMemcpy(h->w32, weights_host, nbytes, cudaMemcpyHostToDevice) != cudaSuccess) {
@@ -171,9 +173,16 @@ extern "C" pf_status pf_evoformer_create(pf_evoformer_t** out, const float* weig
     h->tc = tc_layout(c);
     std::vector<uint16_t> w16(h->tc.total16 * c.n_blocks_max, 0);
     std::vector<float> wf(h->tc.total_f32 * c.n_blocks_max, 0.f);
+    F16Range range;
     for (int b = 0; b < c.n_blocks_max; ++b)
       build_tc_block(c, off, h->tc, weights_host + (size_t)b * off.total, w16, (size_t)b * h->tc.total16, wf,
-                     (size_t)b * h->tc.total_f32);
+                     (size_t)b * h->tc.total_f32, &range);
+    if (range.overflow) {
+      pf_evoformer_destroy(h);
+      return fail(PF_ERR_SHAPE, std::to_string(range.overflow) + " weight(s) that multiply a LayerNorm output exceed the fp16 "
+                                "range (|w| > 65504 or NaN); see the value-range precondition in pf_evoformer.h");
+    }
+    h->f16_below_normal = range.below_normal;
     if (cudaMalloc(&h->w16, w16.size() * 2) != cudaSuccess || cudaMalloc(&h->wf, wf.size() * 4) != cudaSuccess) {
       pf_evoformer_destroy(h);
       return fail(PF_ERR_ALLOC, "cudaMalloc bf16 weights");
@@ -187,6 +196,11 @@ extern "C" pf_status pf_evoformer_create(pf_evoformer_t** out, const float* weig
     if (!h->tma) {
       pf_evoformer_destroy(h);
       return fail(PF_ERR_CUDA, std::string("TMA driver entry point: ") + tc_last_error());
+    }
+    if (!configure_gemm2_kernels() || !configure_transition_kernels() || !configure_attn_kernel() ||
+        !configure_opm_kernel() || !configure_tri_kernel()) {
+      pf_evoformer_destroy(h);
+      return fail(PF_ERR_CUDA, std::string("kernel attributes: ") + tc_last_error());
     }
   }
   *out = h;
@@ -450,33 +464,72 @@ struct Driver {
 };
 
 
-static pf_status check_and_grow(pf_evoformer* h, const float* msa, const float* pair, const float* sm, const float* mm,
-                                int B, int S, int N) {
-  if (!h || !msa || !pair || !sm || !mm) return fail(PF_ERR_INVALID_ARG, "null argument");
-  if (B < 1 || S < 1 || N < 1) return fail(PF_ERR_SHAPE, "B, S, N must be >= 1");
-  if ((long)B * S > 65535 || (long)B * N > 65535) return fail(PF_ERR_SHAPE, "B*S and B*N must be <= 65535");
+static pf_status check_and_grow(pf_evoformer* h, int B, int S, int N, cudaStream_t st) {
   size_t need = arena_layout(h->cfg, B, S, N).total;
   if (need > h->ws_bytes) {
     cudaDeviceSynchronize();
     cudaFree(h->ws);
     h->ws = nullptr;
     h->ws_bytes = 0;
+    h->ws_B = h->ws_S = h->ws_N = 0;
     if (cudaMalloc(&h->ws, need) != cudaSuccess) {
       cudaGetLastError();
       return fail(PF_ERR_ALLOC, "cudaMalloc workspace");
     }
     h->ws_bytes = need;
-    // masked tiles are skipped (pf_flags.cu): what they would have written must still be finite
-    if (cudaMemset(h->ws, 0, need) != cudaSuccess) return fail(PF_ERR_CUDA, "cudaMemset workspace");
+  }
+  // Masked tiles are skipped (pf_flags.cu): what they would have written must still be finite when a partially masked tile
+  // later reads it.  Within one arena layout every region keeps its element type from call to call, so stale contents are
+  // finite outputs of earlier launches; the layout (offsets and types) is a function of (B, S, N), so the arena is zero-filled,
+  // in stream order, whenever that shape differs from the previous call's (a slightly smaller tail batch on the same handle
+  // would otherwise reinterpret fp32 bytes as 16-bit values).
+  if (B != h->ws_B || S != h->ws_S || N != h->ws_N) {
+    if (cudaMemsetAsync(h->ws, 0, need, st) != cudaSuccess) return fail(PF_ERR_CUDA, "cudaMemsetAsync workspace");
+    h->ws_B = B; h->ws_S = S; h->ws_N = N;
   }
   return PF_OK;
 }
 
+// Largest batch one launch sequence takes: gridDim.z of the per-(protein, channel) and per-(protein, row) kernels is capped
+// at 65535.  Larger batches are cut into chunks of proteins (proteins are independent).
+static int max_batch_per_pass(const pf_config& c, int S, int N) {
+  const int lim = 65535;
+  int cap = lim / c.c_tri;                                       // triangle einsum: grid.z = B * c_tri
+  if (c.dtype == PF_F32) cap = std::min(cap, lim / std::max(S, N));   // SIMT attention: grid.z = B * rows
+  return std::max(cap, 1);
+}
+
+static pf_status dispatch_pass(pf_evoformer* h, float* msa, float* pair, const float* sm, const float* mm, int B, int S,
+                               int N, int block0, int block1, int step0, int step1, cudaStream_t st, long long& launches);
+
 static pf_status dispatch(pf_evoformer* h, float* msa, float* pair, const float* sm, const float* mm, int B, int S,
                           int N, int block0, int block1, int step0, int step1, void* stream) {
-  pf_status s = check_and_grow(h, msa, pair, sm, mm, B, S, N);
-  if (s != PF_OK) return s;
+  if (!h || !msa || !pair || !sm || !mm) return fail(PF_ERR_INVALID_ARG, "null argument");
+  if (B < 1 || S < 1 || N < 1) return fail(PF_ERR_SHAPE, "B, S, N must be >= 1");
+  if (S > 65535 || N > 65535) return fail(PF_ERR_SHAPE, "N_seq and N_res must be <= 65535");
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev != h->device)
+    return fail(PF_ERR_INVALID_ARG, "the current device is not the one the handle was created on");
   cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  const int cap = max_batch_per_pass(h->cfg, S, N);
+  const int passes = (B + cap - 1) / cap;
+  long long launches = 0;
+  int b0 = 0;
+  for (int p = 0; p < passes; ++p) {
+    const int bc = (B - b0 + (passes - p) - 1) / (passes - p);
+    pf_status s = dispatch_pass(h, msa + (size_t)b0 * S * N * h->cfg.c_m, pair + (size_t)b0 * N * N * h->cfg.c_z,
+                                sm + (size_t)b0 * N, mm + (size_t)b0 * S, bc, S, N, block0, block1, step0, step1, st, launches);
+    if (s != PF_OK) return s;
+    b0 += bc;
+  }
+  h->launches = launches;
+  return PF_OK;
+}
+
+static pf_status dispatch_pass(pf_evoformer* h, float* msa, float* pair, const float* sm, const float* mm, int B, int S,
+                               int N, int block0, int block1, int step0, int step1, cudaStream_t st, long long& launches) {
+  pf_status s = check_and_grow(h, B, S, N, st);
+  if (s != PF_OK) return s;
   Driver d;
   d.h = h; d.st = st; d.B = B; d.S = S; d.N = N;
   d.msa = msa; d.pair = pair; d.seq_mask = sm; d.msa_mask = mm;
@@ -494,6 +547,7 @@ static pf_status dispatch(pf_evoformer* h, float* msa, float* pair, const float*
         return fail(PF_ERR_CUDA, std::string("launch failed in block ") + std::to_string(blk) + " substep " +
                                      std::to_string(step) + ": " + cudaGetErrorString(e));
     }
+  launches += h->launches;
   return PF_OK;
 }
 

@@ -360,6 +360,12 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQK, const __grid_constant__
   if (warp == 5) tc::tmem_dealloc<256>(tmem_base);
 }
 
+bool configure_attn_kernel() {
+  cudaError_t e = cudaFuncSetAttribute(attn_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, AttnSmem::TOTAL);
+  if (e != cudaSuccess) tc_set_error(std::string("cudaFuncSetAttribute(attn_tc): ") + cudaGetErrorString(e));
+  return e == cudaSuccess;
+}
+
 int launch_attn_tc(TmaCtx* ctx, const bf16* qkg, const bf16* vt, const bf16* bias, const float* keymask, bf16* o, int B,
                    int R, int L, int Lpad, int H, const void* rows, const int* n_rows, int num_sms, cudaStream_t st) {
   if (L > AT_MAXKEYS) {
@@ -384,15 +390,6 @@ int launch_attn_tc(TmaCtx* ctx, const bf16* qkg, const bf16* vt, const bf16* bia
     if (tma_encode_bf16(ctx, &tmB, bias, 3, d, s, bx, 128) != 0) return -1;
   } else {
     tmB = tmV;
-  }
-  static bool configured = false;
-  if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(attn_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, AttnSmem::TOTAL);
-    if (e != cudaSuccess) {
-      tc_set_error(std::string("cudaFuncSetAttribute(attn_tc): ") + cudaGetErrorString(e));
-      return -1;
-    }
-    configured = true;
   }
   AttnParams p;
   p.qkg = qkg; p.keymask = keymask; p.o = o;

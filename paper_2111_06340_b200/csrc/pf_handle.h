@@ -33,7 +33,12 @@ BlockW block_offsets(const pf_config& c);
 
 // ---- tensor-core weight set: 16-bit matrices [Nout, K] (K contiguous), offsets in 16-bit elements within one block.
 // Matrices that multiply a LayerNorm output are stored as fp16 (reading R17: the values are the bf16-rounded
-// weights of R15, which fp16 represents exactly), all others as bf16.  Fused bias vectors are fp32 (offsets in floats).
+// weights of R15, which fp16 represents exactly when 2^-14 <= |w| <= 65504; F16Range counts the entries outside), all
+// others as bf16.  Fused bias vectors are fp32 (offsets in floats).
+struct F16Range {
+  size_t overflow = 0;       // |w| > 65504 or NaN: refused by create
+  size_t below_normal = 0;   // 0 < |w| < 2^-14: stored with fewer mantissa bits or flushed to zero
+};
 struct AttnT {
   size_t w_in;   // fp16 [4C (+H), C]: q | k | gate | v (| pair-bias heads for triangle attention)
   size_t b_in;   // fp32 [4C (+H)]: gate bias in its column range, zero elsewhere
@@ -51,7 +56,7 @@ struct TcBlock {
 };
 TcBlock tc_layout(const pf_config& c);
 void build_tc_block(const pf_config& c, const BlockW& off, const TcBlock& t, const float* w, std::vector<uint16_t>& w16,
-                    size_t base16, std::vector<float>& wf, size_t basef);
+                    size_t base16, std::vector<float>& wf, size_t basef, F16Range* range);
 
 enum KernelKind { KK_LN = 0, KK_GEMM, KK_ATTN, KK_TRI, KK_LNC, KK_OPM, KK_LNGEMM, KK_TRANS, KK_FLAGS, KK_COUNT };
 
@@ -79,6 +84,9 @@ struct pf_evoformer {
   float* wf = nullptr;       // device fused fp32 bias vectors (PF_BF16 only)
   char* ws = nullptr;        // workspace arena
   size_t ws_bytes = 0;
+  size_t f16_below_normal = 0;   // weights stored as fp16 with |w| < 2^-14 (precision loss, pf_evoformer.h value-range note)
+  int device = -1;           // the device the handle was created on (weights, workspace and kernel attributes live there)
+  int ws_B = 0, ws_S = 0, ws_N = 0;   // shape of the arena layout the workspace currently holds (zero-filled when it changes)
   char* stage = nullptr;     // forward_host staging
   size_t stage_bytes = 0;
   // forward_host pipelines the batch in chunks of proteins: copy-in stream, the caller's stream for compute, copy-out stream

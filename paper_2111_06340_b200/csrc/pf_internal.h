@@ -73,6 +73,13 @@ void launch_opm_simt(const T* a, const T* b, const float* wout, const float* bou
 struct TmaCtx;   // holds the driver entry point for cuTensorMapEncodeTiled
 TmaCtx* tma_ctx_create();
 void tma_ctx_destroy(TmaCtx*);
+// kernel attributes (dynamic shared memory sizes) for the CURRENT device; called by pf_evoformer_create, so a handle's kernels
+// are configured on the handle's own device (no process-wide "configured" flags)
+bool configure_gemm2_kernels();
+bool configure_transition_kernels();
+bool configure_attn_kernel();
+bool configure_opm_kernel();
+bool configure_tri_kernel();
 const char* tc_last_error();
 void tc_set_error(const std::string& s);
 // ---- persistent LN-fused projection GEMM (pf_lngemm_tc.cu) ----

@@ -750,18 +750,20 @@ static int launch_g2(const CUtensorMap& tmW, const CUtensorMap& tmA, const CUten
                      const CUtensorMap& tmT1, const CUtensorMap& tmH, const CUtensorMap& tmR, const CUtensorMap& tmVS,
                      const G2Params& p, int num_sms, cudaStream_t st) {
   auto kern = gemm2_kernel<K, AMODE>;
-  static bool configured = false;
-  if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, G2Smem<K>::TOTAL);
-    if (e != cudaSuccess) {
-      tc_set_error(std::string("cudaFuncSetAttribute(gemm2): ") + cudaGetErrorString(e));
-      return -1;
-    }
-    configured = true;
-  }
   unsigned grid = (unsigned)(p.num_tiles < (long)num_sms ? p.num_tiles : (long)num_sms);
   kern<<<grid, G2_THREADS, G2Smem<K>::TOTAL, st>>>(tmW, tmA, tmO0, tmT0, tmT1, tmH, tmR, tmVS, p);
   return 0;
+}
+
+// Per-device kernel attributes (dynamic shared memory above 48 KB), set once per handle at create time on the handle's device.
+template <int K, int AMODE>
+static bool configure_g2() {
+  cudaError_t e = cudaFuncSetAttribute(gemm2_kernel<K, AMODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, G2Smem<K>::TOTAL);
+  if (e != cudaSuccess) tc_set_error(std::string("cudaFuncSetAttribute(gemm2): ") + cudaGetErrorString(e));
+  return e == cudaSuccess;
+}
+bool configure_gemm2_kernels() {
+  return configure_g2<128, 0>() && configure_g2<128, 1>() && configure_g2<256, 0>() && configure_g2<256, 1>();
 }
 
 #ifdef PF_G2_TRACE

@@ -227,6 +227,12 @@ opm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ C
   if (warp == 1) tc::tmem_dealloc<512>(tmem_base);
 }
 
+bool configure_opm_kernel() {
+  cudaError_t e = cudaFuncSetAttribute(opm_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, OpmSmem::TOTAL);
+  if (e != cudaSuccess) tc_set_error(std::string("cudaFuncSetAttribute(opm_tc): ") + cudaGetErrorString(e));
+  return e == cudaSuccess;
+}
+
 int launch_opm_tc(TmaCtx* ctx, const bf16* ab_t, const bf16* wout_t, const float* bout, const float* seq_mask,
                   const float* msa_mask, float* z, int B, int S, int Spad, int N, cudaStream_t st) {
   if (S > OP_MAX_KB * OP_BK) {
@@ -241,15 +247,6 @@ int launch_opm_tc(TmaCtx* ctx, const bf16* ab_t, const bf16* wout_t, const float
   uint64_t dw[2] = {(uint64_t)OP_C * OP_C, OP_CZ}, sw[1] = {(uint64_t)OP_C * OP_C};
   uint32_t bxW[2] = {OP_C, OP_CZ};
   if (tma_encode_bf16(ctx, &tmW, wout_t, 2, dw, sw, bxW, 64) != 0) return -1;
-  static bool configured = false;
-  if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(opm_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, OpmSmem::TOTAL);
-    if (e != cudaSuccess) {
-      tc_set_error(std::string("cudaFuncSetAttribute(opm_tc): ") + cudaGetErrorString(e));
-      return -1;
-    }
-    configured = true;
-  }
   dim3 grid((N + OP_BJ - 1) / OP_BJ, (N + OP_BI - 1) / OP_BI, B);
   opm_tc_kernel<<<grid, OP_THREADS, OpmSmem::TOTAL, st>>>(tmA, tmB, tmW, bout, seq_mask, msa_mask, z, S, N);
   return 0;

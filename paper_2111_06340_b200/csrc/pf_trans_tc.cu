@@ -379,19 +379,18 @@ template <int C>
 static int launch_tr(const CUtensorMap& tmW1, const CUtensorMap& tmW2, const CUtensorMap& tmR, const TrParams& p, int num_sms,
                      cudaStream_t st) {
   auto kern = transition_kernel<C>;
-  static bool configured = false;
-  if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, TrSmem<C>::TOTAL);
-    if (e != cudaSuccess) {
-      tc_set_error(std::string("cudaFuncSetAttribute(transition): ") + cudaGetErrorString(e));
-      return -1;
-    }
-    configured = true;
-  }
   unsigned grid = (unsigned)(p.num_tiles < (long)num_sms ? p.num_tiles : (long)num_sms);
   kern<<<grid, TR_THREADS, TrSmem<C>::TOTAL, st>>>(tmW1, tmW2, tmR, p);
   return 0;
 }
+
+template <int C>
+static bool configure_tr() {
+  cudaError_t e = cudaFuncSetAttribute(transition_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, TrSmem<C>::TOTAL);
+  if (e != cudaSuccess) tc_set_error(std::string("cudaFuncSetAttribute(transition): ") + cudaGetErrorString(e));
+  return e == cudaSuccess;
+}
+bool configure_transition_kernels() { return configure_tr<128>() && configure_tr<256>(); }
 
 // w1t: fp16 [4C, C] (K = C contiguous); w2t: bf16 [C, 4C] (K = 4C contiguous); res: fp32 [R, C] updated in place.
 int launch_transition_tc(TmaCtx* ctx, float* res, long R, int C, const float* gamma, const float* beta, const void* w1t,

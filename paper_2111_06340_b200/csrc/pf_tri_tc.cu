@@ -102,6 +102,12 @@ tri_einsum_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
   if (warp == 1) tc::tmem_dealloc<TRI_BN>(tmem_base);
 }
 
+bool configure_tri_kernel() {
+  cudaError_t e = cudaFuncSetAttribute(tri_einsum_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TRI_SMEM);
+  if (e != cudaSuccess) tc_set_error(std::string("cudaFuncSetAttribute(tri_einsum_tc): ") + cudaGetErrorString(e));
+  return e == cudaSuccess;
+}
+
 int launch_tri_einsum_tc(TmaCtx* ctx, const bf16* a_cm, const bf16* b_cm, float* t_cm, int batch, int N, int Npad,
                          const int* key_tiles, int channels, int num_sms, cudaStream_t st) {
   (void)num_sms;
@@ -110,15 +116,6 @@ int launch_tri_einsum_tc(TmaCtx* ctx, const bf16* a_cm, const bf16* b_cm, float*
   uint32_t bx[3] = {TRI_BK, TRI_BM, 1};
   if (tma_encode_bf16(ctx, &tmA, a_cm, 3, d, s, bx, 128) != 0) return -1;
   if (tma_encode_bf16(ctx, &tmB, b_cm, 3, d, s, bx, 128) != 0) return -1;
-  static bool configured = false;
-  if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(tri_einsum_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TRI_SMEM);
-    if (e != cudaSuccess) {
-      tc_set_error(std::string("cudaFuncSetAttribute(tri_einsum_tc): ") + cudaGetErrorString(e));
-      return -1;
-    }
-    configured = true;
-  }
   dim3 grid((N + TRI_BN - 1) / TRI_BN, (N + TRI_BM - 1) / TRI_BM, batch);
   tri_einsum_tc_kernel<<<grid, TRI_THREADS, TRI_SMEM, st>>>(tmA, tmB, t_cm, N, Npad, key_tiles, channels);
   return 0;

@@ -1,7 +1,8 @@
 // tcgen05 path of the trunk (PF_BF16): device weight layout and the per-sub-step launch sequences of SURVEY.md §8(a).
 // 16-bit MMA operands with fp32 accumulation, fp32 residual streams (R1).  Storage formats (reading R17):
 // LayerNorm outputs and the weights they multiply are fp16 operands (bounded by construction; the weight values are the
-// bf16-rounded ones of R15, exactly representable), sigmoid gates are stored as fp16 (never an MMA operand), every other
+// bf16-rounded ones of R15, which fp16 represents exactly inside its normal range 2^-14 .. 65504 — smaller magnitudes lose
+// bits, larger ones are refused at create time, see F16Range), sigmoid gates are stored as fp16 (never an MMA operand), every other
 // intermediate (q, k, v, P, o, transition hidden, triangle operands, outer-product operands, pair bias) is bf16.
 // No arithmetic of the method lives here except two constants handed to the projection epilogues: log2(e)/sqrt(head_dim) on q
 // (R12) and log2(e) on the pair bias, so that the attention kernel's softmax runs in the exp2 domain.
@@ -30,11 +31,18 @@ static uint16_t f32_to_f16_bits(float f) {
   return b;
 }
 
+static F16Range* g_range = nullptr;   // set for the duration of one build_tc_block call (create is not re-entrant per handle)
+
 // dst[n, k] = src[k, n]  (src row-major [K, ld_src], columns [0, Nout)) as 16-bit
 static void put_transposed(std::vector<uint16_t>& dst, size_t at, const float* src, int K, int Nout, bool f16) {
   for (int n = 0; n < Nout; ++n)
     for (int k = 0; k < K; ++k) {
       float v = src[(size_t)k * Nout + n];
+      if (f16 && g_range) {
+        const float a = v < 0 ? -v : v;
+        if (!(a <= 65504.0f)) g_range->overflow++;           // also catches NaN
+        else if (a != 0.0f && a < 6.103515625e-05f) g_range->below_normal++;
+      }
       dst[at + (size_t)n * K + k] = f16 ? f32_to_f16_bits(v) : f32_to_bf16_bits(v);
     }
 }
@@ -70,7 +78,8 @@ TcBlock tc_layout(const pf_config& c) {
 }
 
 void build_tc_block(const pf_config& c, const BlockW& off, const TcBlock& t, const float* w, std::vector<uint16_t>& w16,
-                    size_t base16, std::vector<float>& wf, size_t basef) {
+                    size_t base16, std::vector<float>& wf, size_t basef, F16Range* range) {
+  g_range = range;
   auto attn = [&](const AttnW& a, const AttnT& d, int ch, int heads, bool self_bias) {
     // column order of the fused projection: [q | k | gate | v (| pair-bias heads)], all fed by LN(x): fp16
     put_transposed(w16, base16 + d.w_in + (size_t)0 * ch * ch, w + a.wq, ch, ch, true);
@@ -124,6 +133,7 @@ void build_tc_block(const pf_config& c, const BlockW& off, const TcBlock& t, con
   };
   tri(off.tri_out, t.to_w, t.to_b, t.to_wz, false);
   tri(off.tri_in, t.ti_w, t.ti_b, t.ti_wz, true);
+  g_range = nullptr;
 }
 
 

@@ -210,3 +210,43 @@ def gemm_flops_per_block(S: int, N: int, d: Dims = AF2) -> float:
             + 4.0 * S * N * cm * co + 2.0 * S * N * N * co * co + 2.0 * N * N * co * co * cz
             + 60.0 * N * N * cz * cz + 12.0 * N ** 3 * cz
             + 2.0 * N * N * cz * d.heads_msa + 4.0 * N * N * cz * d.heads_pair)
+
+
+def make_inputs_device(seed: int, B: int, S: int, N: int, device, d: Dims = AF2, lengths=None,
+                       msa_mask_frac_max: float = 0.0):
+    """make_inputs for batches too large to draw on the host in reasonable time (BASELINE.json configs[2..4] at full size):
+    msa / pair ~ N(0,1) drawn by torch's seeded generator ON ``device`` (torch tensors, garbage in the padding as in
+    make_inputs); the masks follow the same laws (R2, R11) and are returned as numpy arrays.  Whoever needs a protein's
+    values on the host copies that slice back, so the oracle and the CUDA path still see identical bits."""
+    import torch
+    g = torch.Generator(device=device).manual_seed(int(seed))
+    msa = torch.randn((B, S, N, d.c_m), device=device, generator=g, dtype=torch.float32)
+    pair = torch.randn((B, N, N, d.c_z), device=device, generator=g, dtype=torch.float32)
+    seq_mask = np.ones((B, N), dtype=np.float32)
+    if lengths is not None:
+        for b, L in enumerate(lengths):
+            seq_mask[b, int(L):] = 0.0
+    msa_mask = np.ones((B, S), dtype=np.float32)
+    if msa_mask_frac_max > 0.0 and S > 1:
+        gm = rng(seed, 2)
+        for b in range(B):
+            f = gm.uniform(0.0, msa_mask_frac_max)
+            k = int(np.floor(f * S))
+            if k > 0:
+                rows = gm.choice(np.arange(1, S), size=min(k, S - 1), replace=False)
+                msa_mask[b, rows] = 0.0
+    return msa, pair, seq_mask, msa_mask
+
+
+def sample_positions(seed: int, step: int, seq_mask_b, msa_mask_b, n: int):
+    """n output positions of one protein for sub-step ``step`` at which a parity test compares the CUDA path with the
+    sampled oracle: (s, i) with rho_s sigma_i = 1 for steps 1-3, (i, j) with sigma_i sigma_j = 1 for steps 4-9.  The corners
+    of the unmasked region come first (first / last 128-row tile, first / last query and key tile), the rest is uniform."""
+    res = np.flatnonzero(np.asarray(seq_mask_b) > 0.5)
+    rows = np.flatnonzero(np.asarray(msa_mask_b) > 0.5)
+    a, b = (rows, res) if step <= 3 else (res, res)
+    pos = [(a[0], b[0]), (a[-1], b[-1]), (a[0], b[-1]), (a[-1], b[0]), (a[len(a) // 2], b[len(b) // 2])]
+    g = rng(seed, 900 + step)
+    while len(pos) < n:
+        pos.append((a[int(g.integers(len(a)))], b[int(g.integers(len(b)))]))
+    return [(int(p), int(q)) for p, q in pos[:n]]
