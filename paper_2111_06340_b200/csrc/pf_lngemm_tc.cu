@@ -37,10 +37,11 @@ int tma_encode(TmaCtx* ctx, CUtensorMap* out, const void* base, int elem_kind, i
 // Timeline tracing of CTA 0 (experiments only; never defined in the product build): per traced thread a private slot of
 // (tag, clock64) pairs written with plain stores (no atomics: ~10 ns per event).
 __device__ unsigned long long g2_trace_buf[4 * 8192];
+__device__ int g2_trace_nw = 0;   // trace only the launches with this many weight rows (0 = all launches)
 #define G2_TRACE_DECL unsigned g2_trc = 0;
 #define G2_TRACE(slot, tag)                                                         \
   do {                                                                              \
-    if (blockIdx.x == 0 && g2_trc < 4000) {                                         \
+    if (blockIdx.x == 0 && g2_trc < 4000 && (g2_trace_nw == 0 || g2_trace_nw == p.Nw)) { \
       g2_trace_buf[(slot) * 8192 + 2 * g2_trc] = (tag);                             \
       g2_trace_buf[(slot) * 8192 + 2 * g2_trc + 1] = (unsigned long long)clock64(); \
       ++g2_trc;                                                                     \
@@ -767,6 +768,7 @@ bool configure_gemm2_kernels() {
 }
 
 #ifdef PF_G2_TRACE
+extern "C" void pf_debug_g2_trace_select(int nw) { cudaMemcpyToSymbol(g2_trace_nw, &nw, sizeof(int)); }
 extern "C" int pf_debug_g2_trace(unsigned long long* out, int reset) {
   cudaDeviceSynchronize();
   cudaMemcpyFromSymbol(out, g2_trace_buf, sizeof(g2_trace_buf));
