@@ -123,6 +123,11 @@ int pf_evoformer_profile_kinds(void);
 const char* pf_evoformer_profile_name(int kind);
 pf_status pf_evoformer_get_profile(pf_evoformer_t* h, int kind, long long* launches, double* ms, double* flops,
                                    double* bytes);
+/* The same records one by one, in launch order: record `index` in [0, pf_evoformer_profile_records(h)) -> its kind, device
+ * milliseconds, FLOP and byte tags.  Errors: INVALID_ARG (null, index out of range), CUDA (event query failed). */
+long long pf_evoformer_profile_records(const pf_evoformer_t* h);
+pf_status pf_evoformer_get_profile_record(pf_evoformer_t* h, long long index, int* kind, double* ms, double* flops,
+                                          double* bytes);
 
 void pf_evoformer_destroy(pf_evoformer_t* h);
 

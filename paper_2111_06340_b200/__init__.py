@@ -25,7 +25,7 @@ EXPORTED_SYMBOLS = (
     "pf_evoformer_block_floats", "pf_evoformer_create", "pf_evoformer_forward", "pf_evoformer_forward_substep",
     "pf_evoformer_forward_host", "pf_evoformer_workspace_bytes", "pf_evoformer_last_launch_count",
     "pf_evoformer_set_profiling", "pf_evoformer_profile_kinds", "pf_evoformer_profile_name",
-    "pf_evoformer_get_profile", "pf_evoformer_destroy", "pf_last_error", "pf_sched_create", "pf_sched_add", "pf_sched_next_batch",
+    "pf_evoformer_get_profile", "pf_evoformer_profile_records", "pf_evoformer_get_profile_record", "pf_evoformer_destroy", "pf_last_error", "pf_sched_create", "pf_sched_add", "pf_sched_next_batch",
     "pf_sched_bytes_per_protein", "pf_sched_cost", "pf_sched_partition", "pf_sched_destroy",
 )
 
@@ -76,6 +76,11 @@ def lib() -> ctypes.CDLL:
         L.pf_evoformer_get_profile.restype = c_int
         L.pf_evoformer_get_profile.argtypes = [c_void_p, c_int, POINTER(c_longlong), POINTER(ctypes.c_double),
                                                POINTER(ctypes.c_double), POINTER(ctypes.c_double)]
+        L.pf_evoformer_profile_records.restype = c_longlong
+        L.pf_evoformer_profile_records.argtypes = [c_void_p]
+        L.pf_evoformer_get_profile_record.restype = c_int
+        L.pf_evoformer_get_profile_record.argtypes = [c_void_p, c_longlong, POINTER(c_int), POINTER(ctypes.c_double),
+                                                      POINTER(ctypes.c_double), POINTER(ctypes.c_double)]
         L.pf_evoformer_destroy.restype = None
         L.pf_evoformer_destroy.argtypes = [c_void_p]
         L.pf_last_error.restype = c_char_p
@@ -166,6 +171,15 @@ class Evoformer:
             _check(lib().pf_evoformer_get_profile(self._h, k, byref(n), byref(ms), byref(fl), byref(by)))
             out[lib().pf_evoformer_profile_name(k).decode()] = {
                 "launches": n.value, "ms": ms.value, "flops": fl.value, "bytes": by.value}
+        return out
+
+    def get_profile_records(self) -> list:
+        """[(kind name, ms, flops, bytes)] of every launch since set_profiling(True), in launch order."""
+        out = []
+        for i in range(int(lib().pf_evoformer_profile_records(self._h))):
+            k, ms, fl, by = c_int(), ctypes.c_double(), ctypes.c_double(), ctypes.c_double()
+            _check(lib().pf_evoformer_get_profile_record(self._h, i, byref(k), byref(ms), byref(fl), byref(by)))
+            out.append((lib().pf_evoformer_profile_name(k.value).decode(), ms.value, fl.value, by.value))
         return out
 
     def last_launch_count(self) -> int:

@@ -254,6 +254,21 @@ extern "C" pf_status pf_evoformer_get_profile(pf_evoformer_t* h, int kind, long 
   return PF_OK;
 }
 
+extern "C" long long pf_evoformer_profile_records(const pf_evoformer_t* h) { return h ? (long long)h->prof.size() : 0; }
+
+extern "C" pf_status pf_evoformer_get_profile_record(pf_evoformer_t* h, long long index, int* kind, double* ms, double* flops,
+                                                     double* bytes) {
+  if (!h || !kind || !ms || !flops || !bytes) return fail(PF_ERR_INVALID_ARG, "null argument");
+  if (index < 0 || index >= (long long)h->prof.size()) return fail(PF_ERR_INVALID_ARG, "record index out of range");
+  const auto& r = h->prof[(size_t)index];
+  cudaError_t e = cudaEventSynchronize(r.e1);
+  float t = 0.f;
+  if (e == cudaSuccess) e = cudaEventElapsedTime(&t, r.e0, r.e1);
+  if (e != cudaSuccess) return fail(PF_ERR_CUDA, std::string("profile events: ") + cudaGetErrorString(e));
+  *kind = r.kind; *ms = t; *flops = r.flops; *bytes = r.bytes;
+  return PF_OK;
+}
+
 // ------------------------------------------------------------------------------------------------
 // sub-step drivers
 // ------------------------------------------------------------------------------------------------

@@ -6,7 +6,7 @@
 // followed by per-64-column epilogue groups (G2Op): scaled / biased / activated 16-bit row-major stores, gated channel-major
 // triangle operands, pair-bias heads, transposed V / outer-product operands, or "residual += (acc + bias) * gate".
 //
-// One persistent CTA per SM, 18 warps:
+// One persistent CTA per SM, 18 working warps (20 launched: register re-allocation is per warpgroup of four):
 //   warps 0-7   epilogue, two teams of four warps (team t takes the 64-column groups j with j % 2 == t, so one team's TMEM
 //               loads / barriers hide behind the other's arithmetic): tcgen05.ld their TMEM lane quarter -> registers ->
 //               shared-memory staging tile (one per team) -> ONE TMA store per group: row-major 16-bit (128B swizzle),
@@ -52,9 +52,29 @@ __device__ int g2_trace_nw = 0;   // trace only the launches with this many weig
 #define G2_TRACE(slot, tag)
 #endif
 
+#ifdef PF_G2_ABLATE
+// Timing experiments only (never defined in the product build; results are wrong while a bit is set):
+// 1 no TMA stores / staging waits in the epilogue, 2 epilogue groups skipped entirely, 4 LayerNorm producers read no global memory
+__device__ int g2_ablate = 0;
+extern "C" void pf_debug_g2_ablate(int v) { cudaMemcpyToSymbol(g2_ablate, &v, sizeof(int)); }
+#define G2_ABL(bit) (g2_ablate & (bit))
+#else
+#define G2_ABL(bit) 0
+#endif
+
 constexpr int G2_BN = 256;
-constexpr int G2_THREADS = 18 * 32;
+constexpr int G2_THREADS = 20 * 32;   // warps 18, 19 only complete the fourth warpgroup (register re-allocation is per warpgroup)
 constexpr int G2_EPI_WARPS = 8;
+// 20 warps x 96 registers at launch = the CTA's register pool (61440); setmaxnreg moves registers between whole warpgroups
+// inside that pool.  LayerNorm-fed kernels: warps 16-19 drop to 40, which lets the eight epilogue warps grow to 120 (the
+// LayerNorm producers keep 96: 8 x 32 x (120 + 96) + 4 x 32 x 40 = 60416).  TMA-fed kernels: warps 8-19 drop to 40, the
+// epilogue warps grow to 128.  Measured: the epilogue at 96 registers spilled its staging loop (out-projection with gate
+// 300 -> 213 us at cfg2 once it had 128).
+#ifndef PF_G2_EPI_REGS
+#define PF_G2_EPI_REGS 120
+#define PF_G2_MISC_REGS 40
+#endif
+constexpr int G2_EPI_REGS = PF_G2_EPI_REGS, G2_MISC_REGS = PF_G2_MISC_REGS, G2_EPI_REGS_TMA = 128, G2_IDLE_REGS = 40;
 constexpr int G2_PROD_WARPS = 8;
 
 struct G2Params {
@@ -298,7 +318,13 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
   tc::tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
 
+  if (warp >= 16) {   // one site for the whole fourth warpgroup (warps 18, 19 have no other work)
+    if (AMODE == 0) tc::reg_dealloc<G2_MISC_REGS>();
+    else tc::reg_dealloc<G2_IDLE_REGS>();
+  }
   if (warp < G2_EPI_WARPS) {
+    if (AMODE == 0) tc::reg_alloc<G2_EPI_REGS>();
+    else tc::reg_alloc<G2_EPI_REGS_TMA>();
     // =========================================================== epilogue: eight free-running warps.  Warp w owns the 32 tile
     // rows of TMEM lane quarter w % 4 and the 64-column groups j with j % 2 == w / 4; it stages its 32 x 128 B piece in its
     // own shared-memory tile and issues its own TMA store, so no barrier couples it to any other warp.
@@ -353,7 +379,7 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
         for (int j = team; j < 4; j += 2) {
           const G2Op& op = (j == team) ? op_a : op_b;
           const int kind = op.kind;
-          if (kind == G2_SKIP) continue;
+          if (kind == G2_SKIP || G2_ABL(2)) continue;
           if (lane == 0 && quarter == 0) G2_TRACE(team, 0x100 + 3);
           // this group's 64 bias values: inside the table, or the zero pad behind it
           const int bcol = nt * G2_BN + j * 64 - p.bias_lo;
@@ -364,7 +390,7 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
             sb = sb_team + (gcnt++ % NST) * SM::STW_BYTES;
             sb16 = reinterpret_cast<bf16*>(sb);
             if (leader && quarter == 0) G2_TRACE(team, 0x120);
-            if (leader) tc::bulk_wait_read<NST - 1>();
+            if (leader && !G2_ABL(1)) tc::bulk_wait_read<NST - 1>();
             __syncwarp();
             if (leader && quarter == 0) G2_TRACE(team, 0x121);
             {
@@ -390,7 +416,7 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
             tc::fence_proxy_async_smem();
             __syncwarp();
             if (leader && quarter == 0) G2_TRACE(team, 0x123);
-            if (leader) {
+            if (leader && !G2_ABL(1)) {
               tc::tma_store_4d(&tmO0, sb, op.dst_col, tcd.y0 + yw0, tcd.x0 + xw0, tcd.b);
               tc::bulk_commit();
             }
@@ -400,7 +426,7 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
             for (int hf = 0; hf < 2; ++hf) {
               sb = sb_team + (gcnt++ % NST) * SM::STW_BYTES;
             sb16 = reinterpret_cast<bf16*>(sb);
-            if (leader) tc::bulk_wait_read<NST - 1>();
+            if (leader && !G2_ABL(1)) tc::bulk_wait_read<NST - 1>();
               __syncwarp();
               uint32_t v[32];
               float bb[32];
@@ -434,7 +460,7 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
                     make_float4(f[c * 4], f[c * 4 + 1], f[c * 4 + 2], f[c * 4 + 3]);
               tc::fence_proxy_async_smem();
               __syncwarp();
-              if (leader) {
+              if (leader && !G2_ABL(1)) {
                 tc::tma_reduce_add_4d(&tmR, sb, op.dst_col + hf * 32, tcd.y0 + yw0, tcd.x0 + xw0, tcd.b);
                 tc::bulk_commit();
               }
@@ -444,7 +470,7 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
             // consecutive lanes are consecutive in shared memory), one TMA store with box {YT, XT, 64, 1}
             sb = sb_team + (gcnt++ % NST) * SM::STW_BYTES;
             sb16 = reinterpret_cast<bf16*>(sb);
-            if (leader) tc::bulk_wait_read<NST - 1>();
+            if (leader && !G2_ABL(1)) tc::bulk_wait_read<NST - 1>();
             __syncwarp();
 #pragma unroll 1
             for (int hf = 0; hf < 2; ++hf) {
@@ -475,7 +501,7 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
             // pair-bias heads [b, head, x, y]: staging tile [head][x][y], box {YT, XT, n_heads, 1}
             sb = sb_team + (gcnt++ % NST) * SM::STW_BYTES;
             sb16 = reinterpret_cast<bf16*>(sb);
-            if (leader) tc::bulk_wait_read<NST - 1>();
+            if (leader && !G2_ABL(1)) tc::bulk_wait_read<NST - 1>();
             __syncwarp();
             uint32_t v[32];
             tc::tmem_ld32(tacc + j * 64, v);
@@ -496,7 +522,7 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
             const int ch = quarter * 32 + lane;
             const int wcol = nt * G2_BN - p.bias_lo;   // the whole window's bias is in the table (checked by the launcher)
             const float bpv = sbias_tab[wcol + ch], bgv = sbias_tab[wcol + 128 + ch];
-            if (leader) tc::bulk_wait_read<NST - 1>();
+            if (leader && !G2_ABL(1)) tc::bulk_wait_read<NST - 1>();
             __syncwarp();
 #pragma unroll 1
             for (int hf = 0; hf < 2; ++hf) {
@@ -520,7 +546,7 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
             }
             tc::fence_proxy_async_smem();
             __syncwarp();
-            if (leader) {
+            if (leader && !G2_ABL(1)) {
               const int r0 = j * 64;   // first tile row of this group
               tc::tma_store_4d(op.map ? &tmT1 : &tmT0, sb, tcd.y0 + (r0 & (p.YT - 1)), tcd.x0 + (r0 >> p.yt_shift),
                                op.dst_col + quarter * 32, tcd.b);
@@ -530,12 +556,12 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
             // operand-swapped half-window: this thread owns output column (channel) 32 quarter + lane of the half and reads 64
             // consecutive tile rows from TMEM: convert, stage as a 128-byte row, one TMA store {64 y, 32 channels}
             sb = sb_team + (gcnt++ % NST) * SM::STW_BYTES;
-            if (leader) tc::bulk_wait_read<NST - 1>();
+            if (leader && !G2_ABL(1)) tc::bulk_wait_read<NST - 1>();
             __syncwarp();
             g2_row16_plain<0>(tacc + j * 64, sb + lane * 128, 1.0f, sw);
             tc::fence_proxy_async_smem();
             __syncwarp();
-            if (leader) {
+            if (leader && !G2_ABL(1)) {
               const int r0 = (j & 1) * 64;   // first tile row of this group
               tc::tma_store_4d(&tmVS, sb, tcd.y0 + (r0 & (p.YT - 1)), op.dst_col + quarter * 32, tcd.x0 + (r0 >> p.yt_shift), tcd.b);
               tc::bulk_commit();
@@ -544,7 +570,7 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
             // 64 columns written transposed, [(b, x), column, y]: staging tile [x][column][y], box {YT, 64, XT, 1}
             sb = sb_team + (gcnt++ % NST) * SM::STW_BYTES;
             sb16 = reinterpret_cast<bf16*>(sb);
-            if (leader) tc::bulk_wait_read<NST - 1>();
+            if (leader && !G2_ABL(1)) tc::bulk_wait_read<NST - 1>();
             __syncwarp();
             const float mk = op.masked ? mask : 1.0f;
             bf16* dst = sb16 + ((xlw * 64) << p.ytw_shift) + ylw;
@@ -629,7 +655,7 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
 #pragma unroll
           for (int ps = 0; ps < LN::PASSES; ++ps) {
             lr[ps] = pw * 16 + ln.row_of(r0, ps);
-            rp[ps] = src_row(tcd, lr[ps]);
+            rp[ps] = G2_ABL(4) ? nullptr : src_row(tcd, lr[ps]);
           }
           ln.run(rp, lr, abase);
         }
@@ -638,9 +664,10 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
         if (lane == 0 && pw == 0) G2_TRACE(2, 0x202);
         ++it;
       }
-    } else if (warp == 8) {
+    } else {
+      tc::reg_dealloc<G2_IDLE_REGS>();
       // ========================================================= A by TMA (a_mode 1)
-      if (tc::elect_one()) {
+      if (warp == 8 && tc::elect_one()) {
         uint32_t it = 0;
         for (long tile = blockIdx.x; tile < p.num_tiles; tile += gridDim.x) {
           if (!tile_on(tile, p)) continue;
@@ -673,7 +700,7 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
         }
       }
     }
-  } else {
+  } else if (warp == 17) {
     // ============================================================= MMA issue
     if (tc::elect_one()) {
       uint32_t it = 0, wc = 0, ac = 0;

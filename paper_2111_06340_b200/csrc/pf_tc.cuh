@@ -112,6 +112,13 @@ __device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
 // generic-proxy writes to shared memory -> visible to the async proxy (TMA / tcgen05.mma operand reads)
 __device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
+// Register re-allocation between warp roles (whole warpgroups of four consecutive warps): the data-movement warps give
+// registers back to the CTA's pool, the LayerNorm producers take them.
+template <int N>
+__device__ __forceinline__ void reg_dealloc() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
+template <int N>
+__device__ __forceinline__ void reg_alloc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
+
 // ---------------------------------------------------------------- tcgen05
 template <int COLS>
 __device__ __forceinline__ void tmem_alloc(uint32_t* slot_in_smem) {   // whole warp

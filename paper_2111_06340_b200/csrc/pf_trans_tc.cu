@@ -6,7 +6,7 @@
 // operand of GEMM2, which accumulates the C output columns in TMEM over the 4C/128 chunks.  HBM traffic per row is one
 // fp32 read and one fp32 reduce-add of C values (the algorithmic minimum 8C bytes + the L2-resident weights).
 //
-// One persistent CTA per SM, 18 warps:
+// One persistent CTA per SM, 18 working warps (20 launched: register re-allocation is per warpgroup of four):
 //   warps 0-7   epilogue, two teams of four warps.  E1(chunk): team t rectifies columns [64t, 64t+64) of the hidden chunk
 //               (TMEM -> +b1 -> relu -> bf16 -> k-block t of the A2 tile, UMMA 128B-swizzle layout).  E2(tile): the C output
 //               columns + b2 in 32-column fp32 boxes through staging tiles (the idle A2 buffers) -> TMA reduce-add into the
@@ -29,7 +29,7 @@ namespace pf {
 int tma_encode(TmaCtx* ctx, CUtensorMap* out, const void* base, int elem_kind, int rank, const uint64_t* dims,
                const uint64_t* strides_bytes, const uint32_t* box, int swizzle_bytes);
 
-constexpr int TR_THREADS = 18 * 32;
+constexpr int TR_THREADS = 20 * 32;      // warps 18, 19 only complete the fourth warpgroup (setmaxnreg is per warpgroup)
 constexpr int TR_EPI_WARPS = 8;
 constexpr int TR_PROD_WARPS = 8;
 constexpr int TR_HC = 128;              // hidden columns per chunk
@@ -130,7 +130,10 @@ transition_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constan
   tc::tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
 
+  // 20 x 96 registers at launch = the CTA's pool: warps 16-19 drop to 40, the epilogue warps grow to 120
+  if (warp >= 16) tc::reg_dealloc<40>();
   if (warp < TR_EPI_WARPS) {
+    tc::reg_alloc<120>();
     // =========================================================== epilogue (two teams of four warps)
     const int team = warp >> 2, quarter = warp & 3;
     const int lr = quarter * 32 + lane;                // tile row = TMEM lane
@@ -294,7 +297,7 @@ transition_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constan
         g2(NC - 1);
       }
     }
-  } else {
+  } else if (warp == 17) {
     // ============================================================= MMA issue
     if (tc::elect_one()) {
       constexpr uint32_t idesc1 = tc::idesc_f16_f32(128, 128);    // GEMM1: fp16 LayerNorm output x fp16 W1
