@@ -631,13 +631,8 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
       for (long tile = blockIdx.x; tile < p.num_tiles; tile += gridDim.x) {
         if (!tile_on(tile, p)) continue;
         const uint32_t abuf = it & 1;
-        // Short-distance L2 prefetch: while a batch of RU rows is normalised, the next batch of this warp (the first batch of
-        // the next active tile after the last one) is pulled into L2, so the register-staged loads see L2 latency, not HBM
-        // latency (bytes in flight per SM are bounded by the register file).  A whole tile ahead was too far: with the
-        // output stream passing through L2 in between, a third of the prefetched lines were evicted before use.
-        const long nxt = tile + gridDim.x;
-        const bool nxt_on = nxt < p.num_tiles && tile_on(nxt, p);
-        const TileCoord ncd = tile_coord(nxt_on ? nxt : tile, p);
+        // (A bulk L2 prefetch of the next batch of rows used to sit here; once the epilogue stopped spilling it measured as a
+        // small loss — the 128 per-row prefetch operations per tile compete with the weight loads and the stores in the TMA queue.)
         if (lane == 0 && pw == 0) G2_TRACE(2, 0x200);
         tc::mbar_wait(&a_empty[abuf], ((it >> 1) & 1) ^ 1);
         if (lane == 0 && pw == 0) G2_TRACE(2, 0x201);
@@ -645,11 +640,6 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
         uint8_t* abase = smem + SM::A_OFF + abuf * SM::A_BYTES;
 #pragma unroll 1
         for (int r0 = 0; r0 < 16; r0 += RU) {
-          if (lane < RU && (r0 + RU < 16 || nxt_on)) {
-            const bool same = r0 + RU < 16;
-            const float* rp = src_row(same ? tcd : ncd, pw * 16 + (same ? r0 + RU : 0) + lane);
-            if (rp) tc::prefetch_l2_bulk(rp, K * 4);
-          }
           const float* rp[LN::PASSES];
           int lr[LN::PASSES];
 #pragma unroll

@@ -250,3 +250,80 @@ def sample_positions(seed: int, step: int, seq_mask_b, msa_mask_b, n: int):
     while len(pos) < n:
         pos.append((a[int(g.integers(len(a)))], b[int(g.integers(len(b)))]))
     return [(int(p), int(q)) for p, q in pos[:n]]
+
+
+# ----------------------------------------------------------------------------------------------
+# input / recycling embedders (DESIGN.md §2b readings E.1-E.3)
+# ----------------------------------------------------------------------------------------------
+
+@dataclass(frozen=True)
+class EmbedDims:
+    c_m: int = 256
+    c_z: int = 128
+    tf_dim: int = 22          # target features: one break flag + 21 residue classes
+    msa_dim: int = 49         # MSA features: 23 token classes + 2 deletion features + 23 profile entries + 1 deletion mean
+    max_relpos: int = 32
+    n_dist_bins: int = 15
+    first_break: float = 3.25
+    last_break: float = 20.75
+
+
+EMBED = EmbedDims()
+
+
+def embed_spec(d: EmbedDims = EMBED):
+    """Ordered (name, shape, kind) of the embedder weights blob (row-major [in, out], as Appendix B)."""
+    nrel = 2 * d.max_relpos + 1
+    return [("w_a", (d.tf_dim, d.c_z), "W"), ("b_a", (d.c_z,), "bias"),
+            ("w_b", (d.tf_dim, d.c_z), "W"), ("b_b", (d.c_z,), "bias"),
+            ("w_rel", (nrel, d.c_z), "W"), ("b_rel", (d.c_z,), "bias"),
+            ("w_m", (d.msa_dim, d.c_m), "W"), ("b_m", (d.c_m,), "bias"),
+            ("w_t", (d.tf_dim, d.c_m), "W"), ("b_t", (d.c_m,), "bias"),
+            ("ln_m_g", (d.c_m,), "gamma"), ("ln_m_b", (d.c_m,), "beta"),
+            ("ln_z_g", (d.c_z,), "gamma"), ("ln_z_b", (d.c_z,), "beta"),
+            ("w_d", (d.n_dist_bins, d.c_z), "W"), ("b_d", (d.c_z,), "bias")]
+
+
+def make_embed_weights(seed: int, d: EmbedDims = EMBED):
+    """R8 recipe; one-hot inputs select single rows, so W ~ N(0,1) (fan-in of a one-hot is 1) except the dense MSA features."""
+    g = rng(seed, 2000)
+    out = {}
+    for name, shape, kind in embed_spec(d):
+        r = g.standard_normal(shape, dtype=np.float32)
+        if kind == "W":
+            out[name] = (r / np.float32(np.sqrt(shape[0] if name == "w_m" else 1.0))).astype(np.float32)
+        elif kind == "gamma":
+            out[name] = (1.0 + 0.1 * r).astype(np.float32)
+        else:
+            out[name] = (0.1 * r).astype(np.float32)
+    return out
+
+
+def pack_embed_blob(w, d: EmbedDims = EMBED) -> np.ndarray:
+    return np.ascontiguousarray(np.concatenate([np.asarray(w[n], dtype=np.float32).reshape(-1) for n, _, _ in embed_spec(d)]))
+
+
+def make_features(seed: int, B: int, S: int, N: int, d: EmbedDims = EMBED):
+    """Protein-shaped synthetic features (stand-ins for features.pkl, which needs the MSA stage):
+    target_feat[B,N,22] one-hot residue classes, residue_index[B,N] = 0..N-1 with one chain gap, msa_feat[B,S,N,49]
+    (one-hot token, deletion flags, a normalised profile), x_prev[B,N,3] a 3.8 Angstrom random walk (C-alpha-like trace,
+    so pair distances cover all the distance bins)."""
+    g = rng(seed, 2100)
+    aa = g.integers(0, d.tf_dim - 1, size=(B, N))
+    tf = np.zeros((B, N, d.tf_dim), np.float32)
+    np.put_along_axis(tf, (aa + 1)[..., None], 1.0, axis=-1)
+    ri = np.tile(np.arange(N, dtype=np.int32), (B, 1))
+    for b in range(B):
+        ri[b, N // 2:] += 20 * (b % 2)                      # a gap in the numbering of every other protein
+    tok = g.integers(0, 23, size=(B, S, N))
+    mf = np.zeros((B, S, N, d.msa_dim), np.float32)
+    np.put_along_axis(mf[..., :23], tok[..., None], 1.0, axis=-1)
+    mf[..., 23] = (g.uniform(size=(B, S, N)) < 0.1)
+    mf[..., 24] = g.uniform(size=(B, S, N)).astype(np.float32) * mf[..., 23]
+    prof = np.exp(g.standard_normal((B, 1, N, 23), dtype=np.float32))
+    mf[..., 25:48] = prof / prof.sum(-1, keepdims=True)
+    mf[..., 48] = g.uniform(size=(B, 1, N)).astype(np.float32) * 0.2
+    step = g.standard_normal((B, N, 3), dtype=np.float32)
+    step *= np.float32(3.8) / np.linalg.norm(step, axis=-1, keepdims=True)
+    x = np.cumsum(step, axis=1).astype(np.float32)
+    return tf, ri, mf, x
