@@ -320,6 +320,37 @@ def side_workload(h, ps, torch, dev, name, peaks, steps=3, warmup=3):
             "roofline": roof, "kernels": table}
 
 
+def recycled_workload(h, pf, ps, torch, dev, name="cfg3", n_cycles=4, steps=2):
+    """the recycled trunk (three recycling procedures = 4 passes) on configs[2]'s shape:
+    features -> input + recycling embedders -> 48 blocks, four times, through pf_evoformer_forward_recycled.  Context for
+    the paper's whole-model GPU seconds per protein (0.1-0.6 h for the 100-protein medium set on a V100)."""
+    import numpy as np
+    wl = WORKLOADS[name]
+    B, S, N, nb = wl["B"], wl["S"], wl["N"], wl["n_blocks"]
+    emb = pf.Embedder(ps.pack_embed_blob(ps.make_embed_weights(7)), pf.make_embed_config())
+    tf, ri, mf, x = ps.make_features(100, B, S, N)
+    tfd, rid, mfd, xd = [torch.from_numpy(a).to(dev) for a in (tf, ri, mf, x)]
+    smd = torch.ones((B, N), device=dev)
+    mmd = torch.ones((B, S), device=dev)
+    m = torch.empty((B, S, N, 256), device=dev)
+    z = torch.empty((B, N, N, 128), device=dev)
+    pf.forward_recycled(h, emb, tfd, rid, mfd, xd, m, z, smd, mmd, nb, n_cycles)       # warm-up
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(torch.cuda.current_stream())
+    for _ in range(steps):
+        pf.forward_recycled(h, emb, tfd, rid, mfd, xd, m, z, smd, mmd, nb, n_cycles)
+    e1.record(torch.cuda.current_stream())
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / steps
+    launches = h.last_launch_count()
+    finite = bool(torch.isfinite(m).all().item() and torch.isfinite(z).all().item())
+    emb.close()
+    return {"desc": f"{wl['desc']}; {n_cycles} cycles of (input + recycling embedders, {nb} blocks) through "
+                    "pf_evoformer_forward_recycled", "n_cycles": n_cycles, "steps": steps, "ms_per_protein": ms / B,
+            "proteins_per_s": B / (ms * 1e-3), "gpu_launches_per_step": int(launches), "outputs_finite": finite}
+
+
 def cfg5_sweep(h, pf, ps, torch, dev, peaks, n_proteins=2000, S=512, cap=48, nb=48):
     """BASELINE.json configs[4], run for real: 2,000 proteins (lengths R10), buckets {64..320}, N_seq=512, msa_mask R11, every
     batch the length-bucketing scheduler (pf_sched_*) cuts goes through all 48 blocks (48 distinct weight sets).  Inputs are
@@ -513,6 +544,7 @@ def run_ours(args, wl, wl_name):
     torch.cuda.empty_cache()
     if want_sides:
         line["workloads"] = {k: side_workload(h, ps, torch, dev, k, peaks) for k in ("cfg3", "cfg4")}
+        line["workloads"]["cfg3_recycled"] = recycled_workload(h, pf, ps, torch, dev)
     if want_sweep:
         line["cfg5_sweep"] = cfg5_sweep(h, pf, ps, torch, dev, peaks)
     if world == 1 and not args.no_cpu_baseline:

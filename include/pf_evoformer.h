@@ -134,6 +134,55 @@ void pf_evoformer_destroy(pf_evoformer_t* h);
 const char* pf_last_error(void);
 
 /* ------------------------------------------------------------------------------------------------
+ * Input / recycling embedders and the recycled trunk.  ParaFold's GPU stage reads the features its CPU
+ * stage wrote and runs the network with "three recycling procedures" ("recycling",
+ * PAPER.md:61).  PAPER.md prints no formula; the readings E.1-E.3 are:
+ *   E.1 input embedder      z_ij = Lin_a(tf_i) + Lin_b(tf_j) + Lin_rel(onehot(clip(r_i - r_j, -R, R) + R))
+ *                           m_si = Lin_m(msa_feat_si) + Lin_t(tf_i)
+ *   E.2 recycling embedder  z_ij += LN_z(zprev_ij) + Lin_d(onehot_bins(|xprev_i - xprev_j|)),  m_0i += LN_m(mprev_0i)
+ *                           (n_dist_bins lower edges evenly spaced from first_break to last_break; the last bin is open)
+ *   E.3 recycled trunk      n_cycles x (E.1, E.2 with the previous cycle's trunk output — zeros in the first cycle —, trunk)
+ * All arithmetic is fp32.  xprev (previous C-beta positions, Angstrom) would come from the structure module, which this
+ * library does not contain: it is an input, held constant over the cycles; NULL = no previous structure (no bin is set).
+ * ---------------------------------------------------------------------------------------------- */
+typedef struct pf_embedder pf_embedder_t;   /* opaque; owns device weights and a small grow-only workspace */
+typedef struct {
+  int c_m;            /* MSA channels (256) */
+  int c_z;            /* pair channels (128) */
+  int tf_dim;         /* target features per residue (22) */
+  int msa_dim;        /* MSA features per (sequence, residue) (49; at most 64) */
+  int max_relpos;     /* R: relative positions are clipped to [-R, R] (32) */
+  int n_dist_bins;    /* distance bins of the recycled positions (15) */
+  float first_break;  /* lower edge of the first bin, Angstrom (3.25) */
+  float last_break;   /* lower edge of the last bin (20.75) */
+} pf_embed_config;
+
+/* fp32 values in the embedder weights blob, in this order, every matrix row-major [in, out]:
+ * W_a[tf_dim,c_z] b_a | W_b b_b | W_rel[2R+1,c_z] b_rel | W_m[msa_dim,c_m] b_m | W_t[tf_dim,c_m] b_t | LN_m gamma beta [c_m] |
+ * LN_z gamma beta [c_z] | W_d[n_dist_bins,c_z] b_d.  0 for a null / unsupported config. */
+size_t pf_embedder_floats(const pf_embed_config* cfg);
+/* Errors: INVALID_ARG (null), SHAPE (c_m, c_z not in {128, 256}; msa_dim > 64; blob length), ALLOC, CUDA. */
+pf_status pf_embedder_create(pf_embedder_t** out, const float* weights_host, size_t n_weight_floats,
+                             const pf_embed_config* cfg);
+/* E.1 + E.2 for a batch, asynchronously on cuda_stream, IN PLACE: with has_prev != 0 dev msa[B,S,N,c_m] / pair[B,N,N,c_z] hold
+ * the previous cycle's trunk output on entry (only row s = 0 of msa is read); with has_prev == 0 they are not read (previous
+ * representations = 0).  On return they hold the embedded representations.  target_feat_dev [B,N,tf_dim] fp32,
+ * residue_index_dev [B,N] int32, msa_feat_dev [B,S,N,msa_dim] fp32, x_prev_dev [B,N,3] fp32 or NULL.  Every position is
+ * embedded (padding included: the embedders are per position; masks belong to the trunk). */
+pf_status pf_embedder_forward(pf_embedder_t* e, const float* target_feat_dev, const int* residue_index_dev,
+                              const float* msa_feat_dev, const float* x_prev_dev, int has_prev, float* msa_dev,
+                              float* pair_dev, int B, int S, int N, void* cuda_stream);
+long long pf_embedder_last_launch_count(const pf_embedder_t* e);
+void pf_embedder_destroy(pf_embedder_t* e);
+/* E.3: n_cycles x (pf_embedder_forward, pf_evoformer_forward over n_blocks blocks) on cuda_stream; msa_dev / pair_dev are
+ * outputs (their contents on entry are ignored).  n_cycles = 4 is AlphaFold's "three recycling procedures".
+ * Errors: those of the two calls; SHAPE if n_cycles < 1 or the channel dims of the two handles differ. */
+pf_status pf_evoformer_forward_recycled(pf_evoformer_t* h, pf_embedder_t* e, const float* target_feat_dev,
+                                        const int* residue_index_dev, const float* msa_feat_dev, const float* x_prev_dev,
+                                        float* msa_dev, float* pair_dev, const float* seq_mask_dev, const float* msa_mask_dev,
+                                        int B, int S, int N, int n_blocks, int n_cycles, void* cuda_stream);
+
+/* ------------------------------------------------------------------------------------------------
  * Length-bucketing batch scheduler ("sort by length ... share the compiled model";
  * SURVEY.md §3(iv)).  Host only.  Proteins are sorted by descending length (largest first, as the paper
  * compiles for the largest), assigned to the smallest bucket >= length, and cut into batches of at most

@@ -27,6 +27,8 @@ EXPORTED_SYMBOLS = (
     "pf_evoformer_set_profiling", "pf_evoformer_profile_kinds", "pf_evoformer_profile_name",
     "pf_evoformer_get_profile", "pf_evoformer_profile_records", "pf_evoformer_get_profile_record", "pf_evoformer_destroy", "pf_last_error", "pf_sched_create", "pf_sched_add", "pf_sched_next_batch",
     "pf_sched_bytes_per_protein", "pf_sched_cost", "pf_sched_partition", "pf_sched_destroy",
+    "pf_embedder_floats", "pf_embedder_create", "pf_embedder_forward", "pf_embedder_last_launch_count", "pf_embedder_destroy",
+    "pf_evoformer_forward_recycled",
 )
 
 
@@ -34,6 +36,11 @@ class PfConfig(Structure):
     _fields_ = [("c_m", c_int), ("c_z", c_int), ("heads_msa", c_int), ("heads_pair", c_int), ("head_dim", c_int),
                 ("c_opm", c_int), ("c_tri", c_int), ("transition_n", c_int), ("n_blocks_max", c_int),
                 ("dtype", c_int)]
+
+
+class PfEmbedConfig(Structure):
+    _fields_ = [("c_m", c_int), ("c_z", c_int), ("tf_dim", c_int), ("msa_dim", c_int), ("max_relpos", c_int),
+                ("n_dist_bins", c_int), ("first_break", c_float), ("last_break", c_float)]
 
 
 class PfError(RuntimeError):
@@ -98,6 +105,19 @@ def lib() -> ctypes.CDLL:
         L.pf_sched_partition.argtypes = [POINTER(c_int), c_int, POINTER(c_int), c_int, c_int, c_int, POINTER(c_int)]
         L.pf_sched_destroy.restype = None
         L.pf_sched_destroy.argtypes = [c_void_p]
+        L.pf_embedder_floats.restype = c_size_t
+        L.pf_embedder_floats.argtypes = [POINTER(PfEmbedConfig)]
+        L.pf_embedder_create.restype = c_int
+        L.pf_embedder_create.argtypes = [POINTER(c_void_p), c_void_p, c_size_t, POINTER(PfEmbedConfig)]
+        L.pf_embedder_forward.restype = c_int
+        L.pf_embedder_forward.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_int, c_void_p, c_void_p,
+                                          c_int, c_int, c_int, c_void_p]
+        L.pf_embedder_last_launch_count.restype = c_longlong
+        L.pf_embedder_last_launch_count.argtypes = [c_void_p]
+        L.pf_embedder_destroy.restype = None
+        L.pf_embedder_destroy.argtypes = [c_void_p]
+        L.pf_evoformer_forward_recycled.restype = c_int
+        L.pf_evoformer_forward_recycled.argtypes = [c_void_p] * 10 + [c_int] * 5 + [c_void_p]
         _lib = L
     return _lib
 
@@ -195,6 +215,52 @@ class Evoformer:
             self.close()
         except Exception:
             pass
+
+
+def make_embed_config(c_m=256, c_z=128, tf_dim=22, msa_dim=49, max_relpos=32, n_dist_bins=15, first_break=3.25,
+                      last_break=20.75) -> PfEmbedConfig:
+    return PfEmbedConfig(c_m, c_z, tf_dim, msa_dim, max_relpos, n_dist_bins, first_break, last_break)
+
+
+class Embedder:
+    """pf_embedder_* wrapper: input + recycling embedders (pointers and sizes only)."""
+
+    def __init__(self, weights_blob: np.ndarray, cfg: PfEmbedConfig):
+        blob = np.ascontiguousarray(weights_blob, dtype=np.float32)
+        self._e = c_void_p()
+        self.cfg = cfg
+        _check(lib().pf_embedder_create(byref(self._e), blob.ctypes.data, blob.size, byref(cfg)))
+
+    def forward(self, target_feat, residue_index, msa_feat, x_prev, has_prev: bool, msa, pair, stream=None):
+        B, S, N = msa.shape[0], msa.shape[1], msa.shape[2]
+        if stream is None:
+            import torch
+            stream = torch.cuda.current_stream().cuda_stream
+        _check(lib().pf_embedder_forward(self._e, _ptr(target_feat), _ptr(residue_index), _ptr(msa_feat), _ptr(x_prev),
+                                         1 if has_prev else 0, _ptr(msa), _ptr(pair), B, S, N, stream))
+
+    def last_launch_count(self) -> int:
+        return int(lib().pf_embedder_last_launch_count(self._e))
+
+    def close(self):
+        if self._e:
+            lib().pf_embedder_destroy(self._e)
+            self._e = c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def forward_recycled(evo: "Evoformer", emb: Embedder, target_feat, residue_index, msa_feat, x_prev, msa, pair, seq_mask,
+                     msa_mask, n_blocks: int, n_cycles: int, stream=None):
+    """pf_evoformer_forward_recycled: n_cycles x (embedders, trunk); msa / pair receive the result."""
+    B, S, N = msa.shape[0], msa.shape[1], msa.shape[2]
+    _check(lib().pf_evoformer_forward_recycled(evo._h, emb._e, _ptr(target_feat), _ptr(residue_index), _ptr(msa_feat),
+                                               _ptr(x_prev), _ptr(msa), _ptr(pair), _ptr(seq_mask), _ptr(msa_mask),
+                                               B, S, N, n_blocks, n_cycles, evo._stream(stream)))
 
 
 class Scheduler:

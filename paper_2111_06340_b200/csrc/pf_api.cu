@@ -19,6 +19,9 @@ static pf_status fail(pf_status s, const std::string& msg) {
   return s;
 }
 extern "C" const char* pf_last_error(void) { return g_err.c_str(); }
+namespace pf {
+void api_set_error(const std::string& s) { g_err = s; }   // other translation units of the C ABI (pf_embed.cu)
+}
 
 #define CUDA_TRY(expr)                                                                              \
   do {                                                                                              \
