@@ -327,3 +327,80 @@ def make_features(seed: int, B: int, S: int, N: int, d: EmbedDims = EMBED):
     step *= np.float32(3.8) / np.linalg.norm(step, axis=-1, keepdims=True)
     x = np.cumsum(step, axis=1).astype(np.float32)
     return tf, ri, mf, x
+
+
+# ----------------------------------------------------------------------------------------------
+# extra-MSA stack (DESIGN.md §2c readings X.1-X.9)
+# ----------------------------------------------------------------------------------------------
+
+@dataclass(frozen=True)
+class ExtraDims:
+    c_e: int = 64             # extra-MSA channels
+    c_z: int = 128
+    heads_msa: int = 8        # heads of dimension c_e / heads_msa = 8
+    heads_pair: int = 4
+    head_dim_pair: int = 32
+    c_opm: int = 32
+    c_tri: int = 128
+    transition_n: int = 4
+
+    @property
+    def head_dim_msa(self):
+        return self.c_e // self.heads_msa
+
+
+EXTRA = ExtraDims()
+
+
+def extra_block_spec(d: ExtraDims = EXTRA):
+    """Ordered (module, [(name, shape, kind)]) of one extra-MSA block: as block_spec at c_m = c_e, with the column attention
+    replaced by the global one (one shared key / value head of dimension head_dim_msa)."""
+    main = Dims(c_m=d.c_e, c_z=d.c_z, heads_msa=d.heads_msa, heads_pair=d.heads_pair, head_dim=d.head_dim_pair,
+                c_opm=d.c_opm, c_tri=d.c_tri, transition_n=d.transition_n)
+    spec = block_spec(main)
+    c, hd = d.c_e, d.head_dim_msa
+    glob = [("ln_g", (c,), "gamma"), ("ln_b", (c,), "beta"), ("wq", (c, c), "W"), ("wk", (c, hd), "W"), ("wv", (c, hd), "W"),
+            ("wg", (c, c), "W"), ("bg", (c,), "bias"), ("wo", (c, c), "W"), ("bo", (c,), "bias")]
+    return [("col_global", glob) if mod == "col" else (mod, items) for mod, items in spec]
+
+
+def extra_block_floats(d: ExtraDims = EXTRA) -> int:
+    return sum(int(np.prod(shape)) for _, items in extra_block_spec(d) for _, shape, _ in items)
+
+
+def make_extra_weights(seed: int, n_blocks: int, d: ExtraDims = EXTRA, bf16_weights: bool = False):
+    out = []
+    for blk in range(n_blocks):
+        g = rng(seed, 3000 + blk)
+        w = {}
+        for module, items in extra_block_spec(d):
+            mod = {}
+            for name, shape, kind in items:
+                r = g.standard_normal(shape, dtype=np.float32)
+                if kind == "W":
+                    v = r / np.float32(np.sqrt(shape[0]))
+                    mod[name] = round_to_bf16(v) if bf16_weights else v.astype(np.float32)
+                elif kind == "gamma":
+                    mod[name] = (1.0 + 0.1 * r).astype(np.float32)
+                else:
+                    mod[name] = (0.1 * r).astype(np.float32)
+            w[module] = mod
+        out.append(w)
+    return out
+
+
+def pack_extra_blob(blocks, d: ExtraDims = EXTRA) -> np.ndarray:
+    parts = []
+    for w in blocks:
+        for module, items in extra_block_spec(d):
+            for name, shape, _ in items:
+                a = np.asarray(w[module][name], dtype=np.float32)
+                assert a.shape == tuple(shape), (module, name, a.shape, shape)
+                parts.append(a.reshape(-1))
+    return np.ascontiguousarray(np.concatenate(parts))
+
+
+def make_extra_inputs(seed: int, B: int, S: int, N: int, d: ExtraDims = EXTRA, lengths=None, msa_mask_frac_max: float = 0.0):
+    """e[B,S,N,c_e], z[B,N,N,c_z] ~ N(0,1) (garbage in the padding) and the masks of make_inputs."""
+    main = Dims(c_m=d.c_e, c_z=d.c_z)
+    return make_inputs(seed, B, S, N, main, lengths=lengths, msa_mask_frac_max=msa_mask_frac_max)
