@@ -183,6 +183,48 @@ pf_status pf_evoformer_forward_recycled(pf_evoformer_t* h, pf_embedder_t* e, con
                                         int B, int S, int N, int n_blocks, int n_cycles, void* cuda_stream);
 
 /* ------------------------------------------------------------------------------------------------
+ * Extra-MSA stack: the Evoformer block at c_e = 64 MSA channels with GLOBAL column attention over an MSA
+ * of thousands of sequences, updating the same pair representation (part of the network the paper's GPU stage runs,
+ * PAPER.md:61; AlphaFold v2.0.1 CASP14 preset).  PAPER.md prints no formula; readings X.1-X.9:
+ *   X.1 MSA row attention with pair bias (A.1 at c_e channels, heads of dimension c_e / heads_msa)
+ *   X.2 MSA column global attention: x = LN(e); qbar_i = sum_s mu_si x_si / (sum_s mu_si + 1e-10); q[i,h] = Lin0(qbar_i)_h / sqrt(d);
+ *       ONE key / value head k[s,i], v[s,i] in R^d; P = softmax_s(q[i,h].k[s,i] + NEG(mu_si)); o[i,h] = sum_s P v[s,i];
+ *       e[s,i] += Lin_o( sigmoid(Lin_g(x_si)) (.) concat_h o[i,h] )
+ *   X.3 MSA transition (A.3 at c_e), X.4 outer-product-mean (A.4 from e into pair), X.5-X.9 the pair stack A.5-A.9.
+ * 16-bit operands with fp32 accumulation and fp32 residual streams as PF_BF16 (X.2 runs in fp32).  Same conventions, masks
+ * (R2, R3), in-place semantics and error behaviour as pf_evoformer_forward.  Limits: N <= 1024, N_seq <= ~2900, B <= 511.
+ * Weights blob: n_blocks_max blocks of pf_extra_msa_block_floats values, the Appendix-B order at c_m = c_e with the column
+ * attention's entry replaced by: LN gamma beta [c_e], W_q [c_e,c_e], W_k [c_e,d], W_v [c_e,d], W_g [c_e,c_e], b_g, W_o [c_e,c_e], b_o.
+ * ---------------------------------------------------------------------------------------------- */
+typedef struct pf_extra_msa pf_extra_msa_t;
+typedef struct {
+  int c_e;            /* extra-MSA channels (64) */
+  int c_z;            /* pair channels (128) */
+  int heads_msa;      /* 8 heads of dimension c_e / heads_msa = 8 */
+  int heads_pair;     /* 4 */
+  int head_dim_pair;  /* 32 */
+  int c_opm;          /* 32 */
+  int c_tri;          /* 128 */
+  int transition_n;   /* 4 */
+  int n_blocks_max;   /* blocks in the blob (4 in AlphaFold) */
+} pf_extra_config;
+size_t pf_extra_msa_block_floats(const pf_extra_config* cfg);
+pf_status pf_extra_msa_create(pf_extra_msa_t** out, const float* weights_host, size_t n_weight_floats,
+                              const pf_extra_config* cfg);
+/* blocks [0, n_blocks) on dev extra_msa[B,S,N,c_e] and dev pair[B,N,N,c_z], in place, asynchronously on cuda_stream */
+pf_status pf_extra_msa_forward(pf_extra_msa_t* x, float* extra_msa_dev, float* pair_dev, const float* seq_mask_dev,
+                               const float* extra_msa_mask_dev, int B, int S, int N, int n_blocks, void* cuda_stream);
+/* test hook: sub-step `substep` (1..9 = X.1..X.9) of block `block` */
+pf_status pf_extra_msa_forward_substep(pf_extra_msa_t* x, float* extra_msa_dev, float* pair_dev, const float* seq_mask_dev,
+                                       const float* extra_msa_mask_dev, int B, int S, int N, int block, int substep,
+                                       void* cuda_stream);
+long long pf_extra_msa_last_launch_count(const pf_extra_msa_t* x);
+/* per-launch timing as pf_evoformer_set_profiling / pf_evoformer_get_profile (same kinds) */
+pf_status pf_extra_msa_set_profiling(pf_extra_msa_t* x, int enable);
+pf_status pf_extra_msa_get_profile(pf_extra_msa_t* x, int kind, long long* launches, double* ms, double* flops, double* bytes);
+void pf_extra_msa_destroy(pf_extra_msa_t* x);
+
+/* ------------------------------------------------------------------------------------------------
  * Length-bucketing batch scheduler ("sort by length ... share the compiled model";
  * SURVEY.md §3(iv)).  Host only.  Proteins are sorted by descending length (largest first, as the paper
  * compiles for the largest), assigned to the smallest bucket >= length, and cut into batches of at most

@@ -29,6 +29,8 @@ EXPORTED_SYMBOLS = (
     "pf_sched_bytes_per_protein", "pf_sched_cost", "pf_sched_partition", "pf_sched_destroy",
     "pf_embedder_floats", "pf_embedder_create", "pf_embedder_forward", "pf_embedder_last_launch_count", "pf_embedder_destroy",
     "pf_evoformer_forward_recycled",
+    "pf_extra_msa_block_floats", "pf_extra_msa_create", "pf_extra_msa_forward", "pf_extra_msa_forward_substep",
+    "pf_extra_msa_last_launch_count", "pf_extra_msa_set_profiling", "pf_extra_msa_get_profile", "pf_extra_msa_destroy",
 )
 
 
@@ -41,6 +43,11 @@ class PfConfig(Structure):
 class PfEmbedConfig(Structure):
     _fields_ = [("c_m", c_int), ("c_z", c_int), ("tf_dim", c_int), ("msa_dim", c_int), ("max_relpos", c_int),
                 ("n_dist_bins", c_int), ("first_break", c_float), ("last_break", c_float)]
+
+
+class PfExtraConfig(Structure):
+    _fields_ = [("c_e", c_int), ("c_z", c_int), ("heads_msa", c_int), ("heads_pair", c_int), ("head_dim_pair", c_int),
+                ("c_opm", c_int), ("c_tri", c_int), ("transition_n", c_int), ("n_blocks_max", c_int)]
 
 
 class PfError(RuntimeError):
@@ -116,6 +123,23 @@ def lib() -> ctypes.CDLL:
         L.pf_embedder_last_launch_count.argtypes = [c_void_p]
         L.pf_embedder_destroy.restype = None
         L.pf_embedder_destroy.argtypes = [c_void_p]
+        L.pf_extra_msa_block_floats.restype = c_size_t
+        L.pf_extra_msa_block_floats.argtypes = [POINTER(PfExtraConfig)]
+        L.pf_extra_msa_create.restype = c_int
+        L.pf_extra_msa_create.argtypes = [POINTER(c_void_p), c_void_p, c_size_t, POINTER(PfExtraConfig)]
+        L.pf_extra_msa_forward.restype = c_int
+        L.pf_extra_msa_forward.argtypes = fwd + [c_int, c_void_p]
+        L.pf_extra_msa_forward_substep.restype = c_int
+        L.pf_extra_msa_forward_substep.argtypes = fwd + [c_int, c_int, c_void_p]
+        L.pf_extra_msa_last_launch_count.restype = c_longlong
+        L.pf_extra_msa_last_launch_count.argtypes = [c_void_p]
+        L.pf_extra_msa_set_profiling.restype = c_int
+        L.pf_extra_msa_set_profiling.argtypes = [c_void_p, c_int]
+        L.pf_extra_msa_get_profile.restype = c_int
+        L.pf_extra_msa_get_profile.argtypes = [c_void_p, c_int, POINTER(c_longlong), POINTER(ctypes.c_double),
+                                               POINTER(ctypes.c_double), POINTER(ctypes.c_double)]
+        L.pf_extra_msa_destroy.restype = None
+        L.pf_extra_msa_destroy.argtypes = [c_void_p]
         L.pf_evoformer_forward_recycled.restype = c_int
         L.pf_evoformer_forward_recycled.argtypes = [c_void_p] * 10 + [c_int] * 5 + [c_void_p]
         _lib = L
@@ -209,6 +233,64 @@ class Evoformer:
         if self._h:
             lib().pf_evoformer_destroy(self._h)
             self._h = c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def make_extra_config(n_blocks_max: int, c_e=64, c_z=128, heads_msa=8, heads_pair=4, head_dim_pair=32, c_opm=32, c_tri=128,
+                      transition_n=4) -> PfExtraConfig:
+    return PfExtraConfig(c_e, c_z, heads_msa, heads_pair, head_dim_pair, c_opm, c_tri, transition_n, n_blocks_max)
+
+
+class ExtraMsaStack:
+    """pf_extra_msa_* wrapper (pointers and sizes only)."""
+
+    def __init__(self, weights_blob: np.ndarray, cfg: PfExtraConfig):
+        blob = np.ascontiguousarray(weights_blob, dtype=np.float32)
+        self._x = c_void_p()
+        self.cfg = cfg
+        _check(lib().pf_extra_msa_create(byref(self._x), blob.ctypes.data, blob.size, byref(cfg)))
+
+    @staticmethod
+    def _stream(stream):
+        if stream is None:
+            import torch
+            return torch.cuda.current_stream().cuda_stream
+        return stream
+
+    def forward(self, extra_msa, pair, seq_mask, extra_msa_mask, n_blocks: int, stream=None):
+        B, S, N = extra_msa.shape[0], extra_msa.shape[1], extra_msa.shape[2]
+        _check(lib().pf_extra_msa_forward(self._x, _ptr(extra_msa), _ptr(pair), _ptr(seq_mask), _ptr(extra_msa_mask),
+                                          B, S, N, n_blocks, self._stream(stream)))
+
+    def forward_substep(self, extra_msa, pair, seq_mask, extra_msa_mask, block: int, substep: int, stream=None):
+        B, S, N = extra_msa.shape[0], extra_msa.shape[1], extra_msa.shape[2]
+        _check(lib().pf_extra_msa_forward_substep(self._x, _ptr(extra_msa), _ptr(pair), _ptr(seq_mask), _ptr(extra_msa_mask),
+                                                  B, S, N, block, substep, self._stream(stream)))
+
+    def set_profiling(self, enable: bool):
+        _check(lib().pf_extra_msa_set_profiling(self._x, 1 if enable else 0))
+
+    def get_profile(self) -> dict:
+        out = {}
+        for k in range(lib().pf_evoformer_profile_kinds()):
+            n, ms, fl, by = c_longlong(), ctypes.c_double(), ctypes.c_double(), ctypes.c_double()
+            _check(lib().pf_extra_msa_get_profile(self._x, k, byref(n), byref(ms), byref(fl), byref(by)))
+            out[lib().pf_evoformer_profile_name(k).decode()] = {
+                "launches": n.value, "ms": ms.value, "flops": fl.value, "bytes": by.value}
+        return out
+
+    def last_launch_count(self) -> int:
+        return int(lib().pf_extra_msa_last_launch_count(self._x))
+
+    def close(self):
+        if self._x:
+            lib().pf_extra_msa_destroy(self._x)
+            self._x = c_void_p()
 
     def __del__(self):
         try:

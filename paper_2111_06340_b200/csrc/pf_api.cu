@@ -92,7 +92,7 @@ extern "C" size_t pf_evoformer_block_floats(const pf_config* cfg) {
   return block_offsets(*cfg).total;
 }
 
-static const char* const kKindNames[KK_COUNT] = {"ln_rows", "gemm", "attn_core", "tri_einsum", "ln_channels", "opm_core", "ln_gemm", "transition", "mask_flags"};
+static const char* const kKindNames[KK_COUNT] = {"ln_rows", "gemm", "attn_core", "tri_einsum", "ln_channels", "opm_core", "ln_gemm", "transition", "mask_flags", "global_col_attn", "embedders"};
 
 
 Arena pf::arena_layout(const pf_config& c, int B, int S, int N) {
@@ -506,6 +506,12 @@ static pf_status check_and_grow(pf_evoformer* h, int B, int S, int N, cudaStream
     h->ws_B = B; h->ws_S = S; h->ws_N = N;
   }
   return PF_OK;
+}
+
+bool pf::ensure_workspace(pf_evoformer* h, int B, int S, int N, cudaStream_t st, std::string& err) {
+  if (check_and_grow(h, B, S, N, st) == PF_OK) return true;
+  err = g_err;
+  return false;
 }
 
 // Largest batch one launch sequence takes: gridDim.z of the per-(protein, channel) and per-(protein, row) kernels is capped

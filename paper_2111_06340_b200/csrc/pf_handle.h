@@ -58,7 +58,7 @@ TcBlock tc_layout(const pf_config& c);
 void build_tc_block(const pf_config& c, const BlockW& off, const TcBlock& t, const float* w, std::vector<uint16_t>& w16,
                     size_t base16, std::vector<float>& wf, size_t basef, F16Range* range);
 
-enum KernelKind { KK_LN = 0, KK_GEMM, KK_ATTN, KK_TRI, KK_LNC, KK_OPM, KK_LNGEMM, KK_TRANS, KK_FLAGS, KK_COUNT };
+enum KernelKind { KK_LN = 0, KK_GEMM, KK_ATTN, KK_TRI, KK_LNC, KK_OPM, KK_LNGEMM, KK_TRANS, KK_FLAGS, KK_GLOBAL, KK_EMBED, KK_COUNT };
 
 inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 inline int pad8(int v) { return (v + 7) / 8 * 8; }
@@ -130,6 +130,47 @@ struct pf_evoformer {
 };
 
 namespace pf {
+// ---- extra-MSA stack (pf_extra.cu, readings X.1-X.9) ----
+// offsets (floats) within one extra-MSA block of its fp32 blob (the order of pf_synth.extra_block_spec)
+struct GlobalColW {
+  size_t ln_g, ln_b, wq, wk, wv, wg, bg, wo, bo;
+};
+struct ExtraOff {
+  AttnW row;                 // c = c_e, with LN'(z) and the pair-bias projection
+  GlobalColW col;
+  TransW msa_trans;
+  OpmW opm;
+  TriMulW tri_out, tri_in;
+  AttnW tri_start, tri_end;
+  TransW pair_trans;
+  size_t total;
+};
+// prepared device matrices of the MSA-side modules of one extra block: 16-bit offsets / fp32 offsets
+struct ExtraT {
+  size_t row_w_in;           // fp16 [4 * 32 H, c_e]: q | k | gate | v with every head zero-padded from c_e / H to 32 rows
+  size_t row_wo;             // bf16 [c_e, 32 H]
+  size_t tr_w1, tr_w2;       // fp16 [4 c_e, c_e], bf16 [c_e, 4 c_e]
+  size_t opm_wab;            // fp16 [2 c_opm, c_e]
+  size_t total16;
+  size_t row_b_in;           // fp32 [4 * 32 H]: gate bias in its (padded) column range
+  size_t opm_bias_ab;        // fp32 [2 c_opm]
+  size_t total_f32;
+};
+struct ExtraBlockDev {
+  const float* w32;          // fp32 blob of this extra block (LayerNorm parameters, biases, the global attention's matrices)
+  const uint16_t* w16;
+  const float* wf;
+  float* o_glob;             // [B, N, c_e] scratch of the global column attention
+  int c_e, heads, head_dim;
+};
+void launch_extra_global_col(float* e, const float* seq_mask, const float* msa_mask, const float* w32, const GlobalColW& o,
+                             float* o_glob, int B, int S, int N, int c_e, int heads, cudaStream_t st);
+bool tc_run_extra_substep(pf_evoformer* inner, const ExtraOff& xo, const ExtraT& xt, const ExtraBlockDev& xb, float* e,
+                          float* pair, const float* seq_mask, const float* msa_mask, int B, int S, int N, int block, int step,
+                          cudaStream_t st, std::string& err);
+// workspace of `h` for (B, S, N): grown and, when the shape changed, zero-filled in stream order (pf_api.cu)
+bool ensure_workspace(pf_evoformer* h, int B, int S, int N, cudaStream_t st, std::string& err);
+
 // tcgen05 path: one sub-step (1..9) of block `block`; returns false and sets err on failure.
 // mask-derived work flags for one forward call (launched once, before the first block)
 bool tc_prepare_flags(pf_evoformer* h, const float* seq_mask, const float* msa_mask, int B, int S, int N, cudaStream_t st);

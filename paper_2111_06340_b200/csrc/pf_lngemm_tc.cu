@@ -781,7 +781,8 @@ static bool configure_g2() {
   return e == cudaSuccess;
 }
 bool configure_gemm2_kernels() {
-  return configure_g2<128, 0>() && configure_g2<128, 1>() && configure_g2<256, 0>() && configure_g2<256, 1>();
+  return configure_g2<128, 0>() && configure_g2<128, 1>() && configure_g2<256, 0>() && configure_g2<256, 1>() &&
+         configure_g2<64, 0>();
 }
 
 #ifdef PF_G2_TRACE
@@ -798,8 +799,8 @@ extern "C" int pf_debug_g2_trace(unsigned long long* out, int reset) {
 #endif
 
 int launch_gemm2(TmaCtx* ctx, const G2Desc& d, int num_sms, cudaStream_t st) {
-  if (d.K != 128 && d.K != 256) {
-    tc_set_error("gemm2: K must be 128 or 256");
+  if (d.K != 128 && d.K != 256 && !(d.K == 64 && d.a_mode == 0)) {
+    tc_set_error("gemm2: K must be 128 or 256 (or 64 for a LayerNorm-fed GEMM: the extra-MSA stack)");
     return -1;
   }
   G2Params p;
@@ -943,6 +944,7 @@ int launch_gemm2(TmaCtx* ctx, const G2Desc& d, int num_sms, cudaStream_t st) {
   } else {
     tmR = tmW;
   }
+  if (d.K == 64) return launch_g2<64, 0>(tmW, tmA, tmO0, tmT[0], tmT[1], tmH, tmR, tmVS, p, num_sms, st);
   if (d.K == 128) {
     return d.a_mode == 0 ? launch_g2<128, 0>(tmW, tmA, tmO0, tmT[0], tmT[1], tmH, tmR, tmVS, p, num_sms, st)
                          : launch_g2<128, 1>(tmW, tmA, tmO0, tmT[0], tmT[1], tmH, tmR, tmVS, p, num_sms, st);

@@ -38,7 +38,7 @@ struct OpmSmem {
 __global__ void __launch_bounds__(OP_THREADS, 1)
 opm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
               const __grid_constant__ CUtensorMap tmW, const float* __restrict__ bout, const float* __restrict__ seq_mask,
-              const float* __restrict__ msa_mask, float* __restrict__ z, int S, int N) {
+              const float* __restrict__ msa_mask, float* __restrict__ z, int S, int N, int s0, int Sc, int add_bias) {
   using SM = OpmSmem;
   {
     // both residues j of this CTA padded: every output is at a masked position (uniform over the CTA: exit before any setup)
@@ -64,7 +64,9 @@ opm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ C
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int j0 = blockIdx.x * OP_BJ, i0 = blockIdx.y * OP_BI, b = blockIdx.z;
-  const int n_kb = (S + OP_BK - 1) / OP_BK;
+  // this launch contracts the sequences [s0, s0 + Sc) (Sc <= 512: the b operand of the chunk stays resident in shared memory);
+  // the normaliser counts all S sequences, and the chunks add up because the projection is linear (bias with the first chunk)
+  const int n_kb = (Sc + OP_BK - 1) / OP_BK;
 
   if (warp == 0 && lane == 0) {
     tc::prefetch_tmap(&tmA);
@@ -98,14 +100,14 @@ opm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ C
     if (tc::elect_one()) {
       tc::mbar_arrive_expect_tx(b_full, (uint32_t)n_kb * SM::B_KB_BYTES);
       for (int kb = 0; kb < n_kb; ++kb)
-        tc::tma_load_3d(smem + SM::B_OFF + kb * SM::B_KB_BYTES, &tmB, b_full, kb * OP_BK, OP_C, b * N + j0);
+        tc::tma_load_3d(smem + SM::B_OFF + kb * SM::B_KB_BYTES, &tmB, b_full, s0 + kb * OP_BK, OP_C, b * N + j0);
       int it = 0;
       for (int c1 = 0; c1 < OP_C; ++c1) {
         for (int kb = 0; kb < n_kb; ++kb, ++it) {
           int s = it % OP_A_STAGES;
           tc::mbar_wait(&a_empty[s], ((it / OP_A_STAGES) & 1) ^ 1);
           tc::mbar_arrive_expect_tx(&a_full[s], SM::A_BYTES);
-          tc::tma_load_3d(smem + SM::A_OFF + s * SM::A_BYTES, &tmA, &a_full[s], kb * OP_BK, c1, b * N + i0);
+          tc::tma_load_3d(smem + SM::A_OFF + s * SM::A_BYTES, &tmA, &a_full[s], s0 + kb * OP_BK, c1, b * N + i0);
         }
         int ws = c1 & 1;
         tc::mbar_wait(&w_empty[ws], ((c1 >> 1) & 1) ^ 1);
@@ -211,7 +213,7 @@ opm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ C
 #pragma unroll
           for (int e = 0; e < 32; e += 4) {
             float4 o = *reinterpret_cast<float4*>(dst + c0 + e);
-            float4 bo = __ldg(reinterpret_cast<const float4*>(bout + c0 + e));
+            float4 bo = add_bias ? __ldg(reinterpret_cast<const float4*>(bout + c0 + e)) : make_float4(0.f, 0.f, 0.f, 0.f);
             o.x += __uint_as_float(v[e]) * inv + bo.x;
             o.y += __uint_as_float(v[e + 1]) * inv + bo.y;
             o.z += __uint_as_float(v[e + 2]) * inv + bo.z;
@@ -235,10 +237,6 @@ bool configure_opm_kernel() {
 
 int launch_opm_tc(TmaCtx* ctx, const bf16* ab_t, const bf16* wout_t, const float* bout, const float* seq_mask,
                   const float* msa_mask, float* z, int B, int S, int Spad, int N, cudaStream_t st) {
-  if (S > OP_MAX_KB * OP_BK) {
-    tc_set_error("opm_tc: N_seq above 512 not supported");
-    return -1;
-  }
   CUtensorMap tmA, tmB, tmW;
   uint64_t d[3] = {(uint64_t)S, 2 * OP_C, (uint64_t)B * N}, s[2] = {(uint64_t)Spad, (uint64_t)2 * OP_C * Spad};
   uint32_t bxA[3] = {OP_BK, 1, OP_BI}, bxB[3] = {OP_BK, OP_C, OP_BJ};
@@ -248,7 +246,10 @@ int launch_opm_tc(TmaCtx* ctx, const bf16* ab_t, const bf16* wout_t, const float
   uint32_t bxW[2] = {OP_C, OP_CZ};
   if (tma_encode_bf16(ctx, &tmW, wout_t, 2, dw, sw, bxW, 64) != 0) return -1;
   dim3 grid((N + OP_BJ - 1) / OP_BJ, (N + OP_BI - 1) / OP_BI, B);
-  opm_tc_kernel<<<grid, OP_THREADS, OpmSmem::TOTAL, st>>>(tmA, tmB, tmW, bout, seq_mask, msa_mask, z, S, N);
+  const int chunk = OP_MAX_KB * OP_BK;   // 512 sequences per launch; the extra-MSA stack (S in the thousands) takes several
+  for (int s0 = 0; s0 < S; s0 += chunk)
+    opm_tc_kernel<<<grid, OP_THREADS, OpmSmem::TOTAL, st>>>(tmA, tmB, tmW, bout, seq_mask, msa_mask, z, S, N, s0,
+                                                            S - s0 < chunk ? S - s0 : chunk, s0 == 0 ? 1 : 0);
   return 0;
 }
 

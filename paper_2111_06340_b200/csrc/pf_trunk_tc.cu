@@ -9,6 +9,7 @@
 #include "pf_handle.h"
 
 #include <algorithm>
+#include <cmath>
 #include <cstring>
 #include <vector>
 
@@ -145,6 +146,7 @@ namespace {
 constexpr float kLog2e = 1.4426950408889634f;
 
 struct TcDriver {
+  typedef G2Desc G2Desc_;
   pf_evoformer* h;
   cudaStream_t st;
   int B, S, N;
@@ -192,7 +194,23 @@ struct TcDriver {
   // Gated attention sub-step on a residual stream `res` viewed as rows (b, x in D1, y in D2), attention along y.
   //   transposed: rows are gathered from / scattered to the (b, y, x) layout of `res`  (A.2, A.8 via their identities)
   //   f_rows: active-tile flags of this row geometry; rl_off / rl_idx: the compacted row list of this attention (pf_flags.cu)
-  bool attn_substep(float* res, int C, int H, int D1, int D2, bool transposed, const AttnW& a, const AttnT& at,
+  // Where one attention's own parameters live: the handle's blobs for the main block, the extra-MSA stack's own buffers for
+  // its row attention (there the residual stream has Kin = c_e = 64 channels while the attention runs on C = H x 32 columns:
+  // heads of dimension 8 zero-padded to the 32 the attention core is built for).
+  struct AttnPar {
+    int Kin;                          // channels of the residual stream = LayerNorm width = reduction length of the projection
+    const float *ln_g, *ln_b;
+    const void* w_in;                 // fp16 [4C (+H), Kin]
+    const float* b_in;                // fp32 [4C (+H)]
+    const void* wo;                   // bf16 [Kin, C]
+    const float* bo;                  // fp32 [Kin]
+    float qscale;                     // 1 / sqrt(head dimension)  (R12)
+  };
+  AttnPar main_par(int C, const AttnW& a, const AttnT& at) const {
+    return AttnPar{C, w + a.ln_g, w + a.ln_b, w16 + at.w_in, wf + at.b_in, w16 + at.wo, w + a.bo, 0.17677669529663687f};
+  }
+
+  bool attn_substep(float* res, int C, int H, int D1, int D2, bool transposed, const AttnW& a, const AttnPar& px,
                     const float* keymask, bool row_bias, bool self_bias, size_t f_rows, size_t rl_off, int rl_idx) {
     const double f_frac = rl_idx == 0 ? h->frac.msa : rl_idx == 1 ? h->frac.msat : h->frac.pair;
     const double a_frac = rl_idx == 0 ? h->frac.attn_row : rl_idx == 1 ? h->frac.attn_col : h->frac.attn_tri;
@@ -216,9 +234,9 @@ struct TcDriver {
     }
     {
       const int Nw = 4 * C + (self_bias ? H : 0);
-      G2Desc d = desc_base(B, D1, D2, C, Nw);
-      d.src = res; d.src_transposed = transposed ? 1 : 0; d.gamma = w + a.ln_g; d.beta = w + a.ln_b;
-      d.op_fmt = 1; d.Wt = w16 + at.w_in; d.bias = wf + at.b_in;
+      G2Desc d = desc_base(B, D1, D2, px.Kin, Nw);
+      d.src = res; d.src_transposed = transposed ? 1 : 0; d.gamma = px.ln_g; d.beta = px.ln_b;
+      d.op_fmt = 1; d.Wt = px.w_in; d.bias = px.b_in;
       d.bias_lo = 2 * C; d.bias_n = C;   // only the gate columns carry a bias (R7)
       d.row_out[0] = QKG; d.row_ld[0] = 3 * C;
       d.vt_out = VT; d.vt_cols = C; d.Lpad = Lp;
@@ -228,7 +246,7 @@ struct TcDriver {
         int seg = col / C;
         if (seg < 3) {
           d.ops[n] = op(G2_ROW16, col);
-          if (seg == 0) d.ops[n].scale = 0.17677669529663687f * kLog2e;   // log2(e)/sqrt(32)  (R12)
+          if (seg == 0) d.ops[n].scale = px.qscale * kLog2e;   // log2(e)/sqrt(d)  (R12)
           if (seg == 2) { d.ops[n].act = ACT_SIGMOID; d.ops[n].fmt = 1; }
         } else if (g2_pick_yt(D2) >= 64) {
           // V^T comes out of the MMA already transposed: the half-window holding these columns is computed operand-swapped
@@ -257,14 +275,14 @@ struct TcDriver {
       }
       h->prof_end(st);
     }
-    G2Desc d = desc_base(B, D1, D2, C, C);
-    d.a_mode = 1; d.A = O; d.op_fmt = 0; d.Wt = w16 + at.wo; d.bias = w + a.bo;
-    d.resid = res; d.resid_ld = C; d.resid_transposed = transposed ? 1 : 0;
+    G2Desc d = desc_base(B, D1, D2, C, px.Kin);
+    d.a_mode = 1; d.A = O; d.op_fmt = 0; d.Wt = px.wo; d.bias = px.bo;
+    d.resid = res; d.resid_ld = px.Kin; d.resid_transposed = transposed ? 1 : 0;
     int n = 0;
-    for (int col = 0; col < C; col += 64) d.ops[n++] = op(G2_RESID, col);
+    for (int col = 0; col < px.Kin; col += 64) d.ops[n++] = op(G2_RESID, col);
     d.n_ops = n;
     d.tile_active = flags(f_rows);
-    return gemm2(d, R * C * 8.0, f_frac);
+    return gemm2(d, R * px.Kin * 8.0, f_frac);
   }
 
   // A.3 / A.9: one fused kernel, the 4C-wide hidden activation stays on chip
@@ -284,10 +302,6 @@ struct TcDriver {
   bool opm_substep() {
     const pf_config& c = h->cfg;
     const OpmW& o = h->off.opm;
-    if (S > 512) {
-      err = "opm_tc: N_seq above 512 not supported on the tensor-core path";
-      return false;
-    }
     const double M = (double)B * S * N, P = (double)B * N * N, cc = (double)c.c_opm * c.c_opm;
     const int Sp = pad8(S);
     bf16* ABT = buf<bf16>(ar.vt);
@@ -491,6 +505,88 @@ bool tc_prepare_flags(pf_evoformer* h, const float* seq_mask, const float* msa_m
   return cudaGetLastError() == cudaSuccess;
 }
 
+// Extra-MSA stack, MSA-side sub-steps 1-4 of one block (5-9 are the main block's pair stack on the inner handle).  The
+// residual stream e has c_e = 64 channels; its row attention runs on H x 32 = 256 columns (heads zero-padded 8 -> 32), so all
+// intermediates have the main block's shapes and live in the inner handle's arena.
+bool tc_run_extra_substep(pf_evoformer* h, const ExtraOff& xo, const ExtraT& xt, const ExtraBlockDev& xb, float* e, float* pair,
+                          const float* seq_mask, const float* msa_mask, int B, int S, int N, int block, int step,
+                          cudaStream_t st, std::string& err) {
+  const pf_config& c = h->cfg;
+  if (step >= 5) return tc_run_substep(h, e, pair, seq_mask, msa_mask, B, S, N, block, step, st, err);
+  TcDriver d;
+  d.h = h; d.st = st; d.B = B; d.S = S; d.N = N;
+  d.msa = e; d.pair = pair; d.seq_mask = seq_mask; d.msa_mask = msa_mask;
+  d.ar = arena_layout(c, B, S, N);
+  d.w = h->w32 + (size_t)block * h->off.total;
+  d.w16 = h->w16 + (size_t)block * h->tc.total16;
+  d.wf = h->wf + (size_t)block * h->tc.total_f32;
+  const int ce = xb.c_e, H = xb.heads, C = 32 * H;
+  const double M = (double)B * S * N;
+  bool ok = false;
+  if (step == 1) {
+    TcDriver::AttnPar px{ce, xb.w32 + xo.row.ln_g, xb.w32 + xo.row.ln_b, xb.w16 + xt.row_w_in, xb.wf + xt.row_b_in,
+                         xb.w16 + xt.row_wo, xb.w32 + xo.row.bo, 1.0f / sqrtf((float)xb.head_dim)};
+    // LN'(z) and the pair-bias projection of this block sit in the inner handle's blob (same shapes as the main block's)
+    ok = d.attn_substep(e, C, H, S, N, false, h->off.row, px, seq_mask, true, false, d.ar.f_msa, d.ar.rl_row, 0);
+  } else if (step == 2) {
+    h->prof_begin(KK_GLOBAL, 2.0 * M * ce * (2.0 * ce + 2.0 * xb.head_dim), M * ce * 12.0, st);
+    launch_extra_global_col(e, seq_mask, msa_mask, xb.w32, xo.col, xb.o_glob, B, S, N, ce, H, st);
+    h->prof_end(st);
+    h->launches += 1;   // two kernels
+    ok = true;
+  } else if (step == 3) {
+    // X.3 unfused: LN(e) W1 + b1 -> relu -> bf16 hidden [M, 4 c_e] in the arena; hidden W2 + b2 reduce-added into e
+    const int n4 = c.transition_n * ce;
+    bf16* Hb = d.buf<bf16>(d.ar.o);
+    TcDriver::G2Desc_ g1 = TcDriver::desc_base(B, S, N, ce, n4);
+    g1.src = e; g1.gamma = xb.w32 + xo.msa_trans.ln_g; g1.beta = xb.w32 + xo.msa_trans.ln_b;
+    g1.op_fmt = 1; g1.Wt = xb.w16 + xt.tr_w1; g1.bias = xb.w32 + xo.msa_trans.b1;
+    g1.row_out[0] = Hb; g1.row_ld[0] = n4;
+    int n = 0;
+    for (int col = 0; col < n4; col += 64, ++n) {
+      g1.ops[n] = TcDriver::op(G2_ROW16, col);
+      g1.ops[n].act = ACT_RELU;
+    }
+    g1.n_ops = n;
+    g1.tile_active = d.flags(d.ar.f_msa);
+    if (!d.gemm2(g1, M * n4 * 2.0, h->frac.msa)) { err = d.err; return false; }
+    TcDriver::G2Desc_ g2 = TcDriver::desc_base(B, S, N, n4, ce);
+    g2.a_mode = 1; g2.A = Hb; g2.op_fmt = 0; g2.Wt = xb.w16 + xt.tr_w2; g2.bias = xb.w32 + xo.msa_trans.b2;
+    g2.resid = e; g2.resid_ld = ce;
+    g2.ops[0] = TcDriver::op(G2_RESID, 0);
+    g2.n_ops = 1;
+    g2.tile_active = d.flags(d.ar.f_msa);
+    ok = d.gemm2(g2, M * ce * 8.0, h->frac.msa);
+  } else if (step == 4) {
+    const double P = (double)B * N * N, cc = (double)c.c_opm * c.c_opm;
+    const int Sp = pad8(S);
+    bf16* ABT = d.buf<bf16>(d.ar.vt);
+    TcDriver::G2Desc_ g = TcDriver::desc_base(B, N, S, ce, 2 * c.c_opm);
+    g.src = e; g.src_transposed = 1; g.gamma = xb.w32 + xo.opm.ln_g; g.beta = xb.w32 + xo.opm.ln_b;
+    g.op_fmt = 1; g.Wt = xb.w16 + xt.opm_wab; g.bias = xb.wf + xt.opm_bias_ab;
+    g.rowmask = RM_MSA; g.seq_mask = seq_mask; g.msa_mask = msa_mask; g.mask_transposed = 1;
+    g.vt_out = ABT; g.vt_cols = 2 * c.c_opm; g.Lpad = Sp;
+    g.ops[0] = TcDriver::op(G2_VT, 0, 2 * c.c_opm);
+    g.ops[0].masked = 1;
+    g.n_ops = 1;
+    g.tile_active = d.flags(d.ar.f_msat_x);
+    if (!d.gemm2(g, M * 2.0 * c.c_opm * 2.0, h->frac.msat_x)) { err = d.err; return false; }
+    h->prof_begin(KK_OPM, (2.0 * P * cc * S + 2.0 * P * cc * c.c_z) * h->frac.opm,
+                  (2.0 * M * c.c_opm * 2.0 + 8.0 * P * c.c_z) * h->frac.opm, st);
+    if (launch_opm_tc(h->tma, ABT, reinterpret_cast<const bf16*>(d.w16 + h->tc.opm_wout), d.w + h->off.opm.bout, seq_mask,
+                      msa_mask, pair, B, S, Sp, N, st) != 0) {
+      err = std::string("opm_tc: ") + tc_last_error();
+      return false;
+    }
+    h->prof_end(st);
+    ok = true;
+  } else {
+    d.err = "substep not in 1..9";
+  }
+  if (!ok) err = d.err;
+  return ok;
+}
+
 bool tc_run_substep(pf_evoformer* h, float* msa, float* pair, const float* seq_mask, const float* msa_mask, int B, int S,
                     int N, int block, int step, cudaStream_t st, std::string& err) {
   const pf_config& c = h->cfg;
@@ -503,17 +599,17 @@ bool tc_run_substep(pf_evoformer* h, float* msa, float* pair, const float* seq_m
   d.wf = h->wf + (size_t)block * h->tc.total_f32;
   bool ok = false;
   switch (step) {
-    case 1: ok = d.attn_substep(msa, c.c_m, c.heads_msa, S, N, false, h->off.row, h->tc.row, seq_mask, true, false, d.ar.f_msa,
+    case 1: ok = d.attn_substep(msa, c.c_m, c.heads_msa, S, N, false, h->off.row, d.main_par(c.c_m, h->off.row, h->tc.row), seq_mask, true, false, d.ar.f_msa,
                                 d.ar.rl_row, 0); break;
-    case 2: ok = d.attn_substep(msa, c.c_m, c.heads_msa, N, S, true, h->off.col, h->tc.col, msa_mask, false, false, d.ar.f_msat,
+    case 2: ok = d.attn_substep(msa, c.c_m, c.heads_msa, N, S, true, h->off.col, d.main_par(c.c_m, h->off.col, h->tc.col), msa_mask, false, false, d.ar.f_msat,
                                 d.ar.rl_col, 1); break;
     case 3: ok = d.transition_substep(msa, S, N, c.c_m, h->off.msa_trans, h->tc.mt_w1, h->tc.mt_w2, d.ar.f_msa_lin); break;
     case 4: ok = d.opm_substep(); break;
     case 5: ok = d.trimul_substep(false); break;
     case 6: ok = d.trimul_substep(true); break;
-    case 7: ok = d.attn_substep(pair, c.c_z, c.heads_pair, N, N, false, h->off.tri_start, h->tc.tri_start, seq_mask, false,
+    case 7: ok = d.attn_substep(pair, c.c_z, c.heads_pair, N, N, false, h->off.tri_start, d.main_par(c.c_z, h->off.tri_start, h->tc.tri_start), seq_mask, false,
                                 true, d.ar.f_pair, d.ar.rl_tri, 2); break;
-    case 8: ok = d.attn_substep(pair, c.c_z, c.heads_pair, N, N, true, h->off.tri_end, h->tc.tri_end, seq_mask, false,
+    case 8: ok = d.attn_substep(pair, c.c_z, c.heads_pair, N, N, true, h->off.tri_end, d.main_par(c.c_z, h->off.tri_end, h->tc.tri_end), seq_mask, false,
                                 true, d.ar.f_pair, d.ar.rl_tri, 2); break;
     case 9: ok = d.transition_substep(pair, N, N, c.c_z, h->off.pair_trans, h->tc.pt_w1, h->tc.pt_w2, d.ar.f_pair_lin); break;
     default: d.err = "substep not in 1..9";
