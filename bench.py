@@ -320,35 +320,47 @@ def side_workload(h, ps, torch, dev, name, peaks, steps=3, warmup=3):
             "roofline": roof, "kernels": table}
 
 
-def recycled_workload(h, pf, ps, torch, dev, name="cfg3", n_cycles=4, steps=2):
-    """the recycled trunk (three recycling procedures = 4 passes) on configs[2]'s shape:
-    features -> input + recycling embedders -> 48 blocks, four times, through pf_evoformer_forward_recycled.  Context for
-    the paper's whole-model GPU seconds per protein (0.1-0.6 h for the 100-protein medium set on a V100)."""
-    import numpy as np
+def recycled_workload(h, pf, ps, torch, dev, name="cfg3", n_cycles=4, steps=2, S_e=1024, n_extra=4):
+    """the recycled network up to the structure module (three recycling procedures = 4
+    passes) on configs[2]'s shape: features -> input + recycling embedders -> extra-MSA stack (4 blocks, 1,024 extra
+    sequences) -> 48 blocks, four times, through pf_evoformer_forward_recycled.  Context for the paper's whole-model GPU
+    seconds per protein (0.1-0.6 h for the 100-protein medium set on a V100)."""
     wl = WORKLOADS[name]
     B, S, N, nb = wl["B"], wl["S"], wl["N"], wl["n_blocks"]
     emb = pf.Embedder(ps.pack_embed_blob(ps.make_embed_weights(7)), pf.make_embed_config())
+    xst = pf.ExtraMsaStack(ps.pack_extra_blob(ps.make_extra_weights(7, n_extra, bf16_weights=True)), pf.make_extra_config(n_extra))
     tf, ri, mf, x = ps.make_features(100, B, S, N)
-    tfd, rid, mfd, xd = [torch.from_numpy(a).to(dev) for a in (tf, ri, mf, x)]
+    xf = ps.make_extra_features(101, B, S_e, N)
+    tfd, rid, mfd, xd, xfd = [torch.from_numpy(a).to(dev) for a in (tf, ri, mf, x, xf)]
     smd = torch.ones((B, N), device=dev)
     mmd = torch.ones((B, S), device=dev)
+    xmd = torch.ones((B, S_e), device=dev)
     m = torch.empty((B, S, N, 256), device=dev)
     z = torch.empty((B, N, N, 128), device=dev)
-    pf.forward_recycled(h, emb, tfd, rid, mfd, xd, m, z, smd, mmd, nb, n_cycles)       # warm-up
+    e = torch.empty((B, S_e, N, 64), device=dev)
+    kw = dict(extra=xst, extra_msa_feat=xfd, extra_msa=e, extra_msa_mask=xmd, n_extra_blocks=n_extra)
+    pf.forward_recycled(h, emb, tfd, rid, mfd, xd, m, z, smd, mmd, nb, n_cycles, **kw)       # warm-up
     torch.cuda.synchronize()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record(torch.cuda.current_stream())
+    stream = torch.cuda.current_stream()
+    e0, e1, e2 = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+    e0.record(stream)
     for _ in range(steps):
-        pf.forward_recycled(h, emb, tfd, rid, mfd, xd, m, z, smd, mmd, nb, n_cycles)
-    e1.record(torch.cuda.current_stream())
+        pf.forward_recycled(h, emb, tfd, rid, mfd, xd, m, z, smd, mmd, nb, n_cycles, **kw)
+    e1.record(stream)
+    launches = h.last_launch_count()
+    emb.forward_extra(xfd, e)
+    xst.forward(e, z, smd, xmd, n_extra)                        # the extra-MSA stack on its own: one pass of n_extra blocks
+    e2.record(stream)
     torch.cuda.synchronize()
     ms = e0.elapsed_time(e1) / steps
-    launches = h.last_launch_count()
     finite = bool(torch.isfinite(m).all().item() and torch.isfinite(z).all().item())
+    out = {"desc": f"{wl['desc']}; {n_cycles} cycles of (input + recycling embedders, extra-MSA stack: {n_extra} blocks on "
+                   f"{S_e} extra sequences, {nb} blocks) through pf_evoformer_forward_recycled", "n_cycles": n_cycles,
+           "steps": steps, "ms_per_protein": ms / B, "proteins_per_s": B / (ms * 1e-3), "gpu_launches_per_step": int(launches),
+           "extra_msa_stack_ms_per_pass": e1.elapsed_time(e2), "outputs_finite": finite}
     emb.close()
-    return {"desc": f"{wl['desc']}; {n_cycles} cycles of (input + recycling embedders, {nb} blocks) through "
-                    "pf_evoformer_forward_recycled", "n_cycles": n_cycles, "steps": steps, "ms_per_protein": ms / B,
-            "proteins_per_s": B / (ms * 1e-3), "gpu_launches_per_step": int(launches), "outputs_finite": finite}
+    xst.close()
+    return out
 
 
 def cfg5_sweep(h, pf, ps, torch, dev, peaks, n_proteins=2000, S=512, cap=48, nb=48):

@@ -146,6 +146,7 @@ const char* pf_last_error(void);
  * library does not contain: it is an input, held constant over the cycles; NULL = no previous structure (no bin is set).
  * ---------------------------------------------------------------------------------------------- */
 typedef struct pf_embedder pf_embedder_t;   /* opaque; owns device weights and a small grow-only workspace */
+typedef struct pf_extra_msa pf_extra_msa_t; /* the extra-MSA stack, declared further down */
 typedef struct {
   int c_m;            /* MSA channels (256) */
   int c_z;            /* pair channels (128) */
@@ -155,11 +156,13 @@ typedef struct {
   int n_dist_bins;    /* distance bins of the recycled positions (15) */
   float first_break;  /* lower edge of the first bin, Angstrom (3.25) */
   float last_break;   /* lower edge of the last bin (20.75) */
+  int extra_dim;      /* extra-MSA features per (sequence, residue) (25; at most 32) */
+  int c_e;            /* extra-MSA channels (64) */
 } pf_embed_config;
 
 /* fp32 values in the embedder weights blob, in this order, every matrix row-major [in, out]:
  * W_a[tf_dim,c_z] b_a | W_b b_b | W_rel[2R+1,c_z] b_rel | W_m[msa_dim,c_m] b_m | W_t[tf_dim,c_m] b_t | LN_m gamma beta [c_m] |
- * LN_z gamma beta [c_z] | W_d[n_dist_bins,c_z] b_d.  0 for a null / unsupported config. */
+ * LN_z gamma beta [c_z] | W_d[n_dist_bins,c_z] b_d | W_e[extra_dim,c_e] b_e.  0 for a null / unsupported config. */
 size_t pf_embedder_floats(const pf_embed_config* cfg);
 /* Errors: INVALID_ARG (null), SHAPE (c_m, c_z not in {128, 256}; msa_dim > 64; blob length), ALLOC, CUDA. */
 pf_status pf_embedder_create(pf_embedder_t** out, const float* weights_host, size_t n_weight_floats,
@@ -172,15 +175,23 @@ pf_status pf_embedder_create(pf_embedder_t** out, const float* weights_host, siz
 pf_status pf_embedder_forward(pf_embedder_t* e, const float* target_feat_dev, const int* residue_index_dev,
                               const float* msa_feat_dev, const float* x_prev_dev, int has_prev, float* msa_dev,
                               float* pair_dev, int B, int S, int N, void* cuda_stream);
+/* E.4 extra-MSA embedder: dev extra_msa[B,S_e,N,c_e] = Lin_e(dev extra_msa_feat[B,S_e,N,extra_dim]). */
+pf_status pf_embedder_forward_extra(pf_embedder_t* e, const float* extra_msa_feat_dev, float* extra_msa_dev, int B, int S_e,
+                                    int N, void* cuda_stream);
 long long pf_embedder_last_launch_count(const pf_embedder_t* e);
 void pf_embedder_destroy(pf_embedder_t* e);
-/* E.3: n_cycles x (pf_embedder_forward, pf_evoformer_forward over n_blocks blocks) on cuda_stream; msa_dev / pair_dev are
- * outputs (their contents on entry are ignored).  n_cycles = 4 is AlphaFold's "three recycling procedures".
- * Errors: those of the two calls; SHAPE if n_cycles < 1 or the channel dims of the two handles differ. */
-pf_status pf_evoformer_forward_recycled(pf_evoformer_t* h, pf_embedder_t* e, const float* target_feat_dev,
+/* E.3: n_cycles x (pf_embedder_forward [, pf_embedder_forward_extra, pf_extra_msa_forward over n_extra_blocks blocks],
+ * pf_evoformer_forward over n_blocks blocks) on cuda_stream; msa_dev / pair_dev are outputs (their contents on entry are
+ * ignored).  x == NULL skips the extra-MSA stack (its three arguments and S_e, n_extra_blocks are then ignored); otherwise
+ * extra_msa_dev [B,S_e,N,c_e] is a caller-owned scratch buffer and extra_msa_mask_dev [B,S_e] the stack's sequence mask.
+ * n_cycles = 4 is AlphaFold's "three recycling procedures".
+ * Errors: those of the calls it makes; SHAPE if n_cycles < 1 or the channel dims of the handles differ. */
+pf_status pf_evoformer_forward_recycled(pf_evoformer_t* h, pf_embedder_t* e, pf_extra_msa_t* x, const float* target_feat_dev,
                                         const int* residue_index_dev, const float* msa_feat_dev, const float* x_prev_dev,
+                                        const float* extra_msa_feat_dev, float* extra_msa_dev, const float* extra_msa_mask_dev,
                                         float* msa_dev, float* pair_dev, const float* seq_mask_dev, const float* msa_mask_dev,
-                                        int B, int S, int N, int n_blocks, int n_cycles, void* cuda_stream);
+                                        int B, int S, int S_e, int N, int n_blocks, int n_extra_blocks, int n_cycles,
+                                        void* cuda_stream);
 
 /* ------------------------------------------------------------------------------------------------
  * Extra-MSA stack: the Evoformer block at c_e = 64 MSA channels with GLOBAL column attention over an MSA
@@ -196,7 +207,6 @@ pf_status pf_evoformer_forward_recycled(pf_evoformer_t* h, pf_embedder_t* e, con
  * Weights blob: n_blocks_max blocks of pf_extra_msa_block_floats values, the Appendix-B order at c_m = c_e with the column
  * attention's entry replaced by: LN gamma beta [c_e], W_q [c_e,c_e], W_k [c_e,d], W_v [c_e,d], W_g [c_e,c_e], b_g, W_o [c_e,c_e], b_o.
  * ---------------------------------------------------------------------------------------------- */
-typedef struct pf_extra_msa pf_extra_msa_t;
 typedef struct {
   int c_e;            /* extra-MSA channels (64) */
   int c_z;            /* pair channels (128) */

@@ -12,7 +12,8 @@ the reading E.1-E.3 of DESIGN.md §2b (the published AlphaFold 2 algorithm resta
                          bins: K lower edges e_k evenly spaced from first_break to last_break; d falls in bin k when
                          e_k^2 < d^2 < e_{k+1}^2 (e_K = infinity); below e_0 no bin is set (the one-hot is all zero)
   E.3 recycled trunk     for c in 0 .. n_cycles-1: (m, z) = E.1(features); E.2 with the previous cycle's (m_0, z) — zeros in
-                         the first cycle —; (m, z) = trunk(m, z).  xprev comes from the structure module, which is not built
+                         the first cycle —; optionally the extra-MSA stack: e = Lin_e(extra_msa_feat) (E.4), (e, z) =
+                         extra_stack(e, z) (oracle/extra_msa_ref.py), e dropped; (m, z) = trunk(m, z).  xprev comes from the structure module, which is not built
                          (SURVEY.md §8(f)4): it is an input held constant over the cycles (zeros = "no previous structure").
 
 The bin decision is a floating-point comparison deciding an integer: both sides take it in fp32 with the same operation
@@ -25,6 +26,7 @@ from __future__ import annotations
 import numpy as np
 
 from .evoformer_ref import F64, _f64, evoformer_trunk, layer_norm, linear
+from .extra_msa_ref import extra_msa_stack
 
 
 def relpos_index(residue_index, max_relpos):
@@ -81,15 +83,25 @@ def embed_cycle(target_feat, residue_index, msa_feat, m0_prev, z_prev, x_prev, w
     return recycling_embedder(m, z, m0_prev, z_prev, x_prev, w, n_bins, first_break, last_break)
 
 
+def extra_msa_embedder(extra_msa_feat, w):
+    """E.4  e_si = Lin_e(extra_msa_feat_si)."""
+    return linear(_f64(extra_msa_feat), w["w_e"], w["b_e"])
+
+
 def recycled_trunk(target_feat, residue_index, msa_feat, x_prev, seq_mask, msa_mask, w_embed, blocks, n_cycles,
-                   head_dim=32, **kw):
-    """E.3 for one protein -> (m, z) after the last cycle's trunk."""
+                   head_dim=32, extra=None, **kw):
+    """E.3 for one protein -> (m, z) after the last cycle's trunk.
+    extra = (extra_msa_feat[S_e,N,F], extra_msa_mask[S_e], extra_blocks, head_dim_msa) runs the extra-MSA stack between the
+    embedders and the trunk in every cycle."""
     S, N = np.asarray(msa_feat).shape[:2]
     c_m, c_z = np.asarray(w_embed["w_m"]).shape[1], np.asarray(w_embed["w_a"]).shape[1]
     m0_prev, z_prev = np.zeros((N, c_m)), np.zeros((N, N, c_z))
     m = z = None
     for _ in range(n_cycles):
         m, z = embed_cycle(target_feat, residue_index, msa_feat, m0_prev, z_prev, x_prev, w_embed, **kw)
+        if extra is not None:
+            xf, xmask, xblocks, xhd = extra
+            _, z = extra_msa_stack(extra_msa_embedder(xf, w_embed), z, seq_mask, xmask, xblocks, xhd, head_dim)
         m, z = evoformer_trunk(m, z, seq_mask, msa_mask, blocks, head_dim)
         m0_prev, z_prev = m[0], z
     return m, z

@@ -27,7 +27,8 @@ EXPORTED_SYMBOLS = (
     "pf_evoformer_set_profiling", "pf_evoformer_profile_kinds", "pf_evoformer_profile_name",
     "pf_evoformer_get_profile", "pf_evoformer_profile_records", "pf_evoformer_get_profile_record", "pf_evoformer_destroy", "pf_last_error", "pf_sched_create", "pf_sched_add", "pf_sched_next_batch",
     "pf_sched_bytes_per_protein", "pf_sched_cost", "pf_sched_partition", "pf_sched_destroy",
-    "pf_embedder_floats", "pf_embedder_create", "pf_embedder_forward", "pf_embedder_last_launch_count", "pf_embedder_destroy",
+    "pf_embedder_floats", "pf_embedder_create", "pf_embedder_forward", "pf_embedder_forward_extra",
+    "pf_embedder_last_launch_count", "pf_embedder_destroy",
     "pf_evoformer_forward_recycled",
     "pf_extra_msa_block_floats", "pf_extra_msa_create", "pf_extra_msa_forward", "pf_extra_msa_forward_substep",
     "pf_extra_msa_last_launch_count", "pf_extra_msa_set_profiling", "pf_extra_msa_get_profile", "pf_extra_msa_destroy",
@@ -42,7 +43,8 @@ class PfConfig(Structure):
 
 class PfEmbedConfig(Structure):
     _fields_ = [("c_m", c_int), ("c_z", c_int), ("tf_dim", c_int), ("msa_dim", c_int), ("max_relpos", c_int),
-                ("n_dist_bins", c_int), ("first_break", c_float), ("last_break", c_float)]
+                ("n_dist_bins", c_int), ("first_break", c_float), ("last_break", c_float), ("extra_dim", c_int),
+                ("c_e", c_int)]
 
 
 class PfExtraConfig(Structure):
@@ -141,7 +143,9 @@ def lib() -> ctypes.CDLL:
         L.pf_extra_msa_destroy.restype = None
         L.pf_extra_msa_destroy.argtypes = [c_void_p]
         L.pf_evoformer_forward_recycled.restype = c_int
-        L.pf_evoformer_forward_recycled.argtypes = [c_void_p] * 10 + [c_int] * 5 + [c_void_p]
+        L.pf_evoformer_forward_recycled.argtypes = [c_void_p] * 14 + [c_int] * 7 + [c_void_p]
+        L.pf_embedder_forward_extra.restype = c_int
+        L.pf_embedder_forward_extra.argtypes = [c_void_p, c_void_p, c_void_p, c_int, c_int, c_int, c_void_p]
         _lib = L
     return _lib
 
@@ -300,8 +304,8 @@ class ExtraMsaStack:
 
 
 def make_embed_config(c_m=256, c_z=128, tf_dim=22, msa_dim=49, max_relpos=32, n_dist_bins=15, first_break=3.25,
-                      last_break=20.75) -> PfEmbedConfig:
-    return PfEmbedConfig(c_m, c_z, tf_dim, msa_dim, max_relpos, n_dist_bins, first_break, last_break)
+                      last_break=20.75, extra_dim=25, c_e=64) -> PfEmbedConfig:
+    return PfEmbedConfig(c_m, c_z, tf_dim, msa_dim, max_relpos, n_dist_bins, first_break, last_break, extra_dim, c_e)
 
 
 class Embedder:
@@ -321,6 +325,13 @@ class Embedder:
         _check(lib().pf_embedder_forward(self._e, _ptr(target_feat), _ptr(residue_index), _ptr(msa_feat), _ptr(x_prev),
                                          1 if has_prev else 0, _ptr(msa), _ptr(pair), B, S, N, stream))
 
+    def forward_extra(self, extra_msa_feat, extra_msa, stream=None):
+        B, S_e, N = extra_msa.shape[0], extra_msa.shape[1], extra_msa.shape[2]
+        if stream is None:
+            import torch
+            stream = torch.cuda.current_stream().cuda_stream
+        _check(lib().pf_embedder_forward_extra(self._e, _ptr(extra_msa_feat), _ptr(extra_msa), B, S_e, N, stream))
+
     def last_launch_count(self) -> int:
         return int(lib().pf_embedder_last_launch_count(self._e))
 
@@ -337,12 +348,16 @@ class Embedder:
 
 
 def forward_recycled(evo: "Evoformer", emb: Embedder, target_feat, residue_index, msa_feat, x_prev, msa, pair, seq_mask,
-                     msa_mask, n_blocks: int, n_cycles: int, stream=None):
-    """pf_evoformer_forward_recycled: n_cycles x (embedders, trunk); msa / pair receive the result."""
+                     msa_mask, n_blocks: int, n_cycles: int, stream=None, extra: "ExtraMsaStack" = None, extra_msa_feat=None,
+                     extra_msa=None, extra_msa_mask=None, n_extra_blocks: int = 0):
+    """pf_evoformer_forward_recycled: n_cycles x (embedders [, extra-MSA stack], trunk); msa / pair receive the result."""
     B, S, N = msa.shape[0], msa.shape[1], msa.shape[2]
-    _check(lib().pf_evoformer_forward_recycled(evo._h, emb._e, _ptr(target_feat), _ptr(residue_index), _ptr(msa_feat),
-                                               _ptr(x_prev), _ptr(msa), _ptr(pair), _ptr(seq_mask), _ptr(msa_mask),
-                                               B, S, N, n_blocks, n_cycles, evo._stream(stream)))
+    S_e = extra_msa.shape[1] if extra is not None else 0
+    _check(lib().pf_evoformer_forward_recycled(evo._h, emb._e, extra._x if extra is not None else None, _ptr(target_feat),
+                                               _ptr(residue_index), _ptr(msa_feat), _ptr(x_prev), _ptr(extra_msa_feat),
+                                               _ptr(extra_msa), _ptr(extra_msa_mask), _ptr(msa), _ptr(pair), _ptr(seq_mask),
+                                               _ptr(msa_mask), B, S, S_e, N, n_blocks, n_extra_blocks, n_cycles,
+                                               evo._stream(stream)))
 
 
 class Scheduler:

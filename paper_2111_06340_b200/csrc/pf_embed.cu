@@ -25,7 +25,7 @@ struct pf_embedder {
   size_t ws_floats = 0;
   long long launches = 0;
   int device = -1;
-  struct Off { size_t w_a, b_a, w_b, b_b, w_rel, b_rel, w_m, b_m, w_t, b_t, ln_m_g, ln_m_b, ln_z_g, ln_z_b, w_d, b_d, total; } off;
+  struct Off { size_t w_a, b_a, w_b, b_b, w_rel, b_rel, w_m, b_m, w_t, b_t, ln_m_g, ln_m_b, ln_z_g, ln_z_b, w_d, b_d, w_e, b_e, total; } off;
 };
 
 namespace pf { void api_set_error(const std::string& s); }
@@ -47,6 +47,7 @@ static pf_embedder::Off embed_offsets(const pf_embed_config& c) {
   o.ln_m_g = take(c.c_m); o.ln_m_b = take(c.c_m);
   o.ln_z_g = take(c.c_z); o.ln_z_b = take(c.c_z);
   o.w_d = take((size_t)c.n_dist_bins * c.c_z); o.b_d = take(c.c_z);
+  o.w_e = take((size_t)c.extra_dim * c.c_e); o.b_e = take(c.c_e);
   o.total = at;
   return o;
 }
@@ -212,11 +213,33 @@ __global__ void __launch_bounds__(256) embed_pair_kernel(const float* __restrict
   }
 }
 
+// E.4 extra-MSA rows (b, s, i), one warp per row, lane owns two of the c_e = 64 channels: e = extra_msa_feat W_e + b_e
+__global__ void __launch_bounds__(256) embed_extra_kernel(const float* __restrict__ feat, const float* __restrict__ w,
+                                                          pf_embedder::Off o, int extra_dim, float* __restrict__ out, long rows) {
+  extern __shared__ __align__(16) float we[];       // W_e [extra_dim, 64]
+  for (int k = threadIdx.x; k < extra_dim * 64; k += blockDim.x) we[k] = __ldg(w + o.w_e + k);
+  __syncthreads();
+  const int lane = threadIdx.x & 31;
+  const long warp = (long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), nwarps = (long)gridDim.x * (blockDim.x >> 5);
+  const float2 be = __ldg(reinterpret_cast<const float2*>(w + o.b_e) + lane);
+  for (long r = warp; r < rows; r += nwarps) {
+    const float f0 = lane < extra_dim ? __ldg(feat + r * extra_dim + lane) : 0.f;
+    float a0 = be.x, a1 = be.y;
+    for (int k = 0; k < extra_dim; ++k) {
+      const float fk = __shfl_sync(0xffffffffu, f0, k);
+      const float2 wv = reinterpret_cast<const float2*>(we + k * 64)[lane];
+      a0 = fmaf(fk, wv.x, a0);
+      a1 = fmaf(fk, wv.y, a1);
+    }
+    reinterpret_cast<float2*>(out + r * 64)[lane] = make_float2(a0, a1);
+  }
+}
+
 // ------------------------------------------------------------------------------------------------
 // C ABI
 // ------------------------------------------------------------------------------------------------
 static bool embed_cfg_ok(const pf_embed_config& c) {
-  return (c.c_m == 128 || c.c_m == 256) && (c.c_z == 128 || c.c_z == 256) && c.tf_dim >= 1 && c.tf_dim <= 1024 &&
+  return c.extra_dim >= 1 && c.extra_dim <= 32 && c.c_e == 64 && (c.c_m == 128 || c.c_m == 256) && (c.c_z == 128 || c.c_z == 256) && c.tf_dim >= 1 && c.tf_dim <= 1024 &&
          c.msa_dim >= 1 && c.msa_dim <= 64 && c.max_relpos >= 0 && c.max_relpos <= 64 && c.n_dist_bins >= 1 &&
          c.n_dist_bins <= 64 && c.last_break > c.first_break && c.first_break >= 0.f;
 }
@@ -337,18 +360,47 @@ extern "C" pf_status pf_embedder_forward(pf_embedder_t* e, const float* target_f
   return PF_OK;
 }
 
-extern "C" pf_status pf_evoformer_forward_recycled(pf_evoformer_t* h, pf_embedder_t* e, const float* target_feat,
-                                                   const int* residue_index, const float* msa_feat, const float* x_prev,
-                                                   float* msa, float* pair, const float* seq_mask, const float* msa_mask,
-                                                   int B, int S, int N, int n_blocks, int n_cycles, void* stream) {
+extern "C" pf_status pf_embedder_forward_extra(pf_embedder_t* e, const float* extra_msa_feat, float* extra_msa, int B, int S_e,
+                                               int N, void* stream) {
+  if (!e || !extra_msa_feat || !extra_msa) return efail(PF_ERR_INVALID_ARG, "null argument");
+  if (B < 1 || S_e < 1 || N < 1) return efail(PF_ERR_SHAPE, "B, S_e, N must be >= 1");
+  int dev = -1, sms = 148;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev != e->device)
+    return efail(PF_ERR_INVALID_ARG, "the current device is not the one the embedder was created on");
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  const long rows = (long)B * S_e * N;
+  const unsigned grid = (unsigned)std::max(1L, std::min((rows + 7) / 8, (long)sms * 8));
+  embed_extra_kernel<<<grid, 256, e->cfg.extra_dim * 64 * 4, reinterpret_cast<cudaStream_t>(stream)>>>(
+      extra_msa_feat, e->w, e->off, e->cfg.extra_dim, extra_msa, rows);
+  e->launches = 1;
+  cudaError_t ce = cudaGetLastError();
+  if (ce != cudaSuccess) return efail(PF_ERR_CUDA, std::string("extra-MSA embedder launch failed: ") + cudaGetErrorString(ce));
+  return PF_OK;
+}
+
+extern "C" pf_status pf_evoformer_forward_recycled(pf_evoformer_t* h, pf_embedder_t* e, pf_extra_msa_t* x,
+                                                   const float* target_feat, const int* residue_index, const float* msa_feat,
+                                                   const float* x_prev, const float* extra_msa_feat, float* extra_msa,
+                                                   const float* extra_msa_mask, float* msa, float* pair, const float* seq_mask,
+                                                   const float* msa_mask, int B, int S, int S_e, int N, int n_blocks,
+                                                   int n_extra_blocks, int n_cycles, void* stream) {
   if (!h || !e) return efail(PF_ERR_INVALID_ARG, "null handle");
   if (n_cycles < 1) return efail(PF_ERR_SHAPE, "n_cycles must be >= 1");
   if (e->cfg.c_m != h->cfg.c_m || e->cfg.c_z != h->cfg.c_z) return efail(PF_ERR_SHAPE, "embedder and trunk channel dims differ");
+  if (x && (!extra_msa_feat || !extra_msa || !extra_msa_mask)) return efail(PF_ERR_INVALID_ARG, "extra-MSA stack given without its features / buffer / mask");
   long long launches = 0;
   for (int c = 0; c < n_cycles; ++c) {
     pf_status s = pf_embedder_forward(e, target_feat, residue_index, msa_feat, x_prev, c > 0 ? 1 : 0, msa, pair, B, S, N, stream);
     if (s != PF_OK) return s;
     launches += e->launches;
+    if (x) {
+      s = pf_embedder_forward_extra(e, extra_msa_feat, extra_msa, B, S_e, N, stream);
+      if (s != PF_OK) return s;
+      launches += e->launches;
+      s = pf_extra_msa_forward(x, extra_msa, pair, seq_mask, extra_msa_mask, B, S_e, N, n_extra_blocks, stream);
+      if (s != PF_OK) return s;
+      launches += pf_extra_msa_last_launch_count(x);
+    }
     s = pf_evoformer_forward(h, msa, pair, seq_mask, msa_mask, B, S, N, n_blocks, stream);
     if (s != PF_OK) return s;
     launches += h->launches;

@@ -266,6 +266,8 @@ class EmbedDims:
     n_dist_bins: int = 15
     first_break: float = 3.25
     last_break: float = 20.75
+    extra_dim: int = 25       # extra-MSA features: 23 token classes + 2 deletion features
+    c_e: int = 64
 
 
 EMBED = EmbedDims()
@@ -281,7 +283,8 @@ def embed_spec(d: EmbedDims = EMBED):
             ("w_t", (d.tf_dim, d.c_m), "W"), ("b_t", (d.c_m,), "bias"),
             ("ln_m_g", (d.c_m,), "gamma"), ("ln_m_b", (d.c_m,), "beta"),
             ("ln_z_g", (d.c_z,), "gamma"), ("ln_z_b", (d.c_z,), "beta"),
-            ("w_d", (d.n_dist_bins, d.c_z), "W"), ("b_d", (d.c_z,), "bias")]
+            ("w_d", (d.n_dist_bins, d.c_z), "W"), ("b_d", (d.c_z,), "bias"),
+            ("w_e", (d.extra_dim, d.c_e), "W"), ("b_e", (d.c_e,), "bias")]
 
 
 def make_embed_weights(seed: int, d: EmbedDims = EMBED):
@@ -327,6 +330,17 @@ def make_features(seed: int, B: int, S: int, N: int, d: EmbedDims = EMBED):
     step *= np.float32(3.8) / np.linalg.norm(step, axis=-1, keepdims=True)
     x = np.cumsum(step, axis=1).astype(np.float32)
     return tf, ri, mf, x
+
+
+def make_extra_features(seed: int, B: int, S_e: int, N: int, d: EmbedDims = EMBED):
+    """extra_msa_feat[B,S_e,N,25]: one-hot token + deletion flag + deletion value (stand-in for the unclustered sequences)."""
+    g = rng(seed, 2200)
+    tok = g.integers(0, 23, size=(B, S_e, N))
+    xf = np.zeros((B, S_e, N, d.extra_dim), np.float32)
+    np.put_along_axis(xf[..., :23], tok[..., None], 1.0, axis=-1)
+    xf[..., 23] = (g.uniform(size=(B, S_e, N)) < 0.1)
+    xf[..., 24] = g.uniform(size=(B, S_e, N)).astype(np.float32) * xf[..., 23]
+    return xf
 
 
 # ----------------------------------------------------------------------------------------------

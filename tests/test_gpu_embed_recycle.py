@@ -104,3 +104,42 @@ def test_recycled_trunk_matches_oracle():
         assert em <= 3e-2 and ez <= 3e-2 and rm <= 1e-2 and rz <= 1e-2
     emb.close()
     evo.close()
+
+
+def test_recycled_trunk_with_extra_msa_stack_matches_oracle():
+    """E.3 with the extra-MSA stack in every cycle: embedders -> e = Lin_e(extra features) -> one extra block -> one trunk
+    block, two cycles."""
+    import torch
+    B, S, S_e, N, cycles = 2, 8, 70, 40, 2
+    w = ps.make_embed_weights(141)
+    blocks = ps.make_weights(142, 1, bf16_weights=True)
+    xblocks = ps.make_extra_weights(143, 1, bf16_weights=True)
+    tf, ri, mf, x = ps.make_features(144, B, S, N)
+    xf = ps.make_extra_features(145, B, S_e, N)
+    _, _, sm, mm = ps.make_inputs(146, B, S, N, lengths=[40, 31], msa_mask_frac_max=0.3)
+    _, _, _, xm = ps.make_inputs(147, B, S_e, N, msa_mask_frac_max=0.3)
+    emb = pf.Embedder(ps.pack_embed_blob(w), pf.make_embed_config())
+    evo = pf.Evoformer(ps.pack_blob(blocks), pf.make_config(1, pf.PF_BF16))
+    xst = pf.ExtraMsaStack(ps.pack_extra_blob(xblocks), pf.make_extra_config(1))
+    m = torch.empty((B, S, N, 256), device="cuda")
+    z = torch.empty((B, N, N, 128), device="cuda")
+    e = torch.empty((B, S_e, N, 64), device="cuda")
+    tfd, rid, mfd, xd, xfd, xmd, smd, mmd = _dev(tf, ri, mf, x, xf, xm, sm, mm)
+    # E.4 alone first
+    emb.forward_extra(xfd, e)
+    torch.cuda.synchronize()
+    assert np.abs(e[1].cpu().numpy() - er.extra_msa_embedder(xf[1], w)).max() < 1e-4
+    pf.forward_recycled(evo, emb, tfd, rid, mfd, xd, m, z, smd, mmd, 1, cycles, extra=xst, extra_msa_feat=xfd, extra_msa=e,
+                        extra_msa_mask=xmd, n_extra_blocks=1)
+    torch.cuda.synchronize()
+    mo, zo = m.cpu().numpy(), z.cpu().numpy()
+    assert np.isfinite(mo).all() and np.isfinite(zo).all()
+    for b in range(B):
+        mr, zr = er.recycled_trunk(tf[b], ri[b], mf[b], x[b], sm[b], mm[b], w, blocks, cycles, extra=(xf[b], xm[b], xblocks, 8))
+        vm, vz = valid_masks(sm[b:b + 1], mm[b:b + 1])
+        em, rm = errors(mo[b:b + 1], mr[None], vm)
+        ez, rz = errors(zo[b:b + 1], zr[None], vz)
+        print(f"recycled trunk + extra stack protein {b}: m {em:.3e}/{rm:.3e} z {ez:.3e}/{rz:.3e}")
+        assert em <= 3e-2 and ez <= 3e-2 and rm <= 1e-2 and rz <= 1e-2
+    for o in (emb, evo, xst):
+        o.close()

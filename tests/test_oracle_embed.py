@@ -115,3 +115,31 @@ def test_recycled_trunk_is_the_cycle_loop(tiny_dims):
     assert np.abs(got_m - m).max() < 1e-12 and np.abs(got_z - z).max() < 1e-12
     one = er.recycled_trunk(tf[0], ri[0], mf[0], x[0], sig, rho, w, blocks, 1, head_dim=hd)
     assert np.abs(one[1] - got_z).max() > 1e-3              # the second cycle changes the result
+
+
+def test_recycled_trunk_with_extra_msa_stack(tiny_dims):
+    """E.3 with the extra-MSA stack: per cycle embed -> e = Lin_e(features) -> extra stack (only z leaves it) -> trunk, written
+    out by hand; the stack must change the result."""
+    from oracle import extra_msa_ref as xr
+    d = ps.EmbedDims(c_m=tiny_dims.c_m, c_z=tiny_dims.c_z, c_e=4)
+    xd = ps.ExtraDims(c_e=4, c_z=tiny_dims.c_z, heads_msa=2, heads_pair=tiny_dims.heads_pair, head_dim_pair=tiny_dims.head_dim,
+                      c_opm=tiny_dims.c_opm, c_tri=tiny_dims.c_tri, transition_n=tiny_dims.transition_n)
+    w = ps.make_embed_weights(88, d)
+    tf, ri, mf, x = ps.make_features(89, 1, 3, 6, d)
+    xf = ps.make_extra_features(90, 1, 5, 6, d)
+    blocks = ps.make_weights(91, 1, tiny_dims)
+    xblocks = ps.make_extra_weights(92, 1, xd)
+    sig, rho, xrho = np.ones(6), np.ones(3), np.array([1.0, 1, 0, 1, 1])
+    hd = tiny_dims.head_dim
+    got = er.recycled_trunk(tf[0], ri[0], mf[0], x[0], sig, rho, w, blocks, 2, head_dim=hd,
+                            extra=(xf[0], xrho, xblocks, xd.head_dim_msa))
+    m0p, zp = np.zeros((6, d.c_m)), np.zeros((6, 6, d.c_z))
+    for _ in range(2):
+        m, z = er.embed_cycle(tf[0], ri[0], mf[0], m0p, zp, x[0], w)
+        e = xf[0].astype(np.float64) @ w["w_e"].astype(np.float64) + w["b_e"]
+        _, z = xr.extra_msa_stack(e, z, sig, xrho, xblocks, xd.head_dim_msa, hd)
+        m, z = ref.evoformer_trunk(m, z, sig, rho, blocks, hd)
+        m0p, zp = m[0], z
+    assert np.abs(got[0] - m).max() < 1e-12 and np.abs(got[1] - z).max() < 1e-12
+    plain = er.recycled_trunk(tf[0], ri[0], mf[0], x[0], sig, rho, w, blocks, 2, head_dim=hd)
+    assert np.abs(plain[1] - got[1]).max() > 1e-3
