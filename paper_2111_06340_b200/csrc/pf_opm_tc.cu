@@ -19,26 +19,35 @@ int tma_encode_bf16(TmaCtx* ctx, CUtensorMap* out, const void* base, int rank, c
 
 constexpr int OP_BI = 128, OP_BJ = 2, OP_C = 32, OP_CZ = 128, OP_BK = 64;
 constexpr int OP_MAX_KB = 8;       // S <= 512
-constexpr int OP_A_STAGES = 4;
+constexpr int OP_A_STAGES = 10;    // upper bound; the launch uses as many 16 KB stages as fit beside the resident b operand
 constexpr int OP_THREADS = 192;
+constexpr int OP_NB = 4;           // at most 4 outer-product tiles in flight between the two contractions (TMEM: 4 x 64 columns)
+// Per launch: nb = 4 tiles in flight and GEMM2 lagging GEMM1 by 2 when the contraction is short (N_seq <= 256: GEMM1 is too short
+// to hide the relayout of the previous tile behind it), nb = 2 / lag 1 otherwise (the shared memory goes to a deeper a ring,
+// which is what bounds the long contractions).
 
+// Shared memory: W_out tiles, the bf16 outer-product tiles and the barriers at fixed offsets, then the resident b operand
+// (n_kb x 8 KB, n_kb = k-blocks of this launch) and behind it the ring of a tiles: as many 16 KB stages as fit.  The a stream
+// is fetched from L2 with a latency of ~1 us, so its rate is ring bytes / latency (measured: 64 KB in flight gave ~71 GB/s per
+// SM and bounded the kernel; the multicast variant, which cuts L2 traffic instead, was slower).
 struct OpmSmem {
-  static constexpr int B_OFF = 0;                                        // OP_MAX_KB x (64 rows x 128 B) = 64 KB
   static constexpr int B_KB_BYTES = OP_BJ * OP_C * 128;                  // 8 KB
-  static constexpr int A_OFF = B_OFF + OP_MAX_KB * B_KB_BYTES;
   static constexpr int A_BYTES = OP_BI * 128;                            // 16 KB
-  static constexpr int W_OFF = A_OFF + OP_A_STAGES * A_BYTES;
+  static constexpr int W_OFF = 0;
   static constexpr int W_BYTES = OP_CZ * 64;                             // 128 e x 32 c2 bf16 = 8 KB
-  static constexpr int OV_OFF = W_OFF + 2 * W_BYTES;
   static constexpr int OV_TILE = OP_BI * 64;                             // 128 i x 32 c2 bf16 = 8 KB
-  static constexpr int BAR_OFF = OV_OFF + 2 * OP_BJ * OV_TILE;
-  static constexpr int TOTAL = BAR_OFF + 256 + 1024;
+  static constexpr int BAR_OFF = 0;
+  static constexpr int TOTAL = 227 * 1024;
+  static __host__ __device__ int ov_off(int nb) { return 1024 + nb * W_BYTES; }                 // W ring first, at 1024
+  static __host__ __device__ int b_off(int nb) { return ov_off(nb) + nb * OP_BJ * OV_TILE; }
+  static __host__ __device__ int ring_bytes(int nb) { return TOTAL - 1024 - b_off(nb); }        // b operand + a ring
 };
 
 __global__ void __launch_bounds__(OP_THREADS, 1)
 opm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
               const __grid_constant__ CUtensorMap tmW, const float* __restrict__ bout, const float* __restrict__ seq_mask,
-              const float* __restrict__ msa_mask, float* __restrict__ z, int S, int N, int s0, int Sc, int add_bias) {
+              const float* __restrict__ msa_mask, float* __restrict__ z, int S, int N, int s0, int Sc, int add_bias,
+              int a_stages, int nb_shift) {
   using SM = OpmSmem;
   {
     // both residues j of this CTA padded: every output is at a masked position (uniform over the CTA: exit before any setup)
@@ -53,13 +62,13 @@ opm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ C
   uint64_t* b_full = bars;
   uint64_t* a_full = bars + 1;                    // [OP_A_STAGES]
   uint64_t* a_empty = a_full + OP_A_STAGES;       // [OP_A_STAGES]
-  uint64_t* w_full = a_empty + OP_A_STAGES;       // [2]
-  uint64_t* w_empty = w_full + 2;                 // [2]
-  uint64_t* d1_full = w_empty + 2;                // [2]
-  uint64_t* d1_empty = d1_full + 2;               // [2]
-  uint64_t* ov_full = d1_empty + 2;               // [2]
-  uint64_t* ov_empty = ov_full + 2;               // [2]
-  uint64_t* acc_full = ov_empty + 2;
+  uint64_t* w_full = a_empty + OP_A_STAGES;       // [OP_NB]
+  uint64_t* w_empty = w_full + OP_NB;             // [OP_NB]
+  uint64_t* d1_full = w_empty + OP_NB;            // [OP_NB]
+  uint64_t* d1_empty = d1_full + OP_NB;           // [OP_NB]
+  uint64_t* ov_full = d1_empty + OP_NB;           // [OP_NB]
+  uint64_t* ov_empty = ov_full + OP_NB;           // [OP_NB]
+  uint64_t* acc_full = ov_empty + OP_NB;
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(acc_full + 1);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -67,6 +76,9 @@ opm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ C
   // this launch contracts the sequences [s0, s0 + Sc) (Sc <= 512: the b operand of the chunk stays resident in shared memory);
   // the normaliser counts all S sequences, and the chunks add up because the projection is linear (bias with the first chunk)
   const int n_kb = (Sc + OP_BK - 1) / OP_BK;
+  const int nb = 1 << nb_shift, lag = nb >> 1;
+  const int W_OFF = 1024, OV_OFF = SM::ov_off(nb), B_OFF = SM::b_off(nb);
+  const int A_OFF = B_OFF + n_kb * SM::B_KB_BYTES;
 
   if (warp == 0 && lane == 0) {
     tc::prefetch_tmap(&tmA);
@@ -77,7 +89,7 @@ opm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ C
       tc::mbar_init(&a_full[s], 1);
       tc::mbar_init(&a_empty[s], 1);
     }
-    for (int s = 0; s < 2; ++s) {
+    for (int s = 0; s < OP_NB; ++s) {
       tc::mbar_init(&w_full[s], 1);
       tc::mbar_init(&w_empty[s], 1);
       tc::mbar_init(&d1_full[s], 1);
@@ -94,25 +106,26 @@ opm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ C
   tc::tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
   const uint32_t tmem_acc = tmem_base;            // 2 x 128 columns
-  const uint32_t tmem_d1 = tmem_base + 256;       // 2 x 64 columns
+  const uint32_t tmem_d1 = tmem_base + 256;       // OP_NB x 64 columns
 
   if (warp == 0) {
     if (tc::elect_one()) {
       tc::mbar_arrive_expect_tx(b_full, (uint32_t)n_kb * SM::B_KB_BYTES);
       for (int kb = 0; kb < n_kb; ++kb)
-        tc::tma_load_3d(smem + SM::B_OFF + kb * SM::B_KB_BYTES, &tmB, b_full, s0 + kb * OP_BK, OP_C, b * N + j0);
-      int it = 0;
+        tc::tma_load_3d(smem + B_OFF + kb * SM::B_KB_BYTES, &tmB, b_full, s0 + kb * OP_BK, OP_C, b * N + j0);
+      int s = 0;
+      uint32_t ph = 0;                               // ring position and its phase (no divisions on this path)
       for (int c1 = 0; c1 < OP_C; ++c1) {
-        for (int kb = 0; kb < n_kb; ++kb, ++it) {
-          int s = it % OP_A_STAGES;
-          tc::mbar_wait(&a_empty[s], ((it / OP_A_STAGES) & 1) ^ 1);
+        for (int kb = 0; kb < n_kb; ++kb) {
+          tc::mbar_wait(&a_empty[s], ph ^ 1);
           tc::mbar_arrive_expect_tx(&a_full[s], SM::A_BYTES);
-          tc::tma_load_3d(smem + SM::A_OFF + s * SM::A_BYTES, &tmA, &a_full[s], s0 + kb * OP_BK, c1, b * N + i0);
+          tc::tma_load_3d(smem + A_OFF + s * SM::A_BYTES, &tmA, &a_full[s], s0 + kb * OP_BK, c1, b * N + i0);
+          if (++s == a_stages) { s = 0; ph ^= 1; }
         }
-        int ws = c1 & 1;
-        tc::mbar_wait(&w_empty[ws], ((c1 >> 1) & 1) ^ 1);
+        int ws = c1 & (nb - 1);
+        tc::mbar_wait(&w_empty[ws], ((c1 >> nb_shift) & 1) ^ 1);
         tc::mbar_arrive_expect_tx(&w_full[ws], SM::W_BYTES);
-        tc::tma_load_2d(smem + SM::W_OFF + ws * SM::W_BYTES, &tmW, &w_full[ws], c1 * OP_C, 0);
+        tc::tma_load_2d(smem + W_OFF + ws * SM::W_BYTES, &tmW, &w_full[ws], c1 * OP_C, 0);
       }
     }
   } else if (warp == 1) {
@@ -120,34 +133,35 @@ opm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ C
       constexpr uint32_t idesc1 = tc::idesc_bf16_f32(OP_BI, OP_BJ * OP_C);
       constexpr uint32_t idesc2 = tc::idesc_bf16_f32(OP_BI, OP_CZ);
       tc::mbar_wait(b_full, 0);
-      int it = 0;
-      for (int c1 = 0; c1 <= OP_C; ++c1) {
+      int s = 0;
+      uint32_t ph = 0;
+      for (int c1 = 0; c1 < OP_C + lag; ++c1) {
         if (c1 < OP_C) {
-          int buf = c1 & 1;
-          tc::mbar_wait(&d1_empty[buf], ((c1 >> 1) & 1) ^ 1);
+          int buf = c1 & (nb - 1);
+          tc::mbar_wait(&d1_empty[buf], ((c1 >> nb_shift) & 1) ^ 1);
           tc::tc_fence_after();
-          for (int kb = 0; kb < n_kb; ++kb, ++it) {
-            int s = it % OP_A_STAGES;
-            tc::mbar_wait(&a_full[s], (it / OP_A_STAGES) & 1);
+          for (int kb = 0; kb < n_kb; ++kb) {
+            tc::mbar_wait(&a_full[s], ph);
             tc::tc_fence_after();
-            uint64_t a_desc = tc::smem_desc_kmajor<128>(tc::smem_u32(smem + SM::A_OFF + s * SM::A_BYTES));
-            uint64_t b_desc = tc::smem_desc_kmajor<128>(tc::smem_u32(smem + SM::B_OFF + kb * SM::B_KB_BYTES));
+            uint64_t a_desc = tc::smem_desc_kmajor<128>(tc::smem_u32(smem + A_OFF + s * SM::A_BYTES));
+            uint64_t b_desc = tc::smem_desc_kmajor<128>(tc::smem_u32(smem + B_OFF + kb * SM::B_KB_BYTES));
 #pragma unroll
             for (int k = 0; k < OP_BK / 16; ++k)
               tc::mma_bf16(tmem_d1 + buf * 64, a_desc + 2 * k, b_desc + 2 * k, idesc1, (kb | k) != 0);
             tc::mma_commit(&a_empty[s]);
+            if (++s == a_stages) { s = 0; ph ^= 1; }
           }
           tc::mma_commit(&d1_full[buf]);
         }
-        if (c1 >= 1) {
-          int p = c1 - 1, pb = p & 1;
-          tc::mbar_wait(&ov_full[pb], (p >> 1) & 1);
-          tc::mbar_wait(&w_full[pb], (p >> 1) & 1);
+        if (c1 >= lag) {
+          int p = c1 - lag, pb = p & (nb - 1);
+          tc::mbar_wait(&ov_full[pb], (p >> nb_shift) & 1);
+          tc::mbar_wait(&w_full[pb], (p >> nb_shift) & 1);
           tc::tc_fence_after();
-          uint64_t w_desc = tc::smem_desc_kmajor<64>(tc::smem_u32(smem + SM::W_OFF + pb * SM::W_BYTES));
+          uint64_t w_desc = tc::smem_desc_kmajor<64>(tc::smem_u32(smem + W_OFF + pb * SM::W_BYTES));
 #pragma unroll
           for (int j = 0; j < OP_BJ; ++j) {
-            uint64_t o_desc = tc::smem_desc_kmajor<64>(tc::smem_u32(smem + SM::OV_OFF + (pb * OP_BJ + j) * SM::OV_TILE));
+            uint64_t o_desc = tc::smem_desc_kmajor<64>(tc::smem_u32(smem + OV_OFF + (pb * OP_BJ + j) * SM::OV_TILE));
             tc::mma_bf16(tmem_acc + j * OP_CZ, o_desc, w_desc, idesc2, p != 0);
             tc::mma_bf16(tmem_acc + j * OP_CZ, o_desc + 2, w_desc + 2, idesc2, true);
           }
@@ -163,8 +177,8 @@ opm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ C
     const int i = i0 + row;
     const uint32_t lane_addr = (uint32_t)(quarter * 32) << 16;
     for (int c1 = 0; c1 < OP_C; ++c1) {
-      int buf = c1 & 1;
-      tc::mbar_wait(&d1_full[buf], (c1 >> 1) & 1);
+      int buf = c1 & (nb - 1);
+      tc::mbar_wait(&d1_full[buf], (c1 >> nb_shift) & 1);
       tc::tc_fence_after();
       uint32_t v[2][32];
       tc::tmem_ld32(tmem_d1 + buf * 64 + lane_addr, v[0]);
@@ -172,10 +186,10 @@ opm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ C
       tc::tmem_ld_wait();
       tc::tc_fence_before();
       tc::mbar_arrive(&d1_empty[buf]);
-      tc::mbar_wait(&ov_empty[buf], ((c1 >> 1) & 1) ^ 1);
+      tc::mbar_wait(&ov_empty[buf], ((c1 >> nb_shift) & 1) ^ 1);
 #pragma unroll
       for (int j = 0; j < OP_BJ; ++j) {
-        uint8_t* tile = smem + SM::OV_OFF + (buf * OP_BJ + j) * SM::OV_TILE;
+        uint8_t* tile = smem + OV_OFF + (buf * OP_BJ + j) * SM::OV_TILE;
 #pragma unroll
         for (int c = 0; c < 4; ++c) {
           uint32_t pk[4];
@@ -247,9 +261,14 @@ int launch_opm_tc(TmaCtx* ctx, const bf16* ab_t, const bf16* wout_t, const float
   if (tma_encode_bf16(ctx, &tmW, wout_t, 2, dw, sw, bxW, 64) != 0) return -1;
   dim3 grid((N + OP_BJ - 1) / OP_BJ, (N + OP_BI - 1) / OP_BI, B);
   const int chunk = OP_MAX_KB * OP_BK;   // 512 sequences per launch; the extra-MSA stack (S in the thousands) takes several
-  for (int s0 = 0; s0 < S; s0 += chunk)
-    opm_tc_kernel<<<grid, OP_THREADS, OpmSmem::TOTAL, st>>>(tmA, tmB, tmW, bout, seq_mask, msa_mask, z, S, N, s0,
-                                                            S - s0 < chunk ? S - s0 : chunk, s0 == 0 ? 1 : 0);
+  for (int s0 = 0; s0 < S; s0 += chunk) {
+    const int Sc = S - s0 < chunk ? S - s0 : chunk, n_kb = (Sc + OP_BK - 1) / OP_BK;
+    const int nb_shift = Sc <= 256 ? 2 : 1;
+    int stages = (OpmSmem::ring_bytes(1 << nb_shift) - n_kb * OpmSmem::B_KB_BYTES) / OpmSmem::A_BYTES;
+    stages = stages > OP_A_STAGES ? OP_A_STAGES : stages;
+    opm_tc_kernel<<<grid, OP_THREADS, OpmSmem::TOTAL, st>>>(tmA, tmB, tmW, bout, seq_mask, msa_mask, z, S, N, s0, Sc,
+                                                            s0 == 0 ? 1 : 0, stages, nb_shift);
+  }
   return 0;
 }
 
