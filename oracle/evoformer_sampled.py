@@ -168,7 +168,7 @@ def triangle_mult_outgoing_at(z, seq_mask, w, i, j, rnd=None):
     xj = _ln(z[j], w["ln_in_g"], w["ln_in_b"], r)                     # rows (j, k)
     a = _tri_operand(xi, sg[i] * sg, w["w_ap"], w["b_ap"], w["w_ag"], w["b_ag"], r)   # a[k, c] = a[i,k,c]
     b = _tri_operand(xj, sg[j] * sg, w["w_bp"], w["b_bp"], w["w_bg"], w["b_bg"], r)   # b[k, c] = b[j,k,c]
-    t = np.sum(a * b, axis=0)
+    t = r.bf16(np.sum(a * b, axis=0))
     g = r.gate(_lin(xi[j], w["w_g"], w["b_g"], r))
     return _f64(z[i, j]) + g * _lin(_ln(t, w["ln_out_g"], w["ln_out_b"], r), w["w_z"], w["b_z"], r)
 
@@ -181,7 +181,7 @@ def triangle_mult_incoming_at(z, seq_mask, w, i, j, rnd=None):
     xj = _ln(z[:, j], w["ln_in_g"], w["ln_in_b"], r)                  # rows (k, j)
     a = _tri_operand(xi, sg * sg[i], w["w_ap"], w["b_ap"], w["w_ag"], w["b_ag"], r)   # a[k, c] = a[k,i,c]
     b = _tri_operand(xj, sg * sg[j], w["w_bp"], w["b_bp"], w["w_bg"], w["b_bg"], r)   # b[k, c] = b[k,j,c]
-    t = np.sum(a * b, axis=0)
+    t = r.bf16(np.sum(a * b, axis=0))
     xij = _ln(z[i, j], w["ln_in_g"], w["ln_in_b"], r)
     g = r.gate(_lin(xij, w["w_g"], w["b_g"], r))
     return _f64(z[i, j]) + g * _lin(_ln(t, w["ln_out_g"], w["ln_out_b"], r), w["w_z"], w["b_z"], r)

@@ -130,7 +130,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQK, const __grid_constant__
     // ============================================================= TMA producer
     if (tc::elect_one()) {
       const uint32_t stage_tx = SM::K_BYTES + SM::V_BYTES + (p.has_bias ? SM::B_BYTES : 0);
-      uint32_t uc = 0, i = 0;
+      uint32_t uc = 0, s = 0, sph = 0;               // ring position / phase kept as counters: no divisions on the issue paths
       const int units = *p.n_rows * p.H * p.QT;
       int2 ent = attn_row_entry((int)blockIdx.x, units, p);
       for (int u = blockIdx.x; u < units; u += (int)gridDim.x, ++uc) {
@@ -145,14 +145,14 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQK, const __grid_constant__
         uint8_t* qs = smem + SM::Q_OFF + qb * SM::Q_BYTES;
         tc::tma_load_3d(qs, &tmQK, &q_full[qb], h * 32, i0, br);            // box {32, 64, 1} twice: rows i0.., i0+64..
         tc::tma_load_3d(qs + 64 * 64, &tmQK, &q_full[qb], h * 32, i0 + 64, br);
-        for (int kt = 0; kt < n_kt; ++kt, ++i) {
-          const uint32_t s = i % ST;
-          tc::mbar_wait(&kv_empty[s], ((i / ST) & 1) ^ 1);
+        for (int kt = 0; kt < n_kt; ++kt) {
+          tc::mbar_wait(&kv_empty[s], sph ^ 1);
           uint8_t* st = smem + SM::STAGE_OFF + s * p.stage_bytes;
           tc::mbar_arrive_expect_tx(&kv_full[s], stage_tx);
           tc::tma_load_3d(st, &tmQK, &kv_full[s], C + h * 32, kt * AT_BK, br);
           tc::tma_load_2d(st + SM::K_BYTES, &tmV, &kv_full[s], kt * AT_BK, (br * p.H + h) * 32);
           if (p.has_bias) tc::tma_load_3d(st + SM::K_BYTES + SM::V_BYTES, &tmBias, &kv_full[s], kt * AT_BK, i0, b * p.H + h);
+          if (++s == (uint32_t)ST) { s = 0; sph ^= 1; }
         }
         ent = ent_next;
       }
@@ -170,14 +170,15 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQK, const __grid_constant__
       int2 ent = attn_row_entry(cu, units, p), ent_next = make_int2(0, 0);
       int cn = min(ent.y, p.n_kt);
       uint32_t cuc = 0, j = 0, i = 0;
+      uint32_t js = 0, jph = 0, is = 0;              // ring position / phase of the issue side (j) and position of the consume side (i)
       auto issue_s = [&]() -> bool {
         if (cu >= units) return false;
-        const uint32_t qb = cuc & 1, s = j % ST;
+        const uint32_t qb = cuc & 1, s = js;
         if (ckt == 0) {
           ent_next = attn_row_entry(cu + (int)gridDim.x, units, p);   // used when this unit's last S has been issued
           tc::mbar_wait(&q_full[qb], (cuc >> 1) & 1);
         }
-        tc::mbar_wait(&kv_full[s], (j / ST) & 1);
+        tc::mbar_wait(&kv_full[s], jph);
         tc::tc_fence_after();
         const uint64_t q_desc = tc::smem_desc_kmajor<64>(tc::smem_u32(smem + SM::Q_OFF + qb * SM::Q_BYTES));
         const uint64_t k_desc = tc::smem_desc_kmajor<64>(tc::smem_u32(smem + SM::STAGE_OFF + s * p.stage_bytes));
@@ -201,12 +202,14 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQK, const __grid_constant__
           ++ckt;
         }
         ++j;
+        if (++js == (uint32_t)ST) { js = 0; jph ^= 1; }
         return true;
       };
       if (issue_s()) {
         while (true) {
           issue_s();                               // S(i-1) was drained before P(i-1) arrived, so its buffer is free
-          const uint32_t s = i % ST;
+          const uint32_t s = is;
+          if (++is == (uint32_t)ST) is = 0;
           tc::mbar_wait(p_full, i & 1);
           tc::tc_fence_after();
           const uint64_t v_desc = tc::smem_desc_kmajor<128>(tc::smem_u32(smem + SM::STAGE_OFF + s * p.stage_bytes + SM::K_BYTES));

@@ -64,6 +64,8 @@ void launch_tri_einsum_simt(const T* a_cm, const T* b_cm, float* t_cm, int batch
 template <typename T>
 void launch_lnc(const float* t_cm, T* y, const float* gamma, const float* beta, const float* seq_mask /*optional: rows of
                 padded residues are skipped*/, int B, int C, int N, int Npad, cudaStream_t st);
+void launch_lnc_tc(const bf16* t_cm, __half* y, const float* gamma, const float* beta, const float* seq_mask, int B, int N,
+                   int Npad, cudaStream_t st);
 template <typename T>
 void launch_opm_simt(const T* a, const T* b, const float* wout, const float* bout, const float* seq_mask,
                      const float* msa_mask, float* z, int B, int S, int N, int c_opm, int c_z, cudaStream_t st);
@@ -175,7 +177,7 @@ void launch_key_tiles(const float* mask, int B, int L, int* key_tiles, cudaStrea
 int launch_opm_tc(TmaCtx* ctx, const bf16* ab_t, const bf16* wout_t, const float* bout, const float* seq_mask,
                   const float* msa_mask, float* z, int B, int S, int Spad, int N, cudaStream_t st);
 // key_tiles [batch / channels] (optional): the contraction stops after the last unmasked residue's 64-wide k-block
-int launch_tri_einsum_tc(TmaCtx* ctx, const bf16* a_cm, const bf16* b_cm, float* t_cm, int batch, int N, int Npad,
+int launch_tri_einsum_tc(TmaCtx* ctx, const bf16* a_cm, const bf16* b_cm, bf16* t_cm, int batch, int N, int Npad,
                          const int* key_tiles, int channels, int num_sms, cudaStream_t st);
 
 }  // namespace pf

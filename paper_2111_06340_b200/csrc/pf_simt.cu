@@ -283,6 +283,12 @@ __global__ void __launch_bounds__(256) lnc_kernel(const float* __restrict__ t, T
 // holds 16 channels x 2 positions in registers; per-position statistics are the thread's partial sums combined across the
 // eight warps through shared memory (no shuffles); the normalised values are staged [position][channel] in shared memory
 // and leave as coalesced 16-byte stores.
+__device__ __forceinline__ float2 lnc_ld2(const float* p) { return __ldg(reinterpret_cast<const float2*>(p)); }
+__device__ __forceinline__ float2 lnc_ld2(const bf16* p) {
+  const unsigned u = __ldg(reinterpret_cast<const unsigned*>(p));
+  return __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&u));
+}
+
 template <typename T>
 __global__ void __launch_bounds__(256) lnc128_kernel(const float* __restrict__ t, T* __restrict__ y,
                                                      const float* __restrict__ gamma, const float* __restrict__ beta,
@@ -301,7 +307,7 @@ __global__ void __launch_bounds__(256) lnc128_kernel(const float* __restrict__ t
 #pragma unroll
   for (int k = 0; k < 16; ++k) {
     const int c = warp * 16 + k;
-    v[k] = in ? __ldg(reinterpret_cast<const float2*>(t + (((long)b * C + c) * N + i) * Npad + j)) : make_float2(0.f, 0.f);
+    v[k] = in ? lnc_ld2(t + (((long)b * C + c) * N + i) * Npad + j) : make_float2(0.f, 0.f);
   }
   float s0 = 0.f, s1 = 0.f;
 #pragma unroll
@@ -375,6 +381,94 @@ void launch_lnc(const float* t_cm, T* y, const float* gamma, const float* beta, 
   }
   dim3 grid((N + 31) / 32, N, B);
   lnc_kernel<T><<<grid, 256, C * 33 * sizeof(float), st>>>(t_cm, y, gamma, beta, seq_mask, C, N, Npad);
+}
+// The tcgen05 path's variant: bf16 channel-major einsum output -> fp16 rows (the next GEMM's A operand).  Block = one (b, i)
+// row x 128 consecutive j x 128 channels; warp w owns channels [16 w, 16 w + 16), a lane four consecutive positions (one
+// 8-byte load per channel: 256 bytes per warp load as in the fp32 variant), statistics across the eight warps through shared
+// memory, normalised values staged [position][channel] and written as coalesced 16-byte stores.  (Measured alternatives: 16
+// warps x 8 channels and values kept packed in registers were both slower.)
+__global__ void __launch_bounds__(256) lnc128_bf16_kernel(const bf16* __restrict__ t, __half* __restrict__ y,
+                                                          const float* __restrict__ gamma, const float* __restrict__ beta,
+                                                          const float* __restrict__ seq_mask, int N, int Npad) {
+  constexpr int C = 128, PJ = 128, ROWP = C + 8;
+  __shared__ float part[2][8][PJ];
+  __shared__ __align__(16) __half stage[PJ][ROWP];
+  const int j0 = blockIdx.x * PJ, i = blockIdx.y, b = blockIdx.z;
+  if (seq_mask && seq_mask[(long)b * N + i] < 0.5f) return;   // padded row i: every output of it is at a masked position
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int j = j0 + 4 * lane;
+  const bool in = j < Npad;                              // Npad is a multiple of 8: a group of four never straddles the row end
+  float v[16][4];
+#pragma unroll
+  for (int k = 0; k < 16; ++k) {
+    const int c = warp * 16 + k;
+    uint2 u = make_uint2(0u, 0u);
+    if (in) u = __ldg(reinterpret_cast<const uint2*>(t + (((long)b * C + c) * N + i) * Npad + j));
+    const float2 lo = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&u.x));
+    const float2 hi = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&u.y));
+    v[k][0] = lo.x; v[k][1] = lo.y; v[k][2] = hi.x; v[k][3] = hi.y;
+  }
+  float s[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+  for (int k = 0; k < 16; ++k)
+#pragma unroll
+    for (int p = 0; p < 4; ++p) s[p] += v[k][p];
+  *reinterpret_cast<float4*>(&part[0][warp][4 * lane]) = make_float4(s[0], s[1], s[2], s[3]);
+  __syncthreads();
+  float m[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+  for (int w = 0; w < 8; ++w) {
+    const float4 q = *reinterpret_cast<const float4*>(&part[0][w][4 * lane]);
+    m[0] += q.x; m[1] += q.y; m[2] += q.z; m[3] += q.w;
+  }
+  float q2[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+  for (int p = 0; p < 4; ++p) m[p] *= (1.0f / C);
+#pragma unroll
+  for (int k = 0; k < 16; ++k)
+#pragma unroll
+    for (int p = 0; p < 4; ++p) {
+      const float d = v[k][p] - m[p];
+      q2[p] = fmaf(d, d, q2[p]);
+    }
+  *reinterpret_cast<float4*>(&part[1][warp][4 * lane]) = make_float4(q2[0], q2[1], q2[2], q2[3]);
+  __syncthreads();
+  float r[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+  for (int w = 0; w < 8; ++w) {
+    const float4 q = *reinterpret_cast<const float4*>(&part[1][w][4 * lane]);
+    r[0] += q.x; r[1] += q.y; r[2] += q.z; r[3] += q.w;
+  }
+#pragma unroll
+  for (int p = 0; p < 4; ++p) r[p] = rsqrtf(r[p] * (1.0f / C) + 1e-5f);
+  float g[16], be[16];
+#pragma unroll
+  for (int k = 0; k < 16; ++k) {
+    g[k] = __ldg(gamma + warp * 16 + k);
+    be[k] = __ldg(beta + warp * 16 + k);
+  }
+#pragma unroll
+  for (int p = 0; p < 4; ++p) {
+    __align__(16) __half o[16];
+#pragma unroll
+    for (int k = 0; k < 16; ++k) o[k] = __float2half_rn((v[k][p] - m[p]) * r[p] * g[k] + be[k]);
+    reinterpret_cast<uint4*>(&stage[4 * lane + p][warp * 16])[0] = reinterpret_cast<const uint4*>(o)[0];
+    reinterpret_cast<uint4*>(&stage[4 * lane + p][warp * 16])[1] = reinterpret_cast<const uint4*>(o)[1];
+  }
+  __syncthreads();
+  constexpr int CH = C * 2 / 16;                         // 16-byte chunks per position
+  for (int q = threadIdx.x; q < PJ * CH; q += 256) {
+    const int pj = q / CH, ch = q % CH;
+    if (j0 + pj < N)
+      reinterpret_cast<uint4*>(y + (((long)b * N + i) * N + j0 + pj) * C)[ch] = reinterpret_cast<const uint4*>(&stage[pj][0])[ch];
+  }
+}
+
+// tcgen05 path: the einsum output is bf16 channel-major, C = 128, fp16 result (the next GEMM's A operand)
+void launch_lnc_tc(const bf16* t_cm, __half* y, const float* gamma, const float* beta, const float* seq_mask, int B, int N,
+                   int Npad, cudaStream_t st) {
+  dim3 grid((N + 127) / 128, N, B);
+  lnc128_bf16_kernel<<<grid, 256, 0, st>>>(t_cm, y, gamma, beta, seq_mask, N, Npad);
 }
 template void launch_lnc<float>(const float*, float*, const float*, const float*, const float*, int, int, int, int, cudaStream_t);
 template void launch_lnc<bf16>(const float*, bf16*, const float*, const float*, const float*, int, int, int, int, cudaStream_t);

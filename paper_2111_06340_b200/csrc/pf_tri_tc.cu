@@ -2,8 +2,8 @@
 //     t[bc, i, j] = sum_k a[bc, i, k] * b[bc, j, k]        bc = (batch, channel), a/b channel-major bf16 [B*C, N, Npad]
 // = one N x N x N "NT" GEMM per (batch, channel) on tcgen05 tensor cores (north_star: "channel-batched GEMMs").
 // One CTA = one 128 x 128 tile of one channel: 3-D TMA tiles (k, row, bc) with out-of-range k / rows zero-filled,
-// 3-stage ring, fp32 accumulator in TMEM, epilogue stores fp32 rows (128 B per thread per chunk) for the
-// LayerNorm-across-channels kernel that follows.
+// 3-stage ring, fp32 accumulator in TMEM, epilogue stores bf16 rows (64 B per thread per chunk) for the
+// LayerNorm-across-channels kernel that follows (bf16 like the other inter-kernel intermediates: halves this tensor's traffic).
 #include "pf_internal.h"
 #include "pf_device.cuh"
 #include "pf_tc.cuh"
@@ -20,7 +20,7 @@ constexpr int TRI_SMEM = TRI_BAR_OFF + 256 + 1024;
 
 __global__ void __launch_bounds__(TRI_THREADS, 2)
 tri_einsum_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
-                     float* __restrict__ t, int N, int Npad, const int* __restrict__ key_tiles, int channels) {
+                     bf16* __restrict__ t, int N, int Npad, const int* __restrict__ key_tiles, int channels) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = tc::align_smem_1024(smem_raw);
   uint64_t* full = reinterpret_cast<uint64_t*>(smem + TRI_BAR_OFF);
@@ -81,7 +81,7 @@ tri_einsum_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
     tc::mbar_wait(tmem_full, 0);
     tc::tc_fence_after();
     const uint32_t lane_addr = tmem_base + ((uint32_t)(quarter * 32) << 16);
-    float* dst = t + ((long)bc * N + i) * Npad + j0;
+    bf16* dst = t + ((long)bc * N + i) * Npad + j0;
 #pragma unroll 1
     for (int c0 = 0; c0 < TRI_BN; c0 += 32) {
       if (j0 + c0 >= N) break;
@@ -90,10 +90,16 @@ tri_einsum_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
       tc::tmem_ld_wait();
       if (i < N) {
 #pragma unroll
-        for (int j = 0; j < 32; j += 4)   // Npad is a multiple of 8: whole float4 groups stay inside the padded row
-          if (j0 + c0 + j < Npad)
-            *reinterpret_cast<float4*>(dst + c0 + j) = make_float4(__uint_as_float(v[j]), __uint_as_float(v[j + 1]),
-                                                                  __uint_as_float(v[j + 2]), __uint_as_float(v[j + 3]));
+        for (int j = 0; j < 32; j += 8)   // Npad is a multiple of 8: whole 16-byte groups stay inside the padded row
+          if (j0 + c0 + j < Npad) {
+            uint32_t pk[4];
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+              __nv_bfloat162 h = __floats2bfloat162_rn(__uint_as_float(v[j + 2 * e]), __uint_as_float(v[j + 2 * e + 1]));
+              pk[e] = *reinterpret_cast<uint32_t*>(&h);
+            }
+            *reinterpret_cast<uint4*>(dst + c0 + j) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
+          }
       }
     }
   }
@@ -108,7 +114,7 @@ bool configure_tri_kernel() {
   return e == cudaSuccess;
 }
 
-int launch_tri_einsum_tc(TmaCtx* ctx, const bf16* a_cm, const bf16* b_cm, float* t_cm, int batch, int N, int Npad,
+int launch_tri_einsum_tc(TmaCtx* ctx, const bf16* a_cm, const bf16* b_cm, bf16* t_cm, int batch, int N, int Npad,
                          const int* key_tiles, int channels, int num_sms, cudaStream_t st) {
   (void)num_sms;
   CUtensorMap tmA, tmB;

@@ -335,7 +335,7 @@ struct TcDriver {
     bf16* ACM = buf<bf16>(ar.acm);
     bf16* BCM = buf<bf16>(ar.bcm);
     __half* G = buf<__half>(ar.g);
-    float* TCM = buf<float>(ar.tcm);
+    bf16* TCM = buf<bf16>(ar.tcm);
     __half* TN = buf<__half>(ar.tn);
     {
       G2Desc d = desc_base(B, N, N, c.c_z, 5 * ct);
@@ -365,14 +365,14 @@ struct TcDriver {
       if (!gemm2(d, P * 3.0 * ct * 2.0, h->frac.pair_x)) return false;
     }
     h->prof_begin(KK_TRI, 2.0 * B * ct * (double)N * N * N * h->frac.tri_k,
-                  (double)B * ct * N * Np * (4.0 * h->frac.tri_k + 4.0), st);
+                  (double)B * ct * N * Np * (4.0 * h->frac.tri_k + 2.0), st);
     if (launch_tri_einsum_tc(h->tma, ACM, BCM, TCM, B * ct, N, Np, buf<int>(ar.kt_seq), ct, h->num_sms, st) != 0) {
       err = std::string("tri_einsum_tc: ") + tc_last_error();
       return false;
     }
     h->prof_end(st);
-    h->prof_begin(KK_LNC, 0.0, P * ct * 6.0 * h->frac.lnc, st);
-    launch_lnc<__half>(TCM, TN, w + t.ln_out_g, w + t.ln_out_b, seq_mask, B, ct, N, Np, st);
+    h->prof_begin(KK_LNC, 0.0, P * ct * 4.0 * h->frac.lnc, st);
+    launch_lnc_tc(TCM, TN, w + t.ln_out_g, w + t.ln_out_b, seq_mask, B, N, Np, st);
     h->prof_end(st);
     G2Desc d = desc_base(B, N, N, ct, c.c_z);
     d.a_mode = 1; d.A = TN; d.op_fmt = 1; d.Wt = w16 + (incoming ? h->tc.ti_wz : h->tc.to_wz); d.bias = w + t.b_z;
