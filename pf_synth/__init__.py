@@ -418,3 +418,89 @@ def make_extra_inputs(seed: int, B: int, S: int, N: int, d: ExtraDims = EXTRA, l
     """e[B,S,N,c_e], z[B,N,N,c_z] ~ N(0,1) (garbage in the padding) and the masks of make_inputs."""
     main = Dims(c_m=d.c_e, c_z=d.c_z)
     return make_inputs(seed, B, S, N, main, lengths=lengths, msa_mask_frac_max=msa_mask_frac_max)
+
+
+# ----------------------------------------------------------------------------------------------
+# structure module + heads (SURVEY.md §8(f)4; DESIGN.md §2d readings M.0-M.6, H.1-H.3)
+# ----------------------------------------------------------------------------------------------
+
+@dataclass(frozen=True)
+class StructDims:
+    c_m: int = 256
+    c_z: int = 128
+    c_s: int = 384            # single representation
+    heads: int = 12           # IPA heads
+    c_ipa: int = 16           # scalar channels per head
+    n_qp: int = 4             # query / key points per head
+    n_pv: int = 8             # value points per head
+    n_layers: int = 8         # layers, weights shared
+    c_resnet: int = 128       # torsion-angle resnet width
+    n_torsion: int = 7
+    n_dist_bins: int = 64     # distogram head
+    n_msa_classes: int = 23   # masked-MSA head
+    n_lddt_bins: int = 50     # pLDDT head
+    c_lddt: int = 128
+    pos_scale: float = 10.0   # frame translations are in nanometres, positions in Angstrom
+
+    @property
+    def c_cat(self):          # width of the concatenated IPA outputs (M.2)
+        return self.heads * (self.c_z + self.c_ipa + 4 * self.n_pv)
+
+
+STRUCT = StructDims()
+
+
+def struct_spec(d: StructDims = STRUCT):
+    """Ordered (name, shape, kind) of the structure-module / heads blob (row-major [in, out], as Appendix B)."""
+    cs, cz, cm, H, c, cr, cl = d.c_s, d.c_z, d.c_m, d.heads, d.c_ipa, d.c_resnet, d.c_lddt
+    spec = [("w_single", (cm, cs), "W"), ("b_single", (cs,), "bias"),
+            ("ln_s_g", (cs,), "gamma"), ("ln_s_b", (cs,), "beta"), ("ln_z_g", (cz,), "gamma"), ("ln_z_b", (cz,), "beta"),
+            ("w_in", (cs, cs), "W"), ("b_in", (cs,), "bias"),
+            ("w_q", (cs, H * c), "W"), ("w_k", (cs, H * c), "W"), ("w_v", (cs, H * c), "W"),
+            ("w_qp", (cs, H * d.n_qp * 3), "W"), ("w_kp", (cs, H * d.n_qp * 3), "W"), ("w_vp", (cs, H * d.n_pv * 3), "W"),
+            ("w_b", (cz, H), "W"), ("g_head", (H,), "bias"),
+            ("w_out", (d.c_cat, cs), "W"), ("b_out", (cs,), "bias"),
+            ("ln_ipa_g", (cs,), "gamma"), ("ln_ipa_b", (cs,), "beta")]
+    for i in (1, 2, 3):
+        spec += [(f"w_t{i}", (cs, cs), "W"), (f"b_t{i}", (cs,), "bias")]
+    spec += [("ln_tr_g", (cs,), "gamma"), ("ln_tr_b", (cs,), "beta"),
+             ("w_bb", (cs, 6), "W"), ("b_bb", (6,), "bias"),
+             ("w_a1", (cs, cr), "W"), ("b_a1", (cr,), "bias"), ("w_a2", (cs, cr), "W"), ("b_a2", (cr,), "bias")]
+    for r in (1, 2):
+        spec += [(f"w_r{r}a", (cr, cr), "W"), (f"b_r{r}a", (cr,), "bias"), (f"w_r{r}b", (cr, cr), "W"), (f"b_r{r}b", (cr,), "bias")]
+    spec += [("w_alpha", (cr, 2 * d.n_torsion), "W"), ("b_alpha", (2 * d.n_torsion,), "bias"),
+             ("w_dg", (cz, d.n_dist_bins), "W"), ("b_dg", (d.n_dist_bins,), "bias"),
+             ("w_mm", (cm, d.n_msa_classes), "W"), ("b_mm", (d.n_msa_classes,), "bias"),
+             ("ln_l_g", (cs,), "gamma"), ("ln_l_b", (cs,), "beta"),
+             ("w_l1", (cs, cl), "W"), ("b_l1", (cl,), "bias"), ("w_l2", (cl, cl), "W"), ("b_l2", (cl,), "bias"),
+             ("w_l3", (cl, d.n_lddt_bins), "W"), ("b_l3", (d.n_lddt_bins,), "bias")]
+    return spec
+
+
+def struct_floats(d: StructDims = STRUCT) -> int:
+    return sum(int(np.prod(shape)) for _, shape, _ in struct_spec(d))
+
+
+def make_struct_weights(seed: int, d: StructDims = STRUCT):
+    """R8 recipe (the structure module runs in fp32 on both sides: no bf16 rounding of its weights).  The backbone-update
+    Linear is scaled by 0.3 so that eight layers of frame updates stay protein-sized (a walk of a few nanometres)."""
+    g = rng(seed, 4000)
+    out = {}
+    for name, shape, kind in struct_spec(d):
+        r = g.standard_normal(shape, dtype=np.float32)
+        if kind == "W":
+            out[name] = (r / np.float32(np.sqrt(shape[0])) * np.float32(0.3 if name == "w_bb" else 1.0)).astype(np.float32)
+        elif kind == "gamma":
+            out[name] = (1.0 + 0.1 * r).astype(np.float32)
+        else:
+            out[name] = (0.1 * r).astype(np.float32)
+    return out
+
+
+def pack_struct_blob(w, d: StructDims = STRUCT) -> np.ndarray:
+    parts = []
+    for name, shape, _ in struct_spec(d):
+        a = np.asarray(w[name], dtype=np.float32)
+        assert a.shape == tuple(shape), (name, a.shape, shape)
+        parts.append(a.reshape(-1))
+    return np.ascontiguousarray(np.concatenate(parts))
