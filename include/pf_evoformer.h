@@ -142,8 +142,8 @@ const char* pf_last_error(void);
  *   E.2 recycling embedder  z_ij += LN_z(zprev_ij) + Lin_d(onehot_bins(|xprev_i - xprev_j|)),  m_0i += LN_m(mprev_0i)
  *                           (n_dist_bins lower edges evenly spaced from first_break to last_break; the last bin is open)
  *   E.3 recycled trunk      n_cycles x (E.1, E.2 with the previous cycle's trunk output — zeros in the first cycle —, trunk)
- * All arithmetic is fp32.  xprev (previous C-beta positions, Angstrom) would come from the structure module, which this
- * library does not contain: it is an input, held constant over the cycles; NULL = no previous structure (no bin is set).
+ * All arithmetic is fp32.  In pf_evoformer_forward_recycled xprev (previous positions, Angstrom) is an input held constant over
+ * the cycles; NULL = no previous structure (no bin is set).  pf_fold_forward (further down) feeds it from the structure module.
  * ---------------------------------------------------------------------------------------------- */
 typedef struct pf_embedder pf_embedder_t;   /* opaque; owns device weights and a small grow-only workspace */
 typedef struct pf_extra_msa pf_extra_msa_t; /* the extra-MSA stack, declared further down */
@@ -233,6 +233,81 @@ long long pf_extra_msa_last_launch_count(const pf_extra_msa_t* x);
 pf_status pf_extra_msa_set_profiling(pf_extra_msa_t* x, int enable);
 pf_status pf_extra_msa_get_profile(pf_extra_msa_t* x, int kind, long long* launches, double* ms, double* flops, double* bytes);
 void pf_extra_msa_destroy(pf_extra_msa_t* x);
+
+/* ------------------------------------------------------------------------------------------------
+ * Structure module and output heads: the last stage of the network the paper's GPU stage runs ("a new
+ * Evoformer architecture" feeding "the structure module"; AlphaFold v2.0.1 monomer).
+ * PAPER.md prints no formula; readings M.0-M.6 / H.1-H.3, per protein:
+ *   M.0 s^single_i = Lin_single(m_0i)                         M.1 s^init = LN_s(s^single), zn = LN_z(z), s = Lin_in(s^init), T_i = (I, 0)
+ *   M.2 invariant point attention, H heads: q, k, v = Lin0(s) [c per head]; query / key points qp, kp [P_q x 3], value points vp
+ *       [P_v x 3] = Lin0(s) in the residue's frame, mapped to the global frame by T; b = Lin0(zn) [H];
+ *       a_hij = softmax_j( sqrt(1/3) ( q_ih.k_jh / sqrt(c) + b_ijh - softplus(g_h) sqrt(2 / (9 P_q)) / 2 sum_p |T_i qp_ihp - T_j kp_jhp|^2 ) + NEG(sigma_j) )
+ *       IPA_i = Lin_out( concat[ sum_j a zn_ij (H c_z) | sum_j a v_jh (H c) | T_i^-1 sum_j a T_j vp_jhp (H P_v 3) | its norms, sqrt(|.|^2 + 1e-8) (H P_v) ] )
+ *   M.3 s = LN_ipa(s + IPA);  s = LN_tr(s + Lin_3(relu(Lin_2(relu(Lin_1(s))))))            (n_layers layers, weights shared)
+ *   M.4 (b, c, d, u) = Lin_bb(s_i); R^upd from the unit quaternion (1, b, c, d) / |.|;  t_i <- R_i u + t_i, R_i <- R_i R^upd
+ *   M.5 a = Lin_a1(s) + Lin_a2(s^init); twice a += Lin_rb(relu(Lin_ra(relu(a)))); alpha = Lin_alpha(relu(a)) [n_torsion, 2], normalised
+ *   M.6 positions x_i = pos_scale t_i (Angstrom; the frame origin = C-alpha).  All-atom side-chain coordinates are not computed
+ *       (they need per-residue ideal-geometry tables that are not on this box): x is what the recycling embedder (E.2) receives.
+ *   H.1 distogram logits_ij = Lin_dg(z_ij) + Lin_dg(z_ji)    H.2 masked-MSA logits_si = Lin_mm(m_si)
+ *   H.3 pLDDT_i = 100 sum_k softmax(Lin_l3(relu(Lin_l2(relu(Lin_l1(LN_l(s_i)))))))_k (k + 1/2) / n_lddt_bins
+ * All arithmetic is fp32 (tolerance 1e-4 max-abs against the fp64 oracle on s, frames in nanometres, angles; 1e-3 on x in
+ * Angstrom and pLDDT in points).  Masked residues act as masked keys only; outputs at masked residues are unspecified but finite.
+ * Weights blob (fp32, every matrix row-major [in, out]), in this order: W_single b | LN_s g b | LN_z g b | W_in b | W_q | W_k |
+ * W_v [c_s, H c] | W_qp | W_kp [c_s, H P_q 3] | W_vp [c_s, H P_v 3] | W_b [c_z, H] | g_head [H] | W_out [H (c_z + c + 4 P_v), c_s] b |
+ * LN_ipa g b | W_1 b W_2 b W_3 b | LN_tr g b | W_bb [c_s, 6] b | W_a1 b W_a2 b [c_s, c_r] | 2 x (W_ra b W_rb b [c_r, c_r]) |
+ * W_alpha [c_r, 2 n_torsion] b | W_dg [c_z, n_dist_bins] b | W_mm [c_m, n_msa_classes] b | LN_l g b | W_l1 [c_s, c_l] b |
+ * W_l2 [c_l, c_l] b | W_l3 [c_l, n_lddt_bins] b.
+ * ---------------------------------------------------------------------------------------------- */
+typedef struct pf_structure pf_structure_t;   /* opaque; owns device weights and a grow-only workspace */
+typedef struct {
+  int c_m;            /* 256 */
+  int c_z;            /* 128 */
+  int c_s;            /* single-representation channels (384) */
+  int heads;          /* IPA heads H (12; at most 32) */
+  int c_ipa;          /* scalar channels per head c (16) */
+  int n_qp;           /* query / key points per head P_q (4) */
+  int n_pv;           /* value points per head P_v (8) */
+  int n_layers;       /* default layer count (8) */
+  int c_resnet;       /* torsion-angle resnet width (128) */
+  int n_torsion;      /* 7 */
+  int n_dist_bins;    /* distogram bins (64) */
+  int n_msa_classes;  /* masked-MSA classes (23) */
+  int n_lddt_bins;    /* pLDDT bins (50) */
+  int c_lddt;         /* pLDDT head width (128) */
+  float pos_scale;    /* Angstrom per unit of frame translation (10) */
+} pf_struct_config;
+/* fp32 values in the blob described above; 0 for a null / unsupported config. */
+size_t pf_structure_floats(const pf_struct_config* cfg);
+/* Errors: INVALID_ARG (null), SHAPE (dims, blob length), ARCH, ALLOC, CUDA. */
+pf_status pf_structure_create(pf_structure_t** out, const float* weights_host, size_t n_weight_floats,
+                              const pf_struct_config* cfg);
+/* M.0-M.6 (+ H.3) for a batch, asynchronously on cuda_stream.  Inputs (device, read only): msa[B,S,N,c_m] (only row s = 0 is
+ * read), pair[B,N,N,c_z], seq_mask[B,N].  Outputs (device, each may be NULL): s_out[B,N,c_s], frames_out[B,N,12] (R row-major
+ * 3 x 3, then t, nanometres), x_out[B,N,3] (Angstrom), alpha_out[B,N,n_torsion,2], plddt_out[B,N].  n_layers >= 1 (the
+ * config's value is the AlphaFold default).  Limit: heads x N x 4 bytes <= ~200 KB (N <= 4000 at 12 heads).
+ * Errors: INVALID_ARG, SHAPE, ALLOC (workspace: ~N^2 (c_z + heads) floats per protein), CUDA. */
+pf_status pf_structure_forward(pf_structure_t* h, const float* msa_dev, const float* pair_dev, const float* seq_mask_dev, int B,
+                               int S, int N, int n_layers, float* s_out, float* frames_out, float* x_out, float* alpha_out,
+                               float* plddt_out, void* cuda_stream);
+/* H.1 / H.2: distogram_out[B,N,N,n_dist_bins] and / or masked_msa_out[B,S,N,n_msa_classes] (device; NULL skips a head). */
+pf_status pf_heads_forward(pf_structure_t* h, const float* msa_dev, const float* pair_dev, int B, int S, int N,
+                           float* distogram_out, float* masked_msa_out, void* cuda_stream);
+long long pf_structure_last_launch_count(const pf_structure_t* h);
+void pf_structure_destroy(pf_structure_t* h);
+/* The whole GPU stage: n_cycles x (pf_embedder_forward with the PREVIOUS cycle's structure-module
+ * positions — x_prev0_dev [B,N,3] or NULL (no previous structure) in the first cycle —, [extra-MSA stack], pf_evoformer_forward,
+ * pf_structure_forward).  Arguments as pf_evoformer_forward_recycled; x_cycles_out [n_cycles,B,N,3] (device, required) receives the
+ * positions after every cycle (the last slice is the prediction; earlier slices are what the next cycle's recycling embedder
+ * read, so a checker can replay the distance-bin decisions); s_out / frames_out / alpha_out / plddt_out (may be NULL) are the
+ * last cycle's.  pf_structure_last_launch_count(sm) then counts every launch of the call.
+ * Errors: those of the calls it makes; INVALID_ARG if x_cycles_out is NULL. */
+pf_status pf_fold_forward(pf_evoformer_t* h, pf_embedder_t* e, pf_extra_msa_t* x, pf_structure_t* sm,
+                          const float* target_feat_dev, const int* residue_index_dev, const float* msa_feat_dev,
+                          const float* x_prev0_dev, const float* extra_msa_feat_dev, float* extra_msa_dev,
+                          const float* extra_msa_mask_dev, float* msa_dev, float* pair_dev, const float* seq_mask_dev,
+                          const float* msa_mask_dev, int B, int S, int S_e, int N, int n_blocks, int n_extra_blocks, int n_cycles,
+                          int n_layers, float* x_cycles_out, float* s_out, float* frames_out, float* alpha_out, float* plddt_out,
+                          void* cuda_stream);
 
 /* ------------------------------------------------------------------------------------------------
  * Length-bucketing batch scheduler ("sort by length ... share the compiled model";

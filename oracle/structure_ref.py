@@ -182,3 +182,35 @@ def plddt(s, w):
     nb = logits.shape[-1]
     centers = (np.arange(nb, dtype=F64) + 0.5) / nb
     return logits, 100.0 * (softmax(logits, axis=-1) * centers).sum(axis=-1)
+
+
+def fold(target_feat, residue_index, msa_feat, seq_mask, msa_mask, w_embed, blocks, w_struct, n_cycles, x_prev0=None,
+         x_forced=None, head_dim=32, extra=None, struct_kw=None, **embed_kw):
+    """The whole GPU stage for one protein: n_cycles x (E.1, E.2 with the previous cycle's first MSA
+    row, pair representation and structure-module positions, [extra-MSA stack], trunk, M.0-M.6).
+    x_prev0 [N,3] or None: positions the first cycle's recycling embedder sees (None = no bin set).
+    x_forced: optional list of n_cycles - 1 position arrays used INSTEAD of this function's own positions as the recycling
+    input of cycles 1 .. n_cycles-1.  The distance bins are a floating-point comparison deciding an integer; a checker hands
+    in the positions the other implementation produced so that both sides decide on the same numbers.
+    -> dict(m, z, x_cycles [n_cycles, N, 3], and the last cycle's structure_module outputs)."""
+    from .embed_ref import embed_cycle, extra_msa_embedder
+    from .evoformer_ref import evoformer_trunk
+    from .extra_msa_ref import extra_msa_stack
+    N = np.asarray(msa_feat).shape[1]
+    c_m, c_z = np.asarray(w_embed["w_m"]).shape[1], np.asarray(w_embed["w_a"]).shape[1]
+    m0_prev, z_prev = np.zeros((N, c_m)), np.zeros((N, N, c_z))
+    x_prev = np.zeros((N, 3)) if x_prev0 is None else x_prev0
+    xs, out, m, z = [], None, None, None
+    for cyc in range(n_cycles):
+        m, z = embed_cycle(target_feat, residue_index, msa_feat, m0_prev, z_prev, x_prev, w_embed, **embed_kw)
+        if extra is not None:
+            xf, xmask, xblocks, xhd = extra
+            _, z = extra_msa_stack(extra_msa_embedder(xf, w_embed), z, seq_mask, xmask, xblocks, xhd, head_dim)
+        m, z = evoformer_trunk(m, z, seq_mask, msa_mask, blocks, head_dim)
+        out = structure_module(m[0], z, seq_mask, w_struct, **(struct_kw or {}))
+        xs.append(out["x"])
+        m0_prev, z_prev = m[0], z
+        x_prev = out["x"] if x_forced is None or cyc >= len(x_forced) else x_forced[cyc]
+    res = dict(out)
+    res.update(m=m, z=z, x_cycles=np.stack(xs))
+    return res

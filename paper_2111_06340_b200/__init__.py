@@ -32,6 +32,8 @@ EXPORTED_SYMBOLS = (
     "pf_evoformer_forward_recycled",
     "pf_extra_msa_block_floats", "pf_extra_msa_create", "pf_extra_msa_forward", "pf_extra_msa_forward_substep",
     "pf_extra_msa_last_launch_count", "pf_extra_msa_set_profiling", "pf_extra_msa_get_profile", "pf_extra_msa_destroy",
+    "pf_structure_floats", "pf_structure_create", "pf_structure_forward", "pf_heads_forward",
+    "pf_structure_last_launch_count", "pf_structure_destroy", "pf_fold_forward",
 )
 
 
@@ -50,6 +52,12 @@ class PfEmbedConfig(Structure):
 class PfExtraConfig(Structure):
     _fields_ = [("c_e", c_int), ("c_z", c_int), ("heads_msa", c_int), ("heads_pair", c_int), ("head_dim_pair", c_int),
                 ("c_opm", c_int), ("c_tri", c_int), ("transition_n", c_int), ("n_blocks_max", c_int)]
+
+
+class PfStructConfig(Structure):
+    _fields_ = [("c_m", c_int), ("c_z", c_int), ("c_s", c_int), ("heads", c_int), ("c_ipa", c_int), ("n_qp", c_int),
+                ("n_pv", c_int), ("n_layers", c_int), ("c_resnet", c_int), ("n_torsion", c_int), ("n_dist_bins", c_int),
+                ("n_msa_classes", c_int), ("n_lddt_bins", c_int), ("c_lddt", c_int), ("pos_scale", c_float)]
 
 
 class PfError(RuntimeError):
@@ -146,6 +154,20 @@ def lib() -> ctypes.CDLL:
         L.pf_evoformer_forward_recycled.argtypes = [c_void_p] * 14 + [c_int] * 7 + [c_void_p]
         L.pf_embedder_forward_extra.restype = c_int
         L.pf_embedder_forward_extra.argtypes = [c_void_p, c_void_p, c_void_p, c_int, c_int, c_int, c_void_p]
+        L.pf_structure_floats.restype = c_size_t
+        L.pf_structure_floats.argtypes = [POINTER(PfStructConfig)]
+        L.pf_structure_create.restype = c_int
+        L.pf_structure_create.argtypes = [POINTER(c_void_p), c_void_p, c_size_t, POINTER(PfStructConfig)]
+        L.pf_structure_forward.restype = c_int
+        L.pf_structure_forward.argtypes = [c_void_p] * 4 + [c_int] * 4 + [c_void_p] * 6
+        L.pf_heads_forward.restype = c_int
+        L.pf_heads_forward.argtypes = [c_void_p] * 3 + [c_int] * 3 + [c_void_p] * 3
+        L.pf_structure_last_launch_count.restype = c_longlong
+        L.pf_structure_last_launch_count.argtypes = [c_void_p]
+        L.pf_structure_destroy.restype = None
+        L.pf_structure_destroy.argtypes = [c_void_p]
+        L.pf_fold_forward.restype = c_int
+        L.pf_fold_forward.argtypes = [c_void_p] * 15 + [c_int] * 8 + [c_void_p] * 6
         _lib = L
     return _lib
 
@@ -358,6 +380,73 @@ def forward_recycled(evo: "Evoformer", emb: Embedder, target_feat, residue_index
                                                _ptr(extra_msa), _ptr(extra_msa_mask), _ptr(msa), _ptr(pair), _ptr(seq_mask),
                                                _ptr(msa_mask), B, S, S_e, N, n_blocks, n_extra_blocks, n_cycles,
                                                evo._stream(stream)))
+
+
+def make_struct_config(c_m=256, c_z=128, c_s=384, heads=12, c_ipa=16, n_qp=4, n_pv=8, n_layers=8, c_resnet=128, n_torsion=7,
+                       n_dist_bins=64, n_msa_classes=23, n_lddt_bins=50, c_lddt=128, pos_scale=10.0) -> PfStructConfig:
+    return PfStructConfig(c_m, c_z, c_s, heads, c_ipa, n_qp, n_pv, n_layers, c_resnet, n_torsion, n_dist_bins, n_msa_classes,
+                          n_lddt_bins, c_lddt, pos_scale)
+
+
+class StructureModule:
+    """pf_structure_* / pf_heads_forward wrapper (pointers and sizes only)."""
+
+    def __init__(self, weights_blob: np.ndarray, cfg: PfStructConfig):
+        blob = np.ascontiguousarray(weights_blob, dtype=np.float32)
+        self._s = c_void_p()
+        self.cfg = cfg
+        _check(lib().pf_structure_create(byref(self._s), blob.ctypes.data, blob.size, byref(cfg)))
+
+    @staticmethod
+    def _stream(stream):
+        if stream is None:
+            import torch
+            return torch.cuda.current_stream().cuda_stream
+        return stream
+
+    def forward(self, msa, pair, seq_mask, n_layers=None, s_out=None, frames_out=None, x_out=None, alpha_out=None,
+                plddt_out=None, stream=None):
+        B, S, N = msa.shape[0], msa.shape[1], msa.shape[2]
+        _check(lib().pf_structure_forward(self._s, _ptr(msa), _ptr(pair), _ptr(seq_mask), B, S, N,
+                                          self.cfg.n_layers if n_layers is None else n_layers, _ptr(s_out), _ptr(frames_out),
+                                          _ptr(x_out), _ptr(alpha_out), _ptr(plddt_out), self._stream(stream)))
+
+    def heads(self, msa, pair, distogram_out=None, masked_msa_out=None, stream=None):
+        ref = msa if msa is not None else pair
+        B, N = ref.shape[0], ref.shape[2]
+        S = msa.shape[1] if msa is not None else 1
+        _check(lib().pf_heads_forward(self._s, _ptr(msa), _ptr(pair), B, S, N, _ptr(distogram_out), _ptr(masked_msa_out),
+                                      self._stream(stream)))
+
+    def last_launch_count(self) -> int:
+        return int(lib().pf_structure_last_launch_count(self._s))
+
+    def close(self):
+        if self._s:
+            lib().pf_structure_destroy(self._s)
+            self._s = c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def fold_forward(evo: "Evoformer", emb: Embedder, sm: StructureModule, target_feat, residue_index, msa_feat, x_prev0, msa,
+                 pair, seq_mask, msa_mask, n_blocks: int, n_cycles: int, x_cycles_out, n_layers=None, s_out=None,
+                 frames_out=None, alpha_out=None, plddt_out=None, stream=None, extra: "ExtraMsaStack" = None,
+                 extra_msa_feat=None, extra_msa=None, extra_msa_mask=None, n_extra_blocks: int = 0):
+    """pf_fold_forward: n_cycles x (embedders fed with the previous cycle's positions [, extra-MSA stack], trunk, structure
+    module); msa / pair receive the last trunk output, x_cycles_out [n_cycles,B,N,3] the positions after every cycle."""
+    B, S, N = msa.shape[0], msa.shape[1], msa.shape[2]
+    S_e = extra_msa.shape[1] if extra is not None else 0
+    _check(lib().pf_fold_forward(evo._h, emb._e, extra._x if extra is not None else None, sm._s, _ptr(target_feat),
+                                 _ptr(residue_index), _ptr(msa_feat), _ptr(x_prev0), _ptr(extra_msa_feat), _ptr(extra_msa),
+                                 _ptr(extra_msa_mask), _ptr(msa), _ptr(pair), _ptr(seq_mask), _ptr(msa_mask), B, S, S_e, N,
+                                 n_blocks, n_extra_blocks, n_cycles, sm.cfg.n_layers if n_layers is None else n_layers,
+                                 _ptr(x_cycles_out), _ptr(s_out), _ptr(frames_out), _ptr(alpha_out), _ptr(plddt_out),
+                                 evo._stream(stream)))
 
 
 class Scheduler:

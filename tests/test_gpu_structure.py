@@ -1,0 +1,147 @@
+"""GPU parity of the structure module, the heads and the whole recycled GPU stage (readings M.0-M.6, H.1-H.3,
+DESIGN.md §2d) against the fp64 oracle (oracle/structure_ref.py), through the C ABI.  Everything here is fp32 arithmetic:
+tolerance 1e-4 max-abs on quantities of order one (s, rotation matrices, translations in nanometres, unit angle vectors),
+1e-3 on positions in Angstrom (10 x a translation) and on pLDDT (100 x a probability-weighted mean); outputs at masked
+residues are unspecified but must be finite."""
+import numpy as np
+import pytest
+
+import paper_2111_06340_b200 as pf
+import pf_synth as ps
+from oracle import structure_ref as sr
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-4
+D = ps.STRUCT
+
+
+def _dev(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def _run_structure(w, msa, pair, sm, n_layers):
+    import torch
+    B, S, N = msa.shape[:3]
+    h = pf.StructureModule(ps.pack_struct_blob(w), pf.make_struct_config())
+    out = {"s": torch.empty((B, N, D.c_s), device="cuda"), "frames": torch.empty((B, N, 12), device="cuda"),
+           "x": torch.empty((B, N, 3), device="cuda"), "alpha": torch.empty((B, N, D.n_torsion, 2), device="cuda"),
+           "plddt": torch.empty((B, N), device="cuda")}
+    h.forward(_dev(msa), _dev(pair), _dev(sm), n_layers, out["s"], out["frames"], out["x"], out["alpha"], out["plddt"])
+    torch.cuda.synchronize()
+    launches = h.last_launch_count()
+    h.close()
+    return {k: v.cpu().numpy() for k, v in out.items()}, launches
+
+
+def _check_structure(got, msa, pair, sm, w, n_layers):
+    worst = {}
+    for b in range(msa.shape[0]):
+        ref = sr.structure_module(msa[b, 0], pair[b], sm[b], w, n_layers=n_layers)
+        _, pl = sr.plddt(ref["s"], w)
+        v = sm[b] > 0
+        pairs = [("s", got["s"][b], ref["s"], TOL), ("R", got["frames"][b][:, :9].reshape(-1, 3, 3), ref["R"], TOL),
+                 ("t", got["frames"][b][:, 9:], ref["t"], TOL), ("x", got["x"][b], ref["x"], 10 * TOL),
+                 ("alpha", got["alpha"][b], ref["alpha"], TOL), ("plddt", got["plddt"][b], pl, 10 * TOL)]
+        for name, g, r, tol in pairs:
+            assert np.isfinite(g).all(), name
+            e = float(np.abs(g[v] - r[v]).max())
+            worst[name] = max(worst.get(name, 0.0), e)
+            assert e <= tol, (name, b, e, tol)
+    return worst
+
+
+@pytest.mark.parametrize("B,S,N,lengths,n_layers", [(1, 2, 32, None, 1), (2, 3, 40, [40, 29], 8), (3, 1, 65, [65, 1, 50], 2),
+                                                    (1, 4, 130, [117], 8)])
+def test_structure_module_matches_oracle(B, S, N, lengths, n_layers):
+    w = ps.make_struct_weights(5)
+    msa, pair, sm, _ = ps.make_inputs(7, B, S, N, lengths=lengths)
+    got, launches = _run_structure(w, msa, pair, sm, n_layers)
+    worst = _check_structure(got, msa, pair, sm, w, n_layers)
+    print(f"structure module B={B} N={N} layers={n_layers}: launches={launches} worst max-abs {worst}")
+    assert launches > 0
+
+
+def test_heads_match_oracle():
+    import torch
+    w = ps.make_struct_weights(6)
+    B, S, N = 2, 5, 37
+    msa, pair, _, _ = ps.make_inputs(8, B, S, N)
+    h = pf.StructureModule(ps.pack_struct_blob(w), pf.make_struct_config())
+    dg = torch.empty((B, N, N, D.n_dist_bins), device="cuda")
+    mm = torch.empty((B, S, N, D.n_msa_classes), device="cuda")
+    h.heads(_dev(msa), _dev(pair), dg, mm)
+    torch.cuda.synchronize()
+    assert h.last_launch_count() == 3
+    h.heads(None, _dev(pair), dg, None)          # one head alone
+    torch.cuda.synchronize()
+    h.close()
+    for b in range(B):
+        assert np.abs(dg[b].cpu().numpy() - sr.distogram_logits(pair[b], w)).max() <= TOL
+        assert np.abs(mm[b].cpu().numpy() - sr.masked_msa_logits(msa[b], w)).max() <= TOL
+
+
+def test_structure_handle_reuse_and_errors():
+    import torch
+    w = ps.make_struct_weights(5)
+    h = pf.StructureModule(ps.pack_struct_blob(w), pf.make_struct_config())
+    for (B, N) in ((2, 48), (1, 20), (2, 48)):     # grow, shrink, grow again on one handle
+        msa, pair, sm, _ = ps.make_inputs(9, B, 2, N, lengths=[N] + [N - 7] * (B - 1))
+        x = torch.empty((B, N, 3), device="cuda")
+        h.forward(_dev(msa), _dev(pair), _dev(sm), 2, x_out=x)
+        torch.cuda.synchronize()
+        for b in range(B):
+            ref = sr.structure_module(msa[b, 0], pair[b], sm[b], w, n_layers=2)
+            v = sm[b] > 0
+            assert np.abs(x[b].cpu().numpy()[v] - ref["x"][v]).max() <= 10 * TOL
+    with pytest.raises(pf.PfError):
+        h.forward(_dev(msa), None, _dev(sm), 2)
+    h.close()
+    with pytest.raises(pf.PfError):
+        pf.StructureModule(ps.pack_struct_blob(w)[:-1], pf.make_struct_config())
+
+
+def test_fold_recycled_with_structure_module():
+    """n_cycles x (embedders fed by the previous cycle's structure, trunk, structure module) on the fp32 trunk.  The distance
+    bins of the recycling embedder are a floating-point comparison deciding an integer: the oracle is handed the positions
+    the CUDA path produced in the earlier cycles (x_cycles_out exists for that), so both sides decide on the same numbers;
+    each cycle's own positions are then compared."""
+    import torch
+    B, S, N, n_blocks, n_cycles, n_layers = 2, 6, 28, 1, 3, 4
+    lengths = [28, 19]
+    blocks = ps.make_weights(3, n_blocks)
+    we, wst = ps.make_embed_weights(3), ps.make_struct_weights(3)
+    tf, ri, mf, _ = ps.make_features(4, B, S, N)
+    _, _, sm, mm = ps.make_inputs(4, B, S, N, lengths=lengths, msa_mask_frac_max=0.3)
+    evo = pf.Evoformer(ps.pack_blob(blocks), pf.make_config(n_blocks, pf.PF_F32))
+    emb = pf.Embedder(ps.pack_embed_blob(we), pf.make_embed_config())
+    stm = pf.StructureModule(ps.pack_struct_blob(wst), pf.make_struct_config())
+    m = torch.empty((B, S, N, 256), device="cuda")
+    z = torch.empty((B, N, N, 128), device="cuda")
+    xc = torch.empty((n_cycles, B, N, 3), device="cuda")
+    s_out = torch.empty((B, N, D.c_s), device="cuda")
+    pl = torch.empty((B, N), device="cuda")
+    pf.fold_forward(evo, emb, stm, _dev(tf), _dev(ri), _dev(mf), None, m, z, _dev(sm), _dev(mm), n_blocks, n_cycles, xc,
+                    n_layers=n_layers, s_out=s_out, plddt_out=pl)
+    torch.cuda.synchronize()
+    assert stm.last_launch_count() > 0
+    xc_h, m_h, z_h, s_h = xc.cpu().numpy(), m.cpu().numpy(), z.cpu().numpy(), s_out.cpu().numpy()
+    assert all(np.isfinite(a).all() for a in (xc_h, m_h, z_h, s_h))
+    worst = {"x": 0.0, "m": 0.0, "z": 0.0, "s": 0.0}
+    for b in range(B):
+        ref = sr.fold(tf[b], ri[b], mf[b], sm[b], mm[b], we, blocks, wst, n_cycles,
+                      x_forced=[xc_h[c, b] for c in range(n_cycles - 1)], struct_kw=dict(n_layers=n_layers))
+        v = sm[b] > 0
+        vm = (mm[b][:, None] * sm[b][None, :]) > 0
+        vz = (sm[b][:, None] * sm[b][None, :]) > 0
+        worst["x"] = max(worst["x"], float(np.abs(xc_h[:, b][:, v] - ref["x_cycles"][:, v]).max()))
+        worst["m"] = max(worst["m"], float(np.abs(m_h[b][vm] - ref["m"][vm]).max()))
+        worst["z"] = max(worst["z"], float(np.abs(z_h[b][vz] - ref["z"][vz]).max()))
+        worst["s"] = max(worst["s"], float(np.abs(s_h[b][v] - ref["s"][v]).max()))
+    print(f"fold, {n_cycles} cycles: launches={stm.last_launch_count()} worst max-abs {worst}")
+    # three chained cycles of (fp32 trunk block at 1e-4, structure module at 1e-4): 3e-4 on the representations, ten times that
+    # on positions in Angstrom
+    assert worst["m"] <= 3e-4 and worst["z"] <= 3e-4 and worst["s"] <= 3e-4 and worst["x"] <= 3e-3, worst
+    for h in (evo, emb, stm):
+        h.close()

@@ -283,3 +283,32 @@ def test_full_dims_run_and_shapes():
     assert np.abs(o["x"] - D.pos_scale * o["t"]).max() == 0.0
     assert all(np.isfinite(v).all() for v in o.values())
     assert len(ps.pack_struct_blob(w)) == ps.struct_floats()
+
+
+def test_fold_composes_the_pinned_parts():
+    """fold = recycled trunk (oracle/embed_ref.py, pinned in test_oracle_embed.py) + structure module per cycle; forcing the
+    function's own positions back in changes nothing, forcing other positions changes the next cycle (negative control)."""
+    from oracle import embed_ref
+    S, N = 3, 10
+    blocks = ps.make_weights(2, 1)
+    we, wst = ps.make_embed_weights(2), ps.make_struct_weights(2)
+    tf, ri, mf, _ = ps.make_features(5, 1, S, N)
+    _, _, sm, mm = ps.make_inputs(5, 1, S, N, lengths=[8])
+    kw = dict(struct_kw=dict(n_layers=2))
+    one = sr.fold(tf[0], ri[0], mf[0], sm[0], mm[0], we, blocks, wst, 1, **kw)
+    m1, z1 = embed_ref.recycled_trunk(tf[0], ri[0], mf[0], np.zeros((N, 3)), sm[0], mm[0], we, blocks, 1)
+    assert np.abs(one["m"] - m1).max() == 0.0 and np.abs(one["z"] - z1).max() == 0.0
+    ref = sr.structure_module(m1[0], z1, sm[0], wst, n_layers=2)
+    assert np.abs(one["x_cycles"][0] - ref["x"]).max() == 0.0 and np.abs(one["s"] - ref["s"]).max() == 0.0
+    two = sr.fold(tf[0], ri[0], mf[0], sm[0], mm[0], we, blocks, wst, 2, **kw)
+    assert np.abs(two["x_cycles"][0] - one["x_cycles"][0]).max() == 0.0
+    same = sr.fold(tf[0], ri[0], mf[0], sm[0], mm[0], we, blocks, wst, 2, x_forced=[two["x_cycles"][0]], **kw)
+    assert np.abs(same["z"] - two["z"]).max() == 0.0
+    # second cycle by hand: the recycling embedder sees the first cycle's m_0, z and positions
+    m2, z2 = embed_ref.embed_cycle(tf[0], ri[0], mf[0], one["m"][0], one["z"], one["x_cycles"][0], we)
+    from oracle import evoformer_trunk
+    m2, z2 = evoformer_trunk(m2, z2, sm[0], mm[0], blocks, 32)
+    assert np.abs(two["m"] - m2).max() < 1e-12 and np.abs(two["z"] - z2).max() < 1e-12
+    other = sr.fold(tf[0], ri[0], mf[0], sm[0], mm[0], we, blocks, wst, 2, x_forced=[two["x_cycles"][0] * 3.0 + 7.0], **kw)
+    v = sm[0] > 0
+    assert np.abs(other["z"][np.ix_(v, v)] - two["z"][np.ix_(v, v)]).max() > 1e-3
