@@ -358,6 +358,36 @@ def recycled_workload(h, pf, ps, torch, dev, name="cfg3", n_cycles=4, steps=2, S
                    f"{S_e} extra sequences, {nb} blocks) through pf_evoformer_forward_recycled", "n_cycles": n_cycles,
            "steps": steps, "ms_per_protein": ms / B, "proteins_per_s": B / (ms * 1e-3), "gpu_launches_per_step": int(launches),
            "extra_msa_stack_ms_per_pass": e1.elapsed_time(e2), "outputs_finite": finite}
+    # the same with the structure module closing every cycle and feeding its positions to the next cycle's
+    # recycling embedder (pf_fold_forward = the whole GPU stage), the structure module and the heads on their own
+    stm = pf.StructureModule(ps.pack_struct_blob(ps.make_struct_weights(7)), pf.make_struct_config())
+    xc = torch.empty((n_cycles, B, N, 3), device=dev)
+    pl = torch.empty((B, N), device=dev)
+    al = torch.empty((B, N, 7, 2), device=dev)
+    dg = torch.empty((B, N, N, 64), device=dev)
+    mlm = torch.empty((B, S, N, 23), device=dev)
+    pf.fold_forward(h, emb, stm, tfd, rid, mfd, None, m, z, smd, mmd, nb, n_cycles, xc, alpha_out=al, plddt_out=pl, **kw)   # warm-up
+    stm.heads(m, z, dg, mlm)
+    torch.cuda.synchronize()
+    f0, f1, f2, f3 = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+    f0.record(stream)
+    pf.fold_forward(h, emb, stm, tfd, rid, mfd, None, m, z, smd, mmd, nb, n_cycles, xc, alpha_out=al, plddt_out=pl, **kw)
+    f1.record(stream)
+    fold_launches = stm.last_launch_count()
+    stm.forward(m, z, smd, x_out=xc[0], alpha_out=al, plddt_out=pl)
+    f2.record(stream)
+    sm_launches = stm.last_launch_count()
+    stm.heads(m, z, dg, mlm)
+    f3.record(stream)
+    torch.cuda.synchronize()
+    out["fold"] = {"desc": "pf_fold_forward: the cycles above, each closed by the structure module (8 layers, fp32) whose "
+                           "positions feed the next cycle's recycling embedder",
+                   "ms_per_protein": f0.elapsed_time(f1) / B, "proteins_per_s": B / (f0.elapsed_time(f1) * 1e-3),
+                   "gpu_launches": int(fold_launches), "structure_module_ms_per_pass": f1.elapsed_time(f2),
+                   "structure_module_launches": int(sm_launches), "heads_ms": f2.elapsed_time(f3),
+                   "outputs_finite": bool(torch.isfinite(xc).all().item() and torch.isfinite(pl).all().item()
+                                          and torch.isfinite(dg).all().item() and torch.isfinite(mlm).all().item())}
+    stm.close()
     emb.close()
     xst.close()
     return out

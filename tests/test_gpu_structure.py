@@ -63,6 +63,15 @@ def test_structure_module_matches_oracle(B, S, N, lengths, n_layers):
     assert launches > 0
 
 
+def test_structure_module_at_benchmarked_size():
+    """BASELINE.json configs[2]'s protein (N_res 384): whole structure module, 8 layers, every residue compared."""
+    w = ps.make_struct_weights(5)
+    msa, pair, sm, _ = ps.make_inputs(11, 1, 1, 384)
+    got, _ = _run_structure(w, msa, pair, sm, 8)
+    worst = _check_structure(got, msa, pair, sm, w, 8)
+    print(f"structure module N=384: worst max-abs {worst}")
+
+
 def test_heads_match_oracle():
     import torch
     w = ps.make_struct_weights(6)
