@@ -58,7 +58,7 @@ TcBlock tc_layout(const pf_config& c);
 void build_tc_block(const pf_config& c, const BlockW& off, const TcBlock& t, const float* w, std::vector<uint16_t>& w16,
                     size_t base16, std::vector<float>& wf, size_t basef, F16Range* range);
 
-enum KernelKind { KK_LN = 0, KK_GEMM, KK_ATTN, KK_TRI, KK_LNC, KK_OPM, KK_LNGEMM, KK_TRANS, KK_FLAGS, KK_GLOBAL, KK_EMBED, KK_COUNT };
+enum KernelKind { KK_LN = 0, KK_GEMM, KK_ATTN, KK_TRI, KK_LNC, KK_OPM, KK_LNGEMM, KK_TRANS, KK_FLAGS, KK_GLOBAL, KK_EMBED, KK_HEADS, KK_COUNT };
 
 inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 inline int pad8(int v) { return (v + 7) / 8 * 8; }
@@ -107,6 +107,7 @@ struct pf_evoformer {
     double msa = 1, msat = 1, pair = 1, msa_lin = 1, pair_lin = 1, pair_x = 1, msat_x = 1;   // active 128-row tiles per geometry
     double attn_row = 1, attn_col = 1, attn_tri = 1;                 // visited (row, key tile) pairs
     double opm = 1, tri_k = 1, lnc = 1;                              // active j pairs, visited k-blocks, unpadded rows i
+    double pair_rows = 1;                                            // unmasked (i, j) pairs (pair-bias heads kernel)
   } frac;
   cudaEvent_t next_event() {
     if (ev_used == ev_pool.size()) {

@@ -64,6 +64,9 @@ void launch_tri_einsum_simt(const T* a_cm, const T* b_cm, float* t_cm, int batch
 template <typename T>
 void launch_lnc(const float* t_cm, T* y, const float* gamma, const float* beta, const float* seq_mask /*optional: rows of
                 padded residues are skipped*/, int B, int C, int N, int Npad, cudaStream_t st);
+// pair-bias heads of the MSA row attention at c_z = 128, H <= 8 (pf_simt.cu): bias[b,h,i,j] = scale Lin0(LN'(z_ij))_h, W [128, H] fp32
+void launch_ln_heads128(const float* z, const float* gamma, const float* beta, const float* W, float scale, const float* seq_mask,
+                        bf16* out, int B, int N, int Lpad, int H, int num_sms, cudaStream_t st);
 void launch_lnc_tc(const bf16* t_cm, __half* y, const float* gamma, const float* beta, const float* seq_mask, int B, int N,
                    int Npad, cudaStream_t st);
 template <typename T>

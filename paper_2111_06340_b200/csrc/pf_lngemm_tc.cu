@@ -26,7 +26,6 @@
 #include "pf_lnprod.cuh"
 
 #include <cuda_fp16.h>
-#include <cstdlib>
 #include <string>
 
 namespace pf {
@@ -105,7 +104,6 @@ struct G2Params {
   unsigned swap_mask;
   int has_cms;            // some group is G2_CMS: the epilogue warps publish the tile's row masks once per tile
   int bias_lo, bias_n;    // the bias table holds columns [bias_lo, bias_lo + bias_n); all other columns have zero bias
-  int prefetch;           // LayerNorm producers pull the next tile's rows into L2 (launches bound by the producers)
   G2Op ops[G2_MAX_OPS];
 };
 
@@ -633,25 +631,8 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
       for (long tile = blockIdx.x; tile < p.num_tiles; tile += gridDim.x) {
         if (!tile_on(tile, p)) continue;
         const uint32_t abuf = it & 1;
-        if (p.prefetch) {
-          // pull this warp's 16 rows of the NEXT tile into L2: one bulk prefetch when they are contiguous in memory
-          // (YT >= 16, source not transposed), one per row otherwise
-          const long nxt = tile + gridDim.x;
-          if (nxt < p.num_tiles && tile_on(nxt, p)) {
-            const TileCoord nc = tile_coord(nxt, p);
-            if (!p.src_transposed && p.YT >= 16) {
-              const int lr0 = pw * 16;
-              const int x = nc.x0 + (lr0 >> p.yt_shift), y = nc.y0 + (lr0 & (p.YT - 1));
-              int nrows = p.D2 - y;
-              nrows = nrows > 16 ? 16 : nrows;
-              if (lane == 0 && x < p.D1 && nrows > 0)
-                tc::prefetch_l2_bulk(p.src + (((long)nc.b * p.D1 + x) * p.D2 + y) * K, (uint32_t)(nrows * K * 4));
-            } else if (lane < 16) {
-              const float* rp = src_row(nc, pw * 16 + lane);
-              if (rp) tc::prefetch_l2_bulk(rp, K * 4);
-            }
-          }
-        }
+        // (A bulk L2 prefetch of the next batch of rows used to sit here; once the epilogue stopped spilling it measured as a
+        // small loss — the 128 per-row prefetch operations per tile compete with the weight loads and the stores in the TMA queue.)
         if (lane == 0 && pw == 0) G2_TRACE(2, 0x200);
         tc::mbar_wait(&a_empty[abuf], ((it >> 1) & 1) ^ 1);
         if (lane == 0 && pw == 0) G2_TRACE(2, 0x201);
@@ -849,10 +830,6 @@ int launch_gemm2(TmaCtx* ctx, const G2Desc& d, int num_sms, cudaStream_t st) {
   p.vt_out = reinterpret_cast<bf16*>(d.vt_out); p.vt_cols = d.vt_cols;
   p.Lpad = d.Lpad;
   p.tile_active = d.tile_active;
-  {
-    static const int pf_env = getenv("PF_G2_PREFETCH") ? atoi(getenv("PF_G2_PREFETCH")) : 0;
-    p.prefetch = (d.a_mode == 0) && (pf_env == 1 || (pf_env == 2 && d.Nw <= 2 * d.K));
-  }
   p.bias_lo = d.bias_lo;
   p.bias_n = d.bias ? (d.bias_n > 0 ? d.bias_n : d.Nw - d.bias_lo) : 0;
   {

@@ -221,7 +221,14 @@ struct TcDriver {
     bf16* VT = buf<bf16>(ar.vt);
     bf16* O = buf<bf16>(ar.o);
     bf16* BIAS = (row_bias || self_bias) ? buf<bf16>(ar.bias) : nullptr;
-    if (row_bias) {   // A.1: beta[h,i,j] = Lin0(LN'(z[i,j]))_h
+    if (row_bias && c.c_z == 128 && c.heads_msa <= 8 && (double)B * N * N < 4.0e9) {
+      // A.1: beta[h,i,j] = Lin0(LN'(z[i,j]))_h — 16 bytes out per 512 bytes in: a streaming SIMT kernel (pf_simt.cu)
+      h->prof_begin(KK_HEADS, 2.0 * B * N * N * c.c_z * c.heads_msa * h->frac.pair_rows,
+                    (double)B * N * N * (c.c_z * 4.0 + c.heads_msa * 2.0) * h->frac.pair_rows, st);
+      launch_ln_heads128(pair, w + a.ln_z_g, w + a.ln_z_b, w + a.w_bias, kLog2e, seq_mask, BIAS, B, N, pad8(N), c.heads_msa,
+                         h->num_sms, st);
+      h->prof_end(st);
+    } else if (row_bias) {
       G2Desc d = desc_base(B, N, N, c.c_z, c.heads_msa);
       d.src = pair; d.gamma = w + a.ln_z_g; d.beta = w + a.ln_z_b;
       d.op_fmt = 1; d.Wt = w16 + h->tc.row_wbias;
@@ -460,6 +467,15 @@ static void host_work_fractions(pf_evoformer* h, const std::vector<float>& sg, c
     }
     f.opm = (double)on / all;
     f.lnc = (double)rows / ((double)B * N);
+    {
+      double pr = 0;
+      for (int b = 0; b < B; ++b) {
+        long cnt = 0;
+        for (int i = 0; i < N; ++i) cnt += sg[(size_t)b * N + i] > 0.5f;
+        pr += (double)cnt * cnt;
+      }
+      f.pair_rows = pr / ((double)B * N * N);
+    }
     f.tri_k = kb / ((double)B * nkb);
   }
   h->frac = f;
