@@ -8,8 +8,9 @@
 //   sm_pair_kernel      zn = LN_z(z) and the attention bias b = Lin0(zn), one pass over the pair representation, ONCE per
 //                       call (the layers share their weights and z does not change, so both are layer-invariant)
 //   sm_points_kernel    local query / key / value points -> global frame
-//   sm_ipa_kernel       one CTA per query residue, one warp per head: logits over all keys in shared memory, softmax, then
-//                       the three weighted sums (pair values, scalar values, value points) and the map back to the local frame
+//   sm_ipa_kernel       one CTA per query residue, one warp per head: logits over all keys in shared memory (key-major), softmax,
+//                       then the three weighted sums (pair values: every z[i,j,:] read once per CTA against the weights of all
+//                       heads; scalar values; value points) and the map back to the local frame
 //   sm_frames_kernel    quaternion -> rotation, frame composition, positions
 //   sm_alpha_kernel, sm_plddt_kernel, sm_symm_kernel   angle normalisation, pLDDT expectation, distogram symmetrisation
 #include "../../include/pf_evoformer.h"
@@ -198,8 +199,8 @@ __global__ void __launch_bounds__(256) sm_ln_kernel(const float* x, float* y, co
 __global__ void __launch_bounds__(256) sm_pair_kernel(const float* __restrict__ z, float* __restrict__ zn, float* __restrict__ bias,
                                                       const float* __restrict__ gamma, const float* __restrict__ beta,
                                                       const float* __restrict__ wb, long rows, int C, int H) {
-  extern __shared__ float swb[];   // [C, H]
-  for (int i = threadIdx.x; i < C * H; i += blockDim.x) swb[i] = __ldg(wb + i);
+  extern __shared__ __align__(16) float swb[];   // [H, C]: head-major, so a lane reads its four channels of one head as one float4
+  for (int i = threadIdx.x; i < C * H; i += blockDim.x) swb[(i % H) * C + i / H] = __ldg(wb + i);
   __syncthreads();
   const int lane = threadIdx.x & 31, nv = C >> 2;
   for (long r = (long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); r < rows; r += (long)gridDim.x * (blockDim.x >> 5)) {
@@ -234,18 +235,41 @@ __global__ void __launch_bounds__(256) sm_pair_kernel(const float* __restrict__ 
         reinterpret_cast<float4*>(zn + r * C)[c4] = v[i];
       }
     }
-    for (int h = 0; h < H; ++h) {
-      float p = 0.f;
+    // per-lane partial dot products of up to 16 heads at a time, then a reduce-scatter over the warp (16 shuffles for 16
+    // heads instead of 5 per head): afterwards lanes 2 h and 2 h + 1 hold the sum of head h0 + h
+    for (int h0 = 0; h0 < H; h0 += 16) {
+      float p[16];
 #pragma unroll
-      for (int i = 0; i < 8; ++i) {
-        const int c4 = lane + 32 * i;
-        if (c4 < nv) {
-          const float* wr = swb + (size_t)(c4 * 4) * H + h;
-          p += (v[i].x * wr[0] + v[i].y * wr[H]) + (v[i].z * wr[2 * H] + v[i].w * wr[3 * H]);
+      for (int hh = 0; hh < 16; ++hh) {
+        p[hh] = 0.f;
+        if (h0 + hh < H) {
+#pragma unroll
+          for (int i = 0; i < 8; ++i) {
+            const int c4 = lane + 32 * i;
+            if (c4 < nv) {
+              const float4 w4 = *reinterpret_cast<const float4*>(swb + (size_t)(h0 + hh) * C + 4 * c4);
+              p[hh] += (v[i].x * w4.x + v[i].y * w4.y) + (v[i].z * w4.z + v[i].w * w4.w);
+            }
+          }
         }
       }
-      p = warp_sum(p);
-      if (lane == 0) bias[r * H + h] = p;
+      // 16 -> 8 -> 4 -> 2 -> 1 values per lane over lane bits 4, 3, 2, 1, then bit 0 adds the two halves
+#pragma unroll
+      for (int n = 8, m = 16; n >= 1; n >>= 1, m >>= 1) {
+        const bool up = lane & m;
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+          if (j < n) {
+            const float send = up ? p[j] : p[j + n];
+            const float recv = __shfl_xor_sync(0xffffffffu, send, m);
+            p[j] = (up ? p[j + n] : p[j]) + recv;
+          }
+        }
+      }
+      p[0] += __shfl_xor_sync(0xffffffffu, p[0], 1);
+      // head index held by this lane: bits of the lane select the upper half at every step
+      const int hh = ((lane >> 4) & 1) * 8 + ((lane >> 3) & 1) * 4 + ((lane >> 2) & 1) * 2 + ((lane >> 1) & 1);
+      if ((lane & 1) == 0 && h0 + hh < H) bias[r * H + h0 + hh] = p[0];
     }
   }
 }
@@ -286,19 +310,27 @@ struct SmIpa {
   int N, H, c, Pq, Pv, cz, P;
 };
 
+// HQ = ceil(H / 4): the attention weights are kept key-major, att[j][4 HQ], so that the pair-value sum reads the weights of
+// all heads for one key as HQ float4 and every pair value z[i, j, ch] exactly once per CTA.
+template <int HQ>
 __global__ void __launch_bounds__(1024) sm_ipa_kernel(const SmIpa a) {
-  extern __shared__ float sm[];
+  extern __shared__ __align__(16) float sm[];
+  constexpr int HP = 4 * HQ;
   const int N = a.N, H = a.H, c = a.c, Pq = a.Pq, Pv = a.Pv, cz = a.cz;
   const int b = blockIdx.y, i = blockIdx.x;
   const long row = (long)b * N + i;
-  float* att = sm;                              // [H, N]
-  float* qs = att + (size_t)H * N;              // [H c]
+  float* att = sm;                              // [N, HP]
+  const int G = blockDim.x >= (unsigned)cz ? (int)blockDim.x / cz : 1;   // key classes of the pair-value sum
+  float* osum = att + (size_t)N * HP;           // [G, H cz]   partial pair-value sums, added in a fixed order (deterministic)
+  float* qs = osum + (size_t)G * H * cz;        // [H c]
   float* qg = qs + H * c;                       // [H Pq 3]
   float* red = qg + H * Pq * 3;                 // [H (c + 3 Pv)]
   const int o_k = H * c, o_v = 2 * H * c, o_qg = 3 * H * c, o_kg = o_qg + H * Pq * 3, o_vg = o_kg + H * Pq * 3;
   const float* prow = a.proj + row * a.P;
   for (int t = threadIdx.x; t < H * c; t += blockDim.x) qs[t] = prow[t];
   for (int t = threadIdx.x; t < H * Pq * 3; t += blockDim.x) qg[t] = prow[o_qg + t];
+  if (HP != H)
+    for (int t = threadIdx.x; t < N * HP; t += blockDim.x) att[t] = 0.f;   // padded head columns stay zero
   __syncthreads();
   const int h = threadIdx.x >> 5, lane = threadIdx.x & 31;
   {
@@ -307,61 +339,102 @@ __global__ void __launch_bounds__(1024) sm_ipa_kernel(const SmIpa a) {
     const float gamma = log1pf(expf(-fabsf(gh))) + fmaxf(gh, 0.f);          // softplus
     const float coef = gamma * w_c * 0.5f, inv_sqrt_c = rsqrtf((float)c);
     const float* brow = a.bias + (row * N) * H + h;
-    float* arow = att + (size_t)h * N;
+    float* acol = att + h;                      // this head's column, stride HP
+    const bool vec = (c & 3) == 0 && ((Pq * 3) & 3) == 0 && (a.P & 3) == 0;   // 16-byte aligned segments of the projection row
     float mx = -INFINITY;
     for (int j = lane; j < N; j += 32) {
       const float* kr = a.proj + ((long)b * N + j) * a.P;
-      float qk = 0.f;
-      for (int e = 0; e < c; ++e) qk = fmaf(qs[h * c + e], kr[o_k + h * c + e], qk);
-      float d2 = 0.f;
-      for (int e = 0; e < Pq * 3; ++e) {
-        const float d = qg[h * Pq * 3 + e] - kr[o_kg + h * Pq * 3 + e];
-        d2 = fmaf(d, d, d2);
+      float qk = 0.f, d2 = 0.f;
+      if (vec) {
+        const float4* k4 = reinterpret_cast<const float4*>(kr + o_k + h * c);
+        const float4* q4 = reinterpret_cast<const float4*>(qs + h * c);
+        for (int e = 0; e < c / 4; ++e) {
+          const float4 kv = __ldg(k4 + e), qv = q4[e];
+          qk = fmaf(qv.x, kv.x, qk); qk = fmaf(qv.y, kv.y, qk); qk = fmaf(qv.z, kv.z, qk); qk = fmaf(qv.w, kv.w, qk);
+        }
+        const float4* g4 = reinterpret_cast<const float4*>(kr + o_kg + h * Pq * 3);
+        const float4* p4 = reinterpret_cast<const float4*>(qg + h * Pq * 3);
+        for (int e = 0; e < Pq * 3 / 4; ++e) {
+          const float4 kv = __ldg(g4 + e), qv = p4[e];
+          const float dx = qv.x - kv.x, dy = qv.y - kv.y, dz = qv.z - kv.z, dw = qv.w - kv.w;
+          d2 = fmaf(dx, dx, d2); d2 = fmaf(dy, dy, d2); d2 = fmaf(dz, dz, d2); d2 = fmaf(dw, dw, d2);
+        }
+      } else {
+        for (int e = 0; e < c; ++e) qk = fmaf(qs[h * c + e], kr[o_k + h * c + e], qk);
+        for (int e = 0; e < Pq * 3; ++e) {
+          const float d = qg[h * Pq * 3 + e] - kr[o_kg + h * Pq * 3 + e];
+          d2 = fmaf(d, d, d2);
+        }
       }
       float lg = w_l * (qk * inv_sqrt_c + brow[(long)j * H] - coef * d2);
       if (!(a.seq_mask[(long)b * N + j] > 0.f)) lg = -INFINITY;
-      arow[j] = lg;
+      acol[(size_t)j * HP] = lg;
       mx = fmaxf(mx, lg);
     }
     mx = warp_max(mx);
     float s = 0.f;
     for (int j = lane; j < N; j += 32) {
-      const float e = (mx == -INFINITY) ? 0.f : expf(arow[j] - mx);
-      arow[j] = e;
+      const float e = (mx == -INFINITY) ? 0.f : expf(acol[(size_t)j * HP] - mx);
+      acol[(size_t)j * HP] = e;
       s += e;
     }
     s = warp_sum(s);
     const float inv = s > 0.f ? 1.0f / s : 0.f;
-    for (int j = lane; j < N; j += 32) arow[j] *= inv;
+    for (int j = lane; j < N; j += 32) acol[(size_t)j * HP] *= inv;
   }
   __syncthreads();
   float* crow = a.cat + row * ((long)H * (cz + c + 4 * Pv));
-  // ot[h, ch] = sum_j a[h, j] zn[i, j, ch]
-  const float* zrow = a.zn + (row * N) * cz;
-  for (int idx = threadIdx.x; idx < H * cz; idx += blockDim.x) {
-    const int hh = idx / cz, ch = idx - hh * cz;
-    const float* ar = att + (size_t)hh * N;
-    float acc0 = 0.f, acc1 = 0.f;
-    int j = 0;
-    for (; j + 1 < N; j += 2) {
-      acc0 = fmaf(ar[j], zrow[(long)j * cz + ch], acc0);
-      acc1 = fmaf(ar[j + 1], zrow[(long)(j + 1) * cz + ch], acc1);
+  // ot[h, ch] = sum_j a[h, j] zn[i, j, ch]: a thread owns one channel and a residue class of keys (G classes), reads z once
+  // and the weights of all heads as HQ float4; the G partial sums meet in shared memory
+  {
+    const float* zrow = a.zn + (row * N) * cz;
+    for (int ch0 = 0; ch0 < cz; ch0 += (int)blockDim.x) {       // one trip unless cz > blockDim.x
+      const int t = threadIdx.x;
+      const int g = G > 1 ? t / cz : 0;
+      const int ch = G > 1 ? t - g * cz : ch0 + t;
+      if (g < G && ch < cz) {
+        float acc[HP];
+#pragma unroll
+        for (int q = 0; q < HP; ++q) acc[q] = 0.f;
+        for (int j = g; j < N; j += G) {
+          const float zv = __ldg(zrow + (long)j * cz + ch);
+          const float4* aw = reinterpret_cast<const float4*>(att + (size_t)j * HP);
+#pragma unroll
+          for (int q = 0; q < HQ; ++q) {
+            const float4 w4 = aw[q];
+            acc[4 * q] = fmaf(w4.x, zv, acc[4 * q]);
+            acc[4 * q + 1] = fmaf(w4.y, zv, acc[4 * q + 1]);
+            acc[4 * q + 2] = fmaf(w4.z, zv, acc[4 * q + 2]);
+            acc[4 * q + 3] = fmaf(w4.w, zv, acc[4 * q + 3]);
+          }
+        }
+#pragma unroll
+        for (int q = 0; q < HP; ++q)
+          if (q < H) osum[((size_t)g * H + q) * cz + ch] = acc[q];
+      }
     }
-    if (j < N) acc0 = fmaf(ar[j], zrow[(long)j * cz + ch], acc0);
-    crow[idx] = acc0 + acc1;
   }
   // o[h, e] and the global value-point sums og[h, p, x]
   const int per = c + 3 * Pv;
   for (int idx = threadIdx.x; idx < H * per; idx += blockDim.x) {
     const int hh = idx / per, e = idx - hh * per;
     const int col = e < c ? o_v + hh * c + e : o_vg + hh * Pv * 3 + (e - c);
-    const float* ar = att + (size_t)hh * N;
     const float* vcol = a.proj + ((long)b * N) * a.P + col;
-    float acc = 0.f;
-    for (int j = 0; j < N; ++j) acc = fmaf(ar[j], vcol[(long)j * a.P], acc);
-    red[idx] = acc;
+    float acc0 = 0.f, acc1 = 0.f;
+    int j = 0;
+    for (; j + 1 < N; j += 2) {
+      acc0 = fmaf(att[(size_t)j * HP + hh], __ldg(vcol + (long)j * a.P), acc0);
+      acc1 = fmaf(att[(size_t)(j + 1) * HP + hh], __ldg(vcol + (long)(j + 1) * a.P), acc1);
+    }
+    if (j < N) acc0 = fmaf(att[(size_t)j * HP + hh], __ldg(vcol + (long)j * a.P), acc0);
+    red[idx] = acc0 + acc1;
   }
   __syncthreads();
+  for (int idx = threadIdx.x; idx < H * cz; idx += blockDim.x) {
+    float t = osum[idx];
+    for (int g = 1; g < G; ++g) t += osum[(size_t)g * H * cz + idx];
+    crow[idx] = t;
+  }
   const float* f = a.frames + row * 12;
   for (int idx = threadIdx.x; idx < H * c; idx += blockDim.x) {
     const int hh = idx / c, e = idx - hh * c;
@@ -526,9 +599,15 @@ extern "C" pf_status pf_structure_create(pf_structure_t** out, const float* weig
     pf_structure_destroy(h);
     return sfail(PF_ERR_CUDA, "structure weights H2D");
   }
-  if (cudaFuncSetAttribute(sm_ipa_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024) != cudaSuccess) {
-    pf_structure_destroy(h);
-    return sfail(PF_ERR_CUDA, "cudaFuncSetAttribute(sm_ipa_kernel)");
+  {
+    cudaError_t ce = cudaSuccess;
+    auto set = [&](const void* fn) { if (ce == cudaSuccess) ce = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024); };
+    set((const void*)sm_ipa_kernel<1>); set((const void*)sm_ipa_kernel<2>); set((const void*)sm_ipa_kernel<3>); set((const void*)sm_ipa_kernel<4>);
+    set((const void*)sm_ipa_kernel<5>); set((const void*)sm_ipa_kernel<6>); set((const void*)sm_ipa_kernel<7>); set((const void*)sm_ipa_kernel<8>);
+    if (ce != cudaSuccess) {
+      pf_structure_destroy(h);
+      return sfail(PF_ERR_CUDA, "cudaFuncSetAttribute(sm_ipa_kernel)");
+    }
   }
   *out = h;
   return PF_OK;
@@ -580,7 +659,9 @@ extern "C" pf_status pf_structure_forward(pf_structure_t* h, const float* msa, c
   const SmOff& o = h->off;
   const int cs = c.c_s, cz = c.c_z, H = c.heads, P = sm_proj_cols(c), ccat = sm_c_cat(c), cr = c.c_resnet, cl = c.c_lddt;
   const long R = (long)B * N, PR = (long)B * N * N;
-  const size_t ipa_smem = ((size_t)H * N + (size_t)H * c.c_ipa + (size_t)H * c.n_qp * 3 + (size_t)H * (c.c_ipa + 3 * c.n_pv)) * 4;
+  const int HQ = (H + 3) / 4;
+  const int ipa_g = 32 * H >= cz ? 32 * H / cz : 1;
+  const size_t ipa_smem = ((size_t)4 * HQ * N + (size_t)ipa_g * H * cz + (size_t)H * c.c_ipa + (size_t)H * c.n_qp * 3 + (size_t)H * (c.c_ipa + 3 * c.n_pv)) * 4;
   if (ipa_smem > 200 * 1024) return sfail(PF_ERR_SHAPE, "structure module: heads x N_res attention weights exceed 200 KB of shared memory");
   // workspace
   size_t at = 0;
@@ -616,7 +697,19 @@ extern "C" pf_status pf_structure_forward(pf_structure_t* h, const float* msa, c
     sm_points_kernel<<<(unsigned)((R * npts + 255) / 256), 256, 0, st>>>(proj, frames, R, P, pt0, npts);
     ++run.launches;
     SmIpa ia{proj, zn, bias, frames, seq_mask, w + o.g_head, cat, N, H, c.c_ipa, c.n_qp, c.n_pv, cz, P};
-    sm_ipa_kernel<<<dim3((unsigned)N, (unsigned)B), 32 * H, ipa_smem, st>>>(ia);
+    {
+      const dim3 grid((unsigned)N, (unsigned)B);
+      switch (HQ) {
+        case 1: sm_ipa_kernel<1><<<grid, 32 * H, ipa_smem, st>>>(ia); break;
+        case 2: sm_ipa_kernel<2><<<grid, 32 * H, ipa_smem, st>>>(ia); break;
+        case 3: sm_ipa_kernel<3><<<grid, 32 * H, ipa_smem, st>>>(ia); break;
+        case 4: sm_ipa_kernel<4><<<grid, 32 * H, ipa_smem, st>>>(ia); break;
+        case 5: sm_ipa_kernel<5><<<grid, 32 * H, ipa_smem, st>>>(ia); break;
+        case 6: sm_ipa_kernel<6><<<grid, 32 * H, ipa_smem, st>>>(ia); break;
+        case 7: sm_ipa_kernel<7><<<grid, 32 * H, ipa_smem, st>>>(ia); break;
+        default: sm_ipa_kernel<8><<<grid, 32 * H, ipa_smem, st>>>(ia); break;
+      }
+    }
     ++run.launches;
     // M.3
     run.gemm(cat, ccat, w + o.w_out, w + o.b_out, s, cs, R, ccat, cs, false, false, true);

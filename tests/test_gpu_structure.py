@@ -1,7 +1,7 @@
 """GPU parity of the structure module, the heads and the whole recycled GPU stage (readings M.0-M.6, H.1-H.3,
 DESIGN.md §2d) against the fp64 oracle (oracle/structure_ref.py), through the C ABI.  Everything here is fp32 arithmetic:
-tolerance 1e-4 max-abs on quantities of order one (s, rotation matrices, translations in nanometres, unit angle vectors),
-1e-3 on positions in Angstrom (10 x a translation) and on pLDDT (100 x a probability-weighted mean); outputs at masked
+tolerance 1e-4 max-abs on quantities of order one (s, rotation matrices, translations in nanometres), 5e-4 on the unit angle
+vectors (a division by a norm that can be small), 1e-3 on positions in Angstrom (10 x a translation) and on pLDDT (100 x a probability-weighted mean); outputs at masked
 residues are unspecified but must be finite."""
 import numpy as np
 import pytest
@@ -43,7 +43,9 @@ def _check_structure(got, msa, pair, sm, w, n_layers):
         v = sm[b] > 0
         pairs = [("s", got["s"][b], ref["s"], TOL), ("R", got["frames"][b][:, :9].reshape(-1, 3, 3), ref["R"], TOL),
                  ("t", got["frames"][b][:, 9:], ref["t"], TOL), ("x", got["x"][b], ref["x"], 10 * TOL),
-                 ("alpha", got["alpha"][b], ref["alpha"], TOL), ("plddt", got["plddt"][b], pl, 10 * TOL)]
+                 # unit vectors alpha / |alpha|: the division amplifies the fp32 error of alpha (1e-5) by 1 / |alpha|, and
+                 # |alpha| falls to a few hundredths for some residues with random weights
+                 ("alpha", got["alpha"][b], ref["alpha"], 5 * TOL), ("plddt", got["plddt"][b], pl, 10 * TOL)]
         for name, g, r, tol in pairs:
             assert np.isfinite(g).all(), name
             e = float(np.abs(g[v] - r[v]).max())
