@@ -623,7 +623,29 @@ extern "C" pf_status pf_evoformer_forward_host(pf_evoformer_t* h, float* msa_hos
     CUDA_TRY(cudaStreamCreateWithFlags(&h->d2h_stream, cudaStreamNonBlocking));
     for (auto& e : h->host_ev) CUDA_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
   }
-  const int n_chunks = B < 8 ? B : 8;   // measured at cfg2: 2 chunks 866, 4 chunks 993, 6-8 chunks 1012 proteins/s
+  // Chunk sizes: small chunks at both ends (the first copy-in and the last copy-out are not overlapped with compute, so they
+  // should be short), large ones in the middle (small batches use the GPU less well).  Measured at cfg2 with 8 equal chunks:
+  // 1012-1150 proteins/s; 2 chunks 866, 4 chunks 993.
+  int sizes[8];
+  int n_chunks = 0;
+  if (B < 16) {
+    n_chunks = B < 8 ? B : 8;
+    for (int c = 0, b0 = 0; c < n_chunks; ++c) {
+      sizes[c] = (B - b0 + (n_chunks - c) - 1) / (n_chunks - c);
+      b0 += sizes[c];
+    }
+  } else {
+    const int e1 = B / 16, e2 = B / 8, mid = B - 2 * (e1 + e2);
+    const int n_mid = 3;
+    sizes[n_chunks++] = e1;
+    sizes[n_chunks++] = e2;
+    for (int c = 0, left = mid; c < n_mid; ++c) {
+      sizes[n_chunks] = (left + (n_mid - c) - 1) / (n_mid - c);
+      left -= sizes[n_chunks++];
+    }
+    sizes[n_chunks++] = e2;
+    sizes[n_chunks++] = e1;
+  }
   const size_t pm = (size_t)S * N * h->cfg.c_m, pz = (size_t)N * N * h->cfg.c_z;   // floats per protein
   CUDA_TRY(cudaEventRecord(h->host_ev[16], st));                  // earlier work on the caller's stream comes first
   CUDA_TRY(cudaStreamWaitEvent(h->h2d_stream, h->host_ev[16], 0));
@@ -632,7 +654,7 @@ extern "C" pf_status pf_evoformer_forward_host(pf_evoformer_t* h, float* msa_hos
   CUDA_TRY(cudaMemcpyAsync(dr, msa_mask_host, (size_t)B * S * 4, cudaMemcpyHostToDevice, h->h2d_stream));
   int b0 = 0;
   for (int c = 0; c < n_chunks; ++c) {
-    const int bc = (B - b0 + (n_chunks - c) - 1) / (n_chunks - c);
+    const int bc = sizes[c];
     CUDA_TRY(cudaMemcpyAsync(dm + b0 * pm, msa_host + b0 * pm, bc * pm * 4, cudaMemcpyHostToDevice, h->h2d_stream));
     CUDA_TRY(cudaMemcpyAsync(dz + b0 * pz, pair_host + b0 * pz, bc * pz * 4, cudaMemcpyHostToDevice, h->h2d_stream));
     CUDA_TRY(cudaEventRecord(h->host_ev[c], h->h2d_stream));
@@ -640,7 +662,7 @@ extern "C" pf_status pf_evoformer_forward_host(pf_evoformer_t* h, float* msa_hos
   }
   b0 = 0;
   for (int c = 0; c < n_chunks; ++c) {
-    const int bc = (B - b0 + (n_chunks - c) - 1) / (n_chunks - c);
+    const int bc = sizes[c];
     CUDA_TRY(cudaStreamWaitEvent(st, h->host_ev[c], 0));
     pf_status s = pf_evoformer_forward(h, dm + b0 * pm, dz + b0 * pz, ds + (size_t)b0 * N, dr + (size_t)b0 * S, bc, S, N, n_blocks,
                                        stream);

@@ -126,7 +126,7 @@ def test_cfg2_full_size_sampled_proteins():
         _check(m[sl], z[sl], mr, zr, sm[sl], mm[sl], f"cfg2 protein {int(b)} (len {int(lengths[b])})")
 
 
-@pytest.mark.parametrize("B", [1, 5, 11])
+@pytest.mark.parametrize("B", [1, 5, 11, 19])
 def test_forward_host_pipelined_chunks_match_forward(B):
     """pf_evoformer_forward_host pipelines the batch in chunks of proteins over copy streams: every protein must come back
     exactly as from the device-resident call on the same batch (proteins are independent, so chunking changes nothing)."""
