@@ -393,6 +393,36 @@ def recycled_workload(h, pf, ps, torch, dev, name="cfg3", n_cycles=4, steps=2, S
     return out
 
 
+def small_unbatched(h, ps, torch, dev, nb=48):
+    """One small protein at a time (the large set is 50-residue designs): 1,212 launches of kernels with less than
+    one tile per SM, i.e. launch- and tail-bound.  The library replays such calls from a CUDA graph (captured at the first
+    call per buffers + shape); reported: device ms per 48-block forward, host milliseconds spent issuing it, first call."""
+    import time
+    out = {}
+    for (S, N) in ((512, 64), (512, 128)):
+        m, z, sm, mm = ps.make_inputs_device(77, 1, S, N, dev)
+        smd, mmd = torch.from_numpy(sm).to(dev), torch.from_numpy(mm).to(dev)
+        t0 = time.perf_counter()
+        h.forward(m, z, smd, mmd, nb)
+        torch.cuda.synchronize()
+        first = (time.perf_counter() - t0) * 1e3
+        h.forward(m, z, smd, mmd, nb)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        t0 = time.perf_counter()
+        e0.record()
+        for _ in range(3):
+            h.forward(m, z, smd, mmd, nb)
+        issue = (time.perf_counter() - t0) / 3 * 1e3
+        e1.record()
+        torch.cuda.synchronize()
+        out[f"N_res={N},N_seq={S}"] = {"ms_per_forward": e0.elapsed_time(e1) / 3, "host_issue_ms": issue, "first_call_ms": first,
+                                        "launches": int(h.last_launch_count()), "proteins_per_s": 3e3 / e0.elapsed_time(e1),
+                                        "outputs_finite": bool(torch.isfinite(m).all().item() and torch.isfinite(z).all().item())}
+    out["desc"] = "B = 1, 48 blocks, CUDA-graph replay (PF_GRAPH=0 disables: ~10 % slower on the device, 17-25 ms of host time per call)"
+    return out
+
+
 def cfg5_sweep(h, pf, ps, torch, dev, peaks, n_proteins=2000, S=512, cap=48, nb=48):
     """BASELINE.json configs[4], run for real: 2,000 proteins (lengths R10), buckets {64..320}, N_seq=512, msa_mask R11, every
     batch the length-bucketing scheduler (pf_sched_*) cuts goes through all 48 blocks (48 distinct weight sets).  Inputs are
@@ -587,6 +617,7 @@ def run_ours(args, wl, wl_name):
     if want_sides:
         line["workloads"] = {k: side_workload(h, ps, torch, dev, k, peaks) for k in ("cfg3", "cfg4")}
         line["workloads"]["cfg3_recycled"] = recycled_workload(h, pf, ps, torch, dev)
+        line["workloads"]["small_unbatched"] = small_unbatched(h, ps, torch, dev)
     if want_sweep:
         line["cfg5_sweep"] = cfg5_sweep(h, pf, ps, torch, dev, peaks)
     if world == 1 and not args.no_cpu_baseline:

@@ -223,6 +223,8 @@ extern "C" void pf_evoformer_destroy(pf_evoformer_t* h) {
     for (cudaEvent_t e : h->host_ev) cudaEventDestroy(e);
   }
   if (h->tma) tma_ctx_destroy(h->tma);
+  for (auto& g : h->graphs) cudaGraphExecDestroy(g.exec);
+  if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
   for (cudaEvent_t e : h->ev_pool) cudaEventDestroy(e);
   delete h;
 }
@@ -550,10 +552,9 @@ static pf_status dispatch(pf_evoformer* h, float* msa, float* pair, const float*
   return PF_OK;
 }
 
-static pf_status dispatch_pass(pf_evoformer* h, float* msa, float* pair, const float* sm, const float* mm, int B, int S,
-                               int N, int block0, int block1, int step0, int step1, cudaStream_t st, long long& launches) {
-  pf_status s = check_and_grow(h, B, S, N, st);
-  if (s != PF_OK) return s;
+// the launch sequence of one pass (workspace already sized): mask flags, then the sub-steps
+static pf_status pass_launches(pf_evoformer* h, float* msa, float* pair, const float* sm, const float* mm, int B, int S, int N,
+                               int block0, int block1, int step0, int step1, cudaStream_t st) {
   Driver d;
   d.h = h; d.st = st; d.B = B; d.S = S; d.N = N;
   d.msa = msa; d.pair = pair; d.seq_mask = sm; d.msa_mask = mm;
@@ -571,6 +572,68 @@ static pf_status dispatch_pass(pf_evoformer* h, float* msa, float* pair, const f
         return fail(PF_ERR_CUDA, std::string("launch failed in block ") + std::to_string(blk) + " substep " +
                                      std::to_string(step) + ": " + cudaGetErrorString(e));
     }
+  return PF_OK;
+}
+
+// Small problems are launch-bound: 25 launches per block with several tensor-map encodings each cost the host ~10-15 us per
+// launch while the kernels of a single 64-residue protein take less.  Whole forward calls on such shapes are therefore
+// captured once into a CUDA graph per (buffers, shape, block range) and replayed; tensor maps are by-value kernel parameters,
+// so the graph holds them.  Not used while profiling (events per launch), for the fp32 path, or for single sub-steps.
+static bool graph_wanted(const pf_evoformer* h, int B, int S, int N, int block0, int block1, int step0, int step1) {
+  static const int env = getenv("PF_GRAPH") ? atoi(getenv("PF_GRAPH")) : 1;
+  if (!env || h->prof_on || h->cfg.dtype != PF_BF16 || step0 != 1 || step1 != 9 || block1 - block0 < 2) return false;
+  return env == 2 || (double)B * S * N <= 131072.0;
+}
+
+static pf_status dispatch_pass(pf_evoformer* h, float* msa, float* pair, const float* sm, const float* mm, int B, int S,
+                               int N, int block0, int block1, int step0, int step1, cudaStream_t st, long long& launches) {
+  char* const ws_before = h->ws;
+  pf_status s = check_and_grow(h, B, S, N, st);
+  if (s != PF_OK) return s;
+  if (h->ws != ws_before) {   // the arena moved: every captured graph points into the old one
+    for (auto& g : h->graphs) cudaGraphExecDestroy(g.exec);
+    h->graphs.clear();
+  }
+  if (graph_wanted(h, B, S, N, block0, block1, step0, step1)) {
+    for (auto& g : h->graphs)
+      if (g.msa == msa && g.pair == pair && g.sm == sm && g.mm == mm && g.B == B && g.S == S && g.N == N && g.block0 == block0 &&
+          g.block1 == block1) {
+        if (cudaGraphLaunch(g.exec, st) != cudaSuccess) return fail(PF_ERR_CUDA, "cudaGraphLaunch");
+        h->launches = g.launches;
+        launches += g.launches;
+        return PF_OK;
+      }
+    // captured on a stream of the handle's own (the caller's may be the legacy default stream, which cannot be captured;
+    // nothing executes during capture) and replayed on the caller's stream
+    if (!h->cap_stream && cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking) != cudaSuccess) {
+      h->cap_stream = nullptr;
+      cudaGetLastError();
+    }
+    cudaStream_t cs = h->cap_stream;
+    if (cs && cudaStreamBeginCapture(cs, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+      s = pass_launches(h, msa, pair, sm, mm, B, S, N, block0, block1, step0, step1, cs);
+      cudaGraph_t graph = nullptr;
+      cudaError_t ce = cudaStreamEndCapture(cs, &graph);
+      cudaGraphExec_t exec = nullptr;
+      if (s == PF_OK && ce == cudaSuccess && graph && cudaGraphInstantiate(&exec, graph, 0) == cudaSuccess) {
+        cudaGraphDestroy(graph);
+        if (h->graphs.size() >= 16) {   // bounded cache: drop the oldest
+          cudaGraphExecDestroy(h->graphs.front().exec);
+          h->graphs.erase(h->graphs.begin());
+        }
+        h->graphs.push_back({msa, pair, sm, mm, B, S, N, block0, block1, exec, h->launches});
+        if (cudaGraphLaunch(exec, st) != cudaSuccess) return fail(PF_ERR_CUDA, "cudaGraphLaunch");
+        launches += h->launches;
+        return PF_OK;
+      }
+      if (graph) cudaGraphDestroy(graph);
+      cudaGetLastError();   // capture did not work out: fall through to plain launches
+    } else {
+      cudaGetLastError();
+    }
+  }
+  s = pass_launches(h, msa, pair, sm, mm, B, S, N, block0, block1, step0, step1, st);
+  if (s != PF_OK) return s;
   launches += h->launches;
   return PF_OK;
 }

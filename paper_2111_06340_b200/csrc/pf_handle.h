@@ -87,6 +87,10 @@ struct pf_evoformer {
   size_t f16_below_normal = 0;   // weights stored as fp16 with |w| < 2^-14 (precision loss, pf_evoformer.h value-range note)
   int device = -1;           // the device the handle was created on (weights, workspace and kernel attributes live there)
   int ws_B = 0, ws_S = 0, ws_N = 0;   // shape of the arena layout the workspace currently holds (zero-filled when it changes)
+  // CUDA graphs of whole forward calls on launch-bound shapes (pf_api.cu, dispatch_pass)
+  struct GraphEntry { float* msa; float* pair; const float* sm; const float* mm; int B, S, N, block0, block1; cudaGraphExec_t exec; long long launches; };
+  std::vector<GraphEntry> graphs;
+  cudaStream_t cap_stream = nullptr;
   char* stage = nullptr;     // forward_host staging
   size_t stage_bytes = 0;
   // forward_host pipelines the batch in chunks of proteins: copy-in stream, the caller's stream for compute, copy-out stream

@@ -67,3 +67,39 @@ def test_repeated_runs_are_bit_identical():
     h.close()
     for mo, zo in outs[1:]:
         assert np.array_equal(mo, outs[0][0]) and np.array_equal(zo, outs[0][1])
+
+
+def test_cuda_graph_replay_matches_direct_launches():
+    """Small shapes are launch-bound, so whole forward calls on them are captured into a CUDA graph per (buffers, shape) and
+    replayed (pf_api.cu, dispatch_pass).  The graph holds the mask-flag kernels too, so changing the CONTENTS of the masks
+    between replays must give what a direct launch sequence gives (profiling on = no graph), bit for bit."""
+    import torch
+    B, S, N, nb = 2, 10, 72, 2
+    blocks = ps.make_weights(61, nb, bf16_weights=True)
+    msa, pair, sm1, mm1 = ps.make_inputs(62, B, S, N, lengths=[72, 50], msa_mask_frac_max=0.3)
+    _, _, sm2, mm2 = ps.make_inputs(63, B, S, N, lengths=[33, 72], msa_mask_frac_max=0.3)
+    hg = pf.Evoformer(ps.pack_blob(blocks), pf.make_config(nb, pf.PF_BF16))
+    hd = pf.Evoformer(ps.pack_blob(blocks), pf.make_config(nb, pf.PF_BF16))
+    hd.set_profiling(True)
+    m = torch.empty((B, S, N, 256), device="cuda")
+    z = torch.empty((B, N, N, 128), device="cuda")
+    smd = torch.empty((B, N), device="cuda")
+    mmd = torch.empty((B, S), device="cuda")
+    outs = {}
+    for tag, h in (("graph", hg), ("direct", hd)):
+        for k, (sm, mm) in enumerate(((sm1, mm1), (sm2, mm2), (sm1, mm1))):
+            m.copy_(torch.from_numpy(msa))
+            z.copy_(torch.from_numpy(pair))
+            smd.copy_(torch.from_numpy(sm))
+            mmd.copy_(torch.from_numpy(mm))
+            h.forward(m, z, smd, mmd, nb)          # same buffers every time: the second and third call replay the graph
+            torch.cuda.synchronize()
+            outs[(tag, k)] = (m.cpu().numpy().copy(), z.cpu().numpy().copy())
+    hg.close()
+    hd.close()
+    for k, (sm, mm) in enumerate(((sm1, mm1), (sm2, mm2), (sm1, mm1))):
+        vm = (mm[:, :, None] * sm[:, None, :]) > 0
+        vz = (sm[:, :, None] * sm[:, None, :]) > 0
+        assert np.isfinite(outs[("graph", k)][0]).all() and np.isfinite(outs[("graph", k)][1]).all()
+        assert np.array_equal(outs[("graph", k)][0][vm], outs[("direct", k)][0][vm]), k
+        assert np.array_equal(outs[("graph", k)][1][vz], outs[("direct", k)][1][vz]), k
