@@ -88,7 +88,12 @@ pf_status pf_evoformer_create(pf_evoformer_t** out, const float* weights_host, s
  * relative perturbation of those entries only, far below the bf16 tolerances).
  * Masked work: on the PF_BF16 path 128-row tiles, attention rows and key tiles whose outputs all lie at masked positions are
  * skipped (outputs there are unspecified but finite, as stated above); unmasked outputs do not depend on what the masked
- * positions of msa / pair contain. */
+ * positions of msa / pair contain.
+ * Launch-bound shapes (PF_BF16, B * S * N <= 131072, n_blocks >= 2, profiling off): the launch sequence of the call is captured
+ * into a CUDA graph the first time it is seen for these buffer addresses and this shape, and replayed on cuda_stream afterwards
+ * (the mask-derived flags are computed inside the graph, so mask CONTENTS may change between calls).  At most 16 graphs are
+ * kept per handle; a workspace growth drops them.  Environment variable PF_GRAPH=0 turns this off, PF_GRAPH=2 forces it for
+ * every shape. */
 pf_status pf_evoformer_forward(pf_evoformer_t* h, float* msa_dev, float* pair_dev,
                                const float* seq_mask_dev, const float* msa_mask_dev,
                                int B, int S, int N, int n_blocks, void* cuda_stream);
