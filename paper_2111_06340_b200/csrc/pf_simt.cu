@@ -519,129 +519,141 @@ template void launch_opm_simt<bf16>(const bf16*, const bf16*, const float*, cons
 
 // ---------------------------------------------------------------------------------------------
 // Pair-bias heads of the MSA row attention (A.1):  bias[b, h, i, j] = scale * sum_c LN'(z[b,i,j])_c W[c, h],  c_z = 128, H <= 8.
-// 512 bytes in and 2 H bytes out per pair with 2 H c_z FLOP: HBM-bound streaming work, so SIMT in fp32 (as a launch of the
-// projection GEMM it ran at 2.3 TB/s, paced by that kernel's LayerNorm producers).  Eight lanes per pair row (16 channels per
-// lane, coalesced float4 loads), two rows per lane in flight, the projection weights in shared memory with the scale folded
-// in, one reduce-scatter over the eight lanes (7 shuffles for all heads) after which lane h of a row holds head h and stores
-// it (2-byte stores, 3 % of the traffic; no CTA-level synchronisation in the loop, warps run independently).  Pairs with a masked i or j are skipped: the attention masks key j itself and a masked query's output is
+// 512 bytes in and 2 H bytes out per pair with 2 H c_z FLOP: HBM-bound streaming work (as a launch of the projection GEMM it
+// ran at 2.3 TB/s, paced by that kernel's LayerNorm producers; a first SIMT version with the eight dot products on the FMA
+// pipes was bound by instruction issue: 107 warp instructions per row, 2.7 TB/s).  This version: a warp owns 16 consecutive
+// pair rows and holds them in the A-fragment layout of mma.sync.m16n8k16 (lane = (row group g, column group t): rows g and
+// g + 8, columns 16 kb + 2 t + {0, 1, 8, 9} of every 16-wide k-block, loaded as float2), normalises in registers (statistics
+// over the four lanes of a row: two shuffles each), converts xhat to fp16 pairs and issues eight mma.sync against the weight
+// fragments, which hold gamma_c W[c, h] scale as fp16 (LN'(z) W = xhat (gamma . W) + beta W: the affine part of the
+// LayerNorm moves into the weights, the constant beta W is added in fp32 at the end; fp16 operands as the projection GEMM,
+// R17).  Pairs with a masked i or j are skipped: the attention masks key j itself and a masked query's output is
 // unspecified (R3); what the bias buffer holds there is a finite older value.
 // ---------------------------------------------------------------------------------------------
-constexpr int LH_ROWS = 64;   // pair rows per CTA iteration (8 warps x 4 rows x 2 passes)
-__global__ void __launch_bounds__(256, 4) ln_heads128_kernel(const float* __restrict__ z, const float* __restrict__ gamma,
-                                                          const float* __restrict__ beta, const float* __restrict__ W,
-                                                          float scale, const float* __restrict__ seq_mask,
-                                                          bf16* __restrict__ out, int B, int N, int Lpad, int H) {
-  __shared__ __align__(16) float ws[8 * 132];          // [sub][16 channels][8 heads] + 4 floats of padding per sub
-  __shared__ float4 gbs[2][32];                        // LayerNorm gamma / beta
-  for (int t = threadIdx.x; t < 8 * 128; t += 256) {
-    const int sub = t >> 7, k = (t >> 3) & 15, hh = t & 7;              // lane sub owns channels (i * 8 + sub) * 4 + e, k = 4 i + e
-    const int c = ((k >> 2) * 8 + sub) * 4 + (k & 3);
-    ws[sub * 132 + k * 8 + hh] = hh < H ? __ldg(W + c * H + hh) * scale : 0.f;
+__device__ __forceinline__ void mma_16816_f16(float (&d)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1) {
+  asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+               : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
+               : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
+}
+__device__ __forceinline__ uint32_t pack_h2(float a, float b) {
+  __half2 h = __floats2half2_rn(a, b);
+  return *reinterpret_cast<uint32_t*>(&h);
+}
+__device__ __forceinline__ float2 ld_nc_f2(const float2* p) {
+  float2 r;
+  asm volatile("ld.global.nc.L1::no_allocate.v2.f32 {%0,%1}, [%2];" : "=f"(r.x), "=f"(r.y) : "l"(p));
+  return r;
+}
+
+constexpr int LH_WARPS = 8;   // 16 pair rows per warp and iteration
+__global__ void __launch_bounds__(32 * LH_WARPS, 2) ln_heads128_kernel(const float* __restrict__ z, const float* __restrict__ gamma,
+                                                                       const float* __restrict__ beta, const float* __restrict__ W,
+                                                                       float scale, const float* __restrict__ seq_mask,
+                                                                       bf16* __restrict__ out, int B, int N, int Lpad, int H) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, g = lane >> 2, t = lane & 3;
+  // B fragments of the eight k-blocks: b0 = (k = 16 kb + 2t, +1; n = g), b1 = (k = 16 kb + 2t + 8, +9; n = g), n = head
+  uint32_t bw[8][2];
+  float bias_h[2] = {0.f, 0.f};                 // beta W scale for this lane's two output heads (2t, 2t + 1)
+#pragma unroll
+  for (int kb = 0; kb < 8; ++kb) {
+#pragma unroll
+    for (int hf = 0; hf < 2; ++hf) {
+      const int c = 16 * kb + 2 * t + 8 * hf;
+      const float w0 = g < H ? __ldg(gamma + c) * __ldg(W + c * H + g) * scale : 0.f;
+      const float w1 = g < H ? __ldg(gamma + c + 1) * __ldg(W + (c + 1) * H + g) * scale : 0.f;
+      bw[kb][hf] = pack_h2(w0, w1);
+    }
   }
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, sub = lane & 7, rsel = lane >> 3;
-  if (threadIdx.x < 64)
-    gbs[threadIdx.x >> 5][threadIdx.x & 31] = __ldg(reinterpret_cast<const float4*>(threadIdx.x < 32 ? gamma : beta) + (threadIdx.x & 31));
-  __syncthreads();
+  {
+    float part[8];
+#pragma unroll
+    for (int hh = 0; hh < 8; ++hh) {
+      part[hh] = 0.f;
+      if (hh < H)
+        for (int c = lane * 4; c < lane * 4 + 4; ++c) part[hh] = fmaf(__ldg(beta + c) * scale, __ldg(W + c * H + hh), part[hh]);
+      part[hh] = warp_sum(part[hh]);
+    }
+#pragma unroll
+    for (int hh = 0; hh < 8; ++hh) {
+      if (hh == 2 * t) bias_h[0] = part[hh];
+      if (hh == 2 * t + 1) bias_h[1] = part[hh];
+    }
+  }
   const long rows = (long)B * N * N;
-  const float* wl = ws + sub * 132;
-  for (long r0 = (long)blockIdx.x * LH_ROWS; r0 < rows; r0 += (long)gridDim.x * LH_ROWS) {
-    float4 v[2][4];
+  for (long r0 = ((long)blockIdx.x * LH_WARPS + warp) * 16; r0 < rows; r0 += (long)gridDim.x * LH_WARPS * 16) {
     bool on[2];
     long oidx[2];   // output index of head 0 (rows < 2^32 is checked by the launcher: 32-bit divisions only)
+    const float* src[2];
 #pragma unroll
-    for (int ps = 0; ps < 2; ++ps) {
-      const long r = r0 + warp * 8 + ps * 4 + rsel;
-      on[ps] = false;
-      oidx[ps] = 0;
+    for (int q = 0; q < 2; ++q) {
+      const long r = r0 + g + 8 * q;
+      on[q] = false;
+      oidx[q] = 0;
+      src[q] = z;
       if (r < rows) {
         const unsigned ru = (unsigned)r, bx = ru / (unsigned)N, y = ru - bx * (unsigned)N, b = bx / (unsigned)N, x = bx - b * (unsigned)N;
-        on[ps] = seq_mask[bx] > 0.5f && seq_mask[b * (unsigned)N + y] > 0.5f;
-        oidx[ps] = ((long)b * H * N + x) * (long)Lpad + y;
-      }
-      if (on[ps]) {
-        const float4* xp = reinterpret_cast<const float4*>(z + r * 128);
-#pragma unroll
-        for (int i = 0; i < 4; ++i) v[ps][i] = ld_nc_f4(xp + i * 8 + sub);
-      } else {
-#pragma unroll
-        for (int i = 0; i < 4; ++i) v[ps][i] = make_float4(0.f, 0.f, 0.f, 0.f);
+        on[q] = seq_mask[bx] > 0.5f && seq_mask[b * (unsigned)N + y] > 0.5f;
+        oidx[q] = ((long)b * H * N + x) * (long)Lpad + y;
+        src[q] = z + r * 128;
       }
     }
-    float acc[2][8];
+    if (!__any_sync(0xffffffffu, on[0] || on[1])) continue;
+    float2 v[2][8][2];
 #pragma unroll
-    for (int ps = 0; ps < 2; ++ps) {
+    for (int q = 0; q < 2; ++q)
+#pragma unroll
+      for (int kb = 0; kb < 8; ++kb)
+#pragma unroll
+        for (int hf = 0; hf < 2; ++hf)
+          v[q][kb][hf] = on[q] ? ld_nc_f2(reinterpret_cast<const float2*>(src[q] + 16 * kb + 2 * t + 8 * hf)) : make_float2(0.f, 0.f);
+    float acc[4] = {0.f, 0.f, 0.f, 0.f};
+    float rstd[2], nm[2];
+#pragma unroll
+    for (int q = 0; q < 2; ++q) {
       float s = 0.f;
 #pragma unroll
-      for (int i = 0; i < 4; ++i) s += (v[ps][i].x + v[ps][i].y) + (v[ps][i].z + v[ps][i].w);
-#pragma unroll
-      for (int o = 4; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+      for (int kb = 0; kb < 8; ++kb) s += (v[q][kb][0].x + v[q][kb][0].y) + (v[q][kb][1].x + v[q][kb][1].y);
+      s += __shfl_xor_sync(0xffffffffu, s, 1);
+      s += __shfl_xor_sync(0xffffffffu, s, 2);
       const float mean = s * (1.0f / 128);
-      float q = 0.f;
+      float qq = 0.f;
 #pragma unroll
-      for (int i = 0; i < 4; ++i) {
-        const float a = v[ps][i].x - mean, b = v[ps][i].y - mean, c = v[ps][i].z - mean, d = v[ps][i].w - mean;
-        q += (a * a + b * b) + (c * c + d * d);
+      for (int kb = 0; kb < 8; ++kb) {
+        const float a = v[q][kb][0].x - mean, b = v[q][kb][0].y - mean, c = v[q][kb][1].x - mean, d = v[q][kb][1].y - mean;
+        qq += (a * a + b * b) + (c * c + d * d);
       }
-#pragma unroll
-      for (int o = 4; o > 0; o >>= 1) q += __shfl_xor_sync(0xffffffffu, q, o);
-      const float rstd = rsqrtf(q * (1.0f / 128) + 1e-5f);
-      const float nm = -mean * rstd;
-#pragma unroll
-      for (int i = 0; i < 4; ++i) {
-        const float4 gm = gbs[0][i * 8 + sub], bt = gbs[1][i * 8 + sub];
-        v[ps][i].x = fmaf(v[ps][i].x, rstd, nm) * gm.x + bt.x;
-        v[ps][i].y = fmaf(v[ps][i].y, rstd, nm) * gm.y + bt.y;
-        v[ps][i].z = fmaf(v[ps][i].z, rstd, nm) * gm.z + bt.z;
-        v[ps][i].w = fmaf(v[ps][i].w, rstd, nm) * gm.w + bt.w;
-      }
-#pragma unroll
-      for (int hh = 0; hh < 8; ++hh) acc[ps][hh] = 0.f;
+      qq += __shfl_xor_sync(0xffffffffu, qq, 1);
+      qq += __shfl_xor_sync(0xffffffffu, qq, 2);
+      rstd[q] = rsqrtf(qq * (1.0f / 128) + 1e-5f);
+      nm[q] = -mean * rstd[q];
     }
 #pragma unroll
-    for (int i = 0; i < 4; ++i) {
-#pragma unroll
-      for (int e = 0; e < 4; ++e) {
-        const float4 w0 = *reinterpret_cast<const float4*>(wl + (4 * i + e) * 8), w1 = *reinterpret_cast<const float4*>(wl + (4 * i + e) * 8 + 4);
-#pragma unroll
-        for (int ps = 0; ps < 2; ++ps) {
-          const float x = e == 0 ? v[ps][i].x : e == 1 ? v[ps][i].y : e == 2 ? v[ps][i].z : v[ps][i].w;
-          acc[ps][0] = fmaf(x, w0.x, acc[ps][0]); acc[ps][1] = fmaf(x, w0.y, acc[ps][1]);
-          acc[ps][2] = fmaf(x, w0.z, acc[ps][2]); acc[ps][3] = fmaf(x, w0.w, acc[ps][3]);
-          acc[ps][4] = fmaf(x, w1.x, acc[ps][4]); acc[ps][5] = fmaf(x, w1.y, acc[ps][5]);
-          acc[ps][6] = fmaf(x, w1.z, acc[ps][6]); acc[ps][7] = fmaf(x, w1.w, acc[ps][7]);
-        }
-      }
+    for (int kb = 0; kb < 8; ++kb) {
+      uint32_t a[4];   // a0 (row g, cols 2t..), a1 (row g + 8, cols 2t..), a2 (row g, cols 2t + 8..), a3 (row g + 8, cols 2t + 8..)
+      a[0] = pack_h2(fmaf(v[0][kb][0].x, rstd[0], nm[0]), fmaf(v[0][kb][0].y, rstd[0], nm[0]));
+      a[1] = pack_h2(fmaf(v[1][kb][0].x, rstd[1], nm[1]), fmaf(v[1][kb][0].y, rstd[1], nm[1]));
+      a[2] = pack_h2(fmaf(v[0][kb][1].x, rstd[0], nm[0]), fmaf(v[0][kb][1].y, rstd[0], nm[0]));
+      a[3] = pack_h2(fmaf(v[1][kb][1].x, rstd[1], nm[1]), fmaf(v[1][kb][1].y, rstd[1], nm[1]));
+      mma_16816_f16(acc, a, bw[kb][0], bw[kb][1]);
     }
-    // reduce-scatter over the 8 lanes of a row: lane sub ends with the sum of head sub
+    // acc: (row g, head 2t), (row g, head 2t + 1), (row g + 8, head 2t), (row g + 8, head 2t + 1)
+    const long hs = (long)N * Lpad;
 #pragma unroll
-    for (int ps = 0; ps < 2; ++ps) {
-      float a4[4], a2[2];
-      const bool up4 = sub & 4, up2 = sub & 2, up1 = sub & 1;
-#pragma unroll
-      for (int j = 0; j < 4; ++j) {
-        const float send = up4 ? acc[ps][j] : acc[ps][j + 4];
-        const float recv = __shfl_xor_sync(0xffffffffu, send, 4);
-        a4[j] = (up4 ? acc[ps][j + 4] : acc[ps][j]) + recv;
+    for (int q = 0; q < 2; ++q) {
+      if (on[q]) {
+        if (2 * t < H) out[oidx[q] + (long)(2 * t) * hs] = __float2bfloat16_rn(acc[2 * q] + bias_h[0]);
+        if (2 * t + 1 < H) out[oidx[q] + (long)(2 * t + 1) * hs] = __float2bfloat16_rn(acc[2 * q + 1] + bias_h[1]);
       }
-#pragma unroll
-      for (int j = 0; j < 2; ++j) {
-        const float send = up2 ? a4[j] : a4[j + 2];
-        const float recv = __shfl_xor_sync(0xffffffffu, send, 2);
-        a2[j] = (up2 ? a4[j + 2] : a4[j]) + recv;
-      }
-      const float send = up1 ? a2[0] : a2[1];
-      const float recv = __shfl_xor_sync(0xffffffffu, send, 1);
-      const float val = (up1 ? a2[1] : a2[0]) + recv;
-      if (on[ps] && sub < H) out[oidx[ps] + (long)sub * N * Lpad] = __float2bfloat16_rn(val);
     }
   }
 }
 
 void launch_ln_heads128(const float* z, const float* gamma, const float* beta, const float* W, float scale, const float* seq_mask,
                         bf16* out, int B, int N, int Lpad, int H, int num_sms, cudaStream_t st) {
-  const long rows = (long)B * N * N, blocks = (rows + LH_ROWS - 1) / LH_ROWS;
-  const long cap = (long)num_sms * 8;
-  ln_heads128_kernel<<<(unsigned)(blocks < cap ? blocks : cap), 256, 0, st>>>(z, gamma, beta, W, scale, seq_mask, out, B, N, Lpad, H);
+  const long rows = (long)B * N * N, blocks = (rows + LH_WARPS * 16 - 1) / (LH_WARPS * 16);
+  const long cap = (long)num_sms * 2;   // persistent: two CTAs per SM, the weight fragments are built once per CTA
+  ln_heads128_kernel<<<(unsigned)(blocks < cap ? blocks : cap), 32 * LH_WARPS, 0, st>>>(z, gamma, beta, W, scale, seq_mask, out, B, N,
+                                                                                        Lpad, H);
 }
 
 }  // namespace pf
