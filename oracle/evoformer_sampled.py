@@ -12,7 +12,7 @@ of ``evoformer_ref``.
 
 Optional switch ``rnd`` (reading R16, "quantisation-aware oracle"): a ``Rounding`` object rounds
 intermediate values at the points where the bf16 CUDA path stores them in 16 bits (R17:
-LayerNorm outputs and gates fp16; q, k, v, P, o, pair bias, transition hidden, outer-product and
+LayerNorm outputs, gates and pair bias fp16; q, k, v, P, o, transition hidden, outer-product and
 triangle operands bf16).  The arithmetic between those points stays fp64.  With ``rnd=None`` (the
 default) no rounding happens and the functions ARE the plain oracle; the switch exists so that a
 difference GPU - oracle can be split into the part the storage formats cause by themselves
@@ -88,11 +88,11 @@ def _gated_attention_one_query(xq, xk, beta_q, key_mask, w, head_dim, r):
     v = r.bf16(_lin(xk, w["wv"], None, r))
     gate = r.gate(_lin(xq, w["wg"], w["bg"], r))
     if r.on:
-        # storage points of the CUDA path: q carries log2(e)/sqrt(d), the bias log2(e) (both bf16); the softmax runs in the
+        # storage points of the CUDA path: q carries log2(e)/sqrt(d) (bf16), the bias log2(e) (fp16); the softmax runs in the
         # exp2 domain — the same real function (R12)
         q = r.bf16(q * (LOG2E / np.sqrt(float(head_dim)))) / LOG2E * np.sqrt(float(head_dim))
         if beta_q is not None:
-            beta_q = r.bf16(_f64(beta_q) * LOG2E) / LOG2E
+            beta_q = r.f16(_f64(beta_q) * LOG2E) / LOG2E
     o = np.zeros(C, dtype=F64)
     for h in range(H):
         cols = slice(h * head_dim, (h + 1) * head_dim)
@@ -157,7 +157,7 @@ def outer_product_mean_at(m, z, seq_mask, msa_mask, w, i, j, rnd=None):
 
 def _tri_operand(x, pi, wp, bp, wg, bg, r):
     """pi (.) sigmoid(Lin_g(x)) (.) Lin_p(x) for the rows of x ([L, c_z]) with pair masks pi ([L])."""
-    return r.bf16(pi[:, None] * sigmoid(_lin(x, wg, bg, r)) * _lin(x, wp, bp, r))
+    return r.f16(pi[:, None] * sigmoid(_lin(x, wg, bg, r)) * _lin(x, wp, bp, r))
 
 
 def triangle_mult_outgoing_at(z, seq_mask, w, i, j, rnd=None):
@@ -168,7 +168,7 @@ def triangle_mult_outgoing_at(z, seq_mask, w, i, j, rnd=None):
     xj = _ln(z[j], w["ln_in_g"], w["ln_in_b"], r)                     # rows (j, k)
     a = _tri_operand(xi, sg[i] * sg, w["w_ap"], w["b_ap"], w["w_ag"], w["b_ag"], r)   # a[k, c] = a[i,k,c]
     b = _tri_operand(xj, sg[j] * sg, w["w_bp"], w["b_bp"], w["w_bg"], w["b_bg"], r)   # b[k, c] = b[j,k,c]
-    t = r.bf16(np.sum(a * b, axis=0))
+    t = r.f16(np.sum(a * b, axis=0))
     g = r.gate(_lin(xi[j], w["w_g"], w["b_g"], r))
     return _f64(z[i, j]) + g * _lin(_ln(t, w["ln_out_g"], w["ln_out_b"], r), w["w_z"], w["b_z"], r)
 
@@ -181,7 +181,7 @@ def triangle_mult_incoming_at(z, seq_mask, w, i, j, rnd=None):
     xj = _ln(z[:, j], w["ln_in_g"], w["ln_in_b"], r)                  # rows (k, j)
     a = _tri_operand(xi, sg * sg[i], w["w_ap"], w["b_ap"], w["w_ag"], w["b_ag"], r)   # a[k, c] = a[k,i,c]
     b = _tri_operand(xj, sg * sg[j], w["w_bp"], w["b_bp"], w["w_bg"], w["b_bg"], r)   # b[k, c] = b[k,j,c]
-    t = r.bf16(np.sum(a * b, axis=0))
+    t = r.f16(np.sum(a * b, axis=0))
     xij = _ln(z[i, j], w["ln_in_g"], w["ln_in_b"], r)
     g = r.gate(_lin(xij, w["w_g"], w["b_g"], r))
     return _f64(z[i, j]) + g * _lin(_ln(t, w["ln_out_g"], w["ln_out_b"], r), w["w_z"], w["b_z"], r)

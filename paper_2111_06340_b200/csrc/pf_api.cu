@@ -92,7 +92,7 @@ extern "C" size_t pf_evoformer_block_floats(const pf_config* cfg) {
   return block_offsets(*cfg).total;
 }
 
-static const char* const kKindNames[KK_COUNT] = {"ln_rows", "gemm", "attn_core", "tri_einsum", "ln_channels", "opm_core", "ln_gemm", "transition", "mask_flags", "global_col_attn", "embedders", "pair_bias_heads"};
+static const char* const kKindNames[KK_COUNT] = {"ln_rows", "gemm", "attn_core", "tri_einsum", "ln_channels", "opm_core", "ln_gemm", "transition", "mask_flags", "global_col_attn", "embedders", "pair_bias_heads", "opm_operands"};
 
 
 Arena pf::arena_layout(const pf_config& c, int B, int S, int N) {

@@ -116,7 +116,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQK, const __grid_constant__
     __syncthreads();
     if (threadIdx.x < 64) {
       const int j = threadIdx.x;
-      *reinterpret_cast<uint16_t*>(smem + SM::ID_OFF + tc::swz_offset<128>(j, j >> 3) + (j & 7) * 2) = 0x3F80;
+      *reinterpret_cast<uint16_t*>(smem + SM::ID_OFF + tc::swz_offset<128>(j, j >> 3) + (j & 7) * 2) = 0x3C00;   // fp16 1.0: the pair bias is stored as fp16 (R17)
     }
     tc::fence_proxy_async_smem();
   }
@@ -161,6 +161,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQK, const __grid_constant__
     // ============================================================= MMA issue
     if (tc::elect_one()) {
       constexpr uint32_t idesc_s = tc::idesc_bf16_f32(AT_BQ, AT_BK);
+      constexpr uint32_t idesc_b = tc::idesc_f16_f32(AT_BQ, AT_BK);   // bias tile x identity: fp16 operands
       constexpr uint32_t idesc_o = tc::idesc_bf16_f32(AT_BQ, 32);
       const uint64_t p_desc = tc::smem_desc_kmajor<128>(tc::smem_u32(smem + SM::P_OFF));
       const uint64_t id_desc = tc::smem_desc_kmajor<128>(tc::smem_u32(smem + SM::ID_OFF));
@@ -189,7 +190,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQK, const __grid_constant__
           const uint64_t b_desc = tc::smem_desc_kmajor<128>(
               tc::smem_u32(smem + SM::STAGE_OFF + s * p.stage_bytes + SM::K_BYTES + SM::V_BYTES));
 #pragma unroll
-          for (int k = 0; k < AT_BK / 16; ++k) tc::mma_bf16(d, b_desc + 2 * k, id_desc + 2 * k, idesc_s, true);
+          for (int k = 0; k < AT_BK / 16; ++k) tc::mma_bf16(d, b_desc + 2 * k, id_desc + 2 * k, idesc_b, true);
         }
         tc::mma_commit(&s_full[j & 1]);
         if (ckt == cn - 1) {

@@ -58,7 +58,7 @@ TcBlock tc_layout(const pf_config& c);
 void build_tc_block(const pf_config& c, const BlockW& off, const TcBlock& t, const float* w, std::vector<uint16_t>& w16,
                     size_t base16, std::vector<float>& wf, size_t basef, F16Range* range);
 
-enum KernelKind { KK_LN = 0, KK_GEMM, KK_ATTN, KK_TRI, KK_LNC, KK_OPM, KK_LNGEMM, KK_TRANS, KK_FLAGS, KK_GLOBAL, KK_EMBED, KK_HEADS, KK_COUNT };
+enum KernelKind { KK_LN = 0, KK_GEMM, KK_ATTN, KK_TRI, KK_LNC, KK_OPM, KK_LNGEMM, KK_TRANS, KK_FLAGS, KK_GLOBAL, KK_EMBED, KK_HEADS, KK_OPMAB, KK_COUNT };
 
 inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 inline int pad8(int v) { return (v + 7) / 8 * 8; }

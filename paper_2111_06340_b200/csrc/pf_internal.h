@@ -67,6 +67,10 @@ void launch_lnc(const float* t_cm, T* y, const float* gamma, const float* beta, 
 // pair-bias heads of the MSA row attention at c_z = 128, H <= 8 (pf_simt.cu): bias[b,h,i,j] = scale Lin0(LN'(z_ij))_h, W [128, H] fp32
 void launch_ln_heads128(const float* z, const float* gamma, const float* beta, const float* W, float scale, const float* seq_mask,
                         bf16* out, int B, int N, int Lpad, int H, int num_sms, cudaStream_t st);
+// outer-product-mean operands at c_m = 256, c_opm = 32 (pf_simt.cu): ab_t[(b,i), 64, Spad] = mu (LN(m) [W_a | W_b] + [b_a | b_b]), fp32 weights [256, 32]
+void launch_ln_opm_ab256(const float* msa, const float* gamma, const float* beta, const float* Wa, const float* Wb, const float* ba,
+                         const float* bb, const float* seq_mask, const float* msa_mask, bf16* out, int B, int S, int N, int Spad,
+                         int num_sms, cudaStream_t st);
 void launch_lnc_tc(const bf16* t_cm, __half* y, const float* gamma, const float* beta, const float* seq_mask, int B, int N,
                    int Npad, cudaStream_t st);
 template <typename T>

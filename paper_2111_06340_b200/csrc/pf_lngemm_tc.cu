@@ -481,15 +481,15 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
               lds32(sbias + hf * 32, bp);
               lds32(sbias2 + hf * 32, bg);
               tc::tmem_ld_wait();
-              bf16 r[32];
+              __half r[32];   // triangle operands are fp16 (R17, round 2)
 #pragma unroll
               for (int e = 0; e < 32; ++e) {
                 const float pv = __uint_as_float(v[e]) + bp[e];
                 const float gv = fast_sigmoid2(__uint_as_float(g[e]) + bg[e]);
-                r[e] = __float2bfloat16_rn(mask * gv * pv);
+                r[e] = __float2half_rn(mask * gv * pv);
               }
 #pragma unroll
-              for (int e = 0; e < 32; ++e) sb16[(hf * 32 + e) * 32 + lane] = r[e];
+              for (int e = 0; e < 32; ++e) reinterpret_cast<__half*>(sb16)[(hf * 32 + e) * 32 + lane] = r[e];
             }
             tc::fence_proxy_async_smem();
             __syncwarp();
@@ -508,7 +508,7 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
             tc::tmem_ld_wait();
 #pragma unroll
             for (int e = 0; e < 8; ++e)
-              if (e < op.ncols) sb16[e * 32 + lane] = __float2bfloat16_rn(__uint_as_float(v[e]) * op.scale);
+              if (e < op.ncols) reinterpret_cast<__half*>(sb16)[e * 32 + lane] = __float2half_rn(__uint_as_float(v[e]) * op.scale);   // fp16 (R17)
             tc::fence_proxy_async_smem();
             __syncwarp();
             if (leader) {
@@ -537,7 +537,7 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
               for (int e = 0; e < 32; e += 2) {
                 const float o0 = mk[e] * fast_sigmoid2(__uint_as_float(g[e]) + bgv) * (__uint_as_float(v[e]) + bpv);
                 const float o1 = mk[e + 1] * fast_sigmoid2(__uint_as_float(g[e + 1]) + bgv) * (__uint_as_float(v[e + 1]) + bpv);
-                pk[e >> 1] = pack16(o0, o1, 0);
+                pk[e >> 1] = pack16(o0, o1, 1);   // triangle operands are fp16 (R17, round 2)
               }
 #pragma unroll
               for (int c = 0; c < 4; ++c)

@@ -404,8 +404,8 @@ __global__ void __launch_bounds__(256) lnc128_bf16_kernel(const bf16* __restrict
     const int c = warp * 16 + k;
     uint2 u = make_uint2(0u, 0u);
     if (in) u = __ldg(reinterpret_cast<const uint2*>(t + (((long)b * C + c) * N + i) * Npad + j));
-    const float2 lo = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&u.x));
-    const float2 hi = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&u.y));
+    const float2 lo = __half22float2(*reinterpret_cast<const __half2*>(&u.x));   // the einsum output is fp16 (R17, round 2)
+    const float2 hi = __half22float2(*reinterpret_cast<const __half2*>(&u.y));
     v[k][0] = lo.x; v[k][1] = lo.y; v[k][2] = hi.x; v[k][3] = hi.y;
   }
   float s[4] = {0.f, 0.f, 0.f, 0.f};
@@ -641,8 +641,9 @@ __global__ void __launch_bounds__(32 * LH_WARPS, 2) ln_heads128_kernel(const flo
 #pragma unroll
     for (int q = 0; q < 2; ++q) {
       if (on[q]) {
-        if (2 * t < H) out[oidx[q] + (long)(2 * t) * hs] = __float2bfloat16_rn(acc[2 * q] + bias_h[0]);
-        if (2 * t + 1 < H) out[oidx[q] + (long)(2 * t + 1) * hs] = __float2bfloat16_rn(acc[2 * q + 1] + bias_h[1]);
+        __half* oh = reinterpret_cast<__half*>(out);   // the pair bias is held as fp16 (R17): 8x finer than bf16 at |bias| ~ 1
+        if (2 * t < H) oh[oidx[q] + (long)(2 * t) * hs] = __float2half_rn(acc[2 * q] + bias_h[0]);
+        if (2 * t + 1 < H) oh[oidx[q] + (long)(2 * t + 1) * hs] = __float2half_rn(acc[2 * q + 1] + bias_h[1]);
       }
     }
   }
@@ -654,6 +655,130 @@ void launch_ln_heads128(const float* z, const float* gamma, const float* beta, c
   const long cap = (long)num_sms * 2;   // persistent: two CTAs per SM, the weight fragments are built once per CTA
   ln_heads128_kernel<<<(unsigned)(blocks < cap ? blocks : cap), 32 * LH_WARPS, 0, st>>>(z, gamma, beta, W, scale, seq_mask, out, B, N,
                                                                                         Lpad, H);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Outer-product-mean operands (A.4):  ab_t[(b, i), ch, s] = mu_si (LN(m_si) [W_a | W_b] + [b_a | b_b])_ch,  c_m = 256, 64 columns,
+// written transposed (s contiguous) for the outer-product kernel.  1 KB in and 128 bytes out per (s, i) with 32 K FLOP: HBM-bound
+// (as a launch of the projection GEMM it ran at 2.6-2.7 TB/s, paced by that kernel's LayerNorm producers).  Same scheme as the
+// pair-bias heads above: a warp owns 16 consecutive sequences s of one residue (b, i) and keeps the 16 x 256 fp32 values in
+// registers in the A-fragment layout of mma.sync.m16n8k16 (128 registers per lane), normalises them there, and multiplies by
+// gamma . W held as fp16 B fragments in shared memory (32 KB, laid out per lane so that a fragment fetch is four conflict-free
+// 16-byte loads); beta W + bias is added in fp32.  Residues i that are padded are skipped; masked sequences of an unmasked
+// residue are written as exact zeros (they are summed over without a softmax).
+// ---------------------------------------------------------------------------------------------
+constexpr int OA_WARPS = 8;
+__global__ void __launch_bounds__(32 * OA_WARPS, 1)
+ln_opm_ab256_kernel(const float* __restrict__ msa, const float* __restrict__ gamma, const float* __restrict__ beta,
+                    const float* __restrict__ Wa, const float* __restrict__ Wb, const float* __restrict__ ba,
+                    const float* __restrict__ bb, const float* __restrict__ seq_mask, const float* __restrict__ msa_mask,
+                    bf16* __restrict__ out, int B, int S, int N, int Spad) {
+  __shared__ uint4 wfrag[16 * 4 * 32];      // [kb][q][lane]: 16 bytes = fragments (nt = 2q, 2q + 1) x (b0, b1) of this lane
+  __shared__ float cst[64];                 // beta W + bias
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, g = lane >> 2, t = lane & 3;
+  auto wcol = [&](int c, int n) { return n < 32 ? __ldg(Wa + c * 32 + n) : __ldg(Wb + c * 32 + n - 32); };
+  for (int e = threadIdx.x; e < 16 * 4 * 32; e += blockDim.x) {
+    const int ln = e & 31, q = (e >> 5) & 3, kb = e >> 7, gg = ln >> 2, tt = ln & 3;
+    uint32_t w[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {           // j = (nt - 2q) * 2 + hf
+      const int n = 8 * (2 * q + (j >> 1)) + gg, c = 16 * kb + 2 * tt + 8 * (j & 1);
+      w[j] = pack_h2(__ldg(gamma + c) * wcol(c, n), __ldg(gamma + c + 1) * wcol(c + 1, n));
+    }
+    wfrag[e] = make_uint4(w[0], w[1], w[2], w[3]);
+  }
+  if (threadIdx.x < 64) {
+    const int n = threadIdx.x;
+    float a = n < 32 ? __ldg(ba + n) : __ldg(bb + n - 32);
+    for (int c = 0; c < 256; ++c) a = fmaf(__ldg(beta + c), wcol(c, n), a);
+    cst[n] = a;
+  }
+  __syncthreads();
+  const int sblocks = (S + 15) / 16;
+  const long units = (long)B * N * sblocks;
+  for (long u = (long)blockIdx.x * OA_WARPS + warp; u < units; u += (long)gridDim.x * OA_WARPS) {
+    const int sb = (int)(u % sblocks);
+    const long bi = u / sblocks;            // b * N + i
+    if (!(seq_mask[bi] > 0.5f)) continue;   // padded residue: nothing of this unit is read later
+    const int b = (int)(bi / N), i = (int)(bi - (long)b * N);
+    bool on[2], inr[2];
+    const float* src[2];
+#pragma unroll
+    for (int q = 0; q < 2; ++q) {
+      const int sq = sb * 16 + g + 8 * q;
+      inr[q] = sq < S;
+      on[q] = inr[q] && msa_mask[(long)b * S + sq] > 0.5f;
+      src[q] = msa + (((long)b * S + (inr[q] ? sq : 0)) * N + i) * 256;
+    }
+    float2 v[2][16][2];
+#pragma unroll
+    for (int q = 0; q < 2; ++q)
+#pragma unroll
+      for (int kb = 0; kb < 16; ++kb)
+#pragma unroll
+        for (int hf = 0; hf < 2; ++hf)
+          v[q][kb][hf] = on[q] ? ld_nc_f2(reinterpret_cast<const float2*>(src[q] + 16 * kb + 2 * t + 8 * hf)) : make_float2(0.f, 0.f);
+    float rstd[2], nm[2];
+#pragma unroll
+    for (int q = 0; q < 2; ++q) {
+      float sm = 0.f;
+#pragma unroll
+      for (int kb = 0; kb < 16; ++kb) sm += (v[q][kb][0].x + v[q][kb][0].y) + (v[q][kb][1].x + v[q][kb][1].y);
+      sm += __shfl_xor_sync(0xffffffffu, sm, 1);
+      sm += __shfl_xor_sync(0xffffffffu, sm, 2);
+      const float mean = sm * (1.0f / 256);
+      float qq = 0.f;
+#pragma unroll
+      for (int kb = 0; kb < 16; ++kb) {
+        const float a = v[q][kb][0].x - mean, bq = v[q][kb][0].y - mean, c = v[q][kb][1].x - mean, d = v[q][kb][1].y - mean;
+        qq += (a * a + bq * bq) + (c * c + d * d);
+      }
+      qq += __shfl_xor_sync(0xffffffffu, qq, 1);
+      qq += __shfl_xor_sync(0xffffffffu, qq, 2);
+      rstd[q] = rsqrtf(qq * (1.0f / 256) + 1e-5f);
+      nm[q] = -mean * rstd[q];
+    }
+    float acc[8][4];
+#pragma unroll
+    for (int nt = 0; nt < 8; ++nt)
+#pragma unroll
+      for (int e = 0; e < 4; ++e) acc[nt][e] = 0.f;
+#pragma unroll
+    for (int kb = 0; kb < 16; ++kb) {
+      uint32_t a[4];
+      a[0] = pack_h2(fmaf(v[0][kb][0].x, rstd[0], nm[0]), fmaf(v[0][kb][0].y, rstd[0], nm[0]));
+      a[1] = pack_h2(fmaf(v[1][kb][0].x, rstd[1], nm[1]), fmaf(v[1][kb][0].y, rstd[1], nm[1]));
+      a[2] = pack_h2(fmaf(v[0][kb][1].x, rstd[0], nm[0]), fmaf(v[0][kb][1].y, rstd[0], nm[0]));
+      a[3] = pack_h2(fmaf(v[1][kb][1].x, rstd[1], nm[1]), fmaf(v[1][kb][1].y, rstd[1], nm[1]));
+#pragma unroll
+      for (int q = 0; q < 4; ++q) {
+        const uint4 w = wfrag[(kb * 4 + q) * 32 + lane];
+        mma_16816_f16(acc[2 * q], a, w.x, w.y);
+        mma_16816_f16(acc[2 * q + 1], a, w.z, w.w);
+      }
+    }
+    // acc[nt]: (row g, col 8 nt + 2t), (g, + 1), (row g + 8, col 8 nt + 2t), (g + 8, + 1); rows = sequences, written transposed
+    bf16* obase = out + (bi * 64) * (long)Spad;
+#pragma unroll
+    for (int q = 0; q < 2; ++q) {
+      if (!inr[q]) continue;
+      const int sq = sb * 16 + g + 8 * q;
+#pragma unroll
+      for (int nt = 0; nt < 8; ++nt) {
+        const int col = 8 * nt + 2 * t;
+        obase[(long)col * Spad + sq] = __float2bfloat16_rn(on[q] ? acc[nt][2 * q] + cst[col] : 0.f);
+        obase[(long)(col + 1) * Spad + sq] = __float2bfloat16_rn(on[q] ? acc[nt][2 * q + 1] + cst[col + 1] : 0.f);
+      }
+    }
+  }
+}
+
+void launch_ln_opm_ab256(const float* msa, const float* gamma, const float* beta, const float* Wa, const float* Wb, const float* ba,
+                         const float* bb, const float* seq_mask, const float* msa_mask, bf16* out, int B, int S, int N, int Spad,
+                         int num_sms, cudaStream_t st) {
+  const long units = (long)B * N * ((S + 15) / 16), blocks = (units + OA_WARPS - 1) / OA_WARPS;
+  ln_opm_ab256_kernel<<<(unsigned)(blocks < num_sms ? blocks : num_sms), 32 * OA_WARPS, 0, st>>>(msa, gamma, beta, Wa, Wb, ba, bb, seq_mask,
+                                                                                                msa_mask, out, B, S, N, Spad);
 }
 
 }  // namespace pf

@@ -61,7 +61,7 @@ tri_einsum_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
     }
   } else if (warp == 1) {
     if (tc::elect_one()) {
-      constexpr uint32_t idesc = tc::idesc_bf16_f32(TRI_BM, TRI_BN);
+      constexpr uint32_t idesc = tc::idesc_f16_f32(TRI_BM, TRI_BN);   // operands and result fp16 (R17, round 2)
       for (int kb = 0; kb < num_kb; ++kb) {
         int s = kb % TRI_STAGES;
         tc::mbar_wait(&full[s], (kb / TRI_STAGES) & 1);
@@ -95,7 +95,7 @@ tri_einsum_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_const
             uint32_t pk[4];
 #pragma unroll
             for (int e = 0; e < 4; ++e) {
-              __nv_bfloat162 h = __floats2bfloat162_rn(__uint_as_float(v[j + 2 * e]), __uint_as_float(v[j + 2 * e + 1]));
+              __half2 h = __floats2half2_rn(__uint_as_float(v[j + 2 * e]), __uint_as_float(v[j + 2 * e + 1]));
               pk[e] = *reinterpret_cast<uint32_t*>(&h);
             }
             *reinterpret_cast<uint4*>(dst + c0 + j) = make_uint4(pk[0], pk[1], pk[2], pk[3]);

@@ -313,6 +313,15 @@ struct TcDriver {
     const int Sp = pad8(S);
     bf16* ABT = buf<bf16>(ar.vt);
     // rows (b, i, s) gathered from msa[(b, s, i)]: a | b masked and written transposed, [(b,i), 64, Spad], s contiguous
+    static const int opm_env = getenv("PF_OPM_AB") ? atoi(getenv("PF_OPM_AB")) : 1;
+    if (c.c_m == 256 && c.c_opm == 32 && opm_env) {
+      // 128 bytes out per KB in: a streaming kernel with the LayerNorm in registers and mma.sync for the 64 columns (pf_simt.cu)
+      h->prof_begin(KK_OPMAB, 2.0 * M * c.c_m * 2.0 * c.c_opm * h->frac.msat_x,
+                    M * (c.c_m * 4.0 + 2.0 * c.c_opm * 2.0) * h->frac.msat_x, st);
+      launch_ln_opm_ab256(msa, w + o.ln_g, w + o.ln_b, w + o.wa, w + o.wb, w + o.ba, w + o.bb, seq_mask, msa_mask, ABT, B, S, N, Sp,
+                          h->num_sms, st);
+      h->prof_end(st);
+    } else {
     G2Desc d = desc_base(B, N, S, c.c_m, 2 * c.c_opm);
     d.src = msa; d.src_transposed = 1; d.gamma = w + o.ln_g; d.beta = w + o.ln_b;
     d.op_fmt = 1; d.Wt = w16 + h->tc.opm_wab; d.bias = wf + h->tc.opm_bias_ab;
@@ -323,6 +332,7 @@ struct TcDriver {
     d.n_ops = 1;
     d.tile_active = flags(ar.f_msat_x);   // a, b are summed over s: masked s must be written as zeros
     if (!gemm2(d, M * 2.0 * c.c_opm * 2.0, h->frac.msat_x)) return false;
+    }
     h->prof_begin(KK_OPM, (2.0 * P * cc * S + 2.0 * P * cc * c.c_z) * h->frac.opm,
                   (2.0 * M * c.c_opm * 2.0 + 8.0 * P * c.c_z) * h->frac.opm, st);
     if (launch_opm_tc(h->tma, ABT, reinterpret_cast<const bf16*>(w16 + h->tc.opm_wout), w + o.bout, seq_mask, msa_mask,
