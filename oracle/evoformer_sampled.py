@@ -12,8 +12,8 @@ of ``evoformer_ref``.
 
 Optional switch ``rnd`` (reading R16, "quantisation-aware oracle"): a ``Rounding`` object rounds
 intermediate values at the points where the bf16 CUDA path stores them in 16 bits (R17:
-LayerNorm outputs, gates and pair bias fp16; q, k, v, P, o, transition hidden, outer-product and
-triangle operands bf16).  The arithmetic between those points stays fp64.  With ``rnd=None`` (the
+LayerNorm outputs, gates, pair bias, outer-product and triangle operands and results fp16; q, k, v, P, o,
+transition hidden bf16).  The arithmetic between those points stays fp64.  With ``rnd=None`` (the
 default) no rounding happens and the functions ARE the plain oracle; the switch exists so that a
 difference GPU - oracle can be split into the part the storage formats cause by themselves
 (quantised - plain) and the rest (GPU - quantised).  The quantised mode is a model of the storage
@@ -145,9 +145,9 @@ def outer_product_mean_at(m, z, seq_mask, msa_mask, w, i, j, rnd=None):
     rho, sg = _f64(msa_mask), _f64(seq_mask)
     xi = _ln(m[:, i], w["ln_g"], w["ln_b"], r)                        # [S, c_m]
     xj = _ln(m[:, j], w["ln_g"], w["ln_b"], r)
-    a = r.bf16((rho * sg[i])[:, None] * _lin(xi, w["wa"], w["ba"], r))   # a[s, c1] = mu_si Lin_a(x[s,i])
-    b = r.bf16((rho * sg[j])[:, None] * _lin(xj, w["wb"], w["bb"], r))   # b[s, c2] = mu_sj Lin_b(x[s,j])
-    O = r.bf16(a.T @ b)                                               # O[c1, c2] = sum_s a[s,c1] b[s,c2]
+    a = r.f16((rho * sg[i])[:, None] * _lin(xi, w["wa"], w["ba"], r))   # a[s, c1] = mu_si Lin_a(x[s,i])
+    b = r.f16((rho * sg[j])[:, None] * _lin(xj, w["wb"], w["bb"], r))   # b[s, c2] = mu_sj Lin_b(x[s,j])
+    O = r.f16(a.T @ b)                                                # O[c1, c2] = sum_s a[s,c1] b[s,c2]
     n = float(np.sum((rho * sg[i]) * (rho * sg[j])))
     if r.on:
         # the CUDA path contracts the 16-bit outer product with W_out first and divides afterwards (the same by linearity)

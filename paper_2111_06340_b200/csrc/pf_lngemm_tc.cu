@@ -592,11 +592,14 @@ gemm2_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CU
                 tc::tmem_ld32(tacc + j * 64 + hf * 32, v);
                 lds32(sbias + hf * 32, bb);
                 tc::tmem_ld_wait();
-                bf16 r[32];
+                uint16_t r[32];   // op.fmt: 0 bf16, 1 fp16 (the outer-product operands, R17 round 2)
 #pragma unroll
-                for (int e = 0; e < 32; ++e) r[e] = __float2bfloat16_rn((__uint_as_float(v[e]) + bb[e]) * mk);
+                for (int e = 0; e < 32; ++e) {
+                  const float val = (__uint_as_float(v[e]) + bb[e]) * mk;
+                  r[e] = op.fmt ? __half_as_ushort(__float2half_rn(val)) : __bfloat16_as_ushort(__float2bfloat16_rn(val));
+                }
 #pragma unroll
-                for (int e = 0; e < 32; ++e) dst[(hf * 32 + e) << p.ytw_shift] = r[e];
+                for (int e = 0; e < 32; ++e) reinterpret_cast<uint16_t*>(dst)[(hf * 32 + e) << p.ytw_shift] = r[e];
               }
             }
             tc::fence_proxy_async_smem();

@@ -130,8 +130,9 @@ opm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ C
     }
   } else if (warp == 1) {
     if (tc::elect_one()) {
-      constexpr uint32_t idesc1 = tc::idesc_bf16_f32(OP_BI, OP_BJ * OP_C);
-      constexpr uint32_t idesc2 = tc::idesc_bf16_f32(OP_BI, OP_CZ);
+      // a, b, the outer product and W_out are fp16 (R17 round 2: 8x finer rounding than bf16 at the same rate)
+      constexpr uint32_t idesc1 = tc::idesc_f16_f32(OP_BI, OP_BJ * OP_C);
+      constexpr uint32_t idesc2 = tc::idesc_f16_f32(OP_BI, OP_CZ);
       tc::mbar_wait(b_full, 0);
       int s = 0;
       uint32_t ph = 0;
@@ -195,8 +196,7 @@ opm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ C
           uint32_t pk[4];
 #pragma unroll
           for (int e = 0; e < 4; ++e) {
-            __nv_bfloat162 pp = __floats2bfloat162_rn(__uint_as_float(v[j][c * 8 + 2 * e]),
-                                                      __uint_as_float(v[j][c * 8 + 2 * e + 1]));
+            __half2 pp = __floats2half2_rn(__uint_as_float(v[j][c * 8 + 2 * e]), __uint_as_float(v[j][c * 8 + 2 * e + 1]));
             pk[e] = *reinterpret_cast<uint32_t*>(&pp);
           }
           *reinterpret_cast<uint4*>(tile + tc::swz_offset<64>(row, c)) = make_uint4(pk[0], pk[1], pk[2], pk[3]);

@@ -758,7 +758,7 @@ ln_opm_ab256_kernel(const float* __restrict__ msa, const float* __restrict__ gam
       }
     }
     // acc[nt]: (row g, col 8 nt + 2t), (g, + 1), (row g + 8, col 8 nt + 2t), (g + 8, + 1); rows = sequences, written transposed
-    bf16* obase = out + (bi * 64) * (long)Spad;
+    __half* ohalf = reinterpret_cast<__half*>(out) + (bi * 64) * (long)Spad;   // fp16 operands (R17 round 2)
 #pragma unroll
     for (int q = 0; q < 2; ++q) {
       if (!inr[q]) continue;
@@ -766,8 +766,8 @@ ln_opm_ab256_kernel(const float* __restrict__ msa, const float* __restrict__ gam
 #pragma unroll
       for (int nt = 0; nt < 8; ++nt) {
         const int col = 8 * nt + 2 * t;
-        obase[(long)col * Spad + sq] = __float2bfloat16_rn(on[q] ? acc[nt][2 * q] + cst[col] : 0.f);
-        obase[(long)(col + 1) * Spad + sq] = __float2bfloat16_rn(on[q] ? acc[nt][2 * q + 1] + cst[col + 1] : 0.f);
+        ohalf[(long)col * Spad + sq] = __float2half_rn(on[q] ? acc[nt][2 * q] + cst[col] : 0.f);
+        ohalf[(long)(col + 1) * Spad + sq] = __float2half_rn(on[q] ? acc[nt][2 * q + 1] + cst[col + 1] : 0.f);
       }
     }
   }

@@ -109,7 +109,7 @@ void build_tc_block(const pf_config& c, const BlockW& off, const TcBlock& t, con
     wf[basef + t.opm_bias_ab + i] = w[off.opm.ba + i];
     wf[basef + t.opm_bias_ab + c.c_opm + i] = w[off.opm.bb + i];
   }
-  put_transposed(w16, base16 + t.opm_wout, w + off.opm.wout, c.c_opm * c.c_opm, c.c_z, false);
+  put_transposed(w16, base16 + t.opm_wout, w + off.opm.wout, c.c_opm * c.c_opm, c.c_z, true);   // fp16 as the outer product it multiplies
   // triangle multiplication: the einsum kernel contracts buffer 0 (rows i) with buffer 1 (rows j) along k.
   // outgoing (A.5): buffer 0 = a, buffer 1 = b.  incoming (A.6) runs on the transposed rows with a and b swapped
   // (SURVEY.md §0 finding 1): buffer 0 = b, buffer 1 = a.
@@ -328,6 +328,7 @@ struct TcDriver {
     d.rowmask = RM_MSA; d.seq_mask = seq_mask; d.msa_mask = msa_mask; d.mask_transposed = 1;
     d.vt_out = ABT; d.vt_cols = 2 * c.c_opm; d.Lpad = Sp;
     d.ops[0] = op(G2_VT, 0, 2 * c.c_opm);
+    d.ops[0].fmt = 1;   // fp16 operands of the outer product
     d.ops[0].masked = 1;
     d.n_ops = 1;
     d.tile_active = flags(ar.f_msat_x);   // a, b are summed over s: masked s must be written as zeros
@@ -593,6 +594,7 @@ bool tc_run_extra_substep(pf_evoformer* h, const ExtraOff& xo, const ExtraT& xt,
     g.rowmask = RM_MSA; g.seq_mask = seq_mask; g.msa_mask = msa_mask; g.mask_transposed = 1;
     g.vt_out = ABT; g.vt_cols = 2 * c.c_opm; g.Lpad = Sp;
     g.ops[0] = TcDriver::op(G2_VT, 0, 2 * c.c_opm);
+    g.ops[0].fmt = 1;   // fp16 operands of the outer product
     g.ops[0].masked = 1;
     g.n_ops = 1;
     g.tile_active = d.flags(d.ar.f_msat_x);
