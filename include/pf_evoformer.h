@@ -80,8 +80,10 @@ pf_status pf_evoformer_create(pf_evoformer_t** out, const float* weights_host, s
  * N <= 1024 and S <= 1024 (keys per attention row) and S <= 512 (outer-product-mean contraction length).  B is not
  * limited: batches beyond what one launch sequence takes (grid limits) are cut into chunks of proteins internally.
  * The current CUDA device must be the one the handle was created on (PF_ERR_INVALID_ARG otherwise).
- * Value range on the PF_BF16 path (reading R17): LayerNorm outputs, sigmoid gates and the weight matrices that
- * multiply a LayerNorm output are held as fp16.  Precondition: those weights (after bf16 rounding, R15) lie in the fp16
+ * Value range on the PF_BF16 path (reading R17): LayerNorm outputs, sigmoid gates, the weight matrices that
+ * multiply a LayerNorm output, the pair bias, the gated triangle operands and their einsum (sums over N_res of products of
+ * order one), the outer-product operands, the outer product (sums over N_seq) and W_out are held as fp16; q, k, v, the
+ * attention probabilities, o and the transition hidden activation as bf16.  Precondition: those weights (after bf16 rounding, R15) lie in the fp16
  * normal range, 2^-14 <= |w| <= 65504 or w == 0 (smaller magnitudes lose bits or flush to zero), and LayerNorm outputs
  * gamma * xhat + beta stay below 65504 in magnitude (|xhat| <= sqrt(C)).  create() counts weights outside that range and
  * refuses blobs with overflowing ones (PF_ERR_SHAPE); the seeded R8 init has about 0.08 % of entries below 2^-14 (a
