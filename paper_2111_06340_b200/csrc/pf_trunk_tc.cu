@@ -313,8 +313,7 @@ struct TcDriver {
     const int Sp = pad8(S);
     bf16* ABT = buf<bf16>(ar.vt);
     // rows (b, i, s) gathered from msa[(b, s, i)]: a | b masked and written transposed, [(b,i), 64, Spad], s contiguous
-    static const int opm_env = getenv("PF_OPM_AB") ? atoi(getenv("PF_OPM_AB")) : 1;
-    if (c.c_m == 256 && c.c_opm == 32 && opm_env) {
+    if (c.c_m == 256 && c.c_opm == 32) {
       // 128 bytes out per KB in: a streaming kernel with the LayerNorm in registers and mma.sync for the 64 columns (pf_simt.cu)
       h->prof_begin(KK_OPMAB, 2.0 * M * c.c_m * 2.0 * c.c_opm * h->frac.msat_x,
                     M * (c.c_m * 4.0 + 2.0 * c.c_opm * 2.0) * h->frac.msat_x, st);
