@@ -12,8 +12,11 @@
 //                  warps never unpack it; TMEM double buffered) is issued BEFORE waiting for P(i), so the
 //                  tensor core works on the next logits while the softmax warps are busy; O_tile = P V (M=128 N=32 K=4x16)
 //   warps 0-3      thread-per-row online softmax in fp32 from tcgen05.ld (ex2.approx), P (bf16) -> smem in the UMMA
-//                  128B-swizzle layout; o_acc = o_acc * alpha + O_tile in registers; gate (prefetched at unit start) and 1/l
-//                  applied at the end, 64-byte row stores.
+//                  128B-swizzle layout.  O accumulates in TMEM over the key tiles of a unit (P V with accumulate); P is taken
+//                  relative to a reference maximum that moves only when the running maximum has grown by more than 2^8, and
+//                  only then is O rescaled (tcgen05.ld, multiply, tcgen05.st) — the time of this kernel follows the
+//                  instruction count of these warps, and the per-tile "(O + PV) alpha" round trip through registers was 15 %
+//                  of it; gate (prefetched at unit start) and 1/l applied at the end, 64-byte row stores.
 // ~106 KB of shared memory and 256 TMEM columns per CTA -> 2 CTAs per SM overlap each other's softmax and barrier latency.
 #include "pf_internal.h"
 #include "pf_device.cuh"
@@ -172,6 +175,8 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQK, const __grid_constant__
       int cn = min(ent.y, p.n_kt);
       uint32_t cuc = 0, j = 0, i = 0;
       uint32_t js = 0, jph = 0, is = 0;              // ring position / phase of the issue side (j) and position of the consume side (i)
+      // consume side: which key tile of its unit step i is (O accumulates in TMEM over the key tiles of a unit)
+      int pu = blockIdx.x, pkt = 0, pn = cn;
       auto issue_s = [&]() -> bool {
         if (cu >= units) return false;
         const uint32_t qb = cuc & 1, s = js;
@@ -215,9 +220,14 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQK, const __grid_constant__
           tc::tc_fence_after();
           const uint64_t v_desc = tc::smem_desc_kmajor<128>(tc::smem_u32(smem + SM::STAGE_OFF + s * p.stage_bytes + SM::K_BYTES));
 #pragma unroll
-          for (int k = 0; k < AT_BK / 16; ++k) tc::mma_bf16(tmem_O, p_desc + 2 * k, v_desc + 2 * k, idesc_o, k != 0);
+          for (int k = 0; k < AT_BK / 16; ++k) tc::mma_bf16(tmem_O, p_desc + 2 * k, v_desc + 2 * k, idesc_o, (k | pkt) != 0);
           tc::mma_commit(o_full);
           tc::mma_commit(&kv_empty[s]);
+          if (++pkt == pn) {
+            pu += (int)gridDim.x;
+            pn = min(attn_row_entry(pu, units, p).y, p.n_kt);
+            pkt = 0;
+          }
           if (++i == j) break;
         }
       }
@@ -265,10 +275,12 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQK, const __grid_constant__
 #pragma unroll
         for (int d = 0; d < 4; ++d) gq[d] = make_uint4(0u, 0u, 0u, 0u);
       }
-      float m_run = -INFINITY, l_run = 0.f;
-      float oacc[32];
-#pragma unroll
-      for (int d = 0; d < 32; ++d) oacc[d] = 0.f;
+      // Online softmax with the output accumulated by the tensor core: O stays in TMEM over the key tiles of the unit
+      // (P V with accumulate) and P is taken relative to a reference maximum m_ref that is only moved when the running
+      // maximum has grown by more than 2^8 beyond it (P <= 256 then, exact in the exp2 domain: the common factor cancels in
+      // O / l).  Moving it rescales O in TMEM (load, multiply, store) and l; after the first tiles of a row that is rare, so
+      // the per-tile "O = (O + PV) alpha" round trip through registers is gone.
+      float m_run = -INFINITY, m_ref = -INFINITY, l_run = 0.f;
       for (int kt = 0; kt < n_kt; ++kt, ++i) {
         tc::mbar_wait(&s_full[i & 1], (i >> 1) & 1);
         tc::tc_fence_after();
@@ -295,19 +307,29 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQK, const __grid_constant__
           mx2 = fmaxf(mx2, x[j + 2]);
           mx3 = fmaxf(mx3, x[j + 3]);
         }
-        const float m_new = fmaxf(m_run, fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)));
-        const float m_use = (m_new == -INFINITY) ? 0.f : m_new;
-        const float alpha = ex2_approx(m_run - m_use);
-        // PV(i-1) must have finished reading P before it is overwritten; its O tile joins the running output
-        if (kt > 0) {
+        m_run = fmaxf(m_run, fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)));
+        if (kt == 0) {
+          m_ref = m_run;
+        } else {
+          // PV(i-1) must have finished reading P before it is overwritten, and before O is touched
           tc::mbar_wait(o_full, (i - 1) & 1);
           tc::tc_fence_after();
-          uint32_t ov[32];
-          tc::tmem_ld32(tmem_O + lane_addr, ov);
-          tc::tmem_ld_wait();
+          const bool move = m_run > m_ref + 8.0f;          // also true when m_ref is still -inf and a key has appeared
+          if (__any_sync(0xffffffffu, move)) {
+            // rows that do not move multiply by 1; a row whose reference was -inf has O = l = 0: factor 0 keeps that exact
+            const float alpha = !move ? 1.0f : (m_ref == -INFINITY ? 0.0f : ex2_approx(m_ref - m_run));
+            uint32_t ov[32];
+            tc::tmem_ld32(tmem_O + lane_addr, ov);
+            tc::tmem_ld_wait();
 #pragma unroll
-          for (int d = 0; d < 32; ++d) oacc[d] = (oacc[d] + __uint_as_float(ov[d])) * alpha;
+            for (int d = 0; d < 32; ++d) ov[d] = __float_as_uint(__uint_as_float(ov[d]) * alpha);
+            tc::tmem_st32(tmem_O + lane_addr, ov);
+            tc::tmem_st_wait();
+            l_run *= alpha;
+            if (move) m_ref = m_run;
+          }
         }
+        const float m_use = (m_ref == -INFINITY) ? 0.f : m_ref;
         float sum0 = 0.f, sum1 = 0.f;
 #pragma unroll
         for (int c = 0; c < 8; ++c) {
@@ -322,21 +344,21 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQK, const __grid_constant__
           }
           *reinterpret_cast<uint4*>(prow + tc::swz_offset<128>(row, c)) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
         }
-        l_run = l_run * alpha + (sum0 + sum1);
-        m_run = m_new;
+        l_run += sum0 + sum1;
         tc::fence_proxy_async_smem();
         tc::tc_fence_before();
         tc::mbar_arrive(p_full);
       }
-      // last key tile's PV, then normalise, gate and store this row's 32 output channels
+      // the unit's O (all key tiles, relative to m_ref), then normalise, gate and store this row's 32 output channels
       tc::mbar_wait(o_full, (i - 1) & 1);
       tc::tc_fence_after();
+      float oacc[32];
       {
         uint32_t ov[32];
         tc::tmem_ld32(tmem_O + lane_addr, ov);
         tc::tmem_ld_wait();
 #pragma unroll
-        for (int d = 0; d < 32; ++d) oacc[d] += __uint_as_float(ov[d]);
+        for (int d = 0; d < 32; ++d) oacc[d] = __uint_as_float(ov[d]);
       }
       tc::tc_fence_before();
       if (qi < p.L) {
