@@ -241,11 +241,19 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQK, const __grid_constant__
     uint32_t tile_masked = 0;                    // bit kt: key tile kt holds a masked / out-of-range key
     uint32_t i = 0;                              // pipeline step (all units)
     const int units = *p.n_rows * p.H * p.QT;
-    int2 ent = attn_row_entry((int)blockIdx.x, units, p);
-    for (int u = blockIdx.x; u < units; u += (int)gridDim.x) {
-      const int2 ent_next = attn_row_entry(u + (int)gridDim.x, units, p);
+    // unit u = (row entry ridx, head h, query tile qt): advanced incrementally (the integer divisions of the direct form are
+    // long dependent chains through the unit that is busy with the exponentials: ~0.4 us per unit on this critical path)
+    const int G = (int)gridDim.x;
+    const int g_qt = G % p.QT, g_h = (G / p.QT) % p.H, g_r = G / (p.QT * p.H);
+    int qt = (int)blockIdx.x % p.QT, h = ((int)blockIdx.x / p.QT) % p.H, ridx = (int)blockIdx.x / (p.QT * p.H);
+    int2 ent = (int)blockIdx.x < units ? __ldg(p.rows + ridx) : make_int2(0, 0);
+    for (int u = blockIdx.x; u < units; u += G) {
+      // next unit's coordinates and row entry (a plain load, used one unit later)
+      int nqt = qt + g_qt, nh = h + g_h, nr = ridx + g_r;
+      if (nqt >= p.QT) { nqt -= p.QT; ++nh; }
+      if (nh >= p.H) { nh -= p.H; ++nr; }
+      const int2 ent_next = u + G < units ? __ldg(p.rows + nr) : make_int2(0, 0);
       const int br = ent.x, n_kt = min(ent.y, p.n_kt);
-      const int qt = u % p.QT, h = (u / p.QT) % p.H;
       const int b = br / p.R;
       const int qi = qt * AT_BQ + row;
       if (b != cur_b) {
@@ -379,6 +387,7 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQK, const __grid_constant__
         }
       }
       ent = ent_next;
+      qt = nqt; h = nh; ridx = nr;
     }
   }
   tc::tc_fence_before();
