@@ -366,8 +366,9 @@ def recycled_workload(h, pf, ps, torch, dev, name="cfg3", n_cycles=4, steps=2, S
     al = torch.empty((B, N, 7, 2), device=dev)
     dg = torch.empty((B, N, N, 64), device=dev)
     mlm = torch.empty((B, S, N, 23), device=dev)
+    pae = torch.empty((B, N, N, 64), device=dev)
     pf.fold_forward(h, emb, stm, tfd, rid, mfd, None, m, z, smd, mmd, nb, n_cycles, xc, alpha_out=al, plddt_out=pl, **kw)   # warm-up
-    stm.heads(m, z, dg, mlm)
+    stm.heads(m, z, dg, mlm, pae)
     torch.cuda.synchronize()
     f0, f1, f2, f3 = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
     f0.record(stream)
@@ -377,7 +378,7 @@ def recycled_workload(h, pf, ps, torch, dev, name="cfg3", n_cycles=4, steps=2, S
     stm.forward(m, z, smd, x_out=xc[0], alpha_out=al, plddt_out=pl)
     f2.record(stream)
     sm_launches = stm.last_launch_count()
-    stm.heads(m, z, dg, mlm)
+    stm.heads(m, z, dg, mlm, pae)
     f3.record(stream)
     torch.cuda.synchronize()
     out["fold"] = {"desc": "pf_fold_forward: the cycles above, each closed by the structure module (8 layers, fp32) whose "

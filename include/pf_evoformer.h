@@ -244,7 +244,7 @@ void pf_extra_msa_destroy(pf_extra_msa_t* x);
 /* ------------------------------------------------------------------------------------------------
  * Structure module and output heads: the last stage of the network the paper's GPU stage runs ("a new
  * Evoformer architecture" feeding "the structure module"; AlphaFold v2.0.1 monomer).
- * PAPER.md prints no formula; readings M.0-M.6 / H.1-H.3, per protein:
+ * PAPER.md prints no formula; readings M.0-M.6 / H.1-H.5, per protein:
  *   M.0 s^single_i = Lin_single(m_0i)                         M.1 s^init = LN_s(s^single), zn = LN_z(z), s = Lin_in(s^init), T_i = (I, 0)
  *   M.2 invariant point attention, H heads: q, k, v = Lin0(s) [c per head]; query / key points qp, kp [P_q x 3], value points vp
  *       [P_v x 3] = Lin0(s) in the residue's frame, mapped to the global frame by T; b = Lin0(zn) [H];
@@ -257,13 +257,14 @@ void pf_extra_msa_destroy(pf_extra_msa_t* x);
  *       (they need per-residue ideal-geometry tables that are not on this box): x is what the recycling embedder (E.2) receives.
  *   H.1 distogram logits_ij = Lin_dg(z_ij) + Lin_dg(z_ji)    H.2 masked-MSA logits_si = Lin_mm(m_si)
  *   H.3 pLDDT_i = 100 sum_k softmax(Lin_l3(relu(Lin_l2(relu(Lin_l1(LN_l(s_i)))))))_k (k + 1/2) / n_lddt_bins
+ *   H.4 predicted-aligned-error logits_ij = Lin_pae(z_ij) (not symmetrised)   H.5 experimentally-resolved logits_i = Lin_er(s_i)
  * All arithmetic is fp32 (tolerance 1e-4 max-abs against the fp64 oracle on s, frames in nanometres, angles; 1e-3 on x in
  * Angstrom and pLDDT in points).  Masked residues act as masked keys only; outputs at masked residues are unspecified but finite.
  * Weights blob (fp32, every matrix row-major [in, out]), in this order: W_single b | LN_s g b | LN_z g b | W_in b | W_q | W_k |
  * W_v [c_s, H c] | W_qp | W_kp [c_s, H P_q 3] | W_vp [c_s, H P_v 3] | W_b [c_z, H] | g_head [H] | W_out [H (c_z + c + 4 P_v), c_s] b |
  * LN_ipa g b | W_1 b W_2 b W_3 b | LN_tr g b | W_bb [c_s, 6] b | W_a1 b W_a2 b [c_s, c_r] | 2 x (W_ra b W_rb b [c_r, c_r]) |
  * W_alpha [c_r, 2 n_torsion] b | W_dg [c_z, n_dist_bins] b | W_mm [c_m, n_msa_classes] b | LN_l g b | W_l1 [c_s, c_l] b |
- * W_l2 [c_l, c_l] b | W_l3 [c_l, n_lddt_bins] b.
+ * W_l2 [c_l, c_l] b | W_l3 [c_l, n_lddt_bins] b | W_pae [c_z, n_pae_bins] b | W_er [c_s, n_resolved] b.
  * ---------------------------------------------------------------------------------------------- */
 typedef struct pf_structure pf_structure_t;   /* opaque; owns device weights and a grow-only workspace */
 typedef struct {
@@ -281,6 +282,8 @@ typedef struct {
   int n_msa_classes;  /* masked-MSA classes (23) */
   int n_lddt_bins;    /* pLDDT bins (50) */
   int c_lddt;         /* pLDDT head width (128) */
+  int n_pae_bins;     /* predicted-aligned-error bins (64) */
+  int n_resolved;     /* experimentally-resolved classes (37) */
   float pos_scale;    /* Angstrom per unit of frame translation (10) */
 } pf_struct_config;
 /* fp32 values in the blob described above; 0 for a null / unsupported config. */
@@ -290,15 +293,17 @@ pf_status pf_structure_create(pf_structure_t** out, const float* weights_host, s
                               const pf_struct_config* cfg);
 /* M.0-M.6 (+ H.3) for a batch, asynchronously on cuda_stream.  Inputs (device, read only): msa[B,S,N,c_m] (only row s = 0 is
  * read), pair[B,N,N,c_z], seq_mask[B,N].  Outputs (device, each may be NULL): s_out[B,N,c_s], frames_out[B,N,12] (R row-major
- * 3 x 3, then t, nanometres), x_out[B,N,3] (Angstrom), alpha_out[B,N,n_torsion,2], plddt_out[B,N].  n_layers >= 1 (the
+ * 3 x 3, then t, nanometres), x_out[B,N,3] (Angstrom), alpha_out[B,N,n_torsion,2], plddt_out[B,N], resolved_out[B,N,n_resolved]
+ * (H.5 logits).  n_layers >= 1 (the
  * config's value is the AlphaFold default).  Limit: heads x N x 4 bytes <= ~200 KB (N <= 4000 at 12 heads).
  * Errors: INVALID_ARG, SHAPE, ALLOC (workspace: ~N^2 (c_z + heads) floats per protein), CUDA. */
 pf_status pf_structure_forward(pf_structure_t* h, const float* msa_dev, const float* pair_dev, const float* seq_mask_dev, int B,
                                int S, int N, int n_layers, float* s_out, float* frames_out, float* x_out, float* alpha_out,
-                               float* plddt_out, void* cuda_stream);
-/* H.1 / H.2: distogram_out[B,N,N,n_dist_bins] and / or masked_msa_out[B,S,N,n_msa_classes] (device; NULL skips a head). */
+                               float* plddt_out, float* resolved_out, void* cuda_stream);
+/* H.1 / H.2 / H.4: distogram_out[B,N,N,n_dist_bins], masked_msa_out[B,S,N,n_msa_classes], pae_out[B,N,N,n_pae_bins] (device;
+ * NULL skips a head). */
 pf_status pf_heads_forward(pf_structure_t* h, const float* msa_dev, const float* pair_dev, int B, int S, int N,
-                           float* distogram_out, float* masked_msa_out, void* cuda_stream);
+                           float* distogram_out, float* masked_msa_out, float* pae_out, void* cuda_stream);
 long long pf_structure_last_launch_count(const pf_structure_t* h);
 void pf_structure_destroy(pf_structure_t* h);
 /* The whole GPU stage: n_cycles x (pf_embedder_forward with the PREVIOUS cycle's structure-module

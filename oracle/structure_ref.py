@@ -3,7 +3,7 @@ only tests/, __graft_entry__.smoke() and bench.py's reference legs may import it
 
 What it computes: SURVEY.md §8(f)4 — "structure module + heads", the last stage of the network the paper's GPU stage runs
 ("a new Evoformer architecture" feeding "the structure module"; AlphaFold v2.0.1 monomer,
-PAPER.md:127).  PAPER.md prints no formula; what follows is the reading M.0-M.6 / H.1-H.3 of DESIGN.md §2d (the published
+PAPER.md:127).  PAPER.md prints no formula; what follows is the reading M.0-M.6 / H.1-H.5 of DESIGN.md §2d (the published
 AlphaFold 2 algorithm restated in this repository's notation).  One protein, no batch axis:
 
   M.0 single representation   s^single_i = Lin_single(m_0i)                                  (first MSA row, c_m -> c_s)
@@ -27,6 +27,8 @@ AlphaFold 2 algorithm restated in this repository's notation).  One protein, no 
   H.2 masked-MSA              logits_si = Lin_mm(m_si)                                         [S,N,n_msa_classes]
   H.3 pLDDT                   l_i = Lin_l3(relu(Lin_l2(relu(Lin_l1(LN_l(s_i))))))  [n_lddt_bins];  p = softmax(l);
                               plddt_i = 100 sum_k p_k (k + 1/2) / n_lddt_bins
+  H.4 predicted aligned error logits_ij = Lin_pae(z_ij)   [N,N,n_pae_bins]   (NOT symmetrised: error of j in the frame of i)
+  H.5 experimentally resolved logits_i = Lin_er(s_i)      [N,n_resolved]
 
 Masked residues enter only as attention keys (NEG(sigma_j)); outputs at masked residues are unspecified (R3).
 All-atom side-chain coordinates are NOT computed: they need the ideal-geometry tables of the amino acids, which are data of
@@ -182,6 +184,16 @@ def plddt(s, w):
     nb = logits.shape[-1]
     centers = (np.arange(nb, dtype=F64) + 0.5) / nb
     return logits, 100.0 * (softmax(logits, axis=-1) * centers).sum(axis=-1)
+
+
+def pae_logits(z, w):
+    """H.4."""
+    return linear(z, w["w_pae"], w["b_pae"])
+
+
+def resolved_logits(s, w):
+    """H.5."""
+    return linear(s, w["w_er"], w["b_er"])
 
 
 def fold(target_feat, residue_index, msa_feat, seq_mask, msa_mask, w_embed, blocks, w_struct, n_cycles, x_prev0=None,

@@ -57,7 +57,8 @@ class PfExtraConfig(Structure):
 class PfStructConfig(Structure):
     _fields_ = [("c_m", c_int), ("c_z", c_int), ("c_s", c_int), ("heads", c_int), ("c_ipa", c_int), ("n_qp", c_int),
                 ("n_pv", c_int), ("n_layers", c_int), ("c_resnet", c_int), ("n_torsion", c_int), ("n_dist_bins", c_int),
-                ("n_msa_classes", c_int), ("n_lddt_bins", c_int), ("c_lddt", c_int), ("pos_scale", c_float)]
+                ("n_msa_classes", c_int), ("n_lddt_bins", c_int), ("c_lddt", c_int), ("n_pae_bins", c_int), ("n_resolved", c_int),
+                ("pos_scale", c_float)]
 
 
 class PfError(RuntimeError):
@@ -159,9 +160,9 @@ def lib() -> ctypes.CDLL:
         L.pf_structure_create.restype = c_int
         L.pf_structure_create.argtypes = [POINTER(c_void_p), c_void_p, c_size_t, POINTER(PfStructConfig)]
         L.pf_structure_forward.restype = c_int
-        L.pf_structure_forward.argtypes = [c_void_p] * 4 + [c_int] * 4 + [c_void_p] * 6
+        L.pf_structure_forward.argtypes = [c_void_p] * 4 + [c_int] * 4 + [c_void_p] * 7
         L.pf_heads_forward.restype = c_int
-        L.pf_heads_forward.argtypes = [c_void_p] * 3 + [c_int] * 3 + [c_void_p] * 3
+        L.pf_heads_forward.argtypes = [c_void_p] * 3 + [c_int] * 3 + [c_void_p] * 4
         L.pf_structure_last_launch_count.restype = c_longlong
         L.pf_structure_last_launch_count.argtypes = [c_void_p]
         L.pf_structure_destroy.restype = None
@@ -383,9 +384,10 @@ def forward_recycled(evo: "Evoformer", emb: Embedder, target_feat, residue_index
 
 
 def make_struct_config(c_m=256, c_z=128, c_s=384, heads=12, c_ipa=16, n_qp=4, n_pv=8, n_layers=8, c_resnet=128, n_torsion=7,
-                       n_dist_bins=64, n_msa_classes=23, n_lddt_bins=50, c_lddt=128, pos_scale=10.0) -> PfStructConfig:
+                       n_dist_bins=64, n_msa_classes=23, n_lddt_bins=50, c_lddt=128, n_pae_bins=64, n_resolved=37,
+                       pos_scale=10.0) -> PfStructConfig:
     return PfStructConfig(c_m, c_z, c_s, heads, c_ipa, n_qp, n_pv, n_layers, c_resnet, n_torsion, n_dist_bins, n_msa_classes,
-                          n_lddt_bins, c_lddt, pos_scale)
+                          n_lddt_bins, c_lddt, n_pae_bins, n_resolved, pos_scale)
 
 
 class StructureModule:
@@ -405,18 +407,18 @@ class StructureModule:
         return stream
 
     def forward(self, msa, pair, seq_mask, n_layers=None, s_out=None, frames_out=None, x_out=None, alpha_out=None,
-                plddt_out=None, stream=None):
+                plddt_out=None, resolved_out=None, stream=None):
         B, S, N = msa.shape[0], msa.shape[1], msa.shape[2]
         _check(lib().pf_structure_forward(self._s, _ptr(msa), _ptr(pair), _ptr(seq_mask), B, S, N,
                                           self.cfg.n_layers if n_layers is None else n_layers, _ptr(s_out), _ptr(frames_out),
-                                          _ptr(x_out), _ptr(alpha_out), _ptr(plddt_out), self._stream(stream)))
+                                          _ptr(x_out), _ptr(alpha_out), _ptr(plddt_out), _ptr(resolved_out), self._stream(stream)))
 
-    def heads(self, msa, pair, distogram_out=None, masked_msa_out=None, stream=None):
+    def heads(self, msa, pair, distogram_out=None, masked_msa_out=None, pae_out=None, stream=None):
         ref = msa if msa is not None else pair
         B, N = ref.shape[0], ref.shape[2]
         S = msa.shape[1] if msa is not None else 1
         _check(lib().pf_heads_forward(self._s, _ptr(msa), _ptr(pair), B, S, N, _ptr(distogram_out), _ptr(masked_msa_out),
-                                      self._stream(stream)))
+                                      _ptr(pae_out), self._stream(stream)))
 
     def last_launch_count(self) -> int:
         return int(lib().pf_structure_last_launch_count(self._s))

@@ -1,5 +1,5 @@
 // Structure module and output heads ("the structure module"; readings M.0-M.6 and
-// H.1-H.3 of DESIGN.md §2d, restated in include/pf_evoformer.h).  Small FLOPs and many small steps: per protein the eight
+// H.1-H.5 of DESIGN.md §2d, restated in include/pf_evoformer.h).  Small FLOPs and many small steps: per protein the eight
 // shared-weight layers cost ~14 MFLOP per residue plus 2 H N c_z FLOP per residue for the pair-value sum of the invariant
 // point attention, two to three orders of magnitude below the trunk, and every reduction length is 128 .. 2112 over a few
 // hundred to a few thousand rows.  So everything here is fp32 on the SIMT pipes (tolerance 1e-4 against the fp64 oracle):
@@ -34,7 +34,7 @@ static pf_status sfail(pf_status s, const std::string& msg) {
 struct SmOff {
   size_t w_single, b_single, ln_s_g, ln_s_b, ln_z_g, ln_z_b, w_in, b_in, w_q, w_k, w_v, w_qp, w_kp, w_vp, w_b, g_head, w_out,
       b_out, ln_ipa_g, ln_ipa_b, w_t[3], b_t[3], ln_tr_g, ln_tr_b, w_bb, b_bb, w_a1, b_a1, w_a2, b_a2, w_ra[2], b_ra[2],
-      w_rb[2], b_rb[2], w_alpha, b_alpha, w_dg, b_dg, w_mm, b_mm, ln_l_g, ln_l_b, w_l1, b_l1, w_l2, b_l2, w_l3, b_l3, total;
+      w_rb[2], b_rb[2], w_alpha, b_alpha, w_dg, b_dg, w_mm, b_mm, ln_l_g, ln_l_b, w_l1, b_l1, w_l2, b_l2, w_l3, b_l3, w_pae, b_pae, w_er, b_er, total;
 };
 
 struct pf_structure {
@@ -76,6 +76,8 @@ static SmOff sm_offsets(const pf_struct_config& c) {
   o.ln_l_g = take(cs); o.ln_l_b = take(cs);
   o.w_l1 = take(cs * cl); o.b_l1 = take(cl); o.w_l2 = take(cl * cl); o.b_l2 = take(cl);
   o.w_l3 = take(cl * c.n_lddt_bins); o.b_l3 = take(c.n_lddt_bins);
+  o.w_pae = take(cz * c.n_pae_bins); o.b_pae = take(c.n_pae_bins);
+  o.w_er = take(cs * c.n_resolved); o.b_er = take(c.n_resolved);
   o.total = at;
   return o;
 }
@@ -537,7 +539,8 @@ static bool sm_cfg_ok(const pf_struct_config& c) {
   return c.c_m >= 4 && c.c_m % 4 == 0 && c.c_m <= 1024 && c.c_z >= 4 && c.c_z % 4 == 0 && c.c_z <= 1024 && c.c_s >= 4 &&
          c.c_s % 4 == 0 && c.c_s <= 1024 && c.heads >= 1 && c.heads <= 32 && c.c_ipa >= 1 && c.c_ipa <= 64 && c.n_qp >= 1 &&
          c.n_qp <= 16 && c.n_pv >= 1 && c.n_pv <= 16 && c.n_layers >= 1 && c.c_resnet >= 1 && c.n_torsion >= 1 &&
-         c.n_dist_bins >= 1 && c.n_msa_classes >= 1 && c.n_lddt_bins >= 1 && c.c_lddt >= 1 && c.pos_scale > 0.f;
+         c.n_dist_bins >= 1 && c.n_msa_classes >= 1 && c.n_lddt_bins >= 1 && c.c_lddt >= 1 && c.n_pae_bins >= 1 &&
+         c.n_resolved >= 1 && c.pos_scale > 0.f;
 }
 
 extern "C" size_t pf_structure_floats(const pf_struct_config* cfg) {
@@ -648,7 +651,7 @@ bool sm_reserve(pf_structure* h, size_t need) {
 
 extern "C" pf_status pf_structure_forward(pf_structure_t* h, const float* msa, const float* pair, const float* seq_mask, int B,
                                           int S, int N, int n_layers, float* s_out, float* frames_out, float* x_out,
-                                          float* alpha_out, float* plddt_out, void* stream) {
+                                          float* alpha_out, float* plddt_out, float* resolved_out, void* stream) {
   if (!h || !msa || !pair || !seq_mask) return sfail(PF_ERR_INVALID_ARG, "null argument");
   if (B < 1 || S < 1 || N < 1 || n_layers < 1) return sfail(PF_ERR_SHAPE, "B, S, N, n_layers must be >= 1");
   if (B > 65535) return sfail(PF_ERR_SHAPE, "structure module: B <= 65535");
@@ -743,6 +746,8 @@ extern "C" pf_status pf_structure_forward(pf_structure_t* h, const float* msa, c
     sm_plddt_kernel<<<(unsigned)((R + 7) / 8), 256, 0, st>>>(lg, plddt_out, R, c.n_lddt_bins);
     ++run.launches;
   }
+  if (resolved_out)   // H.5
+    run.gemm(s, cs, w + o.w_er, w + o.b_er, resolved_out, c.n_resolved, R, cs, c.n_resolved);
   if (s_out) cudaMemcpyAsync(s_out, s, (size_t)R * cs * 4, cudaMemcpyDeviceToDevice, st);
   if (frames_out) cudaMemcpyAsync(frames_out, frames, (size_t)R * 12 * 4, cudaMemcpyDeviceToDevice, st);
   h->launches = run.launches;
@@ -752,9 +757,9 @@ extern "C" pf_status pf_structure_forward(pf_structure_t* h, const float* msa, c
 }
 
 extern "C" pf_status pf_heads_forward(pf_structure_t* h, const float* msa, const float* pair, int B, int S, int N,
-                                      float* distogram_out, float* masked_msa_out, void* stream) {
+                                      float* distogram_out, float* masked_msa_out, float* pae_out, void* stream) {
   if (!h) return sfail(PF_ERR_INVALID_ARG, "null handle");
-  if ((distogram_out && !pair) || (masked_msa_out && !msa)) return sfail(PF_ERR_INVALID_ARG, "a head was requested without its input");
+  if (((distogram_out || pae_out) && !pair) || (masked_msa_out && !msa)) return sfail(PF_ERR_INVALID_ARG, "a head was requested without its input");
   if (B < 1 || S < 1 || N < 1) return sfail(PF_ERR_SHAPE, "B, S, N must be >= 1");
   int dev = -1;
   if (cudaGetDevice(&dev) != cudaSuccess || dev != h->device)
@@ -769,6 +774,8 @@ extern "C" pf_status pf_heads_forward(pf_structure_t* h, const float* msa, const
     sm_symm_kernel<<<(unsigned)((total + 255) / 256), 256, 0, run.st>>>(distogram_out, N, c.n_dist_bins, total);
     ++run.launches;
   }
+  if (pae_out)           // H.4
+    run.gemm(pair, c.c_z, h->w + o.w_pae, h->w + o.b_pae, pae_out, c.n_pae_bins, (long)B * N * N, c.c_z, c.n_pae_bins);
   if (masked_msa_out)    // H.2
     run.gemm(msa, c.c_m, h->w + o.w_mm, h->w + o.b_mm, masked_msa_out, c.n_msa_classes, (long)B * S * N, c.c_m, c.n_msa_classes);
   h->launches = run.launches;
@@ -809,7 +816,7 @@ extern "C" pf_status pf_fold_forward(pf_evoformer_t* h, pf_embedder_t* e, pf_ext
     launches += pf_evoformer_last_launch_count(h);
     const bool last = c == n_cycles - 1;
     s = pf_structure_forward(sm, msa, pair, seq_mask, B, S, N, n_layers, last ? s_out : nullptr, last ? frames_out : nullptr,
-                             x_cycles_out + (size_t)c * xs, last ? alpha_out : nullptr, last ? plddt_out : nullptr, stream);
+                             x_cycles_out + (size_t)c * xs, last ? alpha_out : nullptr, last ? plddt_out : nullptr, nullptr, stream);
     if (s != PF_OK) return s;
     launches += sm->launches;
   }

@@ -421,7 +421,7 @@ def make_extra_inputs(seed: int, B: int, S: int, N: int, d: ExtraDims = EXTRA, l
 
 
 # ----------------------------------------------------------------------------------------------
-# structure module + heads (DESIGN.md §2d readings M.0-M.6, H.1-H.3)
+# structure module + heads (DESIGN.md §2d readings M.0-M.6, H.1-H.5)
 # ----------------------------------------------------------------------------------------------
 
 @dataclass(frozen=True)
@@ -440,6 +440,8 @@ class StructDims:
     n_msa_classes: int = 23   # masked-MSA head
     n_lddt_bins: int = 50     # pLDDT head
     c_lddt: int = 128
+    n_pae_bins: int = 64      # predicted-aligned-error head
+    n_resolved: int = 37      # experimentally-resolved head (atom types)
     pos_scale: float = 10.0   # frame translations are in nanometres, positions in Angstrom
 
     @property
@@ -473,7 +475,9 @@ def struct_spec(d: StructDims = STRUCT):
              ("w_mm", (cm, d.n_msa_classes), "W"), ("b_mm", (d.n_msa_classes,), "bias"),
              ("ln_l_g", (cs,), "gamma"), ("ln_l_b", (cs,), "beta"),
              ("w_l1", (cs, cl), "W"), ("b_l1", (cl,), "bias"), ("w_l2", (cl, cl), "W"), ("b_l2", (cl,), "bias"),
-             ("w_l3", (cl, d.n_lddt_bins), "W"), ("b_l3", (d.n_lddt_bins,), "bias")]
+             ("w_l3", (cl, d.n_lddt_bins), "W"), ("b_l3", (d.n_lddt_bins,), "bias"),
+             ("w_pae", (cz, d.n_pae_bins), "W"), ("b_pae", (d.n_pae_bins,), "bias"),
+             ("w_er", (cs, d.n_resolved), "W"), ("b_er", (d.n_resolved,), "bias")]
     return spec
 
 

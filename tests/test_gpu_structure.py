@@ -1,4 +1,4 @@
-"""GPU parity of the structure module, the heads and the whole recycled GPU stage (readings M.0-M.6, H.1-H.3,
+"""GPU parity of the structure module, the heads and the whole recycled GPU stage (readings M.0-M.6, H.1-H.5,
 DESIGN.md §2d) against the fp64 oracle (oracle/structure_ref.py), through the C ABI.  Everything here is fp32 arithmetic:
 tolerance 1e-4 max-abs on quantities of order one (s, rotation matrices, translations in nanometres), 5e-4 on the unit angle
 vectors (a division by a norm that can be small), 1e-3 on positions in Angstrom (10 x a translation) and on pLDDT (100 x a probability-weighted mean); outputs at masked
@@ -82,15 +82,28 @@ def test_heads_match_oracle():
     h = pf.StructureModule(ps.pack_struct_blob(w), pf.make_struct_config())
     dg = torch.empty((B, N, N, D.n_dist_bins), device="cuda")
     mm = torch.empty((B, S, N, D.n_msa_classes), device="cuda")
-    h.heads(_dev(msa), _dev(pair), dg, mm)
+    pae = torch.empty((B, N, N, D.n_pae_bins), device="cuda")
+    h.heads(_dev(msa), _dev(pair), dg, mm, pae)
     torch.cuda.synchronize()
-    assert h.last_launch_count() == 3
+    assert h.last_launch_count() == 4
     h.heads(None, _dev(pair), dg, None)          # one head alone
+    torch.cuda.synchronize()
+    # H.5 needs the structure module's single representation: one layer is enough to exercise it
+    lengths = [N, N - 9]
+    sm = np.ones((B, N), np.float32)
+    sm[1, lengths[1]:] = 0
+    s_out = torch.empty((B, N, D.c_s), device="cuda")
+    er = torch.empty((B, N, D.n_resolved), device="cuda")
+    h.forward(_dev(msa), _dev(pair), _dev(sm), 1, s_out=s_out, resolved_out=er)
     torch.cuda.synchronize()
     h.close()
     for b in range(B):
         assert np.abs(dg[b].cpu().numpy() - sr.distogram_logits(pair[b], w)).max() <= TOL
         assert np.abs(mm[b].cpu().numpy() - sr.masked_msa_logits(msa[b], w)).max() <= TOL
+        assert np.abs(pae[b].cpu().numpy() - sr.pae_logits(pair[b], w)).max() <= TOL
+        ref = sr.structure_module(msa[b, 0], pair[b], sm[b], w, n_layers=1)
+        v = sm[b] > 0
+        assert np.abs(er[b].cpu().numpy()[v] - sr.resolved_logits(ref["s"], w)[v]).max() <= TOL
 
 
 def test_structure_handle_reuse_and_errors():

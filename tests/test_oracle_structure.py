@@ -1,4 +1,4 @@
-"""Pins of the structure-module / heads oracle (oracle/structure_ref.py; readings M.0-M.6, H.1-H.3 of DESIGN.md §2d) against
+"""Pins of the structure-module / heads oracle (oracle/structure_ref.py; readings M.0-M.6, H.1-H.5 of DESIGN.md §2d) against
 things other than itself: scipy's Rotation, homogeneous 4x4 matrices, torch's attention and softplus, pure-Python index
 loops, the rigid-motion invariance the attention is named for, closed forms and padding invariance (with negative controls).
 """
@@ -14,7 +14,7 @@ from oracle import structure_ref as sr
 
 D = ps.STRUCT
 SMALL = ps.StructDims(c_m=12, c_z=5, c_s=8, heads=2, c_ipa=3, n_qp=2, n_pv=2, n_layers=2, c_resnet=6, n_torsion=3,
-                      n_dist_bins=7, n_msa_classes=4, n_lddt_bins=5, c_lddt=6)
+                      n_dist_bins=7, n_msa_classes=4, n_lddt_bins=5, c_lddt=6, n_pae_bins=6, n_resolved=3)
 
 
 def _kw(d):
@@ -312,3 +312,20 @@ def test_fold_composes_the_pinned_parts():
     other = sr.fold(tf[0], ri[0], mf[0], sm[0], mm[0], we, blocks, wst, 2, x_forced=[two["x_cycles"][0] * 3.0 + 7.0], **kw)
     v = sm[0] > 0
     assert np.abs(other["z"][np.ix_(v, v)] - two["z"][np.ix_(v, v)]).max() > 1e-3
+
+
+def test_pae_and_resolved_heads_are_row_linears():
+    """H.4 / H.5 against torch's linear; H.4 is not symmetric (unlike the distogram)."""
+    d = SMALL
+    w = ps.make_struct_weights(14, d)
+    g = ps.rng(6, 9)
+    z = g.standard_normal((4, 4, d.c_z))
+    s = g.standard_normal((4, d.c_s))
+    lin = torch.nn.functional.linear
+    pae = sr.pae_logits(z, w)
+    ref = lin(torch.from_numpy(z), torch.from_numpy(w["w_pae"].astype(np.float64).T), torch.from_numpy(w["b_pae"].astype(np.float64))).numpy()
+    assert pae.shape == (4, 4, d.n_pae_bins) and np.abs(pae - ref).max() < 1e-13
+    assert np.abs(pae - np.transpose(pae, (1, 0, 2))).max() > 1e-3
+    er = sr.resolved_logits(s, w)
+    ref = lin(torch.from_numpy(s), torch.from_numpy(w["w_er"].astype(np.float64).T), torch.from_numpy(w["b_er"].astype(np.float64))).numpy()
+    assert er.shape == (4, d.n_resolved) and np.abs(er - ref).max() < 1e-13
