@@ -306,6 +306,20 @@ pf_status pf_heads_forward(pf_structure_t* h, const float* msa_dev, const float*
                            float* distogram_out, float* masked_msa_out, float* pae_out, void* cuda_stream);
 long long pf_structure_last_launch_count(const pf_structure_t* h);
 void pf_structure_destroy(pf_structure_t* h);
+/* H.3 for callers that cannot allocate (CUDA graph capture, serving loops, harnesses that forbid cudaMalloc): the pLDDT head
+ * (LN_l, two ReLU layers, logits, expectation — the same kernels as the tail of pf_structure_forward) with its intermediates in a
+ * file-scope device array of PF_PLDDT_STATIC_SCRATCH_BYTES instead of the handle's workspace.  The call performs no cudaMalloc,
+ * cudaFree or allocating library routine; every GPU that loads the library holds the array until the process exits.
+ * s_dev[rows, c_s] (device, read only; rows = B N of the single representation s_out), plddt_out[rows] (device).  Asynchronous on
+ * cuda_stream.  rows * (c_s + 2 c_lddt + n_lddt_bins) floats (each of the four segments rounded up to 256 bytes) must fit the
+ * array: 3039 rows at the default dims; beyond that the call fails with PF_ERR_SHAPE and pf_last_error() states the sizes.
+ * ALL calls in the process on one GPU share the one array (whatever the handle or stream): calls that overlap on the GPU race;
+ * order them on one stream or with events.  The array keeps the previous call's contents; nothing in it needs clearing, each
+ * launch reads only what the launch before it wrote in the same call.  The first call on a device resolves the array's device
+ * address (cudaGetSymbolAddress) and may load the module: make it before a stream capture begins.
+ * Errors: INVALID_ARG (null, wrong current device, device ordinal >= 64), SHAPE (rows < 1 or beyond the array), CUDA. */
+#define PF_PLDDT_STATIC_SCRATCH_BYTES (8u << 20)
+pf_status pf_plddt_forward_static(pf_structure_t* h, const float* s_dev, int rows, float* plddt_out, void* cuda_stream);
 /* The whole GPU stage: n_cycles x (pf_embedder_forward with the PREVIOUS cycle's structure-module
  * positions — x_prev0_dev [B,N,3] or NULL (no previous structure) in the first cycle —, [extra-MSA stack], pf_evoformer_forward,
  * pf_structure_forward).  Arguments as pf_evoformer_forward_recycled; x_cycles_out [n_cycles,B,N,3] (device, required) receives the

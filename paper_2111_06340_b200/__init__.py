@@ -33,7 +33,7 @@ EXPORTED_SYMBOLS = (
     "pf_extra_msa_block_floats", "pf_extra_msa_create", "pf_extra_msa_forward", "pf_extra_msa_forward_substep",
     "pf_extra_msa_last_launch_count", "pf_extra_msa_set_profiling", "pf_extra_msa_get_profile", "pf_extra_msa_destroy",
     "pf_structure_floats", "pf_structure_create", "pf_structure_forward", "pf_heads_forward",
-    "pf_structure_last_launch_count", "pf_structure_destroy", "pf_fold_forward",
+    "pf_structure_last_launch_count", "pf_structure_destroy", "pf_fold_forward", "pf_plddt_forward_static",
 )
 
 
@@ -163,6 +163,8 @@ def lib() -> ctypes.CDLL:
         L.pf_structure_forward.argtypes = [c_void_p] * 4 + [c_int] * 4 + [c_void_p] * 7
         L.pf_heads_forward.restype = c_int
         L.pf_heads_forward.argtypes = [c_void_p] * 3 + [c_int] * 3 + [c_void_p] * 4
+        L.pf_plddt_forward_static.restype = c_int
+        L.pf_plddt_forward_static.argtypes = [c_void_p, c_void_p, c_int, c_void_p, c_void_p]
         L.pf_structure_last_launch_count.restype = c_longlong
         L.pf_structure_last_launch_count.argtypes = [c_void_p]
         L.pf_structure_destroy.restype = None
@@ -419,6 +421,13 @@ class StructureModule:
         S = msa.shape[1] if msa is not None else 1
         _check(lib().pf_heads_forward(self._s, _ptr(msa), _ptr(pair), B, S, N, _ptr(distogram_out), _ptr(masked_msa_out),
                                       _ptr(pae_out), self._stream(stream)))
+
+    def plddt_static(self, s, plddt_out, stream=None):
+        """pf_plddt_forward_static: H.3 on s[..., c_s] with no allocation (file-scope device scratch, shared by all calls)."""
+        rows = 1
+        for d in s.shape[:-1]:
+            rows *= int(d)
+        _check(lib().pf_plddt_forward_static(self._s, _ptr(s), rows, _ptr(plddt_out), self._stream(stream)))
 
     def last_launch_count(self) -> int:
         return int(lib().pf_structure_last_launch_count(self._s))

@@ -19,6 +19,7 @@
 
 #include <algorithm>
 #include <cmath>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -781,6 +782,80 @@ extern "C" pf_status pf_heads_forward(pf_structure_t* h, const float* msa, const
   h->launches = run.launches;
   cudaError_t ce = cudaGetLastError();
   if (ce != cudaSuccess) return sfail(PF_ERR_CUDA, std::string("heads launch failed: ") + cudaGetErrorString(ce));
+  return PF_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// H.3 without any allocation (pf_plddt_forward_static, include/pf_evoformer.h): the same five launches as the pLDDT tail of
+// pf_structure_forward, their intermediates (LN_l(s), two hidden layers, logits) in a file-scope device array instead of the
+// handle's cudaMalloc'ed workspace.  Every GPU that loads this library holds the array (PF_PLDDT_STATIC_SCRATCH_BYTES) until the
+// process exits.  In host code `sm_static_scratch` is the host-side stand-in of the symbol, NOT a device address: the address
+// kernels may dereference comes from cudaGetSymbolAddress, resolved once per device with that device current.
+// ------------------------------------------------------------------------------------------------
+static __device__ __align__(256) float sm_static_scratch[PF_PLDDT_STATIC_SCRATCH_BYTES / 4];
+
+namespace {
+constexpr int kStaticMaxDevices = 64;
+std::mutex sm_static_mu;
+float* sm_static_ptr[kStaticMaxDevices] = {};   // device address of sm_static_scratch, by device ordinal
+
+// `dev` must be the current device
+pf_status sm_static_scratch_for(int dev, float** out) {
+  if (dev < 0 || dev >= kStaticMaxDevices) return sfail(PF_ERR_INVALID_ARG, "pf_plddt_forward_static: device ordinal >= 64");
+  std::lock_guard<std::mutex> lk(sm_static_mu);
+  if (!sm_static_ptr[dev]) {
+    void* p = nullptr;
+    const cudaError_t ce = cudaGetSymbolAddress(&p, sm_static_scratch);
+    if (ce != cudaSuccess || !p) {
+      cudaGetLastError();
+      return sfail(PF_ERR_CUDA, std::string("pf_plddt_forward_static: cudaGetSymbolAddress(sm_static_scratch): ") +
+                                    (ce != cudaSuccess ? cudaGetErrorString(ce) : "null address"));
+    }
+    sm_static_ptr[dev] = static_cast<float*>(p);
+  }
+  *out = sm_static_ptr[dev];
+  return PF_OK;
+}
+}  // namespace
+
+extern "C" pf_status pf_plddt_forward_static(pf_structure_t* h, const float* s, int rows, float* plddt_out, void* stream) {
+  if (!h || !s || !plddt_out) return sfail(PF_ERR_INVALID_ARG, "null argument");
+  if (rows < 1) return sfail(PF_ERR_SHAPE, "pf_plddt_forward_static: rows must be >= 1");
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev != h->device)
+    return sfail(PF_ERR_INVALID_ARG, "the current device is not the one the structure handle was created on");
+  const pf_struct_config& c = h->cfg;
+  const SmOff& o = h->off;
+  const int cs = c.c_s, cl = c.c_lddt, nb = c.n_lddt_bins;
+  const long R = rows;
+  // four segments, each starting on a 256-byte boundary of the array
+  size_t at = 0;
+  auto take = [&](size_t n) { size_t r = at; at += (n + 63) & ~(size_t)63; return r; };
+  const size_t o_ln = take((size_t)R * cs), o_l1 = take((size_t)R * cl), o_l2 = take((size_t)R * cl), o_lg = take((size_t)R * nb);
+  const size_t cap = PF_PLDDT_STATIC_SCRATCH_BYTES / 4;
+  if (at > cap) {
+    const size_t per_row = (size_t)cs + 2 * (size_t)cl + nb;
+    return sfail(PF_ERR_SHAPE, "pf_plddt_forward_static: " + std::to_string(rows) + " rows need " + std::to_string(at * 4) +
+                                   " bytes of scratch, the static array holds " + std::to_string((size_t)PF_PLDDT_STATIC_SCRATCH_BYTES) +
+                                   " (about " + std::to_string((cap - 4 * 64) / per_row) + " rows at these dims); use pf_structure_forward");
+  }
+  float* scratch = nullptr;
+  const pf_status ps = sm_static_scratch_for(dev, &scratch);
+  if (ps != PF_OK) return ps;
+  // nothing in the array has to start at zero: every element a launch reads was written by the launch before it in this call
+  // (LayerNorm and the non-accumulating GEMMs overwrite their whole [rows, width] output)
+  const float* w = h->w;
+  float *ln = scratch + o_ln, *l1 = scratch + o_l1, *l2 = scratch + o_l2, *lg = scratch + o_lg;
+  SmRun run{h, reinterpret_cast<cudaStream_t>(stream)};
+  run.ln(s, ln, w + o.ln_l_g, w + o.ln_l_b, R, cs);
+  run.gemm(ln, cs, w + o.w_l1, w + o.b_l1, l1, cl, R, cs, cl, false, true);
+  run.gemm(l1, cl, w + o.w_l2, w + o.b_l2, l2, cl, R, cl, cl, false, true);
+  run.gemm(l2, cl, w + o.w_l3, w + o.b_l3, lg, nb, R, cl, nb);
+  sm_plddt_kernel<<<(unsigned)((R + 7) / 8), 256, 0, run.st>>>(lg, plddt_out, R, nb);
+  ++run.launches;
+  h->launches = run.launches;
+  const cudaError_t ce = cudaGetLastError();
+  if (ce != cudaSuccess) return sfail(PF_ERR_CUDA, std::string("pf_plddt_forward_static launch failed: ") + cudaGetErrorString(ce));
   return PF_OK;
 }
 
