@@ -1,21 +1,28 @@
 // Fused transition on tcgen05 tensor cores (sm_100a) — SURVEY.md App. A.3 (MSA, C = 256) and A.9 (pair, C = 128):
 //     res[r, :] += relu(LayerNorm(res[r, :]) W1 + b1) W2 + b2,      W1: C -> 4C,  W2: 4C -> C
 // (north_star: "MSA and pair transitions fused with their residual adds"; §8(a) rows 3 / 9: "hidden stays on-chip").
-// The 4C-wide hidden activation never reaches HBM: per 128-row tile it is produced 128 columns at a time into TMEM
-// (GEMM1), rectified by the epilogue warps into a bf16 K-major shared-memory tile, and immediately consumed as the A
-// operand of GEMM2, which accumulates the C output columns in TMEM over the 4C/128 chunks.  HBM traffic per row is one
-// fp32 read and one fp32 reduce-add of C values (the algorithmic minimum 8C bytes + the L2-resident weights).
+// The 4C-wide hidden activation never reaches HBM and, since round 2, not even shared memory: per 128-row tile it is produced
+// 128 columns at a time into TMEM (GEMM1), rectified by the epilogue warps IN PLACE (tcgen05.ld -> +b1, relu, bf16 pairs ->
+// tcgen05.st over the thread's own fp32 columns) and consumed from tensor memory as the A operand of GEMM2 (tcgen05.mma with a
+// TMEM A operand), which accumulates the C output columns in TMEM over the 4C/128 chunks.  HBM traffic per row is one fp32 read
+// and one fp32 reduce-add of C values (the algorithmic minimum 8C bytes + the L2-resident weights).  The kernel is paced by
+// shared-memory bandwidth (128 B/clk: both operands of a 128 x 128 x 16 MMA from shared memory already take all of it, and the
+// weight tiles arriving by TMA and the staging traffic come on top), so every byte kept out of shared memory is time.
 //
 // One persistent CTA per SM, 18 working warps (20 launched: register re-allocation is per warpgroup of four):
-//   warps 0-7   epilogue, two teams of four warps.  E1(chunk): team t rectifies columns [64t, 64t+64) of the hidden chunk
-//               (TMEM -> +b1 -> relu -> bf16 -> k-block t of the A2 tile, UMMA 128B-swizzle layout).  E2(tile): the C output
-//               columns + b2 in 32-column fp32 boxes through staging tiles (the idle A2 buffers) -> TMA reduce-add into the
-//               residual (the add happens at L2).
+//   warps 0-7   epilogue, two teams of four warps.  E1(chunk): team t rectifies columns [64t, 64t+64) of the hidden chunk into
+//               32-bit columns [64t, 64t+32) of the same accumulator buffer.  E2(tile): the C output columns + b2 in 32-column
+//               fp32 boxes through staging tiles -> TMA reduce-add into the residual (the add happens at L2).  At C = 256 the
+//               staging tiles are the tile's own A1 buffer (idle after its last GEMM1); the team leaders hand it back to the
+//               producers once the reduce-adds have read it.
 //   warps 8-15  LayerNorm producers: warp-per-row, 128-bit loads, warp-shuffle statistics, fp16 result straight into the
-//               UMMA K-major 128B-swizzle layout (A1); the next tile's rows are pulled into L2 by a bulk prefetch.
+//               UMMA K-major 128B-swizzle layout (A1, double buffered: the LayerNorm of tile t+1 runs under the GEMMs of tile
+//               t); the next rows are pulled into L2 by a bulk prefetch.
 //   warp 16     TMA: [128 x 64] weight tiles of W1^T / W2^T through one ring, in the order the MMA thread consumes them
 //   warp 17     TMEM allocation + the single MMA-issuing thread.  Issue order per tile: G1(0), G1(1), G2(0), G1(2), G2(1),
 //               ... so the rectification of chunk c overlaps GEMM1 of chunk c+1 (hidden accumulator double-buffered in TMEM).
+//               GEMM1(c+2) overwrites the buffer GEMM2(c) reads its A operand from: both are issued by this one thread, in
+//               that order, and tcgen05.mma operations of one thread execute in issue order (no barrier in between).
 #include "pf_internal.h"
 #include "pf_device.cuh"
 #include "pf_tc.cuh"
@@ -38,20 +45,25 @@ template <int C>
 struct TrSmem {
   static constexpr int KB1 = C / 64;                       // k-blocks of GEMM1 (K = C)
   static constexpr int NH = C / 128;                       // 128-column halves of the output
-  static constexpr int A1_BUFS = (C == 128) ? 2 : 1;
+  static constexpr int A1_BUFS = 2;
   static constexpr int A1_BYTES = 128 * C * 2;
-  static constexpr int KB_BYTES = 128 * 128;               // one [128 x 64] 16-bit k-block
-  static constexpr int A2_BYTES = 2 * KB_BYTES;            // hidden chunk [128 x 128] bf16
+  static constexpr int KB_BYTES = 128 * 128;               // one [128 x 64] 16-bit k-block = one [128 x 32] fp32 output box
+  static constexpr int ST_BYTES = 4 * KB_BYTES;            // output staging: two teams x two boxes
+  // C = 256: the staging boxes of tile t live in the A1 buffer of tile t (idle once its last GEMM1 has retired; handed back
+  // to the LayerNorm producers when the reduce-adds have read it); C = 128 has room for a region of its own
+  static constexpr bool ST_ALIAS = (C == 256);
   static constexpr int W_STAGE = KB_BYTES;                 // [128 rows x 64 k] 16-bit
   static constexpr int W_STAGES = 5;
   static constexpr int A1_OFF = 0;
-  static constexpr int A2_OFF = A1_OFF + A1_BUFS * A1_BYTES;
-  static constexpr int W_OFF = A2_OFF + 2 * A2_BYTES;
+  static constexpr int ST_OFF = A1_OFF + A1_BUFS * A1_BYTES;
+  static constexpr int W_OFF = ST_OFF + (ST_ALIAS ? 0 : ST_BYTES);
   static constexpr int B1_OFF = W_OFF + W_STAGES * W_STAGE;   // fp32 b1 [4C]
   static constexpr int B2_OFF = B1_OFF + 4 * C * 4;           // fp32 b2 [C]
   static constexpr int BAR_OFF = B2_OFF + C * 4;
   static constexpr int TOTAL = BAR_OFF + 256 + 1024;
   static constexpr int TMEM_ACC2 = 256;                    // acc1[2] at columns 0 / 128, acc2 at [256, 256 + C)
+  static_assert(!ST_ALIAS || A1_BYTES == ST_BYTES, "aliased staging must fit the A1 buffer");
+  static_assert(TOTAL <= 227 * 1024, "shared memory budget");
 };
 
 struct TrParams {
@@ -91,10 +103,8 @@ transition_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constan
   uint64_t* w_full = bars + 4;             // [WS]
   uint64_t* w_empty = w_full + WS;         // [WS]
   uint64_t* acc1_full = w_empty + WS;      // [2]
-  uint64_t* acc1_empty = acc1_full + 2;    // [2]
-  uint64_t* a2_full = acc1_empty + 2;      // [2]
-  uint64_t* a2_empty = a2_full + 2;        // [2]
-  uint64_t* acc2_full = a2_empty + 2;      // 1
+  uint64_t* a2_full = acc1_full + 2;       // [2]
+  uint64_t* acc2_full = a2_full + 2;       // 1
   uint64_t* acc2_empty = acc2_full + 1;    // 1
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(acc2_empty + 1);
   float* sb1 = reinterpret_cast<float*>(smem + SM::B1_OFF);
@@ -108,11 +118,9 @@ transition_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constan
     tc::prefetch_tmap(&tmR);
     for (int i = 0; i < 2; ++i) {
       tc::mbar_init(&a1_full[i], TR_PROD_WARPS * 32);
-      tc::mbar_init(&a1_empty[i], 1);
+      tc::mbar_init(&a1_empty[i], SM::ST_ALIAS ? 2 : 1);   // aliased staging: one arrival per team leader
       tc::mbar_init(&acc1_full[i], 1);
-      tc::mbar_init(&acc1_empty[i], TR_EPI_WARPS * 32);
       tc::mbar_init(&a2_full[i], TR_EPI_WARPS * 32);
-      tc::mbar_init(&a2_empty[i], 1);
     }
     for (int i = 0; i < WS; ++i) {
       tc::mbar_init(&w_full[i], 1);
@@ -148,15 +156,13 @@ transition_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constan
 #pragma unroll 1
       for (int c = 0; c < NC; ++c, ++cc) {
         const uint32_t buf = cc & 1, ph = (cc >> 1) & 1;
+        if (SM::ST_ALIAS && c == 1 && it > 0 && leader) {
+          // the previous tile's reduce-adds have read their staging boxes (its A1 buffer): hand it to the producers
+          tc::bulk_wait_read<0>();
+          tc::mbar_arrive(&a1_empty[(it - 1) % A1B]);
+        }
         tc::mbar_wait(&acc1_full[buf], ph);
         tc::tc_fence_after();
-        tc::mbar_wait(&a2_empty[buf], ph ^ 1);         // GEMM2 of the chunk two steps back has read this A2 buffer
-        if (c < 2) {
-          // the previous tile's E2 staged its output in this A2 buffer: its TMA reads must be complete
-          if (leader) tc::bulk_wait_read<0>();
-          tc::named_bar_sync(bar_id, 128);
-        }
-        uint8_t* arow = smem + SM::A2_OFF + buf * SM::A2_BYTES + team * SM::KB_BYTES + lr * 128;
         const float* bb = sb1 + c * TR_HC + team * 64;
         const uint32_t ta = lane_addr + buf * TR_HC + team * 64;
 #pragma unroll
@@ -177,14 +183,12 @@ transition_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constan
 #pragma unroll
           for (int e = 0; e < 32; e += 2)
             pk[e >> 1] = tr_pack_bf16(fmaxf(__uint_as_float(v[e]) + b1r[e], 0.f), fmaxf(__uint_as_float(v[e + 1]) + b1r[e + 1], 0.f));
-#pragma unroll
-          for (int q = 0; q < 4; ++q)
-            *reinterpret_cast<uint4*>(arow + (((uint32_t)(hf * 4 + q) ^ sw) << 4)) =
-                make_uint4(pk[q * 4], pk[q * 4 + 1], pk[q * 4 + 2], pk[q * 4 + 3]);
+          // bf16 pairs back into tensor memory, over this thread's own (already loaded) fp32 input columns: hidden columns
+          // 64 team + 32 hf + [0, 32) -> 32-bit columns 64 team + 16 hf + [0, 16) of the chunk's accumulator buffer
+          tc::tmem_st16(ta + hf * 16, pk);
         }
+        tc::tmem_st_wait();
         tc::tc_fence_before();
-        tc::mbar_arrive(&acc1_empty[buf]);
-        tc::fence_proxy_async_smem();
         tc::mbar_arrive(&a2_full[buf]);
       }
       // ---- E2: output columns + b2 -> fp32 staging (this team's A2 buffer, two 16 KB boxes) -> TMA reduce-add
@@ -192,11 +196,15 @@ transition_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constan
       tc::tc_fence_after();
       // staging boxes: k-block `team` of both A2 buffers — the region only this team writes in E1, so the team leader's
       // own bulk-group bookkeeping covers every reuse
-      uint8_t* stage = smem + SM::A2_OFF + team * SM::KB_BYTES;
+      uint8_t* stage = smem + (SM::ST_ALIAS ? SM::A1_OFF + (int)(it % A1B) * SM::A1_BYTES : SM::ST_OFF) + team * 2 * SM::KB_BYTES;
       int nbox = 0;
+      if (!SM::ST_ALIAS) {
+        if (leader) tc::bulk_wait_read<0>();           // the previous tile's reduce-adds have read their staging boxes
+        tc::named_bar_sync(bar_id, 128);
+      }
 #pragma unroll 1
       for (int bx = team; bx < C / 32; bx += 2, ++nbox) {
-        uint8_t* sb = stage + (nbox & 1) * SM::A2_BYTES;
+        uint8_t* sb = stage + (nbox & 1) * SM::KB_BYTES;
         if (nbox >= 2) {
           if (leader) tc::bulk_wait_read<1>();
           tc::named_bar_sync(bar_id, 128);
@@ -309,9 +317,9 @@ transition_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constan
         const uint32_t abuf = it % A1B;
         const uint32_t a1_addr = tc::smem_u32(smem + SM::A1_OFF + abuf * SM::A1_BYTES);
         auto gemm1 = [&](int c) {
+          // No wait for the buffer: its previous content (chunk c - 2, rectified in place) was the A operand of GEMM2(c - 2),
+          // issued by this thread before this GEMM1, and tcgen05.mma operations of one thread execute in issue order.
           const uint32_t buf = c1 & 1;
-          tc::mbar_wait(&acc1_empty[buf], ((c1 >> 1) & 1) ^ 1);
-          tc::tc_fence_after();
           const uint32_t d = tmem_base + buf * TR_HC;
 #pragma unroll 1
           for (int kb = 0; kb < KB1; ++kb, ++wc) {
@@ -332,10 +340,9 @@ transition_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constan
           const uint32_t buf = c2 & 1;
           tc::mbar_wait(&a2_full[buf], (c2 >> 1) & 1);
           tc::tc_fence_after();
-          const uint32_t a2_addr = tc::smem_u32(smem + SM::A2_OFF + buf * SM::A2_BYTES);
+          const uint32_t a2_t = tmem_base + buf * TR_HC;   // rectified chunk, bf16 pairs: k-block kb at columns 64 kb + [0, 32)
 #pragma unroll 1
           for (int kb = 0; kb < 2; ++kb) {
-            const uint64_t a_desc = tc::smem_desc_kmajor<128>(a2_addr + kb * SM::KB_BYTES);
 #pragma unroll 1
             for (int nh = 0; nh < NH; ++nh, ++wc) {
               const uint32_t s = wc % WS;
@@ -344,11 +351,10 @@ transition_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constan
               const uint64_t b_desc = tc::smem_desc_kmajor<128>(tc::smem_u32(smem + SM::W_OFF + s * SM::W_STAGE));
 #pragma unroll
               for (int k = 0; k < 4; ++k)
-                tc::mma_bf16(acc2 + nh * 128, a_desc + 2 * k, b_desc + 2 * k, idesc2, (c | kb | k) != 0);
+                tc::mma_bf16_ts(acc2 + nh * 128, a2_t + kb * 64 + k * 8, b_desc + 2 * k, idesc2, (c | kb | k) != 0);
               tc::mma_commit(&w_empty[s]);
             }
           }
-          tc::mma_commit(&a2_empty[buf]);
           ++c2;
         };
         tc::mbar_wait(&a1_full[abuf], (it / A1B) & 1);
@@ -356,7 +362,7 @@ transition_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constan
         gemm1(0);
         for (int c = 1; c < NC; ++c) {
           gemm1(c);
-          if (c == NC - 1) tc::mma_commit(&a1_empty[abuf]);   // every GEMM1 of this tile has been issued: A1 is free when they finish
+          if (!SM::ST_ALIAS && c == NC - 1) tc::mma_commit(&a1_empty[abuf]);   // every GEMM1 of this tile has been issued: A1 is free when they finish
           if (c == 1) {
             // acc2 of the previous tile must have been drained by E2 before the first GEMM2 overwrites it
             tc::mbar_wait(acc2_empty, (it & 1) ^ 1);
