@@ -4,8 +4,10 @@
 // s contiguous), so both operands of the first contraction are K-major tiles TMA can fetch directly.
 // One CTA = 128 residues i x 2 residues j of one protein.  For c1 = 0..31 (software-pipelined over two TMEM buffers):
 //   GEMM1  D1[i, (j,c2)] = sum_s a[s,i,c1] b[s,j,c2]        M=128, N=64,  K=S     (a streamed per c1, b resident)
-//   epilogue warps: D1 fp32 (TMEM) -> bf16 -> two K-major 128x32 tiles in shared memory (64B swizzle)
-//   GEMM2  acc_j[i, e] += sum_c2 D1[i,(j,c2)] W_out[c1*32+c2, e]   M=128, N=128, K=32  per j, accumulated over c1 in TMEM
+//   epilogue warps: D1 fp32 (TMEM) -> fp16 pairs written back over the same TMEM columns (j at 32-bit columns 32 j + [0, 16))
+//   GEMM2  acc_j[i, e] += sum_c2 D1[i,(j,c2)] W_out[c1*32+c2, e]   M=128, N=128, K=32  per j, accumulated over c1 in TMEM,
+//          its A operand read from tensor memory: the kernel is paced by shared-memory bandwidth (GEMM1 alone asks for
+//          192 B/clk at M=128, N=64), so the outer product makes no trip through shared memory
 // so the 32x32 outer product per pair never reaches HBM (north_star bullet 3).  Final: acc_j / (1e-3 + n_ij) + b_out
 // added to the fp32 pair stream, 512 contiguous bytes per thread.
 #include "pf_internal.h"
@@ -19,14 +21,14 @@ int tma_encode_bf16(TmaCtx* ctx, CUtensorMap* out, const void* base, int rank, c
 
 constexpr int OP_BI = 128, OP_BJ = 2, OP_C = 32, OP_CZ = 128, OP_BK = 64;
 constexpr int OP_MAX_KB = 8;       // S <= 512
-constexpr int OP_A_STAGES = 10;    // upper bound; the launch uses as many 16 KB stages as fit beside the resident b operand
+constexpr int OP_A_STAGES = 12;    // upper bound; the launch uses as many 16 KB stages as fit beside the resident b operand
 constexpr int OP_THREADS = 192;
 constexpr int OP_NB = 4;           // at most 4 outer-product tiles in flight between the two contractions (TMEM: 4 x 64 columns)
 // Per launch: nb = 4 tiles in flight and GEMM2 lagging GEMM1 by 2 when the contraction is short (N_seq <= 256: GEMM1 is too short
 // to hide the relayout of the previous tile behind it), nb = 2 / lag 1 otherwise (the shared memory goes to a deeper a ring,
 // which is what bounds the long contractions).
 
-// Shared memory: W_out tiles, the bf16 outer-product tiles and the barriers at fixed offsets, then the resident b operand
+// Shared memory: W_out tiles and the barriers at fixed offsets, then the resident b operand
 // (n_kb x 8 KB, n_kb = k-blocks of this launch) and behind it the ring of a tiles: as many 16 KB stages as fit.  The a stream
 // is fetched from L2 with a latency of ~1 us, so its rate is ring bytes / latency (measured: 64 KB in flight gave ~71 GB/s per
 // SM and bounded the kernel; the multicast variant, which cuts L2 traffic instead, was slower).
@@ -35,11 +37,9 @@ struct OpmSmem {
   static constexpr int A_BYTES = OP_BI * 128;                            // 16 KB
   static constexpr int W_OFF = 0;
   static constexpr int W_BYTES = OP_CZ * 64;                             // 128 e x 32 c2 bf16 = 8 KB
-  static constexpr int OV_TILE = OP_BI * 64;                             // 128 i x 32 c2 bf16 = 8 KB
   static constexpr int BAR_OFF = 0;
   static constexpr int TOTAL = 227 * 1024;
-  static __host__ __device__ int ov_off(int nb) { return 1024 + nb * W_BYTES; }                 // W ring first, at 1024
-  static __host__ __device__ int b_off(int nb) { return ov_off(nb) + nb * OP_BJ * OV_TILE; }
+  static __host__ __device__ int b_off(int nb) { return 1024 + nb * W_BYTES; }                  // W ring first, at 1024
   static __host__ __device__ int ring_bytes(int nb) { return TOTAL - 1024 - b_off(nb); }        // b operand + a ring
 };
 
@@ -65,10 +65,8 @@ opm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ C
   uint64_t* w_full = a_empty + OP_A_STAGES;       // [OP_NB]
   uint64_t* w_empty = w_full + OP_NB;             // [OP_NB]
   uint64_t* d1_full = w_empty + OP_NB;            // [OP_NB]
-  uint64_t* d1_empty = d1_full + OP_NB;           // [OP_NB]
-  uint64_t* ov_full = d1_empty + OP_NB;           // [OP_NB]
-  uint64_t* ov_empty = ov_full + OP_NB;           // [OP_NB]
-  uint64_t* acc_full = ov_empty + OP_NB;
+  uint64_t* ov_full = d1_full + OP_NB;            // [OP_NB]
+  uint64_t* acc_full = ov_full + OP_NB;
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(acc_full + 1);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -77,7 +75,7 @@ opm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ C
   // the normaliser counts all S sequences, and the chunks add up because the projection is linear (bias with the first chunk)
   const int n_kb = (Sc + OP_BK - 1) / OP_BK;
   const int nb = 1 << nb_shift, lag = nb >> 1;
-  const int W_OFF = 1024, OV_OFF = SM::ov_off(nb), B_OFF = SM::b_off(nb);
+  const int W_OFF = 1024, B_OFF = SM::b_off(nb);
   const int A_OFF = B_OFF + n_kb * SM::B_KB_BYTES;
 
   if (warp == 0 && lane == 0) {
@@ -93,9 +91,7 @@ opm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ C
       tc::mbar_init(&w_full[s], 1);
       tc::mbar_init(&w_empty[s], 1);
       tc::mbar_init(&d1_full[s], 1);
-      tc::mbar_init(&d1_empty[s], 128);
       tc::mbar_init(&ov_full[s], 128);
-      tc::mbar_init(&ov_empty[s], 1);
     }
     tc::mbar_init(acc_full, 1);
     tc::fence_barrier_init();
@@ -138,9 +134,9 @@ opm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ C
       uint32_t ph = 0;
       for (int c1 = 0; c1 < OP_C + lag; ++c1) {
         if (c1 < OP_C) {
+          // No wait for the buffer: its previous content (tile c1 - nb, converted in place) was the A operand of GEMM2(c1 - nb),
+          // issued by this thread lag = nb / 2 iterations ago, and tcgen05.mma operations of one thread execute in issue order.
           int buf = c1 & (nb - 1);
-          tc::mbar_wait(&d1_empty[buf], ((c1 >> nb_shift) & 1) ^ 1);
-          tc::tc_fence_after();
           for (int kb = 0; kb < n_kb; ++kb) {
             tc::mbar_wait(&a_full[s], ph);
             tc::tc_fence_after();
@@ -162,11 +158,10 @@ opm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ C
           uint64_t w_desc = tc::smem_desc_kmajor<64>(tc::smem_u32(smem + W_OFF + pb * SM::W_BYTES));
 #pragma unroll
           for (int j = 0; j < OP_BJ; ++j) {
-            uint64_t o_desc = tc::smem_desc_kmajor<64>(tc::smem_u32(smem + OV_OFF + (pb * OP_BJ + j) * SM::OV_TILE));
-            tc::mma_bf16(tmem_acc + j * OP_CZ, o_desc, w_desc, idesc2, p != 0);
-            tc::mma_bf16(tmem_acc + j * OP_CZ, o_desc + 2, w_desc + 2, idesc2, true);
+            const uint32_t o_t = tmem_d1 + pb * 64 + j * 32;   // fp16 pairs: 8 columns per K = 16 step
+            tc::mma_bf16_ts(tmem_acc + j * OP_CZ, o_t, w_desc, idesc2, p != 0);
+            tc::mma_bf16_ts(tmem_acc + j * OP_CZ, o_t + 8, w_desc + 2, idesc2, true);
           }
-          tc::mma_commit(&ov_empty[pb]);
           tc::mma_commit(&w_empty[pb]);
         }
       }
@@ -185,24 +180,18 @@ opm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ C
       tc::tmem_ld32(tmem_d1 + buf * 64 + lane_addr, v[0]);
       tc::tmem_ld32(tmem_d1 + buf * 64 + lane_addr + 32, v[1]);
       tc::tmem_ld_wait();
-      tc::tc_fence_before();
-      tc::mbar_arrive(&d1_empty[buf]);
-      tc::mbar_wait(&ov_empty[buf], ((c1 >> nb_shift) & 1) ^ 1);
 #pragma unroll
       for (int j = 0; j < OP_BJ; ++j) {
-        uint8_t* tile = smem + OV_OFF + (buf * OP_BJ + j) * SM::OV_TILE;
+        uint32_t pk[16];
 #pragma unroll
-        for (int c = 0; c < 4; ++c) {
-          uint32_t pk[4];
-#pragma unroll
-          for (int e = 0; e < 4; ++e) {
-            __half2 pp = __floats2half2_rn(__uint_as_float(v[j][c * 8 + 2 * e]), __uint_as_float(v[j][c * 8 + 2 * e + 1]));
-            pk[e] = *reinterpret_cast<uint32_t*>(&pp);
-          }
-          *reinterpret_cast<uint4*>(tile + tc::swz_offset<64>(row, c)) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
+        for (int e = 0; e < 16; ++e) {
+          __half2 pp = __floats2half2_rn(__uint_as_float(v[j][2 * e]), __uint_as_float(v[j][2 * e + 1]));
+          pk[e] = *reinterpret_cast<uint32_t*>(&pp);
         }
+        tc::tmem_st16(tmem_d1 + buf * 64 + lane_addr + j * 32, pk);   // over this thread's own (already loaded) columns
       }
-      tc::fence_proxy_async_smem();
+      tc::tmem_st_wait();
+      tc::tc_fence_before();
       tc::mbar_arrive(&ov_full[buf]);
     }
     // n_ij = (sum_s rho_s) sigma_i sigma_j   (R5)
