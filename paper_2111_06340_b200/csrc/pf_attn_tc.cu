@@ -11,13 +11,13 @@
 //                  constant 64 x 64 identity, K=4x16: the tensor core adds the bias exactly (fp32 accumulation), so the softmax
 //                  warps never unpack it; TMEM double buffered) is issued BEFORE waiting for P(i), so the
 //                  tensor core works on the next logits while the softmax warps are busy; O_tile = P V (M=128 N=32 K=4x16)
-//   warps 0-3      thread-per-row online softmax in fp32 from tcgen05.ld (ex2.approx), P (bf16) -> smem in the UMMA
-//                  128B-swizzle layout.  O accumulates in TMEM over the key tiles of a unit (P V with accumulate); P is taken
+//   warps 0-3      thread-per-row online softmax in fp32 from tcgen05.ld (ex2.approx), P (bf16 pairs) written back over the
+//                  logits in tensor memory (tcgen05.st) and read by P V as a TMEM A operand.  O accumulates in TMEM over the key tiles of a unit (P V with accumulate); P is taken
 //                  relative to a reference maximum that moves only when the running maximum has grown by more than 2^8, and
 //                  only then is O rescaled (tcgen05.ld, multiply, tcgen05.st) — the time of this kernel follows the
 //                  instruction count of these warps, and the per-tile "(O + PV) alpha" round trip through registers was 15 %
 //                  of it; gate (prefetched at unit start) and 1/l applied at the end, 64-byte row stores.
-// ~106 KB of shared memory and 256 TMEM columns per CTA -> 2 CTAs per SM overlap each other's softmax and barrier latency.
+// ~96 KB of shared memory and 256 TMEM columns per CTA -> 2 CTAs per SM overlap each other's softmax and barrier latency.
 #include "pf_internal.h"
 #include "pf_device.cuh"
 #include "pf_tc.cuh"
@@ -35,8 +35,7 @@ constexpr int AT_MAXKEYS = 1024;  // mask terms kept in shared memory
 struct AttnSmem {
   static constexpr int Q_BYTES = AT_BQ * 64;                       // 128 x 32 bf16, 64B swizzle: 8 KB
   static constexpr int Q_OFF = 0;                                  // two Q buffers
-  static constexpr int P_OFF = Q_OFF + 2 * Q_BYTES;                // 128 x 64 bf16, 128B swizzle: 16 KB
-  static constexpr int STAGE_OFF = P_OFF + AT_BQ * 128;
+  static constexpr int STAGE_OFF = Q_OFF + 2 * Q_BYTES;
   static constexpr int K_BYTES = AT_BK * 64;                       // 64 x 32 bf16: 4 KB
   static constexpr int V_BYTES = 32 * 128;                         // 32 x 64 bf16: 4 KB
   static constexpr int B_BYTES = AT_BQ * 128;                      // 128 x 64 bf16: 16 KB
@@ -45,7 +44,7 @@ struct AttnSmem {
   static constexpr int ID_OFF = STAGE_OFF + POOL_BYTES;            // 64 x 64 bf16 identity, K-major 128B swizzle: 8 KB
   static constexpr int MASK_OFF = ID_OFF + 64 * 128;               // one bit per key: 1 = masked or out of range
   static constexpr int BAR_OFF = MASK_OFF + AT_MAXKEYS / 8;
-  // No alignment slack: two CTAs of 115,072 B fit one SM only without it.  The dynamic shared memory window of a kernel
+  // No alignment slack: two CTAs per SM must fit (98,688 B each).  The dynamic shared memory window of a kernel
   // without static shared memory starts 1024-byte aligned; the kernel traps if it ever does not.
   static constexpr int TOTAL = BAR_OFF + 256;
 };
@@ -166,7 +165,6 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQK, const __grid_constant__
       constexpr uint32_t idesc_s = tc::idesc_bf16_f32(AT_BQ, AT_BK);
       constexpr uint32_t idesc_b = tc::idesc_f16_f32(AT_BQ, AT_BK);   // bias tile x identity: fp16 operands
       constexpr uint32_t idesc_o = tc::idesc_bf16_f32(AT_BQ, 32);
-      const uint64_t p_desc = tc::smem_desc_kmajor<128>(tc::smem_u32(smem + SM::P_OFF));
       const uint64_t id_desc = tc::smem_desc_kmajor<128>(tc::smem_u32(smem + SM::ID_OFF));
       // issue side: S(j) = Q K^T for the next (unit, key tile); consume side: P(i) V.  j runs one step ahead of i.
       const int units = *p.n_rows * p.H * p.QT;
@@ -220,7 +218,8 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQK, const __grid_constant__
           tc::tc_fence_after();
           const uint64_t v_desc = tc::smem_desc_kmajor<128>(tc::smem_u32(smem + SM::STAGE_OFF + s * p.stage_bytes + SM::K_BYTES));
 #pragma unroll
-          for (int k = 0; k < AT_BK / 16; ++k) tc::mma_bf16(tmem_O, p_desc + 2 * k, v_desc + 2 * k, idesc_o, (k | pkt) != 0);
+          for (int k = 0; k < AT_BK / 16; ++k)   // A = P(i): bf16 pairs in the first 32 columns of the S buffer it came from
+            tc::mma_bf16_ts(tmem_O, tmem_S + (i & 1) * AT_BK + k * 8, v_desc + 2 * k, idesc_o, (k | pkt) != 0);
           tc::mma_commit(o_full);
           tc::mma_commit(&kv_empty[s]);
           if (++pkt == pn) {
@@ -236,7 +235,6 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQK, const __grid_constant__
     // ============================================================= softmax warps (thread per query row)
     const int row = warp * 32 + lane;            // warp w reads TMEM lanes [32w, 32w+32)
     const uint32_t lane_addr = (uint32_t)(warp * 32) << 16;
-    uint8_t* prow = smem + SM::P_OFF;
     int cur_b = -1;
     uint32_t tile_masked = 0;                    // bit kt: key tile kt holds a masked / out-of-range key
     uint32_t i = 0;                              // pipeline step (all units)
@@ -316,14 +314,16 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQK, const __grid_constant__
           mx3 = fmaxf(mx3, x[j + 3]);
         }
         m_run = fmaxf(m_run, fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)));
+        bool pv_seen = (kt == 0);   // PV(i-1) observed complete (the previous unit's last one was, at that unit's end)
         if (kt == 0) {
           m_ref = m_run;
         } else {
-          // PV(i-1) must have finished reading P before it is overwritten, and before O is touched
-          tc::mbar_wait(o_full, (i - 1) & 1);
-          tc::tc_fence_after();
           const bool move = m_run > m_ref + 8.0f;          // also true when m_ref is still -inf and a key has appeared
           if (__any_sync(0xffffffffu, move)) {
+            // PV(i-1) must have finished before O is touched
+            tc::mbar_wait(o_full, (i - 1) & 1);
+            tc::tc_fence_after();
+            pv_seen = true;
             // rows that do not move multiply by 1; a row whose reference was -inf has O = l = 0: factor 0 keeps that exact
             const float alpha = !move ? 1.0f : (m_ref == -INFINITY ? 0.0f : ex2_approx(m_ref - m_run));
             uint32_t ov[32];
@@ -339,21 +339,24 @@ attn_tc_kernel(const __grid_constant__ CUtensorMap tmQK, const __grid_constant__
         }
         const float m_use = (m_ref == -INFINITY) ? 0.f : m_ref;
         float sum0 = 0.f, sum1 = 0.f;
+        uint32_t pk[32];
 #pragma unroll
-        for (int c = 0; c < 8; ++c) {
-          uint32_t pk[4];
-#pragma unroll
-          for (int e = 0; e < 4; ++e) {
-            const float p0 = ex2_approx(x[c * 8 + 2 * e] - m_use), p1 = ex2_approx(x[c * 8 + 2 * e + 1] - m_use);
-            sum0 += p0;
-            sum1 += p1;
-            __nv_bfloat162 pp = __floats2bfloat162_rn(p0, p1);
-            pk[e] = *reinterpret_cast<uint32_t*>(&pp);
-          }
-          *reinterpret_cast<uint4*>(prow + tc::swz_offset<128>(row, c)) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
+        for (int e = 0; e < 32; ++e) {
+          const float p0 = ex2_approx(x[2 * e] - m_use), p1 = ex2_approx(x[2 * e + 1] - m_use);
+          sum0 += p0;
+          sum1 += p1;
+          __nv_bfloat162 pp = __floats2bfloat162_rn(p0, p1);
+          pk[e] = *reinterpret_cast<uint32_t*>(&pp);
         }
         l_run += sum0 + sum1;
-        tc::fence_proxy_async_smem();
+        // Steps that did not rescale wait for PV(i-1) only here, after the exponentials (P(i) goes into the buffer S(i) came
+        // from, not the one PV(i-1) reads, so nothing above depended on it).  The wait itself must not be dropped: a one-bit
+        // phase parity is only unambiguous while this thread has seen every phase but the newest, and PV(i) cannot complete
+        // before the arrival below.
+        if (!pv_seen) tc::mbar_wait(o_full, (i - 1) & 1);
+        // P(i) stays in tensor memory: bf16 pairs over the first 32 columns of this thread's own (already loaded) logits
+        tc::tmem_st32(tmem_S + lane_addr + (i & 1) * AT_BK, pk);
+        tc::tmem_st_wait();
         tc::tc_fence_before();
         tc::mbar_arrive(p_full);
       }
