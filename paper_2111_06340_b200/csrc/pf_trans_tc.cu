@@ -191,50 +191,58 @@ transition_kernel(const __grid_constant__ CUtensorMap tmW1, const __grid_constan
         tc::tc_fence_before();
         tc::mbar_arrive(&a2_full[buf]);
       }
-      // ---- E2: output columns + b2 -> fp32 staging (this team's A2 buffer, two 16 KB boxes) -> TMA reduce-add
-      tc::mbar_wait(acc2_full, it & 1);                // all GEMM2 of this tile complete: acc2 final, A2 buffers idle
+      // ---- E2: output columns + b2 -> fp32 staging (two 16 KB boxes per team) -> TMA reduce-add
+      tc::mbar_wait(acc2_full, it & 1);                // all GEMM2 of this tile complete: acc2 final
       tc::tc_fence_after();
-      // staging boxes: k-block `team` of both A2 buffers — the region only this team writes in E1, so the team leader's
-      // own bulk-group bookkeeping covers every reuse
+      // staging boxes: two per team, written only by that team, so the team leader's own bulk-group bookkeeping covers every reuse
       uint8_t* stage = smem + (SM::ST_ALIAS ? SM::A1_OFF + (int)(it % A1B) * SM::A1_BYTES : SM::ST_OFF) + team * 2 * SM::KB_BYTES;
-      int nbox = 0;
       if (!SM::ST_ALIAS) {
         if (leader) tc::bulk_wait_read<0>();           // the previous tile's reduce-adds have read their staging boxes
         tc::named_bar_sync(bar_id, 128);
       }
-#pragma unroll 1
-      for (int bx = team; bx < C / 32; bx += 2, ++nbox) {
-        uint8_t* sb = stage + (nbox & 1) * SM::KB_BYTES;
-        if (nbox >= 2) {
-          if (leader) tc::bulk_wait_read<1>();
-          tc::named_bar_sync(bar_id, 128);
-        }
-        uint32_t v[32];
-        float b2r[32];
-        tc::tmem_ld32(lane_addr + SM::TMEM_ACC2 + bx * 32, v);
+      // One box: registers + b2 -> swizzled fp32 staging tile -> TMA reduce-add into the residual
+      auto emit = [&](int bx, const uint32_t (&v)[32], uint8_t* sb) {
+        const float* bb = sb2 + bx * 32;
 #pragma unroll
         for (int q = 0; q < 8; ++q) {
-          const float4 t = *reinterpret_cast<const float4*>(sb2 + bx * 32 + q * 4);
-          b2r[q * 4 + 0] = t.x;
-          b2r[q * 4 + 1] = t.y;
-          b2r[q * 4 + 2] = t.z;
-          b2r[q * 4 + 3] = t.w;
-        }
-        tc::tmem_ld_wait();
-#pragma unroll
-        for (int q = 0; q < 8; ++q)
+          const float4 t = *reinterpret_cast<const float4*>(bb + q * 4);
           *reinterpret_cast<float4*>(sb + lr * 128 + (((uint32_t)q ^ sw) << 4)) =
-              make_float4(__uint_as_float(v[q * 4 + 0]) + b2r[q * 4 + 0], __uint_as_float(v[q * 4 + 1]) + b2r[q * 4 + 1],
-                          __uint_as_float(v[q * 4 + 2]) + b2r[q * 4 + 2], __uint_as_float(v[q * 4 + 3]) + b2r[q * 4 + 3]);
+              make_float4(__uint_as_float(v[q * 4 + 0]) + t.x, __uint_as_float(v[q * 4 + 1]) + t.y,
+                          __uint_as_float(v[q * 4 + 2]) + t.z, __uint_as_float(v[q * 4 + 3]) + t.w);
+        }
         tc::fence_proxy_async_smem();
         tc::named_bar_sync(bar_id, 128);
         if (leader) {
           tc::tma_reduce_add_2d(&tmR, sb, bx * 32, (int)(tile * 128));
           tc::bulk_commit();
         }
+      };
+      // This team's boxes are bx = team, team + 2, ... (2 at C = 128, 4 at C = 256), two at a time through registers; the
+      // accumulator is handed back to the MMA thread as soon as its last columns are in registers, before they are staged.
+      constexpr int NBOX = C / 64;
+      uint32_t va[32], vb[32];
+      tc::tmem_ld32(lane_addr + SM::TMEM_ACC2 + team * 32, va);
+      tc::tmem_ld32(lane_addr + SM::TMEM_ACC2 + (team + 2) * 32, vb);
+      tc::tmem_ld_wait();
+      if (NBOX == 2) {
+        tc::tc_fence_before();
+        tc::mbar_arrive(acc2_empty);
       }
-      tc::tc_fence_before();
-      tc::mbar_arrive(acc2_empty);
+      emit(team, va, stage);
+      emit(team + 2, vb, stage + SM::KB_BYTES);
+      if (NBOX == 4) {
+        tc::tmem_ld32(lane_addr + SM::TMEM_ACC2 + (team + 4) * 32, va);
+        tc::tmem_ld32(lane_addr + SM::TMEM_ACC2 + (team + 6) * 32, vb);
+        tc::tmem_ld_wait();
+        tc::tc_fence_before();
+        tc::mbar_arrive(acc2_empty);
+        if (leader) tc::bulk_wait_read<1>();           // the first box has been read by its reduce-add
+        tc::named_bar_sync(bar_id, 128);
+        emit(team + 4, va, stage);
+        if (leader) tc::bulk_wait_read<1>();
+        tc::named_bar_sync(bar_id, 128);
+        emit(team + 6, vb, stage + SM::KB_BYTES);
+      }
       ++it;
     }
     if (leader) tc::bulk_wait<0>();

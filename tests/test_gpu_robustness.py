@@ -69,6 +69,36 @@ def test_repeated_runs_are_bit_identical():
         assert np.array_equal(mo, outs[0][0]) and np.array_equal(zo, outs[0][1])
 
 
+def test_tmem_operand_kernels_bit_identical_under_load():
+    """The transition, outer-product and attention kernels keep the intermediate of their two chained GEMMs in tensor memory and
+    let a later tcgen05.mma overwrite columns an earlier one of the same thread read as its A operand, relying on issue-order
+    execution (no barrier in between).  A violated ordering would show as run-to-run differences once every SM works through
+    many tiles: eight repetitions of one block at a batch that gives each persistent CTA dozens of tiles must agree bit for
+    bit on every valid element."""
+    import torch
+    dev = torch.device("cuda:0")
+    B, S, N, nb = 24, 128, 128, 1
+    blocks = ps.make_weights(131, nb, bf16_weights=True)
+    msa, pair, sm, mm = ps.make_inputs(132, B, S, N, lengths=[128 - 3 * i for i in range(B)], msa_mask_frac_max=0.3)
+    smd, mmd = torch.from_numpy(sm).to(dev), torch.from_numpy(mm).to(dev)
+    m0, z0 = torch.from_numpy(msa).to(dev), torch.from_numpy(pair).to(dev)
+    vm, vz = valid_masks(sm, mm)
+    vmd, vzd = torch.from_numpy(vm).to(dev), torch.from_numpy(vz).to(dev)
+    h = pf.Evoformer(ps.pack_blob(blocks), pf.make_config(nb, pf.PF_BF16))
+    ref = None
+    for rep in range(8):
+        m, z = m0.clone(), z0.clone()
+        h.forward(m, z, smd, mmd, nb)
+        torch.cuda.synchronize()
+        m, z = m[vmd], z[vzd]
+        assert bool(torch.isfinite(m).all()) and bool(torch.isfinite(z).all())
+        if ref is None:
+            ref = (m, z)
+        else:
+            assert torch.equal(m, ref[0]) and torch.equal(z, ref[1]), f"run {rep} differs from run 0"
+    h.close()
+
+
 def test_cuda_graph_replay_matches_direct_launches():
     """Small shapes are launch-bound, so whole forward calls on them are captured into a CUDA graph per (buffers, shape) and
     replayed (pf_api.cu, dispatch_pass).  The graph holds the mask-flag kernels too, so changing the CONTENTS of the masks
