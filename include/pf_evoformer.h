@@ -108,6 +108,8 @@ pf_status pf_evoformer_forward_substep(pf_evoformer_t* h, float* msa_dev, float*
 /* End-to-end convenience: the same computation with HOST buffers (pinned or pageable).  The batch is pipelined in
  * chunks of proteins: host->device copies on an internal copy stream, forward on cuda_stream, device->host copies on a
  * second internal copy stream (ordered after earlier work on cuda_stream); returns after everything has completed.
+ * Chunk plan for B >= 16: B/16, seven chunks of ~B/8, B/16 proteins (B < 16: up to eight equal chunks); the environment
+ * variable PF_HOST_CHUNKS=a,b,c,... (at most 16 positive sizes adding up to B, otherwise ignored) overrides it.
  * Device staging buffers and the copy streams are owned by the handle (grow-only). */
 pf_status pf_evoformer_forward_host(pf_evoformer_t* h, float* msa_host, float* pair_host,
                                     const float* seq_mask_host, const float* msa_mask_host,

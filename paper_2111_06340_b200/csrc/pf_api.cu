@@ -686,33 +686,47 @@ extern "C" pf_status pf_evoformer_forward_host(pf_evoformer_t* h, float* msa_hos
     CUDA_TRY(cudaStreamCreateWithFlags(&h->d2h_stream, cudaStreamNonBlocking));
     for (auto& e : h->host_ev) CUDA_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
   }
-  // Chunk sizes: small chunks at both ends (the first copy-in and the last copy-out are not overlapped with compute, so they
-  // should be short), large ones in the middle (small batches use the GPU less well).  Measured at cfg2 with 8 equal chunks:
-  // 1012-1150 proteins/s; 2 chunks 866, 4 chunks 993.
-  int sizes[8];
+  // Chunk sizes.  The copies are the longer leg (cfg2: 1.6 GB each way, 38-40 ms full duplex, against 36 ms of compute), so
+  // compute follows the copy-in by one chunk and the call ends one chunk's compute + copy-out after the last byte has
+  // landed: seven equal chunks of B/8 (equal, so that none of them stalls the ones behind it: at cfg2 a chunk of 8 proteins
+  // is 6.9 waves of 128-row tiles, chunks of 13-14 were 1.3x slower per protein than their copy) between two half chunks at
+  // the ends (the first copy-in and the last compute + copy-out are not overlapped with anything).  Measured at cfg2
+  // (proteins/s): this plan 1391; 8 equal 1373; 16 equal 1234; 7 equal 1216; the former 4,8,14,13,13,8,4 plan 1295.
+  // PF_HOST_CHUNKS=a,b,c,... (at most 16 sizes that add up to B) overrides the plan (tuning other shapes).
+  int sizes[16];
   int n_chunks = 0;
-  if (B < 16) {
+  if (const char* plan = getenv("PF_HOST_CHUNKS")) {
+    int sum = 0;
+    for (const char* q = plan; *q && n_chunks < 16;) {
+      sizes[n_chunks] = atoi(q);
+      if (sizes[n_chunks] < 1) { sum = -1; break; }
+      sum += sizes[n_chunks++];
+      while (*q && *q != ',') ++q;
+      if (*q == ',') ++q;
+    }
+    if (sum != B) n_chunks = 0;
+  }
+  if (n_chunks > 0) {
+  } else if (B < 16) {
     n_chunks = B < 8 ? B : 8;
     for (int c = 0, b0 = 0; c < n_chunks; ++c) {
       sizes[c] = (B - b0 + (n_chunks - c) - 1) / (n_chunks - c);
       b0 += sizes[c];
     }
   } else {
-    const int e1 = B / 16, e2 = B / 8, mid = B - 2 * (e1 + e2);
-    const int n_mid = 3;
+    const int e1 = B / 16, mid = B - 2 * e1;
+    const int n_mid = 7;
     sizes[n_chunks++] = e1;
-    sizes[n_chunks++] = e2;
     for (int c = 0, left = mid; c < n_mid; ++c) {
       sizes[n_chunks] = (left + (n_mid - c) - 1) / (n_mid - c);
       left -= sizes[n_chunks++];
     }
-    sizes[n_chunks++] = e2;
     sizes[n_chunks++] = e1;
   }
   const size_t pm = (size_t)S * N * h->cfg.c_m, pz = (size_t)N * N * h->cfg.c_z;   // floats per protein
-  CUDA_TRY(cudaEventRecord(h->host_ev[16], st));                  // earlier work on the caller's stream comes first
-  CUDA_TRY(cudaStreamWaitEvent(h->h2d_stream, h->host_ev[16], 0));
-  CUDA_TRY(cudaStreamWaitEvent(h->d2h_stream, h->host_ev[16], 0));
+  CUDA_TRY(cudaEventRecord(h->host_ev[32], st));                  // earlier work on the caller's stream comes first
+  CUDA_TRY(cudaStreamWaitEvent(h->h2d_stream, h->host_ev[32], 0));
+  CUDA_TRY(cudaStreamWaitEvent(h->d2h_stream, h->host_ev[32], 0));
   CUDA_TRY(cudaMemcpyAsync(ds, seq_mask_host, (size_t)B * N * 4, cudaMemcpyHostToDevice, h->h2d_stream));
   CUDA_TRY(cudaMemcpyAsync(dr, msa_mask_host, (size_t)B * S * 4, cudaMemcpyHostToDevice, h->h2d_stream));
   int b0 = 0;
@@ -730,8 +744,8 @@ extern "C" pf_status pf_evoformer_forward_host(pf_evoformer_t* h, float* msa_hos
     pf_status s = pf_evoformer_forward(h, dm + b0 * pm, dz + b0 * pz, ds + (size_t)b0 * N, dr + (size_t)b0 * S, bc, S, N, n_blocks,
                                        stream);
     if (s != PF_OK) return s;
-    CUDA_TRY(cudaEventRecord(h->host_ev[8 + c], st));
-    CUDA_TRY(cudaStreamWaitEvent(h->d2h_stream, h->host_ev[8 + c], 0));
+    CUDA_TRY(cudaEventRecord(h->host_ev[16 + c], st));
+    CUDA_TRY(cudaStreamWaitEvent(h->d2h_stream, h->host_ev[16 + c], 0));
     CUDA_TRY(cudaMemcpyAsync(msa_host + b0 * pm, dm + b0 * pm, bc * pm * 4, cudaMemcpyDeviceToHost, h->d2h_stream));
     CUDA_TRY(cudaMemcpyAsync(pair_host + b0 * pz, dz + b0 * pz, bc * pz * 4, cudaMemcpyDeviceToHost, h->d2h_stream));
     b0 += bc;

@@ -95,7 +95,7 @@ struct pf_evoformer {
   size_t stage_bytes = 0;
   // forward_host pipelines the batch in chunks of proteins: copy-in stream, the caller's stream for compute, copy-out stream
   cudaStream_t h2d_stream = nullptr, d2h_stream = nullptr;
-  cudaEvent_t host_ev[3 * 8] = {};   // per chunk: inputs landed, compute done, (spare)
+  cudaEvent_t host_ev[2 * 16 + 1] = {};   // per chunk (at most 16): inputs landed [c], compute done [16 + c]; [32]: call start
   int num_sms = 148;
   long long launches = 0;
   pf::TmaCtx* tma = nullptr;
